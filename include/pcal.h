@@ -1,0 +1,168 @@
+/*
+ * pcal.h -- C ABI of libpcal: B200 (sm_100a) multi-tone phase-calibration (PCal) extraction.
+ *
+ * Method: Wagner & Pogrebenko, "Fast Multi-tone Phase Calibration Signal Extraction"
+ * (cited as PAPER.md:<line> = /root/reference/PAPER.md).  The hot path is
+ *     packed baseband samples --(decode)--> x[n]
+ *     x^[n] = x[n] exp(-j w_offset n)            (rotation, eq. 2.3)
+ *     P[b]  = sum_{n = b mod N_bins} x^[n]       (fold,     eq. 2.2)
+ *     T[i]  = sum_b P[b] exp(-j 2 pi i b/N_bins) ("DFT(P)")
+ * with N_bins = f_s / f_comb.  The rotator comes either from a precomputed look-up table of
+ * length L = lcm(N_bins, N_rotator), N_rotator = f_s / gcd(f_s, f_offset) (eq. 2.4)
+ * or from a recursive sinewave generator with constant phase increment (eq. 2.5-2.9,
+ * PAPER.md:68-120) that is re-derived from the exactly reduced integer phase in fp64 at least
+ * every 2^16 samples.
+ *
+ * Conventions: rotator sign exp(-j...) as eq. 2.3; forward unnormalised
+ * DFT; sample index n = 0 at the first sample after create/reset and running across
+ * pcal_extract calls; frequencies are snapped to a 1 micro-hertz integer grid and the snapped
+ * values define the problem.
+ *
+ * All functions return PCAL_OK (0) or a negative PCAL_ERR_*; nothing throws across the ABI.
+ * There is no CPU fallback: without a usable CUDA device pcal_create fails with PCAL_ERR_DEVICE.
+ * Pointers are marked [host] or [device].  A context is not thread-safe; all calls on one
+ * context must be issued from one thread at a time and use one CUDA stream (or be ordered
+ * externally).
+ */
+#ifndef PCAL_H_
+#define PCAL_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pcal_ctx pcal_ctx;
+
+enum {
+    PCAL_OK = 0,
+    PCAL_ERR_INVALID = -1,     /* bad argument (NULL, non-integer f_s/f_comb, bad bits/encoding/channels) */
+    PCAL_ERR_ALIGNMENT = -2,   /* pointer not 16-byte aligned or segment not a whole number of bytes/words */
+    PCAL_ERR_STATE = -3,       /* call not legal in the current state */
+    PCAL_ERR_UNSUPPORTED = -4, /* valid request this build cannot serve (e.g. LUT of impractical length) */
+    PCAL_ERR_DEVICE = -5,      /* CUDA error / no device */
+    PCAL_ERR_NOMEM = -6
+};
+
+/* Sample encodings (PAPER.md:31 says only "2-bit or higher"; tables defined here, R15).
+ * 2-bit OFFSET_BINARY: code c -> level 2c-3        (0:-3, 1:-1, 2:+1, 3:+3)
+ * 2-bit SIGN_MAG:      code (s<<1)|m, s=1 negative, m=1 magnitude 3   (0:+1, 1:+3, 2:-1, 3:-3)
+ * 8-bit TWOS_COMPLEMENT: int8 value.     32-bit IEEE_FLOAT: float32 value.
+ * Packing: 2-bit single channel, 4 samples per byte, sample m in bits 2(m&3)..2(m&3)+1 of byte
+ * m>>2.  2-bit with C > 1 channels (C a power of two, 2C <= 32): one field of 2C bits per time
+ * sample, fields packed LSB-first into little-endian 32-bit words; channel c in bits 2c..2c+1 of
+ * its field (C = 16: one uint32 per time sample). */
+enum { PCAL_ENC_OFFSET_BINARY = 0, PCAL_ENC_SIGN_MAG = 1, PCAL_ENC_TWOS_COMPLEMENT = 2, PCAL_ENC_IEEE_FLOAT = 3 };
+
+/* Rotator source for eq. 2.3. */
+enum { PCAL_ROT_AUTO = 0, PCAL_ROT_LUT = 1, PCAL_ROT_GENERATOR = 2 };
+
+#define PCAL_MAX_CHANNELS 16
+
+typedef struct pcal_info_t {
+    int32_t n_channels;
+    int32_t n_bins;                 /* N_bins = f_s / f_comb */
+    int32_t bits;
+    int32_t encoding;
+    int32_t rotator_requested;      /* PCAL_ROT_* as set */
+    int32_t rotator_in_effect;      /* PCAL_ROT_LUT or PCAL_ROT_GENERATOR (LUT also when all offsets are 0) */
+    int32_t integer_exact;          /* 1 if integer input and every f_offset == 0 (int64 bins valid) */
+    int32_t k_shift;                /* PAPER.md:97 bin shift in effect */
+    uint64_t n_processed;           /* samples per channel since create/reset */
+    uint64_t fold_period;           /* M: accumulation period of the fold kernel in time samples (LUT mode) */
+    uint64_t lut_len[PCAL_MAX_CHANNELS]; /* L_c = lcm(N_bins, N_rotator) per channel */
+    uint64_t kernel_launches;       /* CUDA kernels launched by this context so far */
+} pcal_info_t;
+
+/*
+ * Create a context (PAPER.md:37-57 problem statement).
+ *   out            [host] receives the context; caller frees with pcal_destroy.
+ *   f_s_hz         sample rate  > 0
+ *   f_comb_hz      comb spacing > 0; f_s/f_comb must be an integer >= 2 (eq. 2.2 needs an integer
+ *                  period), else PCAL_ERR_INVALID
+ *   f_offset_hz    comb offset >= 0 and < f_s, applied to every channel (see pcal_set_channel_offsets)
+ *   bits           2, 8 or 32;  encoding must match (2: OFFSET_BINARY|SIGN_MAG, 8: TWOS_COMPLEMENT,
+ *                  32: IEEE_FLOAT)
+ *   n_channels     1, or a power of two <= 16 with bits == 2
+ * Uses the current CUDA device.  Allocates device accumulators; tables are built lazily at the
+ * first pcal_extract.
+ */
+int pcal_create(pcal_ctx **out, double f_s_hz, double f_comb_hz, double f_offset_hz,
+                int bits, int encoding, int n_channels);
+
+/* Per-channel comb offsets (BASELINE.json config 4).  f_offset_hz: [host] n_channels doubles.
+ * Legal only before the first pcal_extract after create/reset, else PCAL_ERR_STATE. */
+int pcal_set_channel_offsets(pcal_ctx *ctx, const double *f_offset_hz);
+
+/* Choose the rotator source.  AUTO = LUT when the fold period is practical, else GENERATOR.
+ * LUT with an impractical period, or GENERATOR with n_channels > 1 -> PCAL_ERR_UNSUPPORTED
+ * (reported by the next pcal_extract).  Legal only before the first pcal_extract after
+ * create/reset. */
+int pcal_set_rotator(pcal_ctx *ctx, int mode);
+
+/* rotate by w_offset + k w_comb instead of w_offset (0 <= k < N_bins); outputs are
+ * un-shifted back to natural tone order by pcal_finalize (bin reordering) and by
+ * pcal_get_folded (which returns P as if k were 0).  Legal only before the first pcal_extract
+ * after create/reset. */
+int pcal_set_k_shift(pcal_ctx *ctx, int k);
+
+/* Absolute index of the next sample (default 0 after create/reset).  Lets a time-sharded rank
+ * start in the middle of the stream.  Same legality rule as above. */
+int pcal_set_start_index(pcal_ctx *ctx, uint64_t n_start);
+
+/*
+ * Rotate + fold one segment (eq. 2.3 + eq. 2.2) into the context's accumulators.
+ *   dev_samples    [device] 16-byte aligned, caller-owned, valid until the stream work completes
+ *   n_samples      samples PER CHANNEL in this segment; n_samples*bits*n_channels must be a
+ *                  multiple of 8 (whole bytes), else PCAL_ERR_ALIGNMENT.  0 is a no-op.
+ *   cuda_stream    cudaStream_t (NULL = default stream).  Asynchronous: never synchronises.
+ * Successive calls are one continuous stream: the result is invariant to the split points.
+ */
+int pcal_extract(pcal_ctx *ctx, const void *dev_samples, uint64_t n_samples, void *cuda_stream);
+
+/* Same, with the segment in [host] memory (pinned for full speed): copies it to the device in
+ * chunks on cuda_stream and extracts each chunk.  Returns after the last copy has been enqueued
+ * and the host buffer may be reused (it synchronises the stream). */
+int pcal_extract_host(pcal_ctx *ctx, const void *host_samples, uint64_t n_samples, void *cuda_stream);
+
+/*
+ * Tone spectrum: reduce + N_bins-point DFT of the folded period, copy to the host,
+ * synchronise the stream.
+ *   out_tones      [host] n_channels*N_bins*2 doubles; out[(c*N_bins + i)*2 + {0,1}] = Re, Im of
+ *                  T[c][i], natural tone order: tone i sits at frequency i*f_comb + f_offset,c.
+ * Does not reset: integration may continue and finalize may be called again.
+ */
+int pcal_finalize(pcal_ctx *ctx, double *out_tones);
+
+/* As pcal_finalize but only enqueues (DFT + async copy into out_tones, which should be pinned
+ * host memory) on the context's stream; the caller synchronises. */
+int pcal_finalize_async(pcal_ctx *ctx, double *out_tones);
+
+/* Folded period P before the DFT: [host] n_channels*N_bins*2 doubles (Re, Im).  Synchronises. */
+int pcal_get_folded(pcal_ctx *ctx, double *out_bins);
+
+/* Exact integer bins: [host] n_channels*N_bins int64.  Valid only for integer input with every
+ * f_offset == 0 and k_shift == 0 (else PCAL_ERR_STATE).  Synchronises. */
+int pcal_get_folded_i64(pcal_ctx *ctx, int64_t *out_bins);
+
+/* Add externally obtained folded bins (same layout as pcal_get_folded) into the accumulators:
+ * the exchange step of a time-sharded multi-GPU run. */
+int pcal_add_folded(pcal_ctx *ctx, const double *bins);
+
+/* Zero accumulators, sample index <- 0 (on the context's stream); parameters are kept. */
+int pcal_reset(pcal_ctx *ctx);
+
+/* Free everything.  NULL-safe. */
+void pcal_destroy(pcal_ctx *ctx);
+
+/* Describe the context.  info: [host]. */
+int pcal_info(const pcal_ctx *ctx, pcal_info_t *info);
+
+/* Static string for an error code. */
+const char *pcal_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCAL_H_ */

@@ -1,0 +1,222 @@
+"""Thin ctypes binding of libpcal (include/pcal.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for device
+memory (``tensor.data_ptr()``) and streams (``torch.cuda.current_stream().cuda_stream``) only.
+There is no fallback: if the shared library is missing or CUDA is unavailable, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpcal.so")
+_SRC_DIR = os.path.join(_HERE, "csrc")
+_INCLUDE = os.path.join(os.path.dirname(_HERE), "include", "pcal.h")
+
+PCAL_OK = 0
+ENC_OFFSET_BINARY, ENC_SIGN_MAG, ENC_TWOS_COMPLEMENT, ENC_IEEE_FLOAT = 0, 1, 2, 3
+ROT_AUTO, ROT_LUT, ROT_GENERATOR = 0, 1, 2
+MAX_CHANNELS = 16
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-shared", "-Xcompiler", "-fPIC"]
+
+
+class PcalError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {_strerror(code)} ({code})")
+        self.code = code
+
+
+class InfoT(ctypes.Structure):
+    _fields_ = [("n_channels", ctypes.c_int32), ("n_bins", ctypes.c_int32), ("bits", ctypes.c_int32),
+                ("encoding", ctypes.c_int32), ("rotator_requested", ctypes.c_int32),
+                ("rotator_in_effect", ctypes.c_int32), ("integer_exact", ctypes.c_int32),
+                ("k_shift", ctypes.c_int32), ("n_processed", ctypes.c_uint64),
+                ("fold_period", ctypes.c_uint64), ("lut_len", ctypes.c_uint64 * MAX_CHANNELS),
+                ("kernel_launches", ctypes.c_uint64)]
+
+
+def _sources():
+    return sorted(os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)) + [_INCLUDE]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile libpcal.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+    stale = force or not os.path.exists(LIB_PATH) or any(
+        os.path.getmtime(s) > os.path.getmtime(LIB_PATH) for s in _sources())
+    if stale:
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+              ["-o", LIB_PATH, os.path.join(_SRC_DIR, "pcal_api.cu")]
+        subprocess.check_call(cmd)
+    return LIB_PATH
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'`; "
+                               "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, u64, i32, dbl = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_double
+        sig = {
+            "pcal_create": (i32, [ctypes.POINTER(vp), dbl, dbl, dbl, i32, i32, i32]),
+            "pcal_set_channel_offsets": (i32, [vp, vp]),
+            "pcal_set_rotator": (i32, [vp, i32]),
+            "pcal_set_k_shift": (i32, [vp, i32]),
+            "pcal_set_start_index": (i32, [vp, u64]),
+            "pcal_extract": (i32, [vp, vp, u64, vp]),
+            "pcal_extract_host": (i32, [vp, vp, u64, vp]),
+            "pcal_finalize": (i32, [vp, vp]),
+            "pcal_finalize_async": (i32, [vp, vp]),
+            "pcal_get_folded": (i32, [vp, vp]),
+            "pcal_get_folded_i64": (i32, [vp, vp]),
+            "pcal_add_folded": (i32, [vp, vp]),
+            "pcal_reset": (i32, [vp]),
+            "pcal_destroy": (None, [vp]),
+            "pcal_info": (i32, [vp, ctypes.POINTER(InfoT)]),
+            "pcal_strerror": (ctypes.c_char_p, [i32]),
+        }
+        for name, (res, args) in sig.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _strerror(code: int) -> str:
+    try:
+        return lib().pcal_strerror(code).decode()
+    except Exception:  # pragma: no cover
+        return "?"
+
+
+def _check(code: int, what: str):
+    if code != PCAL_OK:
+        raise PcalError(code, what)
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+class Pcal:
+    """One extraction context (``pcal_ctx``).  Method names mirror the C ABI."""
+
+    def __init__(self, f_s_hz: float, f_comb_hz: float, f_offset_hz: float, bits: int, encoding: int,
+                 n_channels: int = 1):
+        h = ctypes.c_void_p()
+        _check(lib().pcal_create(ctypes.byref(h), f_s_hz, f_comb_hz, f_offset_hz, bits, encoding, n_channels),
+               "pcal_create")
+        self._h = h
+        self.n_channels = n_channels
+        self.n_bins = self.info().n_bins
+
+    # -- configuration ---------------------------------------------------------------------
+    def set_channel_offsets(self, f_offset_hz: Sequence[float]):
+        a = np.ascontiguousarray(f_offset_hz, np.float64)
+        assert a.shape == (self.n_channels,)
+        _check(lib().pcal_set_channel_offsets(self._h, a.ctypes.data), "pcal_set_channel_offsets")
+
+    def set_rotator(self, mode: int):
+        _check(lib().pcal_set_rotator(self._h, mode), "pcal_set_rotator")
+
+    def set_k_shift(self, k: int):
+        _check(lib().pcal_set_k_shift(self._h, k), "pcal_set_k_shift")
+
+    def set_start_index(self, n_start: int):
+        _check(lib().pcal_set_start_index(self._h, n_start), "pcal_set_start_index")
+
+    # -- hot path --------------------------------------------------------------------------
+    def extract(self, dev_samples, n_samples: Optional[int] = None, stream=None):
+        """dev_samples: CUDA tensor (or raw device pointer int); n_samples per channel."""
+        if hasattr(dev_samples, "data_ptr"):
+            if not dev_samples.is_cuda:
+                raise ValueError("pcal_extract needs a device buffer; use extract_host for host memory")
+            ptr = dev_samples.data_ptr()
+            if n_samples is None:
+                nbytes = dev_samples.numel() * dev_samples.element_size()
+                inf = self.info()
+                n_samples = nbytes * 8 // (inf.bits * inf.n_channels)
+        else:
+            ptr = int(dev_samples)
+        _check(lib().pcal_extract(self._h, ptr, n_samples, _stream_handle(stream)), "pcal_extract")
+
+    def extract_host(self, host_samples, n_samples: Optional[int] = None, stream=None):
+        """host_samples: CPU tensor / numpy array (pinned for full speed)."""
+        if hasattr(host_samples, "data_ptr"):
+            ptr = host_samples.data_ptr()
+            nbytes = host_samples.numel() * host_samples.element_size()
+        else:
+            ptr = host_samples.ctypes.data
+            nbytes = host_samples.nbytes
+        if n_samples is None:
+            inf = self.info()
+            n_samples = nbytes * 8 // (inf.bits * inf.n_channels)
+        _check(lib().pcal_extract_host(self._h, ptr, n_samples, _stream_handle(stream)), "pcal_extract_host")
+
+    def finalize(self) -> np.ndarray:
+        """complex128 [n_channels, N_bins] tone spectrum T (synchronises)."""
+        out = np.empty((self.n_channels, self.n_bins), np.complex128)
+        _check(lib().pcal_finalize(self._h, out.ctypes.data), "pcal_finalize")
+        return out
+
+    def finalize_async(self, out_pinned):
+        """Enqueue DFT + copy into a pinned complex128 host tensor; caller synchronises."""
+        _check(lib().pcal_finalize_async(self._h, out_pinned.data_ptr()), "pcal_finalize_async")
+
+    def get_folded(self) -> np.ndarray:
+        out = np.empty((self.n_channels, self.n_bins), np.complex128)
+        _check(lib().pcal_get_folded(self._h, out.ctypes.data), "pcal_get_folded")
+        return out
+
+    def get_folded_i64(self) -> np.ndarray:
+        out = np.empty((self.n_channels, self.n_bins), np.int64)
+        _check(lib().pcal_get_folded_i64(self._h, out.ctypes.data), "pcal_get_folded_i64")
+        return out
+
+    def add_folded(self, bins: np.ndarray):
+        b = np.ascontiguousarray(bins, np.complex128)
+        assert b.shape == (self.n_channels, self.n_bins)
+        _check(lib().pcal_add_folded(self._h, b.ctypes.data), "pcal_add_folded")
+
+    def reset(self):
+        _check(lib().pcal_reset(self._h), "pcal_reset")
+
+    def info(self) -> InfoT:
+        inf = InfoT()
+        _check(lib().pcal_info(self._h, ctypes.byref(inf)), "pcal_info")
+        return inf
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().pcal_destroy(self._h)
+            self._h = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def from_workload(w) -> "Pcal":
+    """Context for a ``synth.Workload`` (marshalling only)."""
+    p = Pcal(w.f_s_hz, w.f_comb_hz, w.f_offset_hz[0], w.bits, w.encoding, w.n_channels)
+    if w.n_channels > 1 or any(f != w.f_offset_hz[0] for f in w.f_offset_hz):
+        p.set_channel_offsets(w.f_offset_hz)
+    p.set_rotator({"auto": ROT_AUTO, "lut": ROT_LUT, "generator": ROT_GENERATOR}[w.rotator])
+    return p

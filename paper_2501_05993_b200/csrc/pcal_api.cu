@@ -1,0 +1,499 @@
+// pcal_api.cu -- host side of libpcal: the C ABI declared in include/pcal.h.
+// Validates, derives the geometry (N_bins, rotator lengths, fold period), builds tables in long
+// double on the host, and enqueues the kernels of pcal_fold.cuh / pcal_gen.cuh / pcal_post.cuh on
+// the caller's stream.  No CPU compute path: every step of the hot path runs in those kernels.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/pcal.h"
+#include "pcal_fold.cuh"
+#include "pcal_gen.cuh"
+#include "pcal_post.cuh"
+
+using namespace pcal;
+typedef unsigned __int128 u128;
+
+namespace {
+
+constexpr uint64_t kMaxFoldPeriod = 1ull << 22;   // LUT mode: M*C accumulators at most
+constexpr uint32_t kMaxSlotGroups = 2048;         // LUT mode: q at most
+constexpr uint64_t kMaxLutEntries = 1ull << 22;
+constexpr uint32_t kMaxBins = 4096;
+constexpr uint32_t kMaxIterPerLaunch = 2048;      // keeps the 16-bit lanes of fold_2bit exact
+constexpr size_t kStageBytes = 128ull << 20;
+
+uint64_t gcd64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
+// lcm with saturation
+uint64_t lcm_sat(uint64_t a, uint64_t b, uint64_t cap) {
+    if (a == 0 || b == 0) return 0;
+    u128 l = (u128)(a / gcd64(a, b)) * b;
+    return l > cap ? cap + 1 : (uint64_t)l;
+}
+uint64_t to_uhz(double f_hz) { return (uint64_t)llround(f_hz * 1e6); }
+uint64_t mulmod_host(uint64_t a, uint64_t b, uint64_t m) { return (uint64_t)(((u128)a * b) % m); }
+double2 phasor_neg_host(uint64_t k, uint64_t m) {
+    const long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)m;
+    return make_double2((double)cosl(ang), (double)(-sinl(ang)));
+}
+
+}  // namespace
+
+struct pcal_ctx {
+    // problem
+    uint64_t Fs, Fcomb, Foff[PCAL_MAX_CHANNELS], Feff[PCAL_MAX_CHANNELS];
+    int bits, enc, C, kind, sign_mag;
+    uint32_t n_bins;
+    int rot_req, rot_eff, k_shift;
+    uint64_t n_processed;
+    bool started, prepared, all_zero;
+    // LUT-mode geometry
+    uint32_t spv, F, q, R, grid;
+    uint64_t M, nrot[PCAL_MAX_CHANNELS], lut_len[PCAL_MAX_CHANNELS];
+    // generator-mode geometry
+    uint32_t gen_grid, gen_spt;
+    // device
+    int device, sm_count;
+    cudaStream_t stream;
+    double2 *d_P, *d_T, *d_W, *d_lut, *d_gen_partial, *d_tmp;
+    long long* d_Pint;
+    uint32_t *d_lut_off, *d_lut_len;
+    void *d_partial, *d_acc, *d_stage;
+    double* h_pinned;
+    uint64_t launches;
+};
+
+#define CU(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return PCAL_ERR_DEVICE; } } while (0)
+
+static void free_tables(pcal_ctx* c) {
+    cudaFree(c->d_lut); cudaFree(c->d_lut_off); cudaFree(c->d_lut_len);
+    cudaFree(c->d_partial); cudaFree(c->d_acc); cudaFree(c->d_gen_partial);
+    c->d_lut = nullptr; c->d_lut_off = c->d_lut_len = nullptr;
+    c->d_partial = c->d_acc = nullptr; c->d_gen_partial = nullptr;
+}
+
+extern "C" const char* pcal_strerror(int code) {
+    switch (code) {
+        case PCAL_OK: return "ok";
+        case PCAL_ERR_INVALID: return "invalid argument";
+        case PCAL_ERR_ALIGNMENT: return "pointer or segment length not aligned";
+        case PCAL_ERR_STATE: return "call not legal in this state";
+        case PCAL_ERR_UNSUPPORTED: return "unsupported configuration";
+        case PCAL_ERR_DEVICE: return "CUDA device error";
+        case PCAL_ERR_NOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int pcal_create(pcal_ctx** out, double f_s_hz, double f_comb_hz, double f_offset_hz,
+                           int bits, int encoding, int n_channels) {
+    if (!out) return PCAL_ERR_INVALID;
+    *out = nullptr;
+    if (!(f_s_hz > 0) || !(f_comb_hz > 0) || !(f_offset_hz >= 0) || !(f_offset_hz < f_s_hz)) return PCAL_ERR_INVALID;
+    const uint64_t Fs = to_uhz(f_s_hz), Fc = to_uhz(f_comb_hz), Fo = to_uhz(f_offset_hz);
+    if (Fs == 0 || Fc == 0 || Fs % Fc != 0 || Fs / Fc < 2 || Fs >= (1ull << 62)) return PCAL_ERR_INVALID;
+    if (Fs / Fc > kMaxBins) return PCAL_ERR_UNSUPPORTED;
+    int kind;
+    if (bits == 2 && (encoding == PCAL_ENC_OFFSET_BINARY || encoding == PCAL_ENC_SIGN_MAG)) kind = KIND_2BIT;
+    else if (bits == 8 && encoding == PCAL_ENC_TWOS_COMPLEMENT) kind = KIND_I8;
+    else if (bits == 32 && encoding == PCAL_ENC_IEEE_FLOAT) kind = KIND_F32;
+    else return PCAL_ERR_INVALID;
+    if (n_channels < 1 || n_channels > PCAL_MAX_CHANNELS || (n_channels & (n_channels - 1))) return PCAL_ERR_INVALID;
+    if (n_channels > 1 && bits != 2) return PCAL_ERR_INVALID;
+
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PCAL_ERR_DEVICE; }
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return PCAL_ERR_DEVICE; }
+
+    pcal_ctx* c = new (std::nothrow) pcal_ctx();
+    if (!c) return PCAL_ERR_NOMEM;
+    memset(c, 0, sizeof(*c));
+    c->Fs = Fs; c->Fcomb = Fc;
+    for (int i = 0; i < n_channels; ++i) c->Foff[i] = Fo;
+    c->bits = bits; c->enc = encoding; c->C = n_channels; c->kind = kind;
+    c->sign_mag = (encoding == PCAL_ENC_SIGN_MAG);
+    c->n_bins = (uint32_t)(Fs / Fc);
+    c->rot_req = PCAL_ROT_AUTO;
+    c->device = dev; c->sm_count = sms;
+    const size_t nb = (size_t)c->n_bins * n_channels;
+    bool ok = cudaMalloc(&c->d_P, nb * sizeof(double2)) == cudaSuccess &&
+              cudaMalloc(&c->d_T, nb * sizeof(double2)) == cudaSuccess &&
+              cudaMalloc(&c->d_tmp, nb * sizeof(double2)) == cudaSuccess &&
+              cudaMalloc(&c->d_Pint, nb * sizeof(long long)) == cudaSuccess &&
+              cudaMalloc(&c->d_W, (size_t)c->n_bins * sizeof(double2)) == cudaSuccess &&
+              cudaMallocHost(&c->h_pinned, nb * sizeof(double2)) == cudaSuccess;
+    if (ok) {
+        std::vector<double2> W(c->n_bins);
+        for (uint32_t k = 0; k < c->n_bins; ++k) W[k] = phasor_neg_host(k, c->n_bins);
+        ok = cudaMemcpy(c->d_W, W.data(), W.size() * sizeof(double2), cudaMemcpyHostToDevice) == cudaSuccess &&
+             cudaMemset(c->d_P, 0, nb * sizeof(double2)) == cudaSuccess &&
+             cudaMemset(c->d_Pint, 0, nb * sizeof(long long)) == cudaSuccess;
+    }
+    if (ok && 2 * (size_t)c->n_bins * sizeof(double2) > 48 * 1024)
+        ok = cudaFuncSetAttribute(dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)(2 * (size_t)c->n_bins * sizeof(double2))) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); pcal_destroy(c); return PCAL_ERR_DEVICE; }
+    *out = c;
+    return PCAL_OK;
+}
+
+extern "C" void pcal_destroy(pcal_ctx* c) {
+    if (!c) return;
+    free_tables(c);
+    cudaFree(c->d_P); cudaFree(c->d_T); cudaFree(c->d_tmp); cudaFree(c->d_Pint); cudaFree(c->d_W);
+    cudaFree(c->d_stage);
+    cudaFreeHost(c->h_pinned);
+    cudaGetLastError();
+    delete c;
+}
+
+extern "C" int pcal_set_channel_offsets(pcal_ctx* c, const double* f) {
+    if (!c || !f) return PCAL_ERR_INVALID;
+    if (c->started) return PCAL_ERR_STATE;
+    uint64_t tmp[PCAL_MAX_CHANNELS];
+    for (int i = 0; i < c->C; ++i) {
+        if (!(f[i] >= 0)) return PCAL_ERR_INVALID;
+        tmp[i] = to_uhz(f[i]);
+        if (tmp[i] >= c->Fs) return PCAL_ERR_INVALID;
+    }
+    memcpy(c->Foff, tmp, sizeof(uint64_t) * c->C);
+    c->prepared = false;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_set_rotator(pcal_ctx* c, int mode) {
+    if (!c || mode < PCAL_ROT_AUTO || mode > PCAL_ROT_GENERATOR) return PCAL_ERR_INVALID;
+    if (c->started) return PCAL_ERR_STATE;
+    c->rot_req = mode; c->prepared = false;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_set_k_shift(pcal_ctx* c, int k) {
+    if (!c || k < 0 || (uint32_t)k >= c->n_bins) return PCAL_ERR_INVALID;
+    if (c->started) return PCAL_ERR_STATE;
+    c->k_shift = k; c->prepared = false;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_set_start_index(pcal_ctx* c, uint64_t n_start) {
+    if (!c) return PCAL_ERR_INVALID;
+    if (c->started) return PCAL_ERR_STATE;
+    c->n_processed = n_start;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_info(const pcal_ctx* c, pcal_info_t* info) {
+    if (!c || !info) return PCAL_ERR_INVALID;
+    memset(info, 0, sizeof(*info));
+    info->n_channels = c->C; info->n_bins = (int32_t)c->n_bins; info->bits = c->bits; info->encoding = c->enc;
+    info->rotator_requested = c->rot_req; info->rotator_in_effect = c->prepared ? c->rot_eff : 0;
+    info->integer_exact = (c->prepared && c->all_zero && c->kind != KIND_F32) ? 1 : 0;
+    info->k_shift = c->k_shift;
+    info->n_processed = c->n_processed;
+    info->fold_period = c->prepared && c->rot_eff == PCAL_ROT_LUT ? c->M : 0;
+    for (int i = 0; i < c->C; ++i) {
+        const uint64_t Fe = (c->Foff[i] + (uint64_t)c->k_shift * c->Fcomb) % c->Fs;
+        const uint64_t nrot = Fe ? c->Fs / gcd64(c->Fs, Fe) : 1;
+        info->lut_len[i] = lcm_sat(c->n_bins, nrot, ~0ull >> 1);
+    }
+    info->kernel_launches = c->launches;
+    return PCAL_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Lazy set-up: decide LUT vs generator, derive the geometry, build the rotator tables.
+// ---------------------------------------------------------------------------------------------
+template <typename K>
+static int occupancy_of(K kernel, size_t smem) {
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kThreads, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return occ;
+}
+
+static int prepare(pcal_ctx* c) {
+    if (c->prepared) return PCAL_OK;
+    free_tables(c);
+    c->all_zero = true;
+    uint64_t total_lut = 0;
+    for (int i = 0; i < c->C; ++i) {
+        c->Feff[i] = (c->Foff[i] + (uint64_t)c->k_shift * c->Fcomb) % c->Fs;
+        c->nrot[i] = c->Feff[i] ? c->Fs / gcd64(c->Fs, c->Feff[i]) : 1;   // eq. 2.4
+        if (c->Feff[i]) c->all_zero = false;
+        total_lut += c->nrot[i] > kMaxLutEntries ? kMaxLutEntries + 1 : c->nrot[i];
+    }
+    c->spv = c->kind == KIND_F32 ? 4u : (c->kind == KIND_I8 ? 16u : 64u / (uint32_t)c->C);
+    c->F = c->kind == KIND_F32 ? 4u : (c->kind == KIND_I8 ? 16u : 64u);
+    c->gen_spt = c->kind == KIND_F32 ? 4u : 16u;
+
+    uint64_t M = lcm_sat(c->n_bins, c->spv, kMaxFoldPeriod);
+    for (int i = 0; i < c->C; ++i) M = M > kMaxFoldPeriod ? M : lcm_sat(M, c->nrot[i], kMaxFoldPeriod);
+    bool lut_ok = M <= kMaxFoldPeriod && total_lut <= kMaxLutEntries;
+    uint32_t q = 0;
+    if (lut_ok) {
+        const uint64_t S = M / c->spv;
+        const uint64_t qq = S / gcd64(S, 32);
+        lut_ok = qq <= kMaxSlotGroups;
+        q = (uint32_t)qq;
+    }
+    const bool gen_ok = c->C == 1 && (kThreads * c->gen_spt) % c->n_bins == 0;
+    int mode;
+    if (c->all_zero) mode = PCAL_ROT_LUT;
+    else if (c->rot_req == PCAL_ROT_LUT) mode = lut_ok ? PCAL_ROT_LUT : 0;
+    else if (c->rot_req == PCAL_ROT_GENERATOR) mode = gen_ok ? PCAL_ROT_GENERATOR : 0;
+    else mode = lut_ok ? PCAL_ROT_LUT : (gen_ok ? PCAL_ROT_GENERATOR : 0);
+    if (!mode) return PCAL_ERR_UNSUPPORTED;
+    c->rot_eff = mode;
+
+    if (mode == PCAL_ROT_LUT) {
+        int occ = 0;
+        size_t elem = 0;
+        if (c->kind == KIND_2BIT) { occ = c->sign_mag ? occupancy_of(fold_2bit_kernel<true>, 0) : occupancy_of(fold_2bit_kernel<false>, 0); elem = 2; }
+        else if (c->kind == KIND_I8) { occ = occupancy_of(fold_i8_kernel, 0); elem = 4; }
+        else { occ = occupancy_of(fold_f32_kernel, 0); elem = 8; }
+        if (occ < 1) return PCAL_ERR_DEVICE;
+        const uint32_t slots = (uint32_t)(c->sm_count * occ);
+        c->q = q; c->M = M;
+        c->R = slots / q ? slots / q : 1;
+        c->grid = c->q * c->R;
+        CU(cudaMalloc(&c->d_partial, (size_t)c->grid * c->F * 32 * elem));
+        CU(cudaMalloc(&c->d_acc, (size_t)c->q * c->F * 32 * 8));
+        // rotator tables (eq. 2.4), one per channel, built in long double
+        std::vector<double2> lut;
+        std::vector<uint32_t> off(c->C), len(c->C);
+        for (int i = 0; i < c->C; ++i) {
+            off[i] = (uint32_t)lut.size(); len[i] = (uint32_t)c->nrot[i];
+            for (uint64_t r = 0; r < c->nrot[i]; ++r) lut.push_back(phasor_neg_host(mulmod_host(r, c->Feff[i], c->Fs), c->Fs));
+            c->lut_len[i] = c->nrot[i];
+        }
+        CU(cudaMalloc(&c->d_lut, lut.size() * sizeof(double2)));
+        CU(cudaMalloc(&c->d_lut_off, c->C * sizeof(uint32_t)));
+        CU(cudaMalloc(&c->d_lut_len, c->C * sizeof(uint32_t)));
+        CU(cudaMemcpy(c->d_lut, lut.data(), lut.size() * sizeof(double2), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(c->d_lut_off, off.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    } else {
+        const size_t smem = 2 * (size_t)c->gen_spt * kThreads * sizeof(double);
+        int occ = 0;
+        if (c->kind == KIND_2BIT) { CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, smem); }
+        else if (c->kind == KIND_I8) { CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); occ = occupancy_of(gen_kernel<KIND_I8>, smem); }
+        else { occ = occupancy_of(gen_kernel<KIND_F32>, smem); }
+        if (occ < 1) return PCAL_ERR_DEVICE;
+        c->gen_grid = (uint32_t)(c->sm_count * occ);
+        CU(cudaMalloc(&c->d_gen_partial, (size_t)c->gen_grid * c->n_bins * sizeof(double2)));
+    }
+    c->prepared = true;
+    return PCAL_OK;
+}
+
+// one launch group of the LUT / zero-offset path over n time samples starting at data
+static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
+    const uint64_t n_bytes = n * (uint64_t)c->bits * c->C / 8;
+    const uint64_t n_vec = n_bytes / 16;
+    if (n_vec) {
+        FoldParams fp;
+        fp.data = reinterpret_cast<const uint4*>(data); fp.n_vec = n_vec; fp.q = c->q; fp.R = c->R;
+        const uint64_t NC = (n_vec + 31) / 32, NSR = (NC + c->q - 1) / c->q;
+        uint64_t it = (NSR + (uint64_t)c->R * kWarps - 1) / ((uint64_t)c->R * kWarps);
+        it = (it + kUnroll - 1) / kUnroll * kUnroll;
+        fp.n_iter = (uint32_t)it; fp.partial = c->d_partial;
+        const uint32_t total = c->q * c->F * 32;
+        if (c->kind == KIND_2BIT) {
+            if (c->sign_mag) fold_2bit_kernel<true><<<c->grid, kThreads, 0, st>>>(fp);
+            else fold_2bit_kernel<false><<<c->grid, kThreads, 0, st>>>(fp);
+            reduce_replicas_kernel<uint16_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
+                (const uint16_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
+        } else if (c->kind == KIND_I8) {
+            fold_i8_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+            reduce_replicas_kernel<int32_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
+                (const int32_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
+        } else {
+            fold_f32_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+            reduce_replicas_kernel<double, double><<<(total + 255) / 256, 256, 0, st>>>(
+                (const double*)c->d_partial, (double*)c->d_acc, c->q, c->R, c->F);
+        }
+        c->launches += 2;
+    }
+    RotateParams rp;
+    rp.acc = c->d_acc; rp.lut = c->d_lut; rp.lut_off = c->d_lut_off; rp.lut_len = c->d_lut_len;
+    rp.P = c->d_P; rp.Pint = c->d_Pint; rp.tail = data + n_vec * 16;
+    rp.n0 = c->n_processed; rp.NT = n_vec * c->spv; rp.n_total = n;
+    rp.q = c->q; rp.F = c->F; rp.C = (uint32_t)c->C; rp.spv = c->spv; rp.n_bins = c->n_bins;
+    rp.kind = c->kind; rp.sign_mag = c->sign_mag; rp.integer_exact = c->kind != KIND_F32;
+    rotate_fold_kernel<<<dim3(c->n_bins, c->C), kPostThreads, 0, st>>>(rp);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
+static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
+    const uint32_t spt = c->gen_spt;
+    const uint64_t load_bytes = c->kind == KIND_2BIT ? 4 : 16;
+    const uint64_t n_bytes = n * (uint64_t)c->bits / 8;
+    const uint64_t n_loads = n_bytes / load_bytes;
+    const uint64_t Fs = c->Fs, Fo = c->Feff[0];
+    if (n_loads) {
+        GenParams gp;
+        gp.data = data; gp.n_loads = n_loads;
+        gp.n_tiles = (n_loads * spt + kTileSamples - 1) / kTileSamples;
+        gp.Fs = Fs; gp.Foff = Fo;
+        gp.k0 = mulmod_host(c->n_processed % Fs, Fo, Fs);
+        gp.E = mulmod_host(kTileSamples, Fo, Fs);
+        gp.D = mulmod_host(c->gen_grid, gp.E, Fs);
+        gp.rho = phasor_neg_host(mulmod_host((uint64_t)kThreads * spt, Fo, Fs), Fs);
+        for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
+        gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
+        const size_t smem = 2 * (size_t)spt * kThreads * sizeof(double);
+        if (c->kind == KIND_2BIT) gen_kernel<KIND_2BIT><<<c->gen_grid, kThreads, smem, st>>>(gp);
+        else if (c->kind == KIND_I8) gen_kernel<KIND_I8><<<c->gen_grid, kThreads, smem, st>>>(gp);
+        else gen_kernel<KIND_F32><<<c->gen_grid, kThreads, smem, st>>>(gp);
+        c->launches += 1;
+    }
+    GenReduceParams gr;
+    gr.partial = c->d_gen_partial; gr.P = c->d_P; gr.tail = data + n_loads * load_bytes;
+    gr.n0 = c->n_processed; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
+    gr.grid = n_loads ? c->gen_grid : 0; gr.n_bins = c->n_bins; gr.kind = c->kind; gr.sign_mag = c->sign_mag;
+    gen_reduce_kernel<<<(c->n_bins + 127) / 128, 128, 0, st>>>(gr);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
+extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_samples, void* cuda_stream) {
+    if (!c) return PCAL_ERR_INVALID;
+    if (n_samples == 0) return PCAL_OK;
+    if (!dev_samples) return PCAL_ERR_INVALID;
+    if ((uintptr_t)dev_samples & 15u) return PCAL_ERR_ALIGNMENT;
+    if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
+    const int rc = prepare(c);
+    if (rc != PCAL_OK) return rc;
+    c->started = true;
+    c->stream = (cudaStream_t)cuda_stream;
+    const uint8_t* p = reinterpret_cast<const uint8_t*>(dev_samples);
+    // pieces: bounded per-thread trip count (LUT path) / whole segment (generator path)
+    uint64_t piece = n_samples;
+    if (c->rot_eff == PCAL_ROT_LUT)
+        piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
+    uint64_t done = 0;
+    while (done < n_samples) {
+        const uint64_t n = n_samples - done < piece ? n_samples - done : piece;
+        const uint8_t* base = p + done * (uint64_t)c->bits * c->C / 8;
+        const int r = c->rot_eff == PCAL_ROT_LUT ? extract_piece_lut(c, base, n, c->stream)
+                                                 : extract_piece_gen(c, base, n, c->stream);
+        if (r != PCAL_OK) return r;
+        c->n_processed += n;
+        done += n;
+    }
+    return PCAL_OK;
+}
+
+extern "C" int pcal_extract_host(pcal_ctx* c, const void* host_samples, uint64_t n_samples, void* cuda_stream) {
+    if (!c) return PCAL_ERR_INVALID;
+    if (n_samples == 0) return PCAL_OK;
+    if (!host_samples) return PCAL_ERR_INVALID;
+    if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!c->d_stage) CU(cudaMalloc(&c->d_stage, 2 * kStageBytes));
+    const uint64_t total = n_samples * (uint64_t)c->bits * c->C / 8;
+    const uint8_t* h = reinterpret_cast<const uint8_t*>(host_samples);
+    const uint64_t bits_per_t = (uint64_t)c->bits * c->C;
+    int buf = 0;
+    for (uint64_t off = 0; off < total; off += kStageBytes, buf ^= 1) {
+        const uint64_t bytes = total - off < kStageBytes ? total - off : kStageBytes;
+        uint8_t* d = reinterpret_cast<uint8_t*>(c->d_stage) + (size_t)buf * kStageBytes;
+        CU(cudaMemcpyAsync(d, h + off, bytes, cudaMemcpyHostToDevice, st));
+        const int r = pcal_extract(c, d, bytes * 8 / bits_per_t, st);
+        if (r != PCAL_OK) return r;
+    }
+    CU(cudaStreamSynchronize(st));
+    return PCAL_OK;
+}
+
+static int enqueue_dft(pcal_ctx* c) {
+    const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
+    dft_kernel<<<dim3((c->n_bins + 127) / 128, c->C), 128, smem, c->stream>>>(c->d_P, c->d_W, c->d_T, c->n_bins, (uint32_t)c->k_shift);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
+extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
+    if (!c || !out) return PCAL_ERR_INVALID;
+    const int r = enqueue_dft(c);
+    if (r != PCAL_OK) return r;
+    CU(cudaMemcpyAsync(out, c->d_T, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
+    return PCAL_OK;
+}
+
+extern "C" int pcal_finalize(pcal_ctx* c, double* out) {
+    if (!c || !out) return PCAL_ERR_INVALID;
+    const int r = pcal_finalize_async(c, c->h_pinned);
+    if (r != PCAL_OK) return r;
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(out, c->h_pinned, (size_t)c->n_bins * c->C * sizeof(double2));
+    return PCAL_OK;
+}
+
+// exp(+-j 2 pi k b / N) applied on the host to (un)shift the folded period
+static void kshift_bins(const pcal_ctx* c, double* bins, int sign) {
+    if (!c->k_shift) return;
+    for (int ch = 0; ch < c->C; ++ch)
+        for (uint32_t b = 0; b < c->n_bins; ++b) {
+            const uint64_t k = ((uint64_t)c->k_shift * b) % c->n_bins;
+            const long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)c->n_bins;
+            const long double cs = cosl(ang), sn = sign * sinl(ang);
+            double* z = bins + ((size_t)ch * c->n_bins + b) * 2;
+            const long double re = z[0] * cs - z[1] * sn, im = z[0] * sn + z[1] * cs;
+            z[0] = (double)re; z[1] = (double)im;
+        }
+}
+
+extern "C" int pcal_get_folded(pcal_ctx* c, double* out) {
+    if (!c || !out) return PCAL_ERR_INVALID;
+    const size_t bytes = (size_t)c->n_bins * c->C * sizeof(double2);
+    CU(cudaMemcpyAsync(c->h_pinned, c->d_P, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(out, c->h_pinned, bytes);
+    kshift_bins(c, out, +1);
+    return PCAL_OK;
+}
+
+extern "C" int pcal_get_folded_i64(pcal_ctx* c, int64_t* out) {
+    if (!c || !out) return PCAL_ERR_INVALID;
+    if (c->kind == KIND_F32 || c->k_shift) return PCAL_ERR_STATE;
+    for (int i = 0; i < c->C; ++i) if (c->Foff[i]) return PCAL_ERR_STATE;
+    const size_t bytes = (size_t)c->n_bins * c->C * sizeof(long long);
+    CU(cudaMemcpyAsync(c->h_pinned, c->d_Pint, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(out, c->h_pinned, bytes);
+    return PCAL_OK;
+}
+
+extern "C" int pcal_add_folded(pcal_ctx* c, const double* bins) {
+    if (!c || !bins) return PCAL_ERR_INVALID;
+    const uint32_t n = c->n_bins * (uint32_t)c->C;
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(c->h_pinned, bins, (size_t)n * sizeof(double2));
+    kshift_bins(c, c->h_pinned, -1);
+    CU(cudaMemcpyAsync(c->d_tmp, c->h_pinned, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, c->d_tmp, n);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(c->stream));
+    return PCAL_OK;
+}
+
+extern "C" int pcal_reset(pcal_ctx* c) {
+    if (!c) return PCAL_ERR_INVALID;
+    const uint32_t n = c->n_bins * (uint32_t)c->C;
+    zero_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, c->d_Pint, n);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->n_processed = 0;
+    c->started = false;
+    return PCAL_OK;
+}

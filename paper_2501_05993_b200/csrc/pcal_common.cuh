@@ -1,0 +1,76 @@
+// pcal_common.cuh -- shared device helpers and geometry constants for libpcal (sm_100a).
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pcal {
+
+// One CTA = 8 warps.  A "vector" is one 16-byte (128-bit) global load; a warp load covers 32
+// consecutive vectors = 512 contiguous bytes (4 full 128-byte lines).
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kUnroll = 8;            // independent 128-bit loads in flight per thread
+
+// sample kinds handled by the kernels
+enum Kind : int { KIND_F32 = 0, KIND_I8 = 1, KIND_2BIT = 2 };
+
+// Streaming 128-bit load: read-only path, do not allocate in L1 (each byte is used once).
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ uint32_t lop3_xor3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+__device__ __forceinline__ uint32_t lop3_maj(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE8;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+
+// Carry-save adder on 32 independent bit columns: a + b + c = s + 2*cy (per bit).
+// For words made of 2-bit fields (value = lo + 2*hi) the identity carries over to field values:
+// val(a)+val(b)+val(c) = val(s) + 2*val(cy)  -- two LOP3 compress three packed words into two.
+__device__ __forceinline__ void csa(uint32_t a, uint32_t b, uint32_t c, uint32_t& s, uint32_t& cy) {
+    s = lop3_xor3(a, b, c);
+    cy = lop3_maj(a, b, c);
+}
+
+// SIGN_MAG code (s<<1)|m  ->  OFFSET_BINARY code c' with level = 2c'-3:
+//   c' = x ^ 0b10 ^ (s ? 0b01 : 0)   for every 2-bit field at once (one shift + one LOP3).
+__device__ __forceinline__ uint32_t signmag_to_offset_binary(uint32_t x) {
+    return x ^ 0xAAAAAAAAu ^ ((x >> 1) & 0x55555555u);
+}
+
+__device__ __forceinline__ uint32_t word_of(const uint4& v, int j) {
+    return j == 0 ? v.x : (j == 1 ? v.y : (j == 2 ? v.z : v.w));
+}
+
+// (a * b) mod m for a, b < m < 2^63 without 128-bit division: double-and-add (64 steps worst case).
+// Only used a handful of times per kernel (tails, per-CTA start phases).
+__device__ __forceinline__ uint64_t mulmod_u64(uint64_t a, uint64_t b, uint64_t m) {
+    uint64_t r = 0;
+    a %= m;
+    while (b) {
+        if (b & 1) { r += a; if (r >= m) r -= m; }
+        a += a; if (a >= m) a -= m;
+        b >>= 1;
+    }
+    return r;
+}
+
+// exp(-j 2 pi k / m) in fp64 for an exactly reduced numerator 0 <= k < m.
+__device__ __forceinline__ double2 phasor_neg(uint64_t k, uint64_t m) {
+    double s, c;
+    sincospi(2.0 * ((double)k / (double)m), &s, &c);
+    return make_double2(c, -s);
+}
+
+}  // namespace pcal

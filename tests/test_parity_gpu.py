@@ -1,0 +1,224 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded bytes.  Sizes span many tiles / super-rows and end in a ragged tail.
+
+Bar (north_star): int64 folded bins bit-exact for integer input with f_offset = 0; every tone
+within 1e-5 relative and 1e-5 rad otherwise (R17: every one of the N_bins outputs).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2501_05993_b200 import synth
+from pcal_testlib import assert_close, gpu_run, oracle_fmt, oracle_folded, oracle_tones
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda"
+
+# (config index, n_samples) -- ragged: not a multiple of a 16-byte vector, of L, or of a tile
+SMALL = [
+    (1, 1_300_001),      # float32, f_offset 0
+    (2, 1_300_004),      # 2-bit offset-binary, L = 3200 (LUT)
+    (3, 2_600_036),      # 2-bit, N_bins 512, L = 51200 (LUT)
+    (4, 200_003),        # 16 channels, sign-magnitude, per-channel offsets
+    (5, 1_300_003),      # int8, irrational offset -> generator
+    (6, 1_300_004),      # cfg 2', f_offset 0: integer-exact
+    (7, 1_300_003),      # cfg 5', int8 f_offset 0: integer-exact
+    (8, 1_300_001),      # the paper's benchmark shape: float32 with rotation, L = 1600
+]
+
+
+def make(idx, n):
+    w = synth.config(idx).scaled(n)
+    dev = synth.generate(w, DEV)
+    host = dev.cpu().numpy()
+    return w, dev, host
+
+
+@pytest.mark.parametrize("idx,n", SMALL)
+def test_parity_every_config_small(oracle, idx, n):
+    w, dev, host = make(idx, n)
+    p, T, P = gpu_run(w, dev)
+    inf = p.info()
+    assert inf.n_processed == n
+    for c in range(w.n_channels):
+        pr, pi = oracle_folded(oracle, w, host, c)
+        want_P = pr.astype(np.float64) + 1j * pi.astype(np.float64)
+        assert_close(P[c], want_P, f"cfg{idx} ch{c} folded")
+        assert_close(T[c], oracle.dft(pr, pi), f"cfg{idx} ch{c} tones")
+    if idx in (6, 7):
+        assert inf.integer_exact == 1
+        got = p.get_folded_i64()
+        want = oracle.fold_i64(host, oracle_fmt(oracle, w), 1, 0, 0, 1, n, 0, w.n_bins)
+        assert np.array_equal(got[0], want)          # bit-exact
+        assert np.array_equal(P[0].real, want.astype(np.float64)) and not P[0].imag.any()
+
+
+def test_zero_offset_channel_of_cfg4_is_integer_exact(oracle):
+    """R20: force one zero-offset channel among rotated ones; its bins must be exact integers."""
+    w = synth.config(4).scaled(100_001)
+    w.f_offset_hz[3] = 0.0
+    dev = synth.generate(w, DEV)
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev)
+    want = oracle.fold_i64(host, oracle.TWO_BIT_SIGN_MAG, 16, 3, 0, 1, w.n_samples, 0, w.n_bins)
+    assert np.array_equal(P[3].real, want.astype(np.float64)) and not P[3].imag.any()
+    for c in (0, 3, 15):
+        assert_close(T[c], oracle_tones(oracle, w, host, c), f"ch{c}")
+
+
+@pytest.mark.parametrize("rot", ["lut", "generator"])
+def test_cfg3_both_rotator_variants(oracle, rot):
+    w, dev, host = make(3, 3_000_004)
+    p, T, P = gpu_run(w, dev, rotator=rot)
+    assert p.info().rotator_in_effect == (1 if rot == "lut" else 2)
+    assert_close(T[0], oracle_tones(oracle, w, host, 0), f"cfg3 {rot}")
+
+
+@pytest.mark.parametrize("idx,n", [(2, 700_004), (8, 500_003), (7, 400_001)])
+def test_generator_on_every_sample_type(oracle, idx, n):
+    """2-bit (both encodings), float32 and int8 through the generator kernel."""
+    w, dev, host = make(idx, n)
+    if idx == 7:
+        w = synth.replace(w, f_offset_hz=[1234.567])
+    p, T, P = gpu_run(w, dev, rotator="generator")
+    assert p.info().rotator_in_effect == 2
+    assert_close(T[0], oracle_tones(oracle, w, host, 0), f"gen cfg{idx}")
+    if idx == 2:
+        w2 = synth.replace(w, encoding=synth.ENC_SIGN_MAG)
+        p, T, P = gpu_run(w2, dev, rotator="generator")
+        assert_close(T[0], oracle_tones(oracle, w2, host, 0), "gen sign-mag")
+
+
+@pytest.mark.parametrize("idx,n,splits", [
+    (2, 1_000_004, [64, 64 * 1000, 64 * 9001]),
+    (5, 800_003, [16, 16 * 4099, 16 * 30000]),
+    (1, 500_001, [4, 4 * 77777]),
+    (4, 90_001, [4, 4 * 10001]),
+    (6, 600_004, [64 * 3, 64 * 5000]),
+])
+def test_split_point_invariance(oracle, idx, n, splits):
+    """Successive pcal_extract calls are one continuous stream (R7, R8)."""
+    w, dev, host = make(idx, n)
+    p1, T1, P1 = gpu_run(w, dev)
+    p2, T2, P2 = gpu_run(w, dev, splits=splits)
+    if idx == 6:
+        assert np.array_equal(p1.get_folded_i64(), p2.get_folded_i64())
+    scale = np.abs(P1).max()
+    assert np.abs(P1 - P2).max() <= 1e-9 * scale
+    for c in range(0, w.n_channels, 5):
+        assert_close(T2[c], oracle_tones(oracle, w, host, c), f"split cfg{idx} ch{c}")
+
+
+def test_start_index_and_add_folded_time_sharding(oracle):
+    """Two contexts each take half of the stream at its absolute index; summing P gives the whole."""
+    from paper_2501_05993_b200 import binding
+    w, dev, host = make(2, 1_000_000)
+    half = 64 * 7000
+    flat = dev.view(torch.uint8)
+    a = binding.from_workload(w)
+    a.extract(flat[: half // 4], half)
+    b = binding.from_workload(w)
+    b.set_start_index(half)
+    b.extract(flat[half // 4:], w.n_samples - half)
+    a.add_folded(b.get_folded())
+    assert_close(a.finalize()[0], oracle_tones(oracle, w, host, 0), "time-sharded")
+
+
+@pytest.mark.parametrize("idx", [2, 5])
+def test_k_shift_unshifts_to_natural_order(oracle, idx):
+    """rotate by w_off + k w_comb, reorder the bins back."""
+    w, dev, host = make(idx, 600_004 if idx == 2 else 500_000)
+    p, T, P = gpu_run(w, dev, k_shift=w.n_bins // 4)
+    assert p.info().k_shift == w.n_bins // 4
+    pr, pi = oracle_folded(oracle, w, host, 0)
+    assert_close(T[0], oracle.dft(pr, pi), f"k-shift cfg{idx}")
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"k-shift folded cfg{idx}")
+
+
+def test_bitwise_determinism():
+    w = synth.config(3).scaled(4_000_000)
+    dev = synth.generate(w, DEV)
+    for rot in ("lut", "generator"):
+        _, T1, P1 = gpu_run(w, dev, rotator=rot)
+        _, T2, P2 = gpu_run(w, dev, rotator=rot)
+        assert np.array_equal(T1.view(np.uint64), T2.view(np.uint64))
+        assert np.array_equal(P1.view(np.uint64), P2.view(np.uint64))
+
+
+@pytest.mark.parametrize("idx,n", [(2, 4), (2, 60), (2, 64), (2, 68), (5, 1), (5, 15), (5, 16), (5, 17),
+                                   (1, 1), (1, 3), (1, 4), (1, 5), (4, 1), (4, 3), (4, 4), (4, 5), (3, 2052)])
+def test_tiny_and_ragged_lengths(oracle, idx, n):
+    """Segments shorter than / equal to / just above one 16-byte vector (tail-only and 1-vector paths)."""
+    w, dev, host = make(idx, n)
+    if dev.numel() * dev.element_size() < 16:  # keep the device buffer 16-byte aligned & readable
+        pad = torch.zeros(16, dtype=torch.uint8, device=DEV)
+        pad[: dev.numel() * dev.element_size()] = dev.view(torch.uint8)
+        dev = pad
+    p, T, P = gpu_run(w, dev)
+    for c in range(w.n_channels):
+        pr, pi = oracle_folded(oracle, w, host, c)
+        want = pr.astype(np.float64) + 1j * pi.astype(np.float64)
+        assert np.abs(P[c] - want).max() <= 1e-9 * max(1.0, np.abs(want).max()), (idx, n, c)
+
+
+def test_impulse_and_reset(oracle):
+    """x = delta[n - n1] (float32): T[i] = e^{-j(i w_comb + w_off) n1}; reset restarts the index."""
+    from paper_2501_05993_b200 import binding
+    n1, N = 123_457, 200_000
+    x = torch.zeros(N, dtype=torch.float32, device=DEV)
+    x[n1] = 1.0
+    for rot in (binding.ROT_LUT, binding.ROT_GENERATOR):
+        p = binding.Pcal(32e6, 1e6, 10e3, 32, binding.ENC_IEEE_FLOAT, 1)
+        p.set_rotator(rot)
+        p.extract(x)
+        T = p.finalize()[0]
+        want = oracle.extract(x.cpu().numpy(), oracle.F32, 1, 0, N, 0, 32e6, 1e6, 10e3)
+        assert np.abs(T - want).max() < 1e-6
+        assert abs(abs(T[5]) - 1.0) < 1e-6
+        p.reset()
+        assert p.info().n_processed == 0
+        p.extract(x)
+        assert np.abs(p.finalize()[0] - want).max() < 1e-6
+        p.extract(x)  # continues the stream: second copy starts at absolute index N
+        want2 = want + oracle.extract(x.cpu().numpy(), oracle.F32, 1, 0, N, N, 32e6, 1e6, 10e3)
+        assert np.abs(p.finalize()[0] - want2).max() < 1e-6
+
+
+def test_extract_host_matches_device_path():
+    from paper_2501_05993_b200 import binding
+    w = synth.config(2).scaled(3_000_004)
+    dev = synth.generate(w, DEV)
+    _, T, _ = gpu_run(w, dev)
+    pinned = dev.cpu().pin_memory()
+    p = binding.from_workload(w)
+    p.extract_host(pinned, w.n_samples)
+    assert np.array_equal(p.finalize().view(np.uint64), T.view(np.uint64))
+
+
+def test_error_codes():
+    from paper_2501_05993_b200 import binding as B
+    for args in [(32e6, 3e6, 0.0, 2, 0, 1), (32e6, 1e6, 0.0, 3, 0, 1), (32e6, 1e6, 0.0, 8, 0, 1),
+                 (32e6, 1e6, 0.0, 2, 0, 3), (32e6, 1e6, 0.0, 8, 2, 2), (32e6, 1e6, 40e6, 2, 0, 1)]:
+        with pytest.raises(B.PcalError) as e:
+            B.Pcal(*args)
+        assert e.value.code == -1, args
+    p = B.Pcal(32e6, 1e6, 10e3, 2, B.ENC_OFFSET_BINARY, 1)
+    buf = torch.zeros(4096, dtype=torch.uint8, device=DEV)
+    with pytest.raises(B.PcalError) as e:
+        p.extract(buf[1:], 64)                       # misaligned pointer
+    assert e.value.code == -2
+    p.extract(buf, 0)                                # n = 0 is a no-op
+    assert p.info().n_processed == 0
+    p.extract(buf, 4096 * 4)
+    with pytest.raises(B.PcalError) as e:
+        p.set_rotator(B.ROT_GENERATOR)               # after the first extract
+    assert e.value.code == -3
+    with pytest.raises(B.PcalError) as e:
+        p.get_folded_i64()                           # rotated: no integer bins
+    assert e.value.code == -3
+    q = B.Pcal(1024e6, 1e6, 1234.567, 8, B.ENC_TWOS_COMPLEMENT, 1)
+    q.set_rotator(B.ROT_LUT)
+    with pytest.raises(B.PcalError) as e:
+        q.extract(torch.zeros(4096, dtype=torch.int8, device=DEV))
+    assert e.value.code == -4                        # LUT of impractical length
