@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- PCal extraction throughput on B200 (contract: see the task statement / DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config IDX] [--impl reference] [--all]
+
+A *step* is one pass of the whole hot path over one batch: pcal_reset -> pcal_extract (load/demux,
+decode, rotate, fold, reduce) -> pcal_finalize (DFT + result to the host).  Default workload:
+BASELINE.json configs[1] (single channel, 32 MHz, 2-bit, f_offset 10 kHz, 2^28 samples = 64 MiB).
+
+One JSON line on stdout (rank 0):
+  value      whole-job samples/s, inputs resident in HBM, device-timed over K steps (max over ranks)
+  e2e        same metric through pcal_extract_host: pinned HOST buffer -> device inside the timed
+             region, result read back to the host every step
+  roofline   the fused fold (or generator) kernel: algorithmic input bytes / its average duration,
+             measured live with CUDA events on the launching stream (pcal_set_profiling)
+  cpu_baseline  the CPU oracle timed on this box's host cores on a bounded sample of the workload
+`--impl reference` times the oracle (the only "reference implementation" this paper-only task has).
+With N > 1 (torchrun) the stream is time-sharded: each rank folds its own 2^28-sample range at its
+absolute start index, the bins are exchanged with one NCCL all-gather and summed in rank order
+(weak scaling: per-GPU work fixed).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pcal_extraction_samples_per_s"
+UNIT = "samples/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); smax = float(r[1])
+                for name, v in zip(names, r[4:8]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_fmt(orc, w):
+    from paper_2501_05993_b200 import synth
+    if w.bits == 32:
+        return orc.F32
+    if w.bits == 8:
+        return orc.I8
+    return orc.TWO_BIT_OFFSET_BINARY if w.encoding == synth.ENC_OFFSET_BINARY else orc.TWO_BIT_SIGN_MAG
+
+
+def time_oracle(w, n_sample: int, steps: int = 1):
+    """The oracle as it stands (O-fold + DFT), on n_sample samples of workload w, all host cores."""
+    import numpy as np
+    import oracle as orc
+    from paper_2501_05993_b200 import synth
+    orc.build()
+    ws = w.scaled(n_sample)
+    buf = synth.generate(ws, "cpu").numpy()
+    cores = os.cpu_count() or 1
+    fmt = oracle_fmt(orc, ws)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        for c in range(ws.n_channels):
+            orc.extract(buf, fmt, ws.n_channels, c, n_sample, 0, ws.f_s_hz, ws.f_comb_hz, ws.f_offset_hz[c],
+                        tabulated=True, threads=cores)
+    dt = (time.perf_counter() - t0) / steps
+    return n_sample * ws.n_channels / dt, cores, dt
+
+
+def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do_e2e: bool = True,
+            rotator: str | None = None, n_override: int | None = None):
+    """Run config idx on this rank's GPU; returns the measurement dict (device timing is per rank)."""
+    import torch
+    import torch.distributed as dist
+    from dataclasses import replace
+    from paper_2501_05993_b200 import binding, synth
+
+    w = synth.config(idx)
+    if n_override:
+        w = w.scaled(n_override)
+    if rotator:
+        w = replace(w, rotator=rotator)
+    n, C, nb = w.n_samples, w.n_channels, w.n_bins
+    # distinct input copies so that every step reads from DRAM, not from the 126 MB L2
+    ncopies = 1 if w.n_bytes >= (300 << 20) else min(8, -(-(300 << 20) // w.n_bytes))
+    bufs = [synth.generate(replace(w, seed=w.seed + 100 * i + 7 * rank), device) for i in range(ncopies)]
+    p = binding.from_workload(w)
+    out_pinned = torch.empty((C, nb), dtype=torch.complex128).pin_memory()
+    local = torch.empty(C * nb * 2, dtype=torch.float64, device=device)
+
+    def step(i):
+        p.reset()
+        if world > 1:
+            p.set_start_index(rank * n)
+        p.extract(bufs[i % ncopies], n)
+        if world > 1:  # the one exchange step: all-gather the bins, add them in rank order
+            p.get_folded_dev(local)
+            parts = [torch.empty_like(local) for _ in range(world)]
+            dist.all_gather(parts, local)
+            p.reset()
+            for part in parts:
+                p.add_folded_dev(part)
+        p.finalize_async(out_pinned)
+
+    # clocks are sampled from the start of the warm-up to the end of the timed region (a timed
+    # region of K short steps alone can be shorter than one nvidia-smi period); the warm-up runs
+    # >= W steps and >= 0.5 s of the same steps, so the samples are taken under the same load
+    sampler = ClockSampler(torch.cuda.current_device())
+    if rank == 0:
+        sampler.start()
+    t_w = time.perf_counter()
+    i = 0
+    while i < max(warmup, 3) or (rank == 0 and world == 1 and time.perf_counter() - t_w < 0.5):
+        step(i)
+        i += 1
+        if i % 16 == 0:
+            torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    launches0 = p.info().kernel_launches
+    p.set_profiling(True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    hot_ms, hot_launches = p.get_profile()
+    p.set_profiling(False)
+    launches = p.info().kernel_launches - launches0
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    inf = p.info()
+    res = {
+        "workload": w.name, "n_samples_per_channel": n, "n_channels": C, "n_bins": nb, "bits": w.bits,
+        "input_bytes": w.n_bytes, "rotator": {1: "lut", 2: "generator"}[inf.rotator_in_effect],
+        "fold_period": int(inf.fold_period), "ms_per_step": ms / steps,
+        "value": world * n * C * steps / (ms * 1e-3),
+        "input_gbs": world * w.n_bytes * steps / (ms * 1e-3) / 1e9,
+        "hot_kernel_us": 1e3 * hot_ms / max(hot_launches, 1), "hot_kernel_launches": int(hot_launches),
+        "gpu_launches": int(launches), "l2_policy": f"rotating {ncopies} distinct input copies "
+        f"({ncopies * w.n_bytes / 2**20:.0f} MiB total vs 126 MB L2)" if ncopies > 1 else "input larger than L2",
+        "clocks": clocks,
+    }
+    peak, peak_src = load_peaks()
+    # algorithmic bytes per launch = input bytes of one launch (bits/8 per sample, read once)
+    bytes_per_launch = w.n_bytes * steps / max(hot_launches, 1)
+    achieved = bytes_per_launch / (1e-3 * hot_ms / max(hot_launches, 1)) / 1e9 if hot_ms > 0 else 0.0
+    res["roofline"] = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                       "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                       "kernel": "fold_*_kernel (LUT path)" if inf.rotator_in_effect == 1 else "gen_kernel (generator path)",
+                       "algorithmic_bytes_per_launch": bytes_per_launch}
+    if do_e2e:
+        host = bufs[0].cpu().pin_memory()
+        e2e_steps = max(1, min(steps, 5 if w.n_bytes > (1 << 30) else steps))
+        p.reset(); p.extract_host(host, n); p.finalize()      # warm-up (allocates the staging buffer)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            p.reset()
+            p.extract_host(host, n)
+            T = p.finalize()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        res["e2e"] = {"value": world * n * C * e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": w.n_bytes,
+                      "d2h_bytes_per_step": C * nb * 16, "steps": e2e_steps,
+                      "api": "pcal_reset + pcal_extract_host (pinned host buffer) + pcal_finalize"}
+        del host
+    p.destroy()
+    del bufs
+    torch.cuda.empty_cache()
+    return res, w
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config (1-based); default configs[1]")
+    ap.add_argument("--impl", default="own", choices=["own", "reference"])
+    ap.add_argument("--no-all", action="store_true", help="skip the short per-config table")
+    ap.add_argument("--samples", type=int, default=0, help="override samples per channel (debug)")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2501_05993_b200 import synth
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        w = synth.config(args.config)
+        n_sample = 1 << 24
+        for _ in range(max(args.warmup, 1)):
+            time_oracle(w, 1 << 20)
+        rate, cores, dt = time_oracle(w, n_sample, steps=args.steps)
+        line = {"metric": METRIC, "value": rate, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "sample": f"first {n_sample} samples per step"},
+                "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                 "sample": f"{n_sample} samples of {w.name} per step, O-fold + DFT, {cores} threads"},
+                "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line), flush=True)
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None)
+    line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "int32/fp64 (integer fold, fp64 rotate+DFT)" if res["rotator"] == "lut" else "fp32 MAC / fp64 accumulate",
+            "data": "synthetic", "input_gbs": res["input_gbs"],
+            "config": {"workload": res["workload"], "n_samples_per_channel": res["n_samples_per_channel"],
+                       "n_channels": res["n_channels"], "bits": res["bits"], "n_bins": res["n_bins"],
+                       "rotator": res["rotator"], "input_bytes_per_gpu": res["input_bytes"],
+                       "parallelism": f"time-sharded x{world}" if world > 1 else "single GPU",
+                       "l2": res["l2_policy"]},
+            "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
+            "roofline": res["roofline"], "hot_kernel_us": res["hot_kernel_us"]}
+    if world == 1 and rank == 0:
+        probe, cores, _ = time_oracle(w, 1 << 21)
+        n_sample = int(min(w.n_samples, max(1 << 22, probe * 3.0)))
+        n_sample -= n_sample % 64
+        rate, cores, dt = time_oracle(w, n_sample)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"first {n_sample} samples of {w.name}, O-fold + DFT, {dt:.1f} s wall"}
+        if not args.no_all:
+            table = {}
+            for idx, rot in [(1, None), (2, None), (3, "lut"), (3, "generator"), (4, None), (5, None)]:
+                r, _ = measure(idx, 5 if idx == 5 else 10, 3, 0, 1, device, do_e2e=False, rotator=rot)
+                key = f"cfg{idx}" + (f"_{rot}" if rot else "")
+                table[key] = {k: r[k] for k in ("workload", "rotator", "value", "input_gbs", "ms_per_step", "hot_kernel_us")}
+                table[key]["roofline_frac"] = r["roofline"]["frac"]
+                table[key]["roofline_achieved_gbs"] = r["roofline"]["achieved"]
+            line["all_configs"] = table
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -150,6 +150,21 @@ int pcal_get_folded_i64(pcal_ctx *ctx, int64_t *out_bins);
  * the exchange step of a time-sharded multi-GPU run. */
 int pcal_add_folded(pcal_ctx *ctx, const double *bins);
 
+/* Device-resident variants of pcal_get_folded / pcal_add_folded for an exchange that stays on the
+ * GPU (NCCL all-gather of the bins): dev_bins is [device] n_channels*N_bins*2 doubles.  Asynchronous
+ * on the context's stream.  They move the raw accumulators (no k_shift un-shifting): every rank of
+ * a sharded run must use the same k_shift. */
+int pcal_get_folded_dev(pcal_ctx *ctx, double *dev_bins);
+int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
+
+/* Timing hook for the roofline report: when enabled, every launch of the hot kernel (the fused
+ * load/decode/fold kernel of the LUT path or the generator kernel) is bracketed by CUDA events on
+ * the launching stream.  pcal_get_profile synchronises the stream and returns the summed event time
+ * in milliseconds and the number of hot-kernel launches since profiling was enabled (or since the
+ * last pcal_get_profile). */
+int pcal_set_profiling(pcal_ctx *ctx, int enable);
+int pcal_get_profile(pcal_ctx *ctx, double *hot_kernel_ms, uint64_t *hot_kernel_launches);
+
 /* Zero accumulators, sample index <- 0 (on the context's stream); parameters are kept. */
 int pcal_reset(pcal_ctx *ctx);
 

@@ -103,8 +103,10 @@ def fold_ld(buf, fmt, n_channels, c, m_first, m_step, m_end, n_abs0, f_s_hz, f_c
         pr = np.zeros(nb, np.longdouble)
         pi = np.zeros(nb, np.longdouble)
         if hi > lo:
-            if tabulated and Fo != 0:
-                nrot = L.orc_rotator_len(Fs, Fo)
+            nrot = L.orc_rotator_len(Fs, Fo)
+            # tabulate only a rotator vector of practical length ("impractically long
+            # vector"); otherwise every phasor is computed directly -- the values are identical
+            if tabulated and Fo != 0 and nrot <= (1 << 24):
                 tc = np.empty(nrot, np.float64)
                 ts = np.empty(nrot, np.float64)
                 L.orc_fold_tabulated(_ptr(buf), fmt, n_channels, c, lo, m_step, hi, n_abs0, Fs, Fc, Fo,

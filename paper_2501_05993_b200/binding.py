@@ -82,6 +82,10 @@ def lib():
             "pcal_get_folded": (i32, [vp, vp]),
             "pcal_get_folded_i64": (i32, [vp, vp]),
             "pcal_add_folded": (i32, [vp, vp]),
+            "pcal_get_folded_dev": (i32, [vp, vp]),
+            "pcal_add_folded_dev": (i32, [vp, vp]),
+            "pcal_set_profiling": (i32, [vp, i32]),
+            "pcal_get_profile": (i32, [vp, ctypes.POINTER(dbl), ctypes.POINTER(u64)]),
             "pcal_reset": (i32, [vp]),
             "pcal_destroy": (None, [vp]),
             "pcal_info": (i32, [vp, ctypes.POINTER(InfoT)]),
@@ -192,6 +196,21 @@ class Pcal:
         b = np.ascontiguousarray(bins, np.complex128)
         assert b.shape == (self.n_channels, self.n_bins)
         _check(lib().pcal_add_folded(self._h, b.ctypes.data), "pcal_add_folded")
+
+    def get_folded_dev(self, dev_bins):
+        _check(lib().pcal_get_folded_dev(self._h, dev_bins.data_ptr()), "pcal_get_folded_dev")
+
+    def add_folded_dev(self, dev_bins):
+        _check(lib().pcal_add_folded_dev(self._h, dev_bins.data_ptr()), "pcal_add_folded_dev")
+
+    def set_profiling(self, enable: bool):
+        _check(lib().pcal_set_profiling(self._h, int(enable)), "pcal_set_profiling")
+
+    def get_profile(self):
+        """(summed hot-kernel event time in ms, hot-kernel launches) since the last call."""
+        ms, n = ctypes.c_double(), ctypes.c_uint64()
+        _check(lib().pcal_get_profile(self._h, ctypes.byref(ms), ctypes.byref(n)), "pcal_get_profile")
+        return ms.value, n.value
 
     def reset(self):
         _check(lib().pcal_reset(self._h), "pcal_reset")

@@ -66,7 +66,29 @@ struct pcal_ctx {
     void *d_partial, *d_acc, *d_stage;
     double* h_pinned;
     uint64_t launches;
+    // profiling hook
+    bool profiling;
+    std::vector<cudaEvent_t>* ev;   // pairs (start, stop) recorded so far
+    size_t ev_used;
+    double prof_ms;
+    uint64_t prof_launches;
 };
+
+// bracket the hot kernel with events on the launching stream (only when profiling is on)
+static void prof_mark(pcal_ctx* c, cudaStream_t st) {
+    if (!c->profiling) return;
+    if (!c->ev) c->ev = new std::vector<cudaEvent_t>();
+    if (c->ev_used == c->ev->size()) { cudaEvent_t e; cudaEventCreate(&e); c->ev->push_back(e); }
+    cudaEventRecord((*c->ev)[c->ev_used++], st);
+}
+static void prof_collect(pcal_ctx* c) {
+    for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, (*c->ev)[i], (*c->ev)[i + 1]) == cudaSuccess) { c->prof_ms += ms; c->prof_launches++; }
+    }
+    c->ev_used = 0;
+    cudaGetLastError();
+}
 
 #define CU(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return PCAL_ERR_DEVICE; } } while (0)
 
@@ -148,6 +170,7 @@ extern "C" void pcal_destroy(pcal_ctx* c) {
     cudaFree(c->d_P); cudaFree(c->d_T); cudaFree(c->d_tmp); cudaFree(c->d_Pint); cudaFree(c->d_W);
     cudaFree(c->d_stage);
     cudaFreeHost(c->h_pinned);
+    if (c->ev) { for (cudaEvent_t e : *c->ev) cudaEventDestroy(e); delete c->ev; }
     cudaGetLastError();
     delete c;
 }
@@ -302,17 +325,21 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         it = (it + kUnroll - 1) / kUnroll * kUnroll;
         fp.n_iter = (uint32_t)it; fp.partial = c->d_partial;
         const uint32_t total = c->q * c->F * 32;
+        prof_mark(c, st);
         if (c->kind == KIND_2BIT) {
             if (c->sign_mag) fold_2bit_kernel<true><<<c->grid, kThreads, 0, st>>>(fp);
             else fold_2bit_kernel<false><<<c->grid, kThreads, 0, st>>>(fp);
+            prof_mark(c, st);
             reduce_replicas_kernel<uint16_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
                 (const uint16_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
         } else if (c->kind == KIND_I8) {
             fold_i8_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+            prof_mark(c, st);
             reduce_replicas_kernel<int32_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
                 (const int32_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
         } else {
             fold_f32_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+            prof_mark(c, st);
             reduce_replicas_kernel<double, double><<<(total + 255) / 256, 256, 0, st>>>(
                 (const double*)c->d_partial, (double*)c->d_acc, c->q, c->R, c->F);
         }
@@ -348,9 +375,11 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
         const size_t smem = 2 * (size_t)spt * kThreads * sizeof(double);
+        prof_mark(c, st);
         if (c->kind == KIND_2BIT) gen_kernel<KIND_2BIT><<<c->gen_grid, kThreads, smem, st>>>(gp);
         else if (c->kind == KIND_I8) gen_kernel<KIND_I8><<<c->gen_grid, kThreads, smem, st>>>(gp);
         else gen_kernel<KIND_F32><<<c->gen_grid, kThreads, smem, st>>>(gp);
+        prof_mark(c, st);
         c->launches += 1;
     }
     GenReduceParams gr;
@@ -495,5 +524,38 @@ extern "C" int pcal_reset(pcal_ctx* c) {
     CU(cudaGetLastError());
     c->n_processed = 0;
     c->started = false;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_get_folded_dev(pcal_ctx* c, double* dev_bins) {
+    if (!c || !dev_bins) return PCAL_ERR_INVALID;
+    CU(cudaMemcpyAsync(dev_bins, c->d_P, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
+    return PCAL_OK;
+}
+
+extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
+    if (!c || !dev_bins) return PCAL_ERR_INVALID;
+    const uint32_t n = c->n_bins * (uint32_t)c->C;
+    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_bins), n);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
+extern "C" int pcal_set_profiling(pcal_ctx* c, int enable) {
+    if (!c) return PCAL_ERR_INVALID;
+    CU(cudaStreamSynchronize(c->stream));
+    prof_collect(c);
+    c->profiling = enable != 0;
+    c->prof_ms = 0.0; c->prof_launches = 0;
+    return PCAL_OK;
+}
+
+extern "C" int pcal_get_profile(pcal_ctx* c, double* ms, uint64_t* launches) {
+    if (!c || !ms || !launches) return PCAL_ERR_INVALID;
+    CU(cudaStreamSynchronize(c->stream));
+    prof_collect(c);
+    *ms = c->prof_ms; *launches = c->prof_launches;
+    c->prof_ms = 0.0; c->prof_launches = 0;
     return PCAL_OK;
 }

@@ -1,0 +1,63 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one
+pcal_extract over the whole resident buffer, then pcal_finalize).
+
+Configs 1-4: every folded bin and every tone against the oracle (rotator tabulated, host threads over
+contiguous ranges).  Config 5 (4e9 samples): sampled folded bins the oracle can compute one by one
+(a bin only needs the 1/1024 of the samples that land in it), plus the property that the tones equal
+the oracle's DFT of the GPU's folded period.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2501_05993_b200 import synth
+from pcal_testlib import assert_close, gpu_run, oracle_folded
+
+pytestmark = pytest.mark.gpu
+THREADS = min(32, os.cpu_count() or 1)
+
+
+@pytest.mark.parametrize("idx,rot", [(1, None), (2, None), (3, "lut"), (3, "generator")])
+def test_fullsize_single_channel(oracle, idx, rot):
+    w = synth.config(idx)
+    dev = synth.generate(w, "cuda")
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev, rotator=rot)
+    assert p.info().n_processed == w.n_samples
+    pr, pi = oracle_folded(oracle, w, host, 0, threads=THREADS)
+    rel, _ = assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"cfg{idx} {rot} folded")
+    assert_close(T[0], oracle.dft(pr, pi), f"cfg{idx} {rot} tones")
+    print(f"cfg{idx} {rot}: worst-bin relative error {rel:.3e}")
+
+
+def test_fullsize_cfg4_sixteen_channels(oracle):
+    w = synth.config(4)
+    dev = synth.generate(w, "cuda")
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev)
+    assert p.info().fold_period == 6400
+    for c in (0, 5, 10, 15):
+        pr, pi = oracle_folded(oracle, w, host, c, threads=THREADS)
+        assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"cfg4 ch{c} folded")
+        assert_close(T[c], oracle.dft(pr, pi), f"cfg4 ch{c} tones")
+
+
+def test_fullsize_cfg5_sampled_bins(oracle):
+    w = synth.config(5)
+    dev = synth.generate(w, "cuda")
+    p, T, P = gpu_run(w, dev)
+    assert p.info().rotator_in_effect == 2 and p.info().n_processed == w.n_samples
+    host = dev.cpu().numpy()
+    del dev
+    torch.cuda.empty_cache()
+    bins = [0, 1, 511, 512, 777, 1023]
+    pr, pi = oracle_folded(oracle, w, host, 0, threads=THREADS, tabulated=False, bins=bins)
+    want = pr.astype(np.float64) + 1j * pi.astype(np.float64)
+    assert_close(P[0][bins], want[bins], "cfg5 sampled folded bins")
+    # tones: property that holds at any size -- T == DFT(P) with the oracle's DFT on the GPU's P
+    assert_close(T[0], oracle.dft(P[0].real, P[0].imag), "cfg5 tones vs oracle DFT of folded")
+    # the comb must be visible: in-band tone amplitudes ~ A N / 2 (closed form of eq. 2.1)
+    amp = 2 * np.abs(T[0][1:500]) / w.n_samples
+    assert np.all(np.abs(amp - w.amp) < 0.05), (amp.min(), amp.max())
