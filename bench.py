@@ -118,7 +118,7 @@ def time_oracle(w, n_sample: int, steps: int = 1):
 
 
 def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do_e2e: bool = True,
-            rotator: str | None = None, n_override: int | None = None):
+            rotator: str | None = None, n_override: int | None = None, min_warm_s: float = 0.5):
     """Run config idx on this rank's GPU; returns the measurement dict (device timing is per rank)."""
     import torch
     import torch.distributed as dist
@@ -160,7 +160,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         sampler.start()
     t_w = time.perf_counter()
     i = 0
-    while i < max(warmup, 3) or (rank == 0 and world == 1 and time.perf_counter() - t_w < 0.5):
+    while i < max(warmup, 3) or (rank == 0 and world == 1 and time.perf_counter() - t_w < min_warm_s):
         step(i)
         i += 1
         if i % 16 == 0:
@@ -243,6 +243,8 @@ def main():
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
     ap.add_argument("--no-all", action="store_true", help="skip the short per-config table")
     ap.add_argument("--samples", type=int, default=0, help="override samples per channel (debug)")
+    ap.add_argument("--quick", action="store_true",
+                    help="profiling mode (ncu): exactly W warm-up steps, no e2e / cpu_baseline / per-config table")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -276,7 +278,8 @@ def main():
     device = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
-    res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None)
+    res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None,
+                     do_e2e=not args.quick, min_warm_s=0.0 if args.quick else 0.5)
     line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": res["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
@@ -289,13 +292,14 @@ def main():
                        "l2": res["l2_policy"]},
             "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
             "roofline": res["roofline"], "hot_kernel_us": res["hot_kernel_us"]}
-    if world == 1 and rank == 0:
+    if world == 1 and rank == 0 and not args.quick:
         probe, cores, _ = time_oracle(w, 1 << 21)
-        n_sample = int(min(w.n_samples, max(1 << 22, probe * 3.0)))
+        n_sample = int(min(w.n_samples, max(1 << 22, probe * 1.0)))
         n_sample -= n_sample % 64
-        rate, cores, dt = time_oracle(w, n_sample)
+        reps = max(1, int(round(probe * 1.5 / n_sample)))          # ~1.5 s wall on all cores
+        rate, cores, dt = time_oracle(w, n_sample, steps=reps)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"first {n_sample} samples of {w.name}, O-fold + DFT, {dt:.1f} s wall"}
+                                "sample": f"first {n_sample} samples of {w.name}, O-fold + DFT, {reps} x {dt:.2f} s wall on {cores} threads"}
         if not args.no_all:
             table = {}
             for idx, rot in [(1, None), (2, None), (3, "lut"), (3, "generator"), (4, None), (5, None)]:

@@ -105,7 +105,10 @@ def test_split_point_invariance(oracle, idx, n, splits):
     if idx == 6:
         assert np.array_equal(p1.get_folded_i64(), p2.get_folded_i64())
     scale = np.abs(P1).max()
-    assert np.abs(P1 - P2).max() <= 1e-9 * scale
+    # integer fold + fp64 rotate: only fp64 rounding may differ; fp32-run paths (generator, float32
+    # input) regroup their short fp32 runs when the tiling shifts
+    tol = 1e-6 if (idx in (1, 5)) else 1e-11
+    assert np.abs(P1 - P2).max() <= tol * scale
     for c in range(0, w.n_channels, 5):
         assert_close(T2[c], oracle_tones(oracle, w, host, c), f"split cfg{idx} ch{c}")
 
