@@ -62,5 +62,6 @@ def test_fullsize_cfg5_sampled_bins(oracle):
     # BASELINE.json config 5 compresses the tone amplitudes below the closed form's A N / 2.)
     amp = 2 * np.abs(T[0][1:500]) / w.n_samples
     assert np.all((amp > 0.3 * w.amp) & (amp < 1.05 * w.amp)), (amp.min(), amp.max())
-    noise_bin = 2 * np.abs(T[0][600:1000]) / w.n_samples
-    assert noise_bin.max() < 0.05 * amp.min()
+    # (No "upper bins are noise-only" check here: the clip's odd-order intermodulation products
+    # f_a + f_b - f_c = (a+b-c) f_comb + f_offset fall exactly on comb bins, including the aliased
+    # ones above N_bins/2, so those bins legitimately hold power for this input.)
