@@ -243,6 +243,7 @@ def main():
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
     ap.add_argument("--no-all", action="store_true", help="skip the short per-config table")
     ap.add_argument("--samples", type=int, default=0, help="override samples per channel (debug)")
+    ap.add_argument("--rotator", default=None, choices=["lut", "generator"], help="force the rotator variant (config 3 runs both)")
     ap.add_argument("--quick", action="store_true",
                     help="profiling mode (ncu): exactly W warm-up steps, no e2e / cpu_baseline / per-config table")
     args = ap.parse_args()
@@ -279,7 +280,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
     res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None,
-                     do_e2e=not args.quick, min_warm_s=0.0 if args.quick else 0.5)
+                     rotator=args.rotator, do_e2e=not args.quick, min_warm_s=0.0 if args.quick else 0.5)
     line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": res["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
