@@ -63,9 +63,13 @@ struct pcal_ctx {
     double2 *d_P, *d_T, *d_W, *d_lut, *d_gen_partial, *d_tmp;
     long long* d_Pint;
     uint32_t *d_lut_off, *d_lut_len;
-    void *d_partial, *d_acc, *d_stage;
+    void *d_partial, *d_stage;
+    double* d_val;                  // [q][F][32] replica sums (stage 1 of pcal_post.cuh)
+    uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
+    bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
     uint64_t launches;
+    void (*fold2)(FoldParams);      // the fold_2bit_kernel instantiation in use
     // profiling hook
     bool profiling;
     std::vector<cudaEvent_t>* ev;   // pairs (start, stop) recorded so far
@@ -94,9 +98,11 @@ static void prof_collect(pcal_ctx* c) {
 
 static void free_tables(pcal_ctx* c) {
     cudaFree(c->d_lut); cudaFree(c->d_lut_off); cudaFree(c->d_lut_len);
-    cudaFree(c->d_partial); cudaFree(c->d_acc); cudaFree(c->d_gen_partial);
+    cudaFree(c->d_partial); cudaFree(c->d_gen_partial);
+    cudaFree(c->d_val);
     c->d_lut = nullptr; c->d_lut_off = c->d_lut_len = nullptr;
-    c->d_partial = c->d_acc = nullptr; c->d_gen_partial = nullptr;
+    c->d_partial = nullptr; c->d_gen_partial = nullptr;
+    c->d_val = nullptr;
 }
 
 extern "C" const char* pcal_strerror(int code) {
@@ -228,6 +234,17 @@ extern "C" int pcal_info(const pcal_ctx* c, pcal_info_t* info) {
     return PCAL_OK;
 }
 
+// fold_2bit_kernel instantiations: <SIGN_MAG, loads per block, CTAs per SM>.  The default was
+// chosen on the B200 (profiles/); PCAL_FOLD2_VARIANT=u4b3|u4b4|u8b2 overrides it for tuning runs.
+typedef void (*fold2_fn)(FoldParams);
+static fold2_fn pick_fold2(bool sm) {
+    const char* v = getenv("PCAL_FOLD2_VARIANT");
+    if (v && !strcmp(v, "u4b4")) return sm ? fold_2bit_kernel<true, 4, 4> : fold_2bit_kernel<false, 4, 4>;
+    if (v && !strcmp(v, "u8b2")) return sm ? fold_2bit_kernel<true, 8, 2> : fold_2bit_kernel<false, 8, 2>;
+    if (v && !strcmp(v, "u8b3")) return sm ? fold_2bit_kernel<true, 8, 3> : fold_2bit_kernel<false, 8, 3>;
+    return sm ? fold_2bit_kernel<true, 4, 3> : fold_2bit_kernel<false, 4, 3>;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Lazy set-up: decide LUT vs generator, derive the geometry, build the rotator tables.
 // ---------------------------------------------------------------------------------------------
@@ -275,7 +292,7 @@ static int prepare(pcal_ctx* c) {
     if (mode == PCAL_ROT_LUT) {
         int occ = 0;
         size_t elem = 0;
-        if (c->kind == KIND_2BIT) { occ = c->sign_mag ? occupancy_of(fold_2bit_kernel<true>, 0) : occupancy_of(fold_2bit_kernel<false>, 0); elem = 2; }
+        if (c->kind == KIND_2BIT) { c->fold2 = pick_fold2(c->sign_mag != 0); occ = occupancy_of(c->fold2, 0); elem = 2; }
         else if (c->kind == KIND_I8) { occ = occupancy_of(fold_i8_kernel, 0); elem = 4; }
         else { occ = occupancy_of(fold_f32_kernel, 0); elem = 8; }
         if (occ < 1) return PCAL_ERR_DEVICE;
@@ -284,7 +301,10 @@ static int prepare(pcal_ctx* c) {
         c->R = slots / q ? slots / q : 1;
         c->grid = c->q * c->R;
         CU(cudaMalloc(&c->d_partial, (size_t)c->grid * c->F * 32 * elem));
-        CU(cudaMalloc(&c->d_acc, (size_t)c->q * c->F * 32 * 8));
+        CU(cudaMalloc(&c->d_val, (size_t)c->q * c->F * 32 * sizeof(double)));
+        // rotate_fold_kernel: a warp per (channel, bin) pair, or the whole CTA when a pair has many elements
+        const uint64_t per_pair = (uint64_t)c->q * 32u * c->spv / c->n_bins;
+        c->rot_tpp = per_pair > 256 ? (uint32_t)kPostThreads : 32u;
         // rotator tables (eq. 2.4), one per channel, built in long double
         std::vector<double2> lut;
         std::vector<uint32_t> off(c->C), len(c->C);
@@ -313,6 +333,20 @@ static int prepare(pcal_ctx* c) {
     return PCAL_OK;
 }
 
+// Accumulators hold zeros after pcal_reset only lazily: the first post kernel of the next
+// pcal_extract overwrites them; any other reader zeroes them first.
+static int ensure_zeroed(pcal_ctx* c) {
+    if (!c->zero_pending) return PCAL_OK;
+    const uint32_t n = c->n_bins * (uint32_t)c->C;
+    zero_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, c->d_Pint, n);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->zero_pending = false;
+    return PCAL_OK;
+}
+
+static uint32_t log2_u32(uint32_t v) { uint32_t l = 0; while ((1u << l) < v) ++l; return l; }
+
 // one launch group of the LUT / zero-offset path over n time samples starting at data
 static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
     const uint64_t n_bytes = n * (uint64_t)c->bits * c->C / 8;
@@ -322,36 +356,39 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         fp.data = reinterpret_cast<const uint4*>(data); fp.n_vec = n_vec; fp.q = c->q; fp.R = c->R;
         const uint64_t NC = (n_vec + 31) / 32, NSR = (NC + c->q - 1) / c->q;
         uint64_t it = (NSR + (uint64_t)c->R * kWarps - 1) / ((uint64_t)c->R * kWarps);
-        it = (it + kUnroll - 1) / kUnroll * kUnroll;
+        it = (it + kFoldGroup - 1) / kFoldGroup * kFoldGroup;
         fp.n_iter = (uint32_t)it; fp.partial = c->d_partial;
-        const uint32_t total = c->q * c->F * 32;
+        const uint64_t grid_threads = (uint64_t)c->R * kWarps * c->q * 32u;
+        fp.n_quot = (uint32_t)(n_vec / grid_threads); fp.n_rem = n_vec % grid_threads;
         prof_mark(c, st);
-        if (c->kind == KIND_2BIT) {
-            if (c->sign_mag) fold_2bit_kernel<true><<<c->grid, kThreads, 0, st>>>(fp);
-            else fold_2bit_kernel<false><<<c->grid, kThreads, 0, st>>>(fp);
-            prof_mark(c, st);
-            reduce_replicas_kernel<uint16_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
-                (const uint16_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
-        } else if (c->kind == KIND_I8) {
-            fold_i8_kernel<<<c->grid, kThreads, 0, st>>>(fp);
-            prof_mark(c, st);
-            reduce_replicas_kernel<int32_t, long long><<<(total + 255) / 256, 256, 0, st>>>(
-                (const int32_t*)c->d_partial, (long long*)c->d_acc, c->q, c->R, c->F);
-        } else {
-            fold_f32_kernel<<<c->grid, kThreads, 0, st>>>(fp);
-            prof_mark(c, st);
-            reduce_replicas_kernel<double, double><<<(total + 255) / 256, 256, 0, st>>>(
-                (const double*)c->d_partial, (double*)c->d_acc, c->q, c->R, c->F);
-        }
-        c->launches += 2;
+        if (c->kind == KIND_2BIT) c->fold2<<<c->grid, kThreads, 0, st>>>(fp);
+        else if (c->kind == KIND_I8) fold_i8_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+        else fold_f32_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+        prof_mark(c, st);
+        c->launches += 1;
+    }
+    if (n_vec) {
+        ReplicaParams rr;
+        rr.partial = c->d_partial; rr.val = c->d_val; rr.q = c->q; rr.R = c->R; rr.F = c->F;
+        rr.cnt_quot = (uint32_t)(n_vec / ((uint64_t)c->q * 32u)); rr.cnt_rem = (uint32_t)(n_vec % ((uint64_t)c->q * 32u));
+        rr.kind = c->kind;
+        const uint32_t total = c->q * c->F * 32u;
+        rr.ns = c->R <= 8 ? 1u : (c->R <= 16 ? 2u : (c->R <= 32 ? 4u : 8u));
+        reduce_replicas_kernel<<<total / ((uint32_t)kPostThreads / rr.ns), kPostThreads, 0, st>>>(rr);
+        c->launches += 1;
     }
     RotateParams rp;
-    rp.acc = c->d_acc; rp.lut = c->d_lut; rp.lut_off = c->d_lut_off; rp.lut_len = c->d_lut_len;
+    rp.val = c->d_val; rp.lut = c->d_lut; rp.lut_off = c->d_lut_off; rp.lut_len = c->d_lut_len;
     rp.P = c->d_P; rp.Pint = c->d_Pint; rp.tail = data + n_vec * 16;
     rp.n0 = c->n_processed; rp.NT = n_vec * c->spv; rp.n_total = n;
-    rp.q = c->q; rp.F = c->F; rp.C = (uint32_t)c->C; rp.spv = c->spv; rp.n_bins = c->n_bins;
-    rp.kind = c->kind; rp.sign_mag = c->sign_mag; rp.integer_exact = c->kind != KIND_F32;
-    rotate_fold_kernel<<<dim3(c->n_bins, c->C), kPostThreads, 0, st>>>(rp);
+    rp.q = c->q; rp.F = c->F; rp.C = (uint32_t)c->C; rp.spv = c->spv; rp.spv_log2 = log2_u32(c->spv);
+    rp.n_bins = c->n_bins; rp.tpp = c->rot_tpp; rp.have_val = n_vec ? 1u : 0u;
+    rp.kind = c->kind; rp.sign_mag = c->sign_mag;
+    rp.integer_exact = (c->all_zero && c->kind != KIND_F32) ? 1 : 0;
+    rp.overwrite = c->zero_pending ? 1 : 0;
+    const uint32_t pairs = c->n_bins * (uint32_t)c->C, ppc = (uint32_t)kPostThreads / c->rot_tpp;
+    rotate_fold_kernel<<<(pairs + ppc - 1) / ppc, kPostThreads, 0, st>>>(rp);
+    c->zero_pending = false;
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
@@ -382,11 +419,13 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         prof_mark(c, st);
         c->launches += 1;
     }
-    GenReduceParams gr;
+    GenPostParams gr;
     gr.partial = c->d_gen_partial; gr.P = c->d_P; gr.tail = data + n_loads * load_bytes;
     gr.n0 = c->n_processed; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
     gr.grid = n_loads ? c->gen_grid : 0; gr.n_bins = c->n_bins; gr.kind = c->kind; gr.sign_mag = c->sign_mag;
-    gen_reduce_kernel<<<(c->n_bins + 127) / 128, 128, 0, st>>>(gr);
+    gr.overwrite = c->zero_pending ? 1 : 0;
+    post_gen_kernel<<<(c->n_bins + 31) / 32, kPostThreads, 0, st>>>(gr);
+    c->zero_pending = false;
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
@@ -442,19 +481,35 @@ extern "C" int pcal_extract_host(pcal_ctx* c, const void* host_samples, uint64_t
     return PCAL_OK;
 }
 
-static int enqueue_dft(pcal_ctx* c) {
+// The DFT kernel writes T both to d_T and, when `host_out` is device-visible pinned host memory
+// (cudaHostAlloc / cudaHostRegister under unified addressing), straight into it: no copy node.
+static int enqueue_dft(pcal_ctx* c, double* host_out, bool* wrote_host) {
+    const int rz = ensure_zeroed(c);
+    if (rz != PCAL_OK) return rz;
+    double2* mapped = nullptr;
+    if (host_out) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, host_out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+            mapped = reinterpret_cast<double2*>(at.devicePointer);
+        cudaGetLastError();
+    }
     const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
-    dft_kernel<<<dim3((c->n_bins + 127) / 128, c->C), 128, smem, c->stream>>>(c->d_P, c->d_W, c->d_T, c->n_bins, (uint32_t)c->k_shift);
+    const uint32_t per_cta = kDftThreads / 32;
+    dft_kernel<<<dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream>>>(
+        c->d_P, c->d_W, c->d_T, mapped, c->n_bins, (uint32_t)c->k_shift);
     c->launches += 1;
     CU(cudaGetLastError());
+    *wrote_host = mapped != nullptr;
     return PCAL_OK;
 }
 
 extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
-    const int r = enqueue_dft(c);
+    bool wrote = false;
+    const int r = enqueue_dft(c, out, &wrote);
     if (r != PCAL_OK) return r;
-    CU(cudaMemcpyAsync(out, c->d_T, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
+    if (!wrote)
+        CU(cudaMemcpyAsync(out, c->d_T, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
     return PCAL_OK;
 }
 
@@ -483,6 +538,7 @@ static void kshift_bins(const pcal_ctx* c, double* bins, int sign) {
 
 extern "C" int pcal_get_folded(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
+    { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const size_t bytes = (size_t)c->n_bins * c->C * sizeof(double2);
     CU(cudaMemcpyAsync(c->h_pinned, c->d_P, bytes, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -495,6 +551,7 @@ extern "C" int pcal_get_folded_i64(pcal_ctx* c, int64_t* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
     if (c->kind == KIND_F32 || c->k_shift) return PCAL_ERR_STATE;
     for (int i = 0; i < c->C; ++i) if (c->Foff[i]) return PCAL_ERR_STATE;
+    { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const size_t bytes = (size_t)c->n_bins * c->C * sizeof(long long);
     CU(cudaMemcpyAsync(c->h_pinned, c->d_Pint, bytes, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -504,6 +561,7 @@ extern "C" int pcal_get_folded_i64(pcal_ctx* c, int64_t* out) {
 
 extern "C" int pcal_add_folded(pcal_ctx* c, const double* bins) {
     if (!c || !bins) return PCAL_ERR_INVALID;
+    { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const uint32_t n = c->n_bins * (uint32_t)c->C;
     CU(cudaStreamSynchronize(c->stream));
     memcpy(c->h_pinned, bins, (size_t)n * sizeof(double2));
@@ -518,10 +576,7 @@ extern "C" int pcal_add_folded(pcal_ctx* c, const double* bins) {
 
 extern "C" int pcal_reset(pcal_ctx* c) {
     if (!c) return PCAL_ERR_INVALID;
-    const uint32_t n = c->n_bins * (uint32_t)c->C;
-    zero_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, c->d_Pint, n);
-    c->launches += 1;
-    CU(cudaGetLastError());
+    c->zero_pending = true;   // the next post kernel overwrites; other readers zero first
     c->n_processed = 0;
     c->started = false;
     return PCAL_OK;
@@ -529,12 +584,14 @@ extern "C" int pcal_reset(pcal_ctx* c) {
 
 extern "C" int pcal_get_folded_dev(pcal_ctx* c, double* dev_bins) {
     if (!c || !dev_bins) return PCAL_ERR_INVALID;
+    { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     CU(cudaMemcpyAsync(dev_bins, c->d_P, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
     return PCAL_OK;
 }
 
 extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
     if (!c || !dev_bins) return PCAL_ERR_INVALID;
+    { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const uint32_t n = c->n_bins * (uint32_t)c->C;
     add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_bins), n);
     c->launches += 1;

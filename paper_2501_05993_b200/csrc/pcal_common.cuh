@@ -10,6 +10,7 @@ namespace pcal {
 // consecutive vectors = 512 contiguous bytes (4 full 128-byte lines).
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
+constexpr int kMaxChannels = 16;      // == PCAL_MAX_CHANNELS of include/pcal.h
 constexpr int kUnroll = 8;            // independent 128-bit loads in flight per thread
 
 // sample kinds handled by the kernels

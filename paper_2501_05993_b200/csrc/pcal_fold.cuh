@@ -28,7 +28,9 @@ struct FoldParams {
     uint64_t n_vec;         // complete 16-byte vectors in this launch
     uint32_t q;             // slot groups
     uint32_t R;             // replicas per slot group (gridDim.x == q*R)
-    uint32_t n_iter;        // loop trips per warp (multiple of kUnroll)
+    uint32_t n_iter;        // loop trips per warp (multiple of 16)
+    uint32_t n_quot;        // n_vec / (threads in the grid): loads every thread makes ...
+    uint64_t n_rem;         // ... plus one for the threads whose first vector index is < n_vec % threads
     void* partial;          // [device] per-CTA partial sums, layout [cta][field][lane]
 };
 
@@ -40,118 +42,132 @@ __device__ __forceinline__ uint64_t fold_first_vec(const FoldParams& P, int w, i
 // ---------------------------------------------------------------------------------------------
 // 2-bit samples: 64 fields per vector.  Per-field sums of the (offset-binary) codes.
 //
-// Eight loads of one thread are compressed with a carry-save adder tree (7 CSAs = 14 LOP3 per
-// word position) into running planes of weight 1, 2, 4 plus one word of weight 8 per group; only
-// that word (one per 8 loads) goes through SWAR widening 2 -> 4 -> 8 -> 16 bits.  About 0.17
-// integer instructions per sample, all exact.
+// The loads of one thread feed a streaming vertical counter (Harley-Seal): csa(plane, x0, x1)
+// keeps the running plane of weight w and emits one carry word of weight 2w; 15 CSAs (30 LOP3)
+// per word position turn 16 loads into the running planes O, T, F, E (weights 1, 2, 4, 8) and
+// ONE word of weight 16, which alone is widened by SWAR (2-bit -> 4-bit lanes in registers,
+// -> 16-bit lanes in shared memory every 5 groups).  About 0.15 integer instructions per
+// sample, all exact.  Loads are software-pipelined: the next block of U 128-bit loads is issued
+// before the current block is reduced, so every warp always has U..2U loads in flight.
 // Output: uint16 partial[cta][64 fields][32 lanes], field f = bit pair 2f..2f+1 of the vector.
-// Host guarantees n_iter <= 2048 so that 8 warps * 3 * n_iter < 65536.
+// Host guarantees n_iter <= 2048 (8 warps * 3 * n_iter < 65536) and n_iter % 16 == 0.
 // ---------------------------------------------------------------------------------------------
-template <bool SIGN_MAG>
-__global__ void __launch_bounds__(kThreads, 2) fold_2bit_kernel(FoldParams P) {
-    __shared__ uint32_t sh[kWarps][32][32];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    uint64_t idx = fold_first_vec(P, w, lane);
+constexpr int kFoldGroup = 16;   // loads per complete counter cascade
+
+template <bool SIGN_MAG, int U, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P) {
+    static_assert(U == 4 || U == 8, "block of 4 or 8 loads");
+    __shared__ uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const uint64_t first = fold_first_vec(P, w, lane);
     const uint64_t stride = (uint64_t)P.R * kWarps * P.q * 32u;
+    const uint32_t n_valid = P.n_quot + (first < P.n_rem ? 1u : 0u);   // this thread's real loads
+    const uint4* base = P.data + first;
     // a vector that does not exist must add 0 to every code sum: raw pattern whose code is 0
     const uint32_t fill = SIGN_MAG ? 0xFFFFFFFFu : 0u;
 
-    uint32_t ones[4] = {0, 0, 0, 0}, twos[4] = {0, 0, 0, 0}, fours[4] = {0, 0, 0, 0};
-    uint32_t nib[8], byt[16], hlf[32];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) nib[k] = 0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) byt[k] = 0;
-#pragma unroll
-    for (int k = 0; k < 32; ++k) hlf[k] = 0;
+    for (int h = 0; h < 32; ++h) hlf[h][tid] = 0;
+    uint32_t O[4] = {0, 0, 0, 0}, T[4] = {0, 0, 0, 0}, F[4] = {0, 0, 0, 0}, E[4] = {0, 0, 0, 0};
+    uint32_t nib[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // weight 16, 4-bit lanes: [2j+par] nibble i = field 2i+par
+    uint32_t d[4], e[4];                             // pending carries of weight 4 and 8
 
-    uint32_t i = 0;
-    while (i < P.n_iter) {
-        for (int mid = 0; mid < 16 && i < P.n_iter; ++mid) {
-            for (int inner = 0; inner < 5 && i < P.n_iter; ++inner, i += kUnroll) {
-                uint4 v[kUnroll];
+    auto load_block = [&](uint4(&v)[U], uint32_t i0) {
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) {
-                    const uint64_t a = idx + (uint64_t)u * stride;
-                    v[u] = (a < P.n_vec) ? ldg_stream(P.data + a) : make_uint4(fill, fill, fill, fill);
-                }
-                idx += (uint64_t)kUnroll * stride;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    uint32_t x[kUnroll];
-#pragma unroll
-                    for (int u = 0; u < kUnroll; ++u) {
-                        x[u] = word_of(v[u], j);
-                        if (SIGN_MAG) x[u] = signmag_to_offset_binary(x[u]);
-                    }
-                    uint32_t s1, c1, s2, c2, s3, c3, s4, c4, t1, d1, t2, d2, f1, e1;
-                    csa(x[0], x[1], x[2], s1, c1);
-                    csa(x[3], x[4], x[5], s2, c2);
-                    csa(s1, s2, x[6], s3, c3);
-                    csa(s3, x[7], ones[j], s4, c4);
-                    ones[j] = s4;
-                    csa(c1, c2, c3, t1, d1);
-                    csa(t1, c4, twos[j], t2, d2);
-                    twos[j] = t2;
-                    csa(d1, d2, fours[j], f1, e1);
-                    fours[j] = f1;
-                    // e1: fields of weight 8, values 0..3 -> 4-bit lanes (<= 5 additions)
-                    nib[2 * j] += e1 & 0x33333333u;
-                    nib[2 * j + 1] += (e1 >> 2) & 0x33333333u;
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {  // 4-bit -> 8-bit lanes (<= 16*15 = 240)
-                byt[2 * k] += nib[k] & 0x0F0F0F0Fu;
-                byt[2 * k + 1] += (nib[k] >> 4) & 0x0F0F0F0Fu;
-                nib[k] = 0;
-            }
+        for (int u = 0; u < U; ++u) {
+            const uint32_t i = i0 + u;
+            v[u] = (i < n_valid) ? ldg_stream(base + (uint64_t)i * stride) : make_uint4(fill, fill, fill, fill);
         }
+    };
+    // four loads -> planes O, T updated, one carry word of weight 4 per word position
+    auto quad = [&](const uint4& v0, const uint4& v1, const uint4& v2, const uint4& v3, uint32_t(&out4)[4]) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {  // 8-bit -> 16-bit lanes
-            hlf[2 * k] += byt[k] & 0x00FF00FFu;
-            hlf[2 * k + 1] += (byt[k] >> 8) & 0x00FF00FFu;
-            byt[k] = 0;
+        for (int j = 0; j < 4; ++j) {
+            uint32_t x0 = word_of(v0, j), x1 = word_of(v1, j), x2 = word_of(v2, j), x3 = word_of(v3, j);
+            if (SIGN_MAG) {
+                x0 = signmag_to_offset_binary(x0); x1 = signmag_to_offset_binary(x1);
+                x2 = signmag_to_offset_binary(x2); x3 = signmag_to_offset_binary(x3);
+            }
+            uint32_t ca, cb;
+            csa(O[j], x0, x1, O[j], ca);
+            csa(O[j], x2, x3, O[j], cb);
+            csa(T[j], ca, cb, T[j], out4[j]);
         }
+    };
+    auto fold8 = [&](const uint32_t(&d0)[4], const uint32_t(&d1)[4], uint32_t(&out8)[4]) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) csa(F[j], d0[j], d1[j], F[j], out8[j]);
+    };
+    auto fold16 = [&](const uint32_t(&e0)[4], const uint32_t(&e1)[4]) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            uint32_t g;
+            csa(E[j], e0[j], e1[j], E[j], g);
+            nib[2 * j] += g & 0x33333333u;
+            nib[2 * j + 1] += (g >> 2) & 0x33333333u;
+        }
+    };
+    auto flush_nib = [&]() {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int j = r >> 1, par = r & 1;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) hlf[8 * j + 2 * k + par][tid] += (nib[r] >> (4 * k)) & 0x000F000Fu;
+            nib[r] = 0;
+        }
+    };
+    // one block of U loads; `phase` = index of the block inside its group of 16 loads
+    auto reduce_block = [&](const uint4(&v)[U], int phase) {
+        uint32_t d1[4], e1[4];
+        if (U == 4) {
+            if (phase == 0) quad(v[0], v[1], v[2], v[3], d);
+            else if (phase == 1) { quad(v[0], v[1], v[2], v[3], d1); fold8(d, d1, e); }
+            else if (phase == 2) quad(v[0], v[1], v[2], v[3], d);
+            else { quad(v[0], v[1], v[2], v[3], d1); fold8(d, d1, e1); fold16(e, e1); }
+        } else {
+            quad(v[0], v[1], v[2], v[3], d);
+            quad(v[4 % U], v[5 % U], v[6 % U], v[7 % U], d1);
+            if (phase == 0) fold8(d, d1, e);
+            else { fold8(d, d1, e1); fold16(e, e1); }
+        }
+    };
+
+    uint4 bufA[U], bufB[U];
+    load_block(bufA, 0);
+    uint32_t groups_since_flush = 0;
+    for (uint32_t i = 0; i < P.n_iter; i += kFoldGroup) {
+#pragma unroll
+        for (int b = 0; b < kFoldGroup / U; b += 2) {
+            load_block(bufB, i + (b + 1) * U);
+            reduce_block(bufA, b);
+            load_block(bufA, i + (b + 2) * U);
+            reduce_block(bufB, b + 1);
+        }
+        if (++groups_since_flush == 5) { flush_nib(); groups_since_flush = 0; }   // 4-bit lanes hold <= 15
     }
+    flush_nib();
 
-    // total = 8*hlf + 4*val(fours) + 2*val(twos) + val(ones), all in the 16-bit lane layout:
-    // register h = ((2j + par)*2 + hi4)*2 + hi8 holds fields 16j + a + 4*hi8 (+8 in the upper
-    // half-word), a = par + 2*hi4.
+    // total = 16*hlf + val(O) + 2 val(T) + 4 val(F) + 8 val(E), assembled in 16-bit lanes
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
 #pragma unroll
-        for (int par = 0; par < 2; ++par) {
-            const uint32_t m3 = 0x33333333u;
-            const uint32_t n1 = (par ? (ones[j] >> 2) : ones[j]) & m3;
-            const uint32_t n2 = (par ? (twos[j] >> 2) : twos[j]) & m3;
-            const uint32_t n4 = (par ? (fours[j] >> 2) : fours[j]) & m3;
-#pragma unroll
-            for (int hi4 = 0; hi4 < 2; ++hi4) {
-                const uint32_t b1 = (hi4 ? (n1 >> 4) : n1) & 0x0F0F0F0Fu;
-                const uint32_t b2 = (hi4 ? (n2 >> 4) : n2) & 0x0F0F0F0Fu;
-                const uint32_t b4 = (hi4 ? (n4 >> 4) : n4) & 0x0F0F0F0Fu;
-                const uint32_t bs = b1 + 2u * b2 + 4u * b4;  // <= 21 per byte
-#pragma unroll
-                for (int hi8 = 0; hi8 < 2; ++hi8) {
-                    const int h = ((2 * j + par) * 2 + hi4) * 2 + hi8;
-                    hlf[h] = 8u * hlf[h] + ((hi8 ? (bs >> 8) : bs) & 0x00FF00FFu);
-                }
-            }
+        for (int a = 0; a < 4; ++a) {
+            const uint32_t m = 0x03030303u;   // byte i = field 4i + a
+            const uint32_t v = ((O[j] >> (2 * a)) & m) + 2u * ((T[j] >> (2 * a)) & m) +
+                               4u * ((F[j] >> (2 * a)) & m) + 8u * ((E[j] >> (2 * a)) & m);   // <= 45 per byte
+            hlf[8 * j + a][tid] = 16u * hlf[8 * j + a][tid] + (v & 0x00FF00FFu);
+            hlf[8 * j + a + 4][tid] = 16u * hlf[8 * j + a + 4][tid] + ((v >> 8) & 0x00FF00FFu);
         }
     }
-#pragma unroll
-    for (int h = 0; h < 32; ++h) sh[w][h][lane] = hlf[h];
     __syncthreads();
     uint16_t* out = reinterpret_cast<uint16_t*>(P.partial) + (size_t)blockIdx.x * 64 * 32;
 #pragma unroll
-    for (int e = threadIdx.x; e < 32 * 32; e += kThreads) {
-        const int h = e >> 5, ln = e & 31;
+    for (int x = tid; x < 32 * 32; x += kThreads) {
+        const int h = x >> 5, ln = x & 31;
         uint32_t s = 0;
 #pragma unroll
-        for (int ww = 0; ww < kWarps; ++ww) s += sh[ww][h][ln];  // 16-bit lanes, < 65536 by host cap
-        const int hi8 = h & 1, hi4 = (h >> 1) & 1, par = (h >> 2) & 1, j = h >> 3;
-        const int f = 16 * j + par + 2 * hi4 + 4 * hi8;
+        for (int ww = 0; ww < kWarps; ++ww) s += hlf[h][ww * 32 + ln];  // 16-bit lanes, < 65536 by host cap
+        const int f = 16 * (h >> 3) + (h & 7);
         out[f * 32 + ln] = (uint16_t)(s & 0xFFFFu);
         out[(f + 8) * 32 + ln] = (uint16_t)(s >> 16);
     }

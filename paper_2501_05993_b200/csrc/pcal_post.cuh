@@ -1,160 +1,291 @@
 // pcal_post.cuh -- the small deterministic kernels behind the hot loop:
-//   reduce_replicas_kernel   per-CTA partials -> one accumulator per (slot group, field, lane)
-//                            (the "binary tree stepping" the paper leaves to the host)
-//   rotate_fold_kernel       A[r] * exp(-j w_off r) folded to N_bins (eq. 2.3 + 2.2 after the
-//                            reordering of PAPER.md:200), plus the ragged tail (< 1 vector)
-//   gen_reduce_kernel        per-CTA generator partials -> bins
-//   dft_kernel               T[i] = sum_b P[b] exp(-j 2 pi i b / N_bins)
-// All sums run in a fixed order (no atomics): two runs give bit-identical results.
+//   reduce_replicas_kernel  per-CTA partials of the fold kernels -> one sum per (slot, field, lane)
+//                       (the "binary tree stepping" the paper leaves to the host)
+//   rotate_fold_kernel  A[r] * exp(-j w_off r) folded to N_bins (eq. 2.3 + 2.2 after the reordering
+//                       of PAPER.md:200), ragged tail (< 1 vector), accumulate into the context
+//   post_gen_kernel     per-CTA generator partials -> bins, ragged tail, accumulate
+//   dft_kernel          T[i] = sum_b P[b] exp(-j 2 pi i b / N_bins)
+// All sums run in a fixed order (no floating-point atomics): two runs give bit-identical results.
 #pragma once
 #include "pcal_common.cuh"
 
 namespace pcal {
 
-constexpr int kPostThreads = 128;
+constexpr int kPostThreads = 256;
 
-// ---- stage 1: sum the R replicas of each slot group -------------------------------------------
-// in : T partial[(rho0*q + p)][F][32]      out: int64/double acc[p][F][32]
-template <typename Tin, typename Tacc>
-__global__ void reduce_replicas_kernel(const Tin* __restrict__ partial, Tacc* __restrict__ acc,
-                                       uint32_t q, uint32_t R, uint32_t F) {
-    const uint32_t per_group = F * 32u;
-    const uint32_t total = q * per_group;
-    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x >= total) return;
-    Tacc s = 0;
-    for (uint32_t r = 0; r < R; ++r) s += (Tacc)partial[(size_t)r * total + x];  // fixed order
-    acc[x] = s;
-}
-
-struct RotateParams {
-    const void* acc;          // [device] int64 or double acc[q][F][32]
-    const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
-    const uint32_t* lut_off;  // [device] per channel: first entry
-    const uint32_t* lut_len;  // [device] per channel: L_c (1 => no rotation)
-    double2* P;               // [device] folded bins [C][N_bins], accumulated into
-    long long* Pint;          // [device] exact integer bins [C][N_bins] (valid when no rotation)
-    const uint8_t* tail;      // [device] first byte after the last complete vector
-    uint64_t n0;              // absolute index of the first sample of this call
-    uint64_t NT;              // time samples covered by complete vectors
-    uint64_t n_total;         // time samples in this call
-    uint32_t q, F, C;         // slot groups, fields per vector, channels
-    uint32_t spv;             // time samples per vector
-    uint32_t n_bins;
-    int kind;                 // KIND_*
-    int sign_mag;
-    int integer_exact;        // also accumulate Pint
+// ---- stage 1: sum the R replicas of every slot group -------------------------------------------
+// in : elem partial[(rho*q + p)][F][32]          out: double val[p][F][32]
+// For 2-bit data the partials are code sums; val = 2*sum - 3*(vectors folded into this slot) is the
+// level sum.  Integer sums are exact in a double (|val| < 2^53).  One thread per element; the
+// replica loads are issued eight at a time and added in replica order (deterministic for fp64).
+struct ReplicaParams {
+    const void* partial;
+    double* val;
+    uint32_t q, R, F, ns;        // ns: replica slices per element (1, 2, 4 or 8)
+    uint32_t cnt_quot, cnt_rem;   // vectors per slot: cnt_quot + (p*32 + lane < cnt_rem)
+    int kind;
 };
 
-// decode one tail sample (time index t relative to the first tail byte's first sample)
-__device__ __forceinline__ double tail_value(const RotateParams& P, uint32_t t, uint32_t c) {
-    if (P.kind == KIND_F32) return (double)reinterpret_cast<const float*>(P.tail)[t];
-    if (P.kind == KIND_I8) return (double)reinterpret_cast<const int8_t*>(P.tail)[t];
-    const uint32_t bit = (t * P.C + c) * 2u;
-    const uint32_t code = (P.tail[bit >> 3] >> (bit & 7u)) & 3u;
-    if (P.sign_mag) return (code & 2u) ? -(double)(1 + 2 * (code & 1u)) : (double)(1 + 2 * (code & 1u));
+// replicas r = first, first + step, ... < R, eight loads in flight, added in replica order
+template <typename Tin, typename Tacc>
+__device__ __forceinline__ Tacc replica_sum(const Tin* src, size_t stride, uint32_t first, uint32_t step, uint32_t R) {
+    Tacc a = 0;
+    for (uint32_t r0 = first; r0 < R; r0 += 8 * step) {
+        Tin t[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) t[k] = (r0 + k * step < R) ? __ldcg(src + (size_t)(r0 + k * step) * stride) : (Tin)0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a += (Tacc)t[k];
+    }
+    return a;
+}
+
+// A CTA serves 256/ns consecutive elements with ns replica slices (ns = 1, 2, 4 or 8, chosen by
+// the host so that a slice has at most ~8 replicas): thread = (slice, element), consecutive
+// threads read consecutive elements (coalesced); the slice sums are then added in slice order.
+__global__ void __launch_bounds__(kPostThreads) reduce_replicas_kernel(ReplicaParams P) {
+    __shared__ double sd[kPostThreads];
+    __shared__ long long si[kPostThreads];
+    const uint32_t E = P.F * 32u, total = P.q * E;          // total is a multiple of 256
+    const uint32_t epc = kPostThreads / P.ns;                // elements per CTA
+    const uint32_t sl = threadIdx.x / epc, e = threadIdx.x % epc;
+    const uint32_t i = blockIdx.x * epc + e;
+    if (P.kind == KIND_F32) sd[threadIdx.x] = replica_sum<double, double>(reinterpret_cast<const double*>(P.partial) + i, total, sl, P.ns, P.R);
+    else if (P.kind == KIND_I8) si[threadIdx.x] = replica_sum<int32_t, long long>(reinterpret_cast<const int32_t*>(P.partial) + i, total, sl, P.ns, P.R);
+    else si[threadIdx.x] = replica_sum<uint16_t, long long>(reinterpret_cast<const uint16_t*>(P.partial) + i, total, sl, P.ns, P.R);
+    __syncthreads();
+    if (sl != 0) return;
+    double v;
+    if (P.kind == KIND_F32) {
+        v = 0.0;
+        for (uint32_t k = 0; k < P.ns; ++k) v += sd[k * epc + e];
+    } else {
+        long long a = 0;
+        for (uint32_t k = 0; k < P.ns; ++k) a += si[k * epc + e];
+        if (P.kind == KIND_2BIT) {
+            const uint32_t vslot = (i / E) * 32u + (i & 31u);
+            a = 2 * a - 3ll * (long long)(P.cnt_quot + (vslot < P.cnt_rem ? 1u : 0u));
+        }
+        v = (double)a;
+    }
+    P.val[i] = v;
+}
+
+// ---- stage 2: rotate and fold to N_bins --------------------------------------------------------
+struct RotateParams {
+    const double* val;        // [device] val[q][F][32] from stage 1
+    const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
+    const uint32_t* lut_off;  // [device] per channel: first entry
+    const uint32_t* lut_len;  // [device] per channel: N_rotator,c (1 => no rotation)
+    double2* P;               // [device] folded bins [C][N_bins]
+    long long* Pint;          // [device] exact integer bins [C][N_bins]
+    const uint8_t* tail;      // [device] first byte after the last complete vector
+    uint64_t n0;              // absolute index of the first sample of this piece
+    uint64_t NT;              // time samples covered by complete vectors
+    uint64_t n_total;         // time samples in this piece
+    uint32_t q, F, C;         // slot groups, fields per vector, channels
+    uint32_t spv, spv_log2;   // time samples per vector (power of two)
+    uint32_t n_bins;
+    uint32_t tpp;             // threads per (channel, bin) pair: 32 (a warp) or 256 (the CTA)
+    uint32_t have_val;        // 0 when the piece has no complete vector
+    int kind;                 // KIND_*
+    int sign_mag;
+    int integer_exact;        // every channel unrotated and integer input: keep Pint
+    int overwrite;            // first piece after reset: P = new instead of P += new
+};
+
+__device__ __forceinline__ double decode_tail(int kind, int sign_mag, const uint8_t* tail, uint32_t t, uint32_t c, uint32_t C) {
+    if (kind == KIND_F32) return (double)reinterpret_cast<const float*>(tail)[t];
+    if (kind == KIND_I8) return (double)reinterpret_cast<const int8_t*>(tail)[t];
+    const uint32_t bit = (t * C + c) * 2u;
+    const uint32_t code = (tail[bit >> 3] >> (bit & 7u)) & 3u;
+    if (sign_mag) return (code & 2u) ? -(double)(1 + 2 * (code & 1u)) : (double)(1 + 2 * (code & 1u));
     return (double)(2 * (int)code - 3);
 }
 
-// ---- stage 2: one block per (channel, bin) ---------------------------------------------------
-// The super-row (q*32 vectors = SR time samples, a multiple of M and of N_bins) is the index space
-// of acc: offset o in [0, SR) <-> (p, lane, time-in-vector).  Bin b collects the offsets
-// o = o_b + j*N_bins.  For 2-bit data acc holds code sums; level sum = 2*acc - 3*count(o).
+// The super-row (q*32 vectors = SR time samples, a multiple of the fold period and of N_bins) is
+// the index space of val: offset o in [0, SR) <-> slot group o / (32 spv), lane, time-in-vector.
+// Bin b of channel c collects the offsets o = o_b + j*N_bins.  A pair is served by `tpp` threads:
+// thread u adds its elements j = u, u + tpp, ... in order (four look-ups in flight), then the
+// lane sums are combined by a fixed butterfly (and, for tpp = 256, the 8 warp sums in warp order).
 __global__ void __launch_bounds__(kPostThreads) rotate_fold_kernel(RotateParams P) {
-    __shared__ double sre[kPostThreads], sim[kPostThreads];
-    __shared__ long long sint[kPostThreads];
-    const uint32_t c = blockIdx.y, b = blockIdx.x;
-    const uint64_t SR = (uint64_t)P.q * 32u * P.spv;
+    __shared__ double sre[kPostThreads / 32], sim[kPostThreads / 32];
+    __shared__ long long sint[kPostThreads / 32];
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
+    const uint32_t pairs = P.C * P.n_bins;
+    const uint32_t ppc = kPostThreads / P.tpp;                  // pairs per CTA: 8 or 1
+    const uint32_t pp = blockIdx.x * ppc + (P.tpp == 32 ? w : 0);
+    const bool active = pp < pairs;                              // uniform per warp
+    const uint32_t u = P.tpp == 32 ? lane : tid;
+    const uint32_t c = active ? pp / P.n_bins : 0, b = active ? pp % P.n_bins : 0;
     const uint32_t L = P.lut_len[c];
     const double2* lut = P.lut + P.lut_off[c];
-    const uint32_t o_b = (uint32_t)(((uint64_t)b + P.n_bins - (P.n0 % P.n_bins)) % P.n_bins);
-    const uint32_t n0L = (uint32_t)(P.n0 % L);
+    const uint32_t SR = P.q * 32u * P.spv;
     double are = 0.0, aim = 0.0;
-    long long aint = 0;
-    for (uint64_t o = o_b + (uint64_t)threadIdx.x * P.n_bins; o < SR; o += (uint64_t)kPostThreads * P.n_bins) {
-        if (o >= P.NT) break;
-        const uint32_t vec = (uint32_t)(o / P.spv), tf = (uint32_t)(o % P.spv);
-        const uint32_t p = vec >> 5, lane = vec & 31u;
-        const uint32_t f = tf * P.C + c;
-        const size_t x = ((size_t)p * P.F + f) * 32u + lane;
-        double val;
-        long long ival = 0;
-        if (P.kind == KIND_F32) {
-            val = reinterpret_cast<const double*>(P.acc)[x];
-        } else {
-            ival = reinterpret_cast<const long long*>(P.acc)[x];
-            if (P.kind == KIND_2BIT) {
-                const long long cnt = (long long)((P.NT - o - 1) / SR + 1);
-                ival = 2 * ival - 3 * cnt;
-            }
-            val = (double)ival;
-        }
+    long long ai = 0;
+    if (active && P.have_val) {
+        const uint32_t E = P.F * 32u, span_log2 = 5u + P.spv_log2;
+        const uint32_t o_b = (uint32_t)(((uint64_t)b + P.n_bins - (P.n0 % P.n_bins)) % P.n_bins);
+        uint32_t o = o_b + u * P.n_bins;
+        const uint32_t ostep = P.tpp * P.n_bins;
+        auto at = [&](uint32_t oo) -> uint32_t {   // element index of super-row offset oo, channel c
+            const uint32_t p = oo >> span_log2, d = oo & ((1u << span_log2) - 1u);
+            return p * E + (((d & (P.spv - 1u)) * P.C + c) << 5) + (d >> P.spv_log2);
+        };
         if (L > 1) {
-            const double2 ph = lut[(n0L + (uint32_t)(o % L)) % L];
-            are += val * ph.x;
-            aim += val * ph.y;
+            uint32_t k = (uint32_t)((P.n0 % L + o) % L);
+            const uint32_t kstep = ostep % L;
+            for (; o < SR; o += 4u * ostep) {
+                double2 ph[4];
+                double v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t oo = o + j * ostep;
+                    const bool ok = oo < SR;
+                    ph[j] = ok ? __ldg(lut + k) : make_double2(0.0, 0.0);
+                    v[j] = ok ? __ldcg(P.val + at(oo)) : 0.0;
+                    k += kstep; if (k >= L) k -= L;
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { are += v[j] * ph[j].x; aim += v[j] * ph[j].y; }
+            }
         } else {
-            are += val;
-            aint += ival;
-        }
-    }
-    sre[threadIdx.x] = are; sim[threadIdx.x] = aim; sint[threadIdx.x] = aint;
-    __syncthreads();
-    for (int s = kPostThreads / 2; s > 0; s >>= 1) {  // fixed tree
-        if (threadIdx.x < s) {
-            sre[threadIdx.x] += sre[threadIdx.x + s];
-            sim[threadIdx.x] += sim[threadIdx.x + s];
-            sint[threadIdx.x] += sint[threadIdx.x + s];
-        }
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) {
-        double tre = sre[0], tim = sim[0];
-        long long tint = sint[0];
-        // ragged tail: samples NT .. n_total-1 (fewer than one vector)
-        for (uint64_t t = P.NT; t < P.n_total; ++t) {
-            if ((P.n0 + t) % P.n_bins != b) continue;
-            const double v = tail_value(P, (uint32_t)(t - P.NT), c);
-            if (L > 1) {
-                const double2 ph = lut[(n0L + (uint32_t)(t % L)) % L];
-                tre += v * ph.x; tim += v * ph.y;
-            } else {
-                tre += v; tint += (long long)v;
+            for (; o < SR; o += 4u * ostep) {
+                double v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { const uint32_t oo = o + j * ostep; v[j] = (oo < SR) ? __ldcg(P.val + at(oo)) : 0.0; }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { are += v[j]; ai += (long long)v[j]; }
             }
         }
-        double2 cur = P.P[(size_t)c * P.n_bins + b];
-        cur.x += tre; cur.y += tim;
-        P.P[(size_t)c * P.n_bins + b] = cur;
-        if (P.integer_exact) P.Pint[(size_t)c * P.n_bins + b] += tint;
     }
+#pragma unroll
+    for (uint32_t s = 16; s > 0; s >>= 1) {
+        are += __shfl_xor_sync(0xFFFFFFFFu, are, s);
+        aim += __shfl_xor_sync(0xFFFFFFFFu, aim, s);
+        ai += __shfl_xor_sync(0xFFFFFFFFu, ai, s);
+    }
+    if (P.tpp != 32) {
+        if (lane == 0) { sre[w] = are; sim[w] = aim; sint[w] = ai; }
+        __syncthreads();
+        are = 0.0; aim = 0.0; ai = 0;
+#pragma unroll
+        for (int ww = 0; ww < kPostThreads / 32; ++ww) { are += sre[ww]; aim += sim[ww]; ai += sint[ww]; }
+        if (tid != 0) return;
+    } else if (lane != 0) {
+        return;
+    }
+    if (!active) return;
+    const uint32_t n_tail = (uint32_t)(P.n_total - P.NT);
+    if (n_tail) {   // ragged tail: samples NT .. n_total-1 (fewer than one vector)
+        uint32_t bb = (uint32_t)((P.n0 + P.NT) % P.n_bins);
+        uint32_t k = L > 1 ? (uint32_t)((P.n0 + P.NT) % L) : 0;
+        for (uint32_t t = 0; t < n_tail; ++t) {
+            if (bb == b) {
+                const double v = decode_tail(P.kind, P.sign_mag, P.tail, t, c, P.C);
+                if (L > 1) { const double2 ph = lut[k]; are += v * ph.x; aim += v * ph.y; }
+                else { are += v; ai += (long long)v; }
+            }
+            if (++bb == P.n_bins) bb = 0;
+            if (L > 1 && ++k == L) k = 0;
+        }
+    }
+    if (!P.overwrite) {
+        const double2 cur = P.P[pp];
+        are += cur.x; aim += cur.y;
+        if (P.integer_exact) ai += P.Pint[pp];
+    }
+    P.P[pp] = make_double2(are, aim);
+    if (P.integer_exact) P.Pint[pp] = ai;
+}
+
+// ---- generator path: per-CTA partial bins -> context bins ------------------------------------
+struct GenPostParams {
+    const double2* partial;  // [device] [grid][n_bins], bin index relative to the piece start
+    double2* P;              // [device] [n_bins] accumulated into (or overwritten)
+    const uint8_t* tail;     // [device] first byte after the last complete load
+    uint64_t n0, n_done, n_total, Fs, Foff;
+    uint32_t grid, n_bins;
+    int kind, sign_mag, overwrite;
+};
+
+// One CTA per 32 consecutive bins: warp w sums the CTAs w, w+8, ... (coalesced 512-byte rows),
+// the 8 warp sums are added in warp order, then the ragged tail with exactly reduced phases.
+__global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G) {
+    __shared__ double sre[kPostThreads / 32][32], sim[kPostThreads / 32][32];
+    const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    const uint32_t b = blockIdx.x * 32u + lane;
+    const bool ok = b < G.n_bins;
+    const uint32_t shift = (uint32_t)(G.n0 % G.n_bins);
+    const uint32_t s = ok ? (b + G.n_bins - shift) % G.n_bins : 0;
+    double re = 0.0, im = 0.0;
+    if (ok)
+        for (uint32_t c = w; c < G.grid; c += kPostThreads / 32) {
+            const double2 v = G.partial[(size_t)c * G.n_bins + s];
+            re += v.x; im += v.y;
+        }
+    sre[w][lane] = re; sim[w][lane] = im;
+    __syncthreads();
+    if (w != 0 || !ok) return;
+    re = 0.0; im = 0.0;
+#pragma unroll
+    for (int ww = 0; ww < kPostThreads / 32; ++ww) { re += sre[ww][lane]; im += sim[ww][lane]; }
+    const uint32_t n_tail = (uint32_t)(G.n_total - G.n_done);
+    if (n_tail) {
+        uint32_t bb = (uint32_t)((G.n0 + G.n_done) % G.n_bins);
+        for (uint32_t t = 0; t < n_tail; ++t) {
+            if (bb == b) {
+                const double v = decode_tail(G.kind, G.sign_mag, G.tail, t, 0, 1);
+                const double2 ph = phasor_neg(mulmod_u64(G.Foff, G.n0 + G.n_done + t, G.Fs), G.Fs);
+                re += v * ph.x; im += v * ph.y;
+            }
+            if (++bb == G.n_bins) bb = 0;
+        }
+    }
+    if (!G.overwrite) { const double2 cur = G.P[b]; re += cur.x; im += cur.y; }
+    G.P[b] = make_double2(re, im);
 }
 
 // ---- DFT of the folded period ------------------------------------------------------------------
 // T[c][i] = sum_b P[c][b] * W[(i'*b) mod N], i' = (i - k_shift) mod N, W[k] = exp(-j 2 pi k/N)
-// (twiddle table built on the host in long double).  One thread per output, fixed order in b.
-__global__ void dft_kernel(const double2* __restrict__ P, const double2* __restrict__ W,
-                           double2* __restrict__ T, uint32_t N, uint32_t k_shift) {
-    extern __shared__ double2 sm[];  // [N] bins of this channel, [N] twiddles
-    double2* sp = sm;
-    double2* sw = sm + N;
+// (twiddle table built on the host in long double).  One warp per output: lane l sums the terms
+// b = l, l+32, ... in order, then a fixed xor-butterfly adds the 32 lane sums.  The twiddle index
+// is stepped in integers, never formed as a floating-point angle.
+constexpr int kDftThreads = 256;
+__global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restrict__ P, const double2* __restrict__ W,
+                                                          double2* __restrict__ T, double2* __restrict__ T_host,
+                                                          uint32_t N, uint32_t k_shift) {
+    extern __shared__ double2 dft_sm[];  // [N] bins of this channel, [N] twiddles
+    double2* sp = dft_sm;
+    double2* sw = dft_sm + N;
     const uint32_t c = blockIdx.y;
-    for (uint32_t t = threadIdx.x; t < N; t += blockDim.x) {
+    for (uint32_t t = threadIdx.x; t < N; t += kDftThreads) {
         sp[t] = P[(size_t)c * N + t];
         sw[t] = W[t];
     }
     __syncthreads();
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t i = blockIdx.x * (kDftThreads / 32) + (threadIdx.x >> 5);
+    if (i >= N) return;                                   // whole warp leaves together
     const uint32_t ii = (i + N - k_shift % N) % N;
+    uint32_t k = (uint32_t)(((uint64_t)ii * lane) % N);
+    const uint32_t kstep = (uint32_t)(((uint64_t)ii * 32u) % N);
     double re = 0.0, im = 0.0;
-    uint32_t k = 0;
-    for (uint32_t b = 0; b < N; ++b) {
+    for (uint32_t b = lane; b < N; b += 32u) {
         const double2 p = sp[b], w = sw[k];
         re += p.x * w.x - p.y * w.y;
         im += p.x * w.y + p.y * w.x;
-        k += ii; if (k >= N) k -= N;
+        k += kstep; if (k >= N) k -= N;
     }
-    T[(size_t)c * N + i] = make_double2(re, im);
+#pragma unroll
+    for (uint32_t s = 16; s > 0; s >>= 1) {
+        re += __shfl_xor_sync(0xFFFFFFFFu, re, s);
+        im += __shfl_xor_sync(0xFFFFFFFFu, im, s);
+    }
+    if (lane == 0) {
+        T[(size_t)c * N + i] = make_double2(re, im);
+        if (T_host) T_host[(size_t)c * N + i] = make_double2(re, im);   // mapped pinned host memory
+    }
 }
 
 __global__ void zero_kernel(double2* P, long long* Pint, uint32_t n) {
