@@ -57,6 +57,7 @@ struct pcal_ctx {
     uint64_t M, nrot[PCAL_MAX_CHANNELS], lut_len[PCAL_MAX_CHANNELS];
     // generator-mode geometry
     uint32_t gen_grid, gen_spt;
+    size_t gen_smem;
     // device
     int device, sm_count;
     cudaStream_t stream;
@@ -320,11 +321,10 @@ static int prepare(pcal_ctx* c) {
         CU(cudaMemcpy(c->d_lut_off, off.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
         CU(cudaMemcpy(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
     } else {
-        const size_t smem = 2 * (size_t)c->gen_spt * kThreads * sizeof(double);
         int occ = 0;
-        if (c->kind == KIND_2BIT) { CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, smem); }
-        else if (c->kind == KIND_I8) { CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); occ = occupancy_of(gen_kernel<KIND_I8>, smem); }
-        else { occ = occupancy_of(gen_kernel<KIND_F32>, smem); }
+        if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
+        else if (c->kind == KIND_I8) { c->gen_smem = gen_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_I8>, c->gen_smem); }
+        else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
         if (occ < 1) return PCAL_ERR_DEVICE;
         c->gen_grid = (uint32_t)(c->sm_count * occ);
         CU(cudaMalloc(&c->d_gen_partial, (size_t)c->gen_grid * c->n_bins * sizeof(double2)));
@@ -411,7 +411,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.rho = phasor_neg_host(mulmod_host((uint64_t)kThreads * spt, Fo, Fs), Fs);
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
-        const size_t smem = 2 * (size_t)spt * kThreads * sizeof(double);
+        const size_t smem = c->gen_smem;
         prof_mark(c, st);
         if (c->kind == KIND_2BIT) gen_kernel<KIND_2BIT><<<c->gen_grid, kThreads, smem, st>>>(gp);
         else if (c->kind == KIND_I8) gen_kernel<KIND_I8><<<c->gen_grid, kThreads, smem, st>>>(gp);
@@ -446,6 +446,8 @@ extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_sam
     uint64_t piece = n_samples;
     if (c->rot_eff == PCAL_ROT_LUT)
         piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
+    else
+        piece = (uint64_t)kGenMaxTiles * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
     uint64_t done = 0;
     while (done < n_samples) {
         const uint64_t n = n_samples - done < piece ? n_samples - done : piece;

@@ -23,6 +23,7 @@
 // fp32 partial sums live for one tile (<= 64 additions), then are added to fp64 accumulators in
 // shared memory.
 #pragma once
+#include <type_traits>
 #include "pcal_common.cuh"
 
 namespace pcal {
@@ -99,146 +100,173 @@ __device__ __forceinline__ void gen_decode<KIND_2BIT>(const uint32_t& v, float* 
     }
 }
 
+// ---- own-thread asynchronous copies: global -> this thread's slot of a shared-memory ring ----
+// Every thread prefetches ITS OWN future loads (cp.async), so completion is tracked per thread with
+// cp.async.wait_group and no barrier is needed; the bytes in flight per SM (DEPTH loads per thread)
+// do not cost registers.
+template <int BYTES>
+__device__ __forceinline__ void cp_async_own(void* smem_dst, const void* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int kGenMaxTiles = 256;   // tiles per CTA per launch (host splits longer segments)
+
+template <int KIND> struct GenCfg;
+// LPT loads per thread per 2^16-sample tile; RUN tiles between fp32 -> fp64 flushes (<= 64 additions,
+// 16 for the 2-bit affine code whose sums carry a DC term); DEPTH loads in flight per thread.
+template <> struct GenCfg<KIND_F32>  { static constexpr int LB = 16, LPT = 64, RUN = 1, DEPTH = 16; };
+template <> struct GenCfg<KIND_I8>   { static constexpr int LB = 16, LPT = 16, RUN = 4, DEPTH = 8; };
+template <> struct GenCfg<KIND_2BIT> { static constexpr int LB = 4,  LPT = 16, RUN = 1, DEPTH = 16; };
+
 template <int KIND>
-__device__ __forceinline__ typename GenTraits<KIND>::Vec gen_load(const void* base, uint64_t i);
-template <> __device__ __forceinline__ uint4 gen_load<KIND_F32>(const void* b, uint64_t i) { return ldg_stream(reinterpret_cast<const uint4*>(b) + i); }
-template <> __device__ __forceinline__ uint4 gen_load<KIND_I8>(const void* b, uint64_t i) { return ldg_stream(reinterpret_cast<const uint4*>(b) + i); }
-template <> __device__ __forceinline__ uint32_t gen_load<KIND_2BIT>(const void* b, uint64_t i) {
-    uint32_t r;
-    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(reinterpret_cast<const uint32_t*>(b) + i));
-    return r;
+constexpr size_t gen_smem_bytes() {
+    return (size_t)GenTraits<KIND>::SPT * kThreads * sizeof(double2) + (size_t)kGenMaxTiles * sizeof(double2) +
+           (size_t)GenCfg<KIND>::DEPTH * kThreads * GenCfg<KIND>::LB;
 }
 
 template <int KIND>
 __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     constexpr int SPT = GenTraits<KIND>::SPT;
-    constexpr uint32_t SPAN = kThreads * SPT;               // samples per CTA iteration
-    constexpr uint32_t ITERS = kTileSamples / SPAN;         // iterations per tile
-    constexpr int U = 4;                                     // loads in flight per thread
+    constexpr int LB = GenCfg<KIND>::LB, LPT = GenCfg<KIND>::LPT, RUN = GenCfg<KIND>::RUN, DEPTH = GenCfg<KIND>::DEPTH;
+    constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration
+    static_assert((uint32_t)LPT * SPAN == kTileSamples, "a tile is 2^16 samples");
     using Vec = typename GenTraits<KIND>::Vec;
-    extern __shared__ double sacc[];                         // [2*SPT][kThreads] re then im
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    double2* acc = reinterpret_cast<double2*>(gen_smem);                 // [SPT][kThreads] (re, im)
+    double2* base = acc + SPT * kThreads;                                 // [kGenMaxTiles] tile-start phasors
+    unsigned char* ring = reinterpret_cast<unsigned char*>(base + kGenMaxTiles);   // [DEPTH][kThreads][LB]
     const int tid = threadIdx.x;
 #pragma unroll
-    for (int k = 0; k < 2 * SPT; ++k) sacc[k * kThreads + tid] = 0.0;
+    for (int k = 0; k < SPT; ++k) acc[k * kThreads + tid] = make_double2(0.0, 0.0);
 
-    const uint64_t koff = mulmod_u64(P.Foff, (uint64_t)tid * SPT, P.Fs);
-    uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
-    if (k_cta >= P.Fs) k_cta -= P.Fs;
+    // this CTA's tiles: T_i = blockIdx.x + i * gridDim.x, i < nt
+    const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    // ---- resync table: the exactly reduced INTEGER phase of every tile start -> fp64 phasor ----
+    {
+        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
+        if (k_cta >= P.Fs) k_cta -= P.Fs;
+        for (uint32_t i = tid; i < nt; i += kThreads) {
+            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
+            if (k >= P.Fs) k -= P.Fs;
+            base[i] = phasor_neg(k, P.Fs);
+        }
+    }
+    const double2 theta = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * SPT, P.Fs), P.Fs);   // exp(-j w tid SPT)
+    __syncthreads();
+
+    const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
+    unsigned char* my_ring = ring + (size_t)tid * LB;
+    static_assert(LPT % DEPTH == 0, "ring slot of load j is j % DEPTH, a compile-time constant");
+    constexpr uint64_t LOAD_STRIDE = (uint64_t)kThreads * LB;            // bytes between a thread's loads
+    constexpr uint64_t TILE_BYTES = (uint64_t)LPT * LOAD_STRIDE;
+    const uint64_t end_off = P.n_loads * LB;                              // first byte past the last complete load
+    const uint64_t tile_stride = (uint64_t)gridDim.x * TILE_BYTES;
+    uint64_t off = (uint64_t)blockIdx.x * TILE_BYTES + (uint64_t)tid * LB;   // this thread's load 0 of tile i
+
+    float2 ar[SPT / 2], ai[SPT / 2];
+#pragma unroll
+    for (int k2 = 0; k2 < SPT / 2; ++k2) { ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f); }
+    float pr = 0.f, pi = 0.f;
     double sphr = 0.0, sphi = 0.0;                           // sum of phasors of valid loads (2-bit)
 
-    for (uint64_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
-        // ---- resync: exact integer phase -> fp64 phasor ----
-        uint64_t k = k_cta + koff;
-        if (k >= P.Fs) k -= P.Fs;
-        double2 ph = phasor_neg(k, P.Fs);
-        k_cta += P.D;
-        if (k_cta >= P.Fs) k_cta -= P.Fs;
-
-        float2 ar[SPT / 2], ai[SPT / 2];
 #pragma unroll
-        for (int k2 = 0; k2 < SPT / 2; ++k2) { ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f); }
-        float pr = 0.f, pi = 0.f;
-        uint64_t li = (tile * ITERS) * kThreads + tid;       // this thread's load index
-#pragma unroll 1
-        for (uint32_t it = 0; it < ITERS; it += U) {
-            Vec v[U];
-            bool ok[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                ok[u] = (li + (uint64_t)u * kThreads) < P.n_loads;
-                if (ok[u]) v[u] = gen_load<KIND>(P.data, li + (uint64_t)u * kThreads);
-            }
-            li += (uint64_t)U * kThreads;
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const float c = (float)ph.x, s = (float)ph.y;
-                if (ok[u]) {
-                    float x[SPT];
-                    gen_decode<KIND>(v[u], x, P.sign_mag);
-                    const float2 cc = make_float2(c, c), ss = make_float2(s, s);
-#pragma unroll
-                    for (int k2 = 0; k2 < SPT / 2; ++k2) {
-                        const float2 xx = make_float2(x[2 * k2], x[2 * k2 + 1]);
-                        ffma2(ar[k2], xx, cc);
-                        ffma2(ai[k2], xx, ss);
-                    }
-                    if (KIND == KIND_2BIT) { pr += c; pi += s; }
-                }
-                // coupled-form oscillator step (eq. 2.6): ph *= rho, fp64
-                const double nx = ph.x * P.rho.x - ph.y * P.rho.y;
-                const double ny = ph.x * P.rho.y + ph.y * P.rho.x;
-                ph.x = nx; ph.y = ny;
-            }
-        }
-        // ---- flush the tile's fp32 sums into the fp64 accumulators ----
-#pragma unroll
-        for (int k2 = 0; k2 < SPT / 2; ++k2) {
-            sacc[(2 * k2) * kThreads + tid] += (double)ar[k2].x;
-            sacc[(2 * k2 + 1) * kThreads + tid] += (double)ar[k2].y;
-            sacc[(SPT + 2 * k2) * kThreads + tid] += (double)ai[k2].x;
-            sacc[(SPT + 2 * k2 + 1) * kThreads + tid] += (double)ai[k2].y;
-        }
-        sphr += (double)pr; sphi += (double)pi;
+    for (int j = 0; j < DEPTH; ++j) {                        // prologue: the first DEPTH loads of tile 0
+        if (nt > 0 && off + j * LOAD_STRIDE < end_off)
+            cp_async_own<LB>(my_ring + (size_t)j * LOAD_STRIDE, gdata + off + j * LOAD_STRIDE);
+        cp_async_commit();
     }
+
+    // one tile; CHECK = false when this tile and the next one are complete (no per-load tests)
+    auto tile_body = [&](auto check_tag, double2 ph, bool next_exists) {
+        constexpr bool CHECK = decltype(check_tag)::value;
+#pragma unroll
+        for (int j = 0; j < LPT; ++j) {
+            constexpr int dummy = 0; (void)dummy;
+            const int slot = j % DEPTH;                      // compile-time after unrolling
+            cp_async_wait<DEPTH - 1>();
+            const Vec v = *reinterpret_cast<const Vec*>(my_ring + (size_t)slot * LOAD_STRIDE);
+            const float c = (float)ph.x, sn = (float)ph.y;
+            bool ok = true;
+            if (CHECK) ok = off + j * LOAD_STRIDE < end_off;
+            if (ok) {
+                float x[SPT];
+                gen_decode<KIND>(v, x, P.sign_mag);
+                const float2 cc = make_float2(c, c), ss = make_float2(sn, sn);
+#pragma unroll
+                for (int k2 = 0; k2 < SPT / 2; ++k2) {
+                    const float2 xx = make_float2(x[2 * k2], x[2 * k2 + 1]);
+                    ffma2(ar[k2], xx, cc);
+                    ffma2(ai[k2], xx, ss);
+                }
+                if (KIND == KIND_2BIT) { pr += c; pi += sn; }
+            }
+            // refill the slot just consumed with the load DEPTH ahead (same tile or the next one)
+            {
+                const uint64_t o = (j + DEPTH < LPT) ? off + (uint64_t)(j + DEPTH) * LOAD_STRIDE
+                                                     : off + tile_stride + (uint64_t)(j + DEPTH - LPT) * LOAD_STRIDE;
+                bool go = true;
+                if (CHECK) go = ((j + DEPTH < LPT) || next_exists) && o < end_off;
+                if (go) cp_async_own<LB>(my_ring + (size_t)slot * LOAD_STRIDE, gdata + o);
+                cp_async_commit();
+            }
+            // coupled-form oscillator step (eq. 2.6): ph *= rho, fp64
+            const double nx = ph.x * P.rho.x - ph.y * P.rho.y;
+            const double ny = ph.x * P.rho.y + ph.y * P.rho.x;
+            ph.x = nx; ph.y = ny;
+        }
+    };
+
+    for (uint32_t i = 0; i < nt; ++i, off += tile_stride) {
+        // oscillator re-seeded at the tile start: exact tile phase x this thread's offset phasor
+        const double2 b = base[i];
+        const double2 ph0 = make_double2(b.x * theta.x - b.y * theta.y, b.x * theta.y + b.y * theta.x);
+        const uint64_t tile0 = off - (uint64_t)tid * LB;     // first byte of tile i
+        const bool next_exists = i + 1 < nt;
+        const bool fast = next_exists && tile0 + tile_stride + TILE_BYTES <= end_off;   // tiles i and i+1 complete
+        if (fast) tile_body(std::false_type{}, ph0, true);
+        else tile_body(std::true_type{}, ph0, next_exists);
+        if ((i + 1) % RUN == 0 || i + 1 == nt) {
+            // ---- flush the fp32 sums (<= 64 additions each) into the fp64 accumulators ----
+#pragma unroll
+            for (int k2 = 0; k2 < SPT / 2; ++k2) {
+                double2 a0 = acc[(2 * k2) * kThreads + tid], a1 = acc[(2 * k2 + 1) * kThreads + tid];
+                a0.x += (double)ar[k2].x; a0.y += (double)ai[k2].x;
+                a1.x += (double)ar[k2].y; a1.y += (double)ai[k2].y;
+                acc[(2 * k2) * kThreads + tid] = a0; acc[(2 * k2 + 1) * kThreads + tid] = a1;
+                ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f);
+            }
+            sphr += (double)pr; sphi += (double)pi;
+            pr = 0.f; pi = 0.f;
+        }
+    }
+    cp_async_wait<0>();
 
     // ---- post-twiddle by exp(-j w k), undo the 2-bit affine code, reduce positions to bins ----
     double zr[SPT], zi[SPT];
 #pragma unroll
     for (int k = 0; k < SPT; ++k) {
-        double re = sacc[k * kThreads + tid], im = sacc[(SPT + k) * kThreads + tid];
+        const double2 a = acc[k * kThreads + tid];
+        double re = a.x, im = a.y;
         if (KIND == KIND_2BIT) { re = 8.0 * re - 11.0 * sphr; im = 8.0 * im - 11.0 * sphi; }
         zr[k] = re * P.tw[k].x - im * P.tw[k].y;
         zi[k] = re * P.tw[k].y + im * P.tw[k].x;
     }
     __syncthreads();
-    double* pos_re = sacc;                 // [SPAN]
-    double* pos_im = sacc + SPAN;          // [SPAN]
+    double* pos_re = reinterpret_cast<double*>(gen_smem);   // [SPAN]
+    double* pos_im = pos_re + SPAN;                           // [SPAN]   (together == the acc region)
 #pragma unroll
     for (int k = 0; k < SPT; ++k) { pos_re[tid * SPT + k] = zr[k]; pos_im[tid * SPT + k] = zi[k]; }
     __syncthreads();
-    for (uint32_t s = tid; s < P.n_bins; s += kThreads) {
+    for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
         double re = 0.0, im = 0.0;
-        for (uint32_t pos = s; pos < SPAN; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
-        P.partial[(size_t)blockIdx.x * P.n_bins + s] = make_double2(re, im);
+        for (uint32_t pos = sb; pos < SPAN; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
+        P.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
     }
-}
-
-struct GenReduceParams {
-    const double2* partial;  // [grid][n_bins]
-    double2* P;              // [n_bins] accumulated into
-    const uint8_t* tail;     // first byte after the last complete load
-    uint64_t n0, n_done, n_total, Fs, Foff;
-    uint32_t grid, n_bins;
-    int kind, sign_mag;
-};
-
-// one thread per bin: fixed-order sum over CTAs, then the ragged tail with exact phases
-__global__ void gen_reduce_kernel(GenReduceParams G) {
-    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= G.n_bins) return;
-    const uint32_t s = (uint32_t)(((uint64_t)b + G.n_bins - G.n0 % G.n_bins) % G.n_bins);
-    double re = 0.0, im = 0.0;
-    for (uint32_t c = 0; c < G.grid; ++c) {
-        const double2 v = G.partial[(size_t)c * G.n_bins + s];
-        re += v.x; im += v.y;
-    }
-    for (uint64_t t = G.n_done; t < G.n_total; ++t) {
-        if ((G.n0 + t) % G.n_bins != b) continue;
-        const uint32_t r = (uint32_t)(t - G.n_done);
-        double v;
-        if (G.kind == KIND_F32) v = (double)reinterpret_cast<const float*>(G.tail)[r];
-        else if (G.kind == KIND_I8) v = (double)reinterpret_cast<const int8_t*>(G.tail)[r];
-        else {
-            const uint32_t code = (G.tail[r >> 2] >> (2 * (r & 3u))) & 3u;
-            v = G.sign_mag ? ((code & 2u) ? -(double)(1 + 2 * (code & 1u)) : (double)(1 + 2 * (code & 1u)))
-                           : (double)(2 * (int)code - 3);
-        }
-        const double2 ph = phasor_neg(mulmod_u64(G.Foff, G.n0 + t, G.Fs), G.Fs);
-        re += v * ph.x; im += v * ph.y;
-    }
-    double2 cur = G.P[b];
-    cur.x += re; cur.y += im;
-    G.P[b] = cur;
 }
 
 }  // namespace pcal
