@@ -37,6 +37,19 @@ METRIC = "pcal_extraction_samples_per_s"
 UNIT = "samples/s"
 
 
+def load_traffic(workload: str, rotator: str):
+    """dram bytes per launch of the hot kernel from the committed ncu capture (profiles/r1_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    try:
+        for line in open(path).read().splitlines()[1:]:
+            wl, rot, b = line.split(",")
+            if wl == workload and rot == rotator:
+                return int(b)
+    except Exception:
+        pass
+    return None
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -234,13 +247,40 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         "clocks": clocks,
     }
     peak, peak_src = load_peaks()
+    # calibration: a pure streaming read of the same buffers, same grid/loads, bracketed by events
+    # on the same stream in the same way as the hot kernel above
+    floor_us = None
+    if rank == 0:
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for i in range(3):
+            p.read_probe(bufs[i % ncopies])
+        for i, (a, b) in enumerate(evs):
+            a.record(); p.read_probe(bufs[i % ncopies]); b.record()
+        torch.cuda.synchronize()
+        floor_us = 1e3 * sum(a.elapsed_time(b) for a, b in evs) / len(evs)
     # algorithmic bytes per launch = input bytes of one launch (bits/8 per sample, read once)
     bytes_per_launch = w.n_bytes * steps / max(hot_launches, 1)
-    achieved = bytes_per_launch / (1e-3 * hot_ms / max(hot_launches, 1)) / 1e9 if hot_ms > 0 else 0.0
+    hot_s = 1e-3 * hot_ms / max(hot_launches, 1)
+    achieved = bytes_per_launch / hot_s / 1e9 if hot_ms > 0 else 0.0
+    gen = inf.rotator_in_effect == 2
     res["roofline"] = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                        "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                       "kernel": "fold_*_kernel (LUT path)" if inf.rotator_in_effect == 1 else "gen_kernel (generator path)",
+                       "kernel": "gen_kernel (generator path)" if gen else "fold_*_kernel (LUT path)",
                        "algorithmic_bytes_per_launch": bytes_per_launch}
+    res["roofline"]["traffic"] = load_traffic(w.name, res["rotator"]) if not n_override else None
+    if floor_us:
+        res["roofline"]["read_floor"] = {
+            "us": floor_us, "gbs": w.n_bytes / floor_us / 1e3, "frac_of_floor": floor_us / (hot_s * 1e6),
+            "what": "pcal_read_probe: pure streaming read of the same buffer (no decode/fold), same event bracketing"}
+    if gen and w.bits == 2:
+        # 2-bit generator variant: >= 3 thread-instructions per sample (shift, LOP3, one FFMA2 lane-op)
+        # against the issue rate 148 SMs x 4 schedulers x 32 lanes x f_SM
+        sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        alu_peak = 148 * 4 * 32 * sm_mhz * 1e6 / 1e9                     # G thread-instr/s
+        alu_ach = 3.0 * (n * C * steps / max(hot_launches, 1)) / hot_s / 1e9
+        res["roofline"].update({"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Ginstr/s",
+                                "frac": alu_ach / alu_peak, "peak_source": "derived: 148 SMs x 4 x 32 lanes x sm_max_mhz",
+                                "hbm_frac": achieved / peak, "hbm_achieved_gbs": achieved})
     if do_e2e:
         host = bufs[0].cpu().pin_memory()
         e2e_steps = max(1, min(steps, 5 if w.n_bytes > (1 << 30) else steps))

@@ -165,6 +165,12 @@ int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
 int pcal_set_profiling(pcal_ctx *ctx, int enable);
 int pcal_get_profile(pcal_ctx *ctx, double *hot_kernel_ms, uint64_t *hot_kernel_launches);
 
+/* Calibration for the roofline report: enqueue a pure streaming read (no decode, no fold) of
+ * n_bytes from dev ([device], 16-byte aligned) on cuda_stream, with the load instruction, block
+ * size and pipelining of the fold kernels.  Asynchronous; computes nothing; the caller times it.
+ * What it reaches on a given size is the practical ceiling of a read-once kernel of that size. */
+int pcal_read_probe(pcal_ctx *ctx, const void *dev, uint64_t n_bytes, void *cuda_stream);
+
 /* Zero accumulators, sample index <- 0 (on the context's stream); parameters are kept. */
 int pcal_reset(pcal_ctx *ctx);
 

@@ -77,6 +77,7 @@ def lib():
             "pcal_set_start_index": (i32, [vp, u64]),
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
+            "pcal_read_probe": (i32, [vp, vp, u64, vp]),
             "pcal_finalize": (i32, [vp, vp]),
             "pcal_finalize_async": (i32, [vp, vp]),
             "pcal_get_folded": (i32, [vp, vp]),
@@ -202,6 +203,11 @@ class Pcal:
 
     def add_folded_dev(self, dev_bins):
         _check(lib().pcal_add_folded_dev(self._h, dev_bins.data_ptr()), "pcal_add_folded_dev")
+
+    def read_probe(self, dev_buf, stream=None):
+        """Calibration: enqueue a pure streaming read of the whole device tensor (roofline report)."""
+        nbytes = dev_buf.numel() * dev_buf.element_size()
+        _check(lib().pcal_read_probe(self._h, dev_buf.data_ptr(), nbytes, _stream_handle(stream)), "pcal_read_probe")
 
     def set_profiling(self, enable: bool):
         _check(lib().pcal_set_profiling(self._h, int(enable)), "pcal_set_profiling")

@@ -411,6 +411,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.rho = phasor_neg_host(mulmod_host((uint64_t)kThreads * spt, Fo, Fs), Fs);
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
+        gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
         if (c->kind == KIND_2BIT) gen_kernel<KIND_2BIT><<<c->gen_grid, kThreads, smem, st>>>(gp);
@@ -596,6 +597,18 @@ extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
     { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const uint32_t n = c->n_bins * (uint32_t)c->C;
     add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_bins), n);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
+extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, void* cuda_stream) {
+    if (!c || !dev) return PCAL_ERR_INVALID;
+    if ((uintptr_t)dev & 15u) return PCAL_ERR_ALIGNMENT;
+    int occ = occupancy_of(read_probe_kernel, 0);
+    if (occ < 1) return PCAL_ERR_DEVICE;
+    read_probe_kernel<<<c->sm_count * occ, kThreads, 0, (cudaStream_t)cuda_stream>>>(
+        reinterpret_cast<const uint4*>(dev), n_bytes / 16, reinterpret_cast<uint32_t*>(c->d_tmp));
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;

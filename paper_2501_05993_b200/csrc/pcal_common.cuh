@@ -75,3 +75,28 @@ __device__ __forceinline__ double2 phasor_neg(uint64_t k, uint64_t m) {
 }
 
 }  // namespace pcal
+
+// ---- calibration: a pure streaming read of `n_vec` 16-byte vectors (no decode, no fold) --------
+// Same load instruction, block size and software pipelining as the fold kernels; what it reaches
+// on a given buffer size is the practical ceiling for any read-once kernel of that size
+// (bench.py reports it beside the roofline fraction).  The xor of all words lands in out[0] only
+// if it equals a magic value, so the loads cannot be optimised away.
+namespace pcal {
+__global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __restrict__ d, uint64_t n_vec, uint32_t* out) {
+    const uint64_t stride = (uint64_t)gridDim.x * kThreads;
+    uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
+    uint32_t acc = 0;
+    uint4 v[4], w[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const uint64_t a = i + u * stride; v[u] = a < n_vec ? ldg_stream(d + a) : make_uint4(0, 0, 0, 0); }
+    for (i += 4 * stride; i < n_vec + 4 * stride; i += 4 * stride) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const uint64_t a = i + u * stride; w[u] = a < n_vec ? ldg_stream(d + a) : make_uint4(0, 0, 0, 0); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = w[u];
+    }
+    if (acc == 0x5ca1ab1eu) out[0] = acc;
+}
+}  // namespace pcal

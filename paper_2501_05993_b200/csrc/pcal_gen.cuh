@@ -41,6 +41,7 @@ struct GenParams {
     double2* partial;        // [device] [cta][n_bins]
     uint32_t n_bins;
     int sign_mag;
+    uint32_t dec_mask, dec_one;   // 0x00600000, 0x3F800000 (2-bit decode, see lop3_and_or)
 };
 
 __device__ __forceinline__ void ffma2(float2& acc, const float2 x, const float2 c) {
@@ -90,13 +91,20 @@ __device__ __forceinline__ void gen_decode<KIND_I8>(const uint4& v, float* x, in
         }
     }
 }
-template <>
-__device__ __forceinline__ void gen_decode<KIND_2BIT>(const uint32_t& v, float* x, int sign_mag) {
+// (a & b) | c in ONE LOP3.  b and c are the decode constants 0x00600000 / 0x3F800000 handed over
+// as kernel parameters (GenParams::dec_mask / dec_one): with immediates ptxas needs two LOP3,
+// because one instruction can encode only one immediate.
+__device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+__device__ __forceinline__ void gen_decode_2bit(uint32_t v, float* x, int sign_mag, uint32_t dec_mask, uint32_t dec_one) {
     const uint32_t w = sign_mag ? signmag_to_offset_binary(v) : v;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         const uint32_t sh = (2 * k <= 21) ? (w << (21 - 2 * k)) : (w >> (2 * k - 21));
-        x[k] = __uint_as_float((sh & 0x00600000u) | 0x3F800000u);  // 1 + c/4
+        x[k] = __uint_as_float(lop3_and_or(sh, dec_mask, dec_one));  // 1 + c/4
     }
 }
 
@@ -141,6 +149,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     double2* base = acc + SPT * kThreads;                                 // [kGenMaxTiles] tile-start phasors
     unsigned char* ring = reinterpret_cast<unsigned char*>(base + kGenMaxTiles);   // [DEPTH][kThreads][LB]
     const int tid = threadIdx.x;
+    const uint32_t dec_mask = P.dec_mask, dec_one = P.dec_one;   // opaque to ptxas: see lop3_and_or
 #pragma unroll
     for (int k = 0; k < SPT; ++k) acc[k * kThreads + tid] = make_double2(0.0, 0.0);
 
@@ -195,7 +204,8 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
             if (CHECK) ok = off + j * LOAD_STRIDE < end_off;
             if (ok) {
                 float x[SPT];
-                gen_decode<KIND>(v, x, P.sign_mag);
+                if constexpr (KIND == KIND_2BIT) gen_decode_2bit(v, x, P.sign_mag, dec_mask, dec_one);
+                else gen_decode<KIND>(v, x, P.sign_mag);
                 const float2 cc = make_float2(c, c), ss = make_float2(sn, sn);
 #pragma unroll
                 for (int k2 = 0; k2 < SPT / 2; ++k2) {
