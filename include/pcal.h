@@ -139,6 +139,23 @@ int pcal_finalize(pcal_ctx *ctx, double *out_tones);
  * host memory) on the context's stream; the caller synchronises. */
 int pcal_finalize_async(pcal_ctx *ctx, double *out_tones);
 
+/*
+ * PCal data analysis on the device (R23-R25): enqueues the DFT and
+ * one analysis kernel, copies the results to the host, synchronises the stream.
+ *   out_summary    [host] n_channels*PCAL_N_SUMMARY doubles, per channel:
+ *                  [0] b*      bin of the largest |P[b]|^2 (first one on ties)
+ *                  [1] delta   three-point vertex offset in (-1/2, 1/2), cyclic neighbours
+ *                  [2] pulse (group) delay (b* + delta)/f_s in seconds (bin i <-> delay i/f_s)
+ *                  [3] |P[b*]|^2   [4] sum_b |P[b]|^2
+ *                  [5] cable delay t_d of eq. 2.1 from the least-squares slope of the unwrapped tone
+ *                      phases arg T[i] + pi/2 over the in-band tones (branch |t_d| < 1/(2 f_comb))
+ *                  [6] intercept of that line in radians   [7] rms residual in radians
+ *   out_bandpass   [host] n_channels*N_bins*2 doubles or NULL: group-delay corrected band-pass
+ *                  B[c][i] = T[c][i] exp(+j 2 pi i (b* + delta)/N_bins).
+ */
+#define PCAL_N_SUMMARY 8
+int pcal_analyze(pcal_ctx *ctx, double *out_summary, double *out_bandpass);
+
 /* Folded period P before the DFT: [host] n_channels*N_bins*2 doubles (Re, Im).  Synchronises. */
 int pcal_get_folded(pcal_ctx *ctx, double *out_bins);
 

@@ -78,6 +78,7 @@ def lib():
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
+            "pcal_analyze": (i32, [vp, vp, vp]),
             "pcal_finalize": (i32, [vp, vp]),
             "pcal_finalize_async": (i32, [vp, vp]),
             "pcal_get_folded": (i32, [vp, vp]),
@@ -182,6 +183,13 @@ class Pcal:
     def finalize_async(self, out_pinned):
         """Enqueue DFT + copy into a pinned complex128 host tensor; caller synchronises."""
         _check(lib().pcal_finalize_async(self._h, out_pinned.data_ptr()), "pcal_finalize_async")
+
+    def analyze(self, bandpass: bool = True):
+        """(summary float64 [n_channels, 8], corrected band-pass complex128 [n_channels, N_bins] or None)."""
+        summ = np.empty((self.n_channels, 8), np.float64)
+        bp = np.empty((self.n_channels, self.n_bins), np.complex128) if bandpass else None
+        _check(lib().pcal_analyze(self._h, summ.ctypes.data, bp.ctypes.data if bandpass else None), "pcal_analyze")
+        return summ, bp
 
     def get_folded(self) -> np.ndarray:
         out = np.empty((self.n_channels, self.n_bins), np.complex128)

@@ -15,6 +15,7 @@
 #include "pcal_fold.cuh"
 #include "pcal_gen.cuh"
 #include "pcal_post.cuh"
+#include "pcal_analysis.cuh"
 
 using namespace pcal;
 typedef unsigned __int128 u128;
@@ -69,6 +70,8 @@ struct pcal_ctx {
     uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
+    double *d_summary, *h_ana;      // analysis outputs: [C][8] + band-pass [C][N] complex
+    double2* d_B;
     uint64_t launches;
     void (*fold2)(FoldParams);      // the fold_2bit_kernel instantiation in use
     // profiling hook
@@ -155,7 +158,10 @@ extern "C" int pcal_create(pcal_ctx** out, double f_s_hz, double f_comb_hz, doub
               cudaMalloc(&c->d_tmp, nb * sizeof(double2)) == cudaSuccess &&
               cudaMalloc(&c->d_Pint, nb * sizeof(long long)) == cudaSuccess &&
               cudaMalloc(&c->d_W, (size_t)c->n_bins * sizeof(double2)) == cudaSuccess &&
-              cudaMallocHost(&c->h_pinned, nb * sizeof(double2)) == cudaSuccess;
+              cudaMallocHost(&c->h_pinned, nb * sizeof(double2)) == cudaSuccess &&
+              cudaMalloc(&c->d_summary, (size_t)n_channels * kNSummary * sizeof(double)) == cudaSuccess &&
+              cudaMalloc(&c->d_B, nb * sizeof(double2)) == cudaSuccess &&
+              cudaMallocHost(&c->h_ana, (size_t)n_channels * kNSummary * sizeof(double) + nb * sizeof(double2)) == cudaSuccess;
     if (ok) {
         std::vector<double2> W(c->n_bins);
         for (uint32_t k = 0; k < c->n_bins; ++k) W[k] = phasor_neg_host(k, c->n_bins);
@@ -176,7 +182,8 @@ extern "C" void pcal_destroy(pcal_ctx* c) {
     free_tables(c);
     cudaFree(c->d_P); cudaFree(c->d_T); cudaFree(c->d_tmp); cudaFree(c->d_Pint); cudaFree(c->d_W);
     cudaFree(c->d_stage);
-    cudaFreeHost(c->h_pinned);
+    cudaFreeHost(c->h_pinned); cudaFreeHost(c->h_ana);
+    cudaFree(c->d_summary); cudaFree(c->d_B);
     if (c->ev) { for (cudaEvent_t e : *c->ev) cudaEventDestroy(e); delete c->ev; }
     cudaGetLastError();
     delete c;
@@ -522,6 +529,30 @@ extern "C" int pcal_finalize(pcal_ctx* c, double* out) {
     if (r != PCAL_OK) return r;
     CU(cudaStreamSynchronize(c->stream));
     memcpy(out, c->h_pinned, (size_t)c->n_bins * c->C * sizeof(double2));
+    return PCAL_OK;
+}
+
+// PCal data analysis: DFT, then one analysis CTA per channel.
+extern "C" int pcal_analyze(pcal_ctx* c, double* out_summary, double* out_bandpass) {
+    if (!c || !out_summary) return PCAL_ERR_INVALID;
+    bool wrote = false;
+    const int r = enqueue_dft(c, nullptr, &wrote);
+    if (r != PCAL_OK) return r;
+    AnalyzeParams ap;
+    ap.P = c->d_P; ap.T = c->d_T; ap.summary = c->d_summary; ap.B = c->d_B;
+    ap.f_s_hz = (double)c->Fs * 1e-6; ap.f_comb_hz = (double)c->Fcomb * 1e-6; ap.N = c->n_bins;
+    ap.zero_offset_mask = 0;
+    for (int i = 0; i < c->C; ++i) if (c->Foff[i] == 0) ap.zero_offset_mask |= 1u << i;
+    const size_t smem = (size_t)c->n_bins * sizeof(double);
+    analyze_kernel<<<c->C, kAnaThreads, smem, c->stream>>>(ap);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    const size_t sb = (size_t)c->C * kNSummary * sizeof(double), bb = (size_t)c->n_bins * c->C * sizeof(double2);
+    CU(cudaMemcpyAsync(c->h_ana, c->d_summary, sb, cudaMemcpyDeviceToHost, c->stream));
+    if (out_bandpass) CU(cudaMemcpyAsync(reinterpret_cast<char*>(c->h_ana) + sb, c->d_B, bb, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(out_summary, c->h_ana, sb);
+    if (out_bandpass) memcpy(out_bandpass, reinterpret_cast<char*>(c->h_ana) + sb, bb);
     return PCAL_OK;
 }
 
