@@ -121,6 +121,21 @@ int pcal_set_start_index(pcal_ctx *ctx, uint64_t n_start);
  */
 int pcal_extract(pcal_ctx *ctx, const void *dev_samples, uint64_t n_samples, void *cuda_stream);
 
+/*
+ * A time series of integrations in one call ("112 integrated time-integrated PCal
+ * results", 10 s each): period k = samples [k, k+1)*n_per_period of the segment.  The accumulators
+ * restart at every period, the sample index (rotator phase, bin alignment) runs on, so period k equals
+ * what pcal_set_start_index(n0 + k*n_per_period) + pcal_extract + pcal_finalize would give.
+ *   dev_samples     [device] 16-byte aligned; n_per_period*bits*n_channels must be a multiple of 128
+ *                   (every period starts 16-byte aligned), else PCAL_ERR_ALIGNMENT
+ *   dev_out_tones   [device] n_periods*n_channels*N_bins*2 doubles: T of every period (layout of
+ *                   pcal_finalize per period)
+ *   dev_out_folded  [device] same size or NULL: P of every period (needs k_shift == 0)
+ * Asynchronous on cuda_stream.  Afterwards the context holds the LAST period's accumulators.
+ */
+int pcal_extract_series(pcal_ctx *ctx, const void *dev_samples, uint64_t n_per_period, uint32_t n_periods,
+                        void *cuda_stream, double *dev_out_tones, double *dev_out_folded);
+
 /* Same, with the segment in [host] memory (pinned for full speed): copies it to the device in
  * chunks on cuda_stream and extracts each chunk.  Returns after the last copy has been enqueued
  * and the host buffer may be reused (it synchronises the stream). */

@@ -78,6 +78,7 @@ def lib():
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
+            "pcal_extract_series": (i32, [vp, vp, u64, ctypes.c_uint32, vp, vp, vp]),
             "pcal_analyze": (i32, [vp, vp, vp]),
             "pcal_finalize": (i32, [vp, vp]),
             "pcal_finalize_async": (i32, [vp, vp]),
@@ -160,6 +161,13 @@ class Pcal:
         else:
             ptr = int(dev_samples)
         _check(lib().pcal_extract(self._h, ptr, n_samples, _stream_handle(stream)), "pcal_extract")
+
+    def extract_series(self, dev_samples, n_per_period: int, n_periods: int, out_tones, out_folded=None, stream=None):
+        """Time series of integrations: out_tones / out_folded are CUDA complex128 tensors
+        [n_periods, n_channels, N_bins] (caller-owned); asynchronous."""
+        _check(lib().pcal_extract_series(self._h, dev_samples.data_ptr(), n_per_period, n_periods, _stream_handle(stream),
+                                         out_tones.data_ptr(), out_folded.data_ptr() if out_folded is not None else None),
+               "pcal_extract_series")
 
     def extract_host(self, host_samples, n_samples: Optional[int] = None, stream=None):
         """host_samples: CPU tensor / numpy array (pinned for full speed)."""

@@ -439,19 +439,11 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     return PCAL_OK;
 }
 
-extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_samples, void* cuda_stream) {
-    if (!c) return PCAL_ERR_INVALID;
-    if (n_samples == 0) return PCAL_OK;
-    if (!dev_samples) return PCAL_ERR_INVALID;
-    if ((uintptr_t)dev_samples & 15u) return PCAL_ERR_ALIGNMENT;
-    if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
-    const int rc = prepare(c);
-    if (rc != PCAL_OK) return rc;
-    c->started = true;
-    c->stream = (cudaStream_t)cuda_stream;
-    const uint8_t* p = reinterpret_cast<const uint8_t*>(dev_samples);
-    // pieces: bounded per-thread trip count (LUT path) / whole segment (generator path)
-    uint64_t piece = n_samples;
+static int enqueue_dft(pcal_ctx* c, double2* second_dst);
+
+// pieces: bounded per-thread trip count (LUT path) / bounded resync table (generator path)
+static int extract_segment(pcal_ctx* c, const uint8_t* p, uint64_t n_samples) {
+    uint64_t piece;
     if (c->rot_eff == PCAL_ROT_LUT)
         piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
     else
@@ -465,6 +457,48 @@ extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_sam
         if (r != PCAL_OK) return r;
         c->n_processed += n;
         done += n;
+    }
+    return PCAL_OK;
+}
+
+extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_samples, void* cuda_stream) {
+    if (!c) return PCAL_ERR_INVALID;
+    if (n_samples == 0) return PCAL_OK;
+    if (!dev_samples) return PCAL_ERR_INVALID;
+    if ((uintptr_t)dev_samples & 15u) return PCAL_ERR_ALIGNMENT;
+    if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
+    const int rc = prepare(c);
+    if (rc != PCAL_OK) return rc;
+    c->started = true;
+    c->stream = (cudaStream_t)cuda_stream;
+    return extract_segment(c, reinterpret_cast<const uint8_t*>(dev_samples), n_samples);
+}
+
+// A time series of integrations (112 pulses of 10 s each): period k covers the
+// samples [k, k+1) * n_per_period of the segment; the accumulators restart at every period while the
+// sample index -- hence the rotator phase -- runs on.
+extern "C" int pcal_extract_series(pcal_ctx* c, const void* dev_samples, uint64_t n_per_period, uint32_t n_periods,
+                                   void* cuda_stream, double* dev_out_tones, double* dev_out_folded) {
+    if (!c || !dev_out_tones) return PCAL_ERR_INVALID;
+    if (n_periods == 0 || n_per_period == 0) return PCAL_OK;
+    if (!dev_samples) return PCAL_ERR_INVALID;
+    const uint64_t bits_per_period = n_per_period * (uint64_t)c->bits * c->C;
+    if (((uintptr_t)dev_samples & 15u) || bits_per_period % 128) return PCAL_ERR_ALIGNMENT;   // every period 16-byte aligned
+    if (dev_out_folded && c->k_shift) return PCAL_ERR_STATE;
+    const int rc = prepare(c);
+    if (rc != PCAL_OK) return rc;
+    c->started = true;
+    c->stream = (cudaStream_t)cuda_stream;
+    const size_t nb = (size_t)c->n_bins * c->C;
+    const uint8_t* p = reinterpret_cast<const uint8_t*>(dev_samples);
+    for (uint32_t k = 0; k < n_periods; ++k) {
+        c->zero_pending = true;                       // the period's first post kernel overwrites the bins
+        int r = extract_segment(c, p + (size_t)k * (bits_per_period / 8), n_per_period);
+        if (r != PCAL_OK) return r;
+        r = enqueue_dft(c, reinterpret_cast<double2*>(dev_out_tones) + (size_t)k * nb);
+        if (r != PCAL_OK) return r;
+        if (dev_out_folded)
+            CU(cudaMemcpyAsync(dev_out_folded + (size_t)k * nb * 2, c->d_P, nb * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
     }
     return PCAL_OK;
 }
@@ -493,32 +527,28 @@ extern "C" int pcal_extract_host(pcal_ctx* c, const void* host_samples, uint64_t
 
 // The DFT kernel writes T both to d_T and, when `host_out` is device-visible pinned host memory
 // (cudaHostAlloc / cudaHostRegister under unified addressing), straight into it: no copy node.
-static int enqueue_dft(pcal_ctx* c, double* host_out, bool* wrote_host) {
+static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const int rz = ensure_zeroed(c);
     if (rz != PCAL_OK) return rz;
-    double2* mapped = nullptr;
-    if (host_out) {
-        cudaPointerAttributes at;
-        if (cudaPointerGetAttributes(&at, host_out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
-            mapped = reinterpret_cast<double2*>(at.devicePointer);
-        cudaGetLastError();
-    }
     const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
     const uint32_t per_cta = kDftThreads / 32;
     dft_kernel<<<dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream>>>(
-        c->d_P, c->d_W, c->d_T, mapped, c->n_bins, (uint32_t)c->k_shift);
+        c->d_P, c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift);
     c->launches += 1;
     CU(cudaGetLastError());
-    *wrote_host = mapped != nullptr;
     return PCAL_OK;
 }
 
 extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
-    bool wrote = false;
-    const int r = enqueue_dft(c, out, &wrote);
+    double2* mapped = nullptr;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+        mapped = reinterpret_cast<double2*>(at.devicePointer);
+    cudaGetLastError();
+    const int r = enqueue_dft(c, mapped);
     if (r != PCAL_OK) return r;
-    if (!wrote)
+    if (!mapped)
         CU(cudaMemcpyAsync(out, c->d_T, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
     return PCAL_OK;
 }
@@ -535,8 +565,7 @@ extern "C" int pcal_finalize(pcal_ctx* c, double* out) {
 // PCal data analysis: DFT, then one analysis CTA per channel.
 extern "C" int pcal_analyze(pcal_ctx* c, double* out_summary, double* out_bandpass) {
     if (!c || !out_summary) return PCAL_ERR_INVALID;
-    bool wrote = false;
-    const int r = enqueue_dft(c, nullptr, &wrote);
+    const int r = enqueue_dft(c, nullptr);
     if (r != PCAL_OK) return r;
     AnalyzeParams ap;
     ap.P = c->d_P; ap.T = c->d_T; ap.summary = c->d_summary; ap.B = c->d_B;

@@ -106,6 +106,14 @@ __device__ __forceinline__ void gen_decode_2bit(uint32_t v, float* x, int sign_m
         const uint32_t sh = (2 * k <= 21) ? (w << (21 - 2 * k)) : (w >> (2 * k - 21));
         x[k] = __uint_as_float(lop3_and_or(sh, dec_mask, dec_one));  // 1 + c/4
     }
+    // centre the code: (1 + c/4) - 1.375 = level/8 exactly.  Without it every fp32 sum would carry a
+    // DC term ~ sum of phasors, whose rounding (not the signal's) would set the error floor.
+    const float2 bias = make_float2(-1.375f, -1.375f);
+#pragma unroll
+    for (int k = 0; k < 16; k += 2) {
+        const float2 p = fadd2(make_float2(x[k], x[k + 1]), bias);
+        x[k] = p.x; x[k + 1] = p.y;
+    }
 }
 
 // ---- own-thread asynchronous copies: global -> this thread's slot of a shared-memory ring ----
@@ -126,10 +134,10 @@ constexpr int kGenMaxTiles = 256;   // tiles per CTA per launch (host splits lon
 
 template <int KIND> struct GenCfg;
 // LPT loads per thread per 2^16-sample tile; RUN tiles between fp32 -> fp64 flushes (<= 64 additions,
-// 16 for the 2-bit affine code whose sums carry a DC term); DEPTH loads in flight per thread.
+// the 2-bit code is centred to level/8 at decode, so its sums carry no DC term); DEPTH loads in flight per thread.
 template <> struct GenCfg<KIND_F32>  { static constexpr int LB = 16, LPT = 64, RUN = 1, DEPTH = 16; };
 template <> struct GenCfg<KIND_I8>   { static constexpr int LB = 16, LPT = 16, RUN = 4, DEPTH = 8; };
-template <> struct GenCfg<KIND_2BIT> { static constexpr int LB = 4,  LPT = 16, RUN = 1, DEPTH = 16; };
+template <> struct GenCfg<KIND_2BIT> { static constexpr int LB = 4,  LPT = 16, RUN = 4, DEPTH = 16; };
 
 template <int KIND>
 constexpr size_t gen_smem_bytes() {
@@ -180,8 +188,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     float2 ar[SPT / 2], ai[SPT / 2];
 #pragma unroll
     for (int k2 = 0; k2 < SPT / 2; ++k2) { ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f); }
-    float pr = 0.f, pi = 0.f;
-    double sphr = 0.0, sphi = 0.0;                           // sum of phasors of valid loads (2-bit)
 
 #pragma unroll
     for (int j = 0; j < DEPTH; ++j) {                        // prologue: the first DEPTH loads of tile 0
@@ -213,7 +219,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
                     ffma2(ar[k2], xx, cc);
                     ffma2(ai[k2], xx, ss);
                 }
-                if (KIND == KIND_2BIT) { pr += c; pi += sn; }
             }
             // refill the slot just consumed with the load DEPTH ahead (same tile or the next one)
             {
@@ -250,8 +255,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
                 acc[(2 * k2) * kThreads + tid] = a0; acc[(2 * k2 + 1) * kThreads + tid] = a1;
                 ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f);
             }
-            sphr += (double)pr; sphi += (double)pi;
-            pr = 0.f; pi = 0.f;
         }
     }
     cp_async_wait<0>();
@@ -262,7 +265,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     for (int k = 0; k < SPT; ++k) {
         const double2 a = acc[k * kThreads + tid];
         double re = a.x, im = a.y;
-        if (KIND == KIND_2BIT) { re = 8.0 * re - 11.0 * sphr; im = 8.0 * im - 11.0 * sphi; }
+        if (KIND == KIND_2BIT) { re *= 8.0; im *= 8.0; }      // sums of level/8
         zr[k] = re * P.tw[k].x - im * P.tw[k].y;
         zi[k] = re * P.tw[k].y + im * P.tw[k].x;
     }
