@@ -443,11 +443,15 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst);
 
 // pieces: bounded per-thread trip count (LUT path) / bounded resync table (generator path)
 static int extract_segment(pcal_ctx* c, const uint8_t* p, uint64_t n_samples) {
+    // PCAL_SMALL_PIECES=1 (tests only) shrinks both limits so that a few million samples already
+    // span several launches; the arithmetic is unchanged.
+    const char* sp = getenv("PCAL_SMALL_PIECES");
+    const bool small = sp && sp[0] == '1';
     uint64_t piece;
     if (c->rot_eff == PCAL_ROT_LUT)
-        piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
+        piece = (uint64_t)(small ? 16u : kMaxIterPerLaunch) * c->R * kWarps * c->q * 32ull * c->spv;
     else
-        piece = (uint64_t)kGenMaxTiles * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
+        piece = (uint64_t)(small ? 2 : kGenMaxTiles) * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
     uint64_t done = 0;
     while (done < n_samples) {
         const uint64_t n = n_samples - done < piece ? n_samples - done : piece;

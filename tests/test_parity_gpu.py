@@ -225,3 +225,22 @@ def test_error_codes():
     with pytest.raises(B.PcalError) as e:
         q.extract(torch.zeros(4096, dtype=torch.int8, device=DEV))
     assert e.value.code == -4                        # LUT of impractical length
+
+
+@pytest.mark.parametrize("idx,n,rot", [(2, 250_000_004, None), (4, 14_000_003, None), (5, 90_000_003, None),
+                                       (3, 90_000_004, "generator"), (8, 40_000_001, "generator")])
+def test_segments_longer_than_one_launch(oracle, idx, n, rot, monkeypatch):
+    """A segment that exceeds the per-launch limits (16-bit lanes of the fold kernel, 256-entry resync
+    table of the generator kernel) is cut into several launches by the host; PCAL_SMALL_PIECES=1 lowers
+    both limits so that this size already needs 2-4 of them.  Result = one continuous stream."""
+    monkeypatch.setenv("PCAL_SMALL_PIECES", "1")
+    w, dev, host = make(idx, n)
+    p, T, P = gpu_run(w, dev, rotator=rot)
+    n_fold = 3 if rot is None and idx != 5 else 2          # kernels per piece: fold+reduce+rotate / gen+post
+    assert p.info().kernel_launches >= 2 * n_fold + 1, p.info().kernel_launches
+    for c in range(0, w.n_channels, 6):
+        assert_close(T[c], oracle_tones(oracle, w, host, c, threads=8), f"cfg{idx} ch{c} multi-launch")
+    monkeypatch.delenv("PCAL_SMALL_PIECES")
+    p2, T2, _ = gpu_run(w, dev, rotator=rot)
+    assert p2.info().kernel_launches < p.info().kernel_launches
+    assert_close(T, T2, f"cfg{idx} pieces vs single launch")
