@@ -197,6 +197,25 @@ int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
 int pcal_set_profiling(pcal_ctx *ctx, int enable);
 int pcal_get_profile(pcal_ctx *ctx, double *hot_kernel_ms, uint64_t *hot_kernel_launches);
 
+/*
+ * Accuracy of the sinewave generators over many cycles (eq. 2.6/2.7, PAPER.md:142-153
+ * direct method, PAPER.md:97 k-shift; R26).  One device thread per case runs the
+ * recursion for n = 1..n_steps with every operation rounded once to the case's precision and records
+ * out_err[case*n_chk + j] = max over the j-th of n_chk equal intervals of |y[n] - exp(-j n dphi)|, the
+ * exact phasor taken from the exactly reduced integer phase (fp64).  For a k-shift give
+ * f_rot_hz = f_offset + k f_comb.  cases: [host]; out_err: [host] n_cases*n_chk doubles.  Synchronous,
+ * default stream of the current device, no context needed.
+ */
+enum { PCAL_GEN_CFO = 0, PCAL_GEN_MCO = 1, PCAL_GEN_DFR = 2, PCAL_GEN_DFR_FMA = 3, PCAL_GEN_DIRECT = 4 };
+typedef struct pcal_gen_case_t {
+    int32_t form;        /* PCAL_GEN_* */
+    int32_t precision;   /* 32 or 64 (PCAL_GEN_DIRECT always computes its phase in float32) */
+    double f_s_hz;
+    double f_rot_hz;     /* rotator frequency, 0 <= f_rot < f_s */
+} pcal_gen_case_t;
+int pcal_generator_study(const pcal_gen_case_t *cases, uint32_t n_cases, uint64_t n_steps, uint32_t n_chk,
+                         double *out_err);
+
 /* Calibration for the roofline report: enqueue a pure streaming read (no decode, no fold) of
  * n_bytes from dev ([device], 16-byte aligned) on cuda_stream, with the load instruction, block
  * size and pipelining of the fold kernels.  Asynchronous; computes nothing; the caller times it.

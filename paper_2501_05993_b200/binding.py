@@ -78,6 +78,7 @@ def lib():
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
+            "pcal_generator_study": (i32, [vp, ctypes.c_uint32, u64, ctypes.c_uint32, vp]),
             "pcal_extract_series": (i32, [vp, vp, u64, ctypes.c_uint32, vp, vp, vp]),
             "pcal_analyze": (i32, [vp, vp, vp]),
             "pcal_finalize": (i32, [vp, vp]),
@@ -252,6 +253,23 @@ class Pcal:
             self.destroy()
         except Exception:
             pass
+
+
+GEN_CFO, GEN_MCO, GEN_DFR, GEN_DFR_FMA, GEN_DIRECT = 0, 1, 2, 3, 4
+
+
+class GenCaseT(ctypes.Structure):
+    _fields_ = [("form", ctypes.c_int32), ("precision", ctypes.c_int32), ("f_s_hz", ctypes.c_double),
+                ("f_rot_hz", ctypes.c_double)]
+
+
+def generator_study(cases, n_steps: int, n_chk: int) -> np.ndarray:
+    """cases: sequence of (form, precision, f_s_hz, f_rot_hz); returns float64 [n_cases, n_chk] max errors."""
+    arr = (GenCaseT * len(cases))(*[GenCaseT(int(f), int(p), float(fs), float(fr)) for f, p, fs, fr in cases])
+    out = np.empty((len(cases), n_chk), np.float64)
+    _check(lib().pcal_generator_study(ctypes.cast(arr, ctypes.c_void_p), len(cases), n_steps, n_chk, out.ctypes.data),
+           "pcal_generator_study")
+    return out
 
 
 def from_workload(w) -> "Pcal":

@@ -16,6 +16,7 @@
 #include "pcal_gen.cuh"
 #include "pcal_post.cuh"
 #include "pcal_analysis.cuh"
+#include "pcal_genstudy.cuh"
 
 using namespace pcal;
 typedef unsigned __int128 u128;
@@ -676,6 +677,38 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
+}
+
+// Generator accuracy study: one device thread per case.
+extern "C" int pcal_generator_study(const pcal_gen_case_t* cases, uint32_t n_cases, uint64_t n_steps, uint32_t n_chk,
+                                    double* out_err) {
+    if (!cases || !out_err || n_cases == 0 || n_chk == 0 || n_steps == 0 || n_steps >= (1ull << 40)) return PCAL_ERR_INVALID;
+    std::vector<GenStudyCase> h(n_cases);
+    for (uint32_t i = 0; i < n_cases; ++i) {
+        const pcal_gen_case_t& u = cases[i];
+        if (u.form < PCAL_GEN_CFO || u.form > PCAL_GEN_DIRECT || (u.precision != 32 && u.precision != 64)) return PCAL_ERR_INVALID;
+        if (!(u.f_s_hz > 0) || !(u.f_rot_hz >= 0) || !(u.f_rot_hz < u.f_s_hz)) return PCAL_ERR_INVALID;
+        GenStudyCase& g = h[i];
+        g.form = u.form; g.precision = u.precision; g.Fs = to_uhz(u.f_s_hz); g.F = to_uhz(u.f_rot_hz);
+        if (g.Fs == 0 || g.Fs >= (1ull << 61)) return PCAL_ERR_INVALID;
+        const double dphi = 2.0 * M_PI * (double)g.F / (double)g.Fs;         // eq. 2.5
+        g.cn = cos(dphi); g.sn = sin(dphi); g.eps = 2.0 * sin(0.5 * dphi); g.two_c = 2.0 * cos(dphi);
+        g.s_half = sin(0.5 * dphi); g.dphi32 = (float)dphi;
+    }
+    GenStudyCase* d_cases = nullptr;
+    double* d_err = nullptr;
+    const size_t eb = (size_t)n_cases * n_chk * sizeof(double);
+    if (cudaMalloc(&d_cases, n_cases * sizeof(GenStudyCase)) != cudaSuccess || cudaMalloc(&d_err, eb) != cudaSuccess) {
+        cudaFree(d_cases); cudaGetLastError(); return PCAL_ERR_DEVICE;
+    }
+    int rc = PCAL_OK;
+    if (cudaMemcpy(d_cases, h.data(), n_cases * sizeof(GenStudyCase), cudaMemcpyHostToDevice) != cudaSuccess) rc = PCAL_ERR_DEVICE;
+    if (rc == PCAL_OK) {
+        gen_study_kernel<<<(n_cases + 31) / 32, 32>>>(d_cases, n_cases, n_steps, n_chk, d_err);
+        if (cudaGetLastError() != cudaSuccess || cudaMemcpy(out_err, d_err, eb, cudaMemcpyDeviceToHost) != cudaSuccess) rc = PCAL_ERR_DEVICE;
+    }
+    cudaFree(d_cases); cudaFree(d_err); cudaGetLastError();
+    return rc;
 }
 
 extern "C" int pcal_set_profiling(pcal_ctx* c, int enable) {
