@@ -99,6 +99,26 @@ static void prof_collect(pcal_ctx* c) {
     cudaGetLastError();
 }
 
+// Programmatic dependent launch: the kernels of one step form a chain; each is launched with
+// programmatic stream serialization so that its CTAs can be scheduled while its predecessor is still
+// running (hiding the launch latency), and each starts with griddepcontrol.wait (pdl_wait_release in
+// pcal_common.cuh), i.e. touches memory only after the predecessor has completed and flushed.
+// PCAL_NO_PDL=1 falls back to plain stream order.
+static bool use_pdl() {
+    static const bool on = [] { const char* e = getenv("PCAL_NO_PDL"); return !(e && e[0] == '1'); }();
+    return on;
+}
+template <typename... KArgs, typename... Args>
+static void launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = use_pdl() ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 #define CU(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return PCAL_ERR_DEVICE; } } while (0)
 
 static void free_tables(pcal_ctx* c) {
@@ -369,9 +389,9 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         const uint64_t grid_threads = (uint64_t)c->R * kWarps * c->q * 32u;
         fp.n_quot = (uint32_t)(n_vec / grid_threads); fp.n_rem = n_vec % grid_threads;
         prof_mark(c, st);
-        if (c->kind == KIND_2BIT) c->fold2<<<c->grid, kThreads, 0, st>>>(fp);
-        else if (c->kind == KIND_I8) fold_i8_kernel<<<c->grid, kThreads, 0, st>>>(fp);
-        else fold_f32_kernel<<<c->grid, kThreads, 0, st>>>(fp);
+        if (c->kind == KIND_2BIT) launch_chain(c->fold2, c->grid, kThreads, 0, st, fp);
+        else if (c->kind == KIND_I8) launch_chain(fold_i8_kernel, c->grid, kThreads, 0, st, fp);
+        else launch_chain(fold_f32_kernel, c->grid, kThreads, 0, st, fp);
         prof_mark(c, st);
         c->launches += 1;
     }
@@ -382,7 +402,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         rr.kind = c->kind;
         const uint32_t total = c->q * c->F * 32u;
         rr.ns = c->R <= 8 ? 1u : (c->R <= 16 ? 2u : (c->R <= 32 ? 4u : 8u));
-        reduce_replicas_kernel<<<total / ((uint32_t)kPostThreads / rr.ns), kPostThreads, 0, st>>>(rr);
+        launch_chain(reduce_replicas_kernel, total / ((uint32_t)kPostThreads / rr.ns), kPostThreads, 0, st, rr);
         c->launches += 1;
     }
     RotateParams rp;
@@ -395,7 +415,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     rp.integer_exact = (c->all_zero && c->kind != KIND_F32) ? 1 : 0;
     rp.overwrite = c->zero_pending ? 1 : 0;
     const uint32_t pairs = c->n_bins * (uint32_t)c->C, ppc = (uint32_t)kPostThreads / c->rot_tpp;
-    rotate_fold_kernel<<<(pairs + ppc - 1) / ppc, kPostThreads, 0, st>>>(rp);
+    launch_chain(rotate_fold_kernel, (pairs + ppc - 1) / ppc, kPostThreads, 0, st, rp);
     c->zero_pending = false;
     c->launches += 1;
     CU(cudaGetLastError());
@@ -422,9 +442,9 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
-        if (c->kind == KIND_2BIT) gen_kernel<KIND_2BIT><<<c->gen_grid, kThreads, smem, st>>>(gp);
-        else if (c->kind == KIND_I8) gen_kernel<KIND_I8><<<c->gen_grid, kThreads, smem, st>>>(gp);
-        else gen_kernel<KIND_F32><<<c->gen_grid, kThreads, smem, st>>>(gp);
+        if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
+        else if (c->kind == KIND_I8) launch_chain(gen_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
+        else launch_chain(gen_kernel<KIND_F32>, c->gen_grid, kThreads, smem, st, gp);
         prof_mark(c, st);
         c->launches += 1;
     }
@@ -433,7 +453,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     gr.n0 = c->n_processed; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
     gr.grid = n_loads ? c->gen_grid : 0; gr.n_bins = c->n_bins; gr.kind = c->kind; gr.sign_mag = c->sign_mag;
     gr.overwrite = c->zero_pending ? 1 : 0;
-    post_gen_kernel<<<(c->n_bins + 31) / 32, kPostThreads, 0, st>>>(gr);
+    launch_chain(post_gen_kernel, (c->n_bins + 31) / 32, kPostThreads, 0, st, gr);
     c->zero_pending = false;
     c->launches += 1;
     CU(cudaGetLastError());
@@ -537,8 +557,8 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     if (rz != PCAL_OK) return rz;
     const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
     const uint32_t per_cta = kDftThreads / 32;
-    dft_kernel<<<dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream>>>(
-        c->d_P, c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift);
+    launch_chain(dft_kernel, dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream,
+                 (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;

@@ -25,6 +25,14 @@ __device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
     return r;
 }
 
+// First statement of every kernel of the per-step chain (see launch_chain in pcal_api.cu): wait
+// until the predecessor grid has completed and its writes are visible, then allow the successor's
+// CTAs to be scheduled behind this grid.  A no-op when the kernel was launched in plain stream order.
+__device__ __forceinline__ void pdl_wait_release() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 __device__ __forceinline__ uint32_t lop3_xor3(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t r;
     asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(r) : "r"(a), "r"(b), "r"(c));

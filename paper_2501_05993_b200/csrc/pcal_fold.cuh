@@ -56,6 +56,7 @@ constexpr int kFoldGroup = 16;   // loads per complete counter cascade
 
 template <bool SIGN_MAG, int U, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P) {
+    pdl_wait_release();
     static_assert(U == 4 || U == 8, "block of 4 or 8 loads");
     __shared__ uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -178,6 +179,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
 // Output: int32 partial[cta][16][32].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
+    pdl_wait_release();
     __shared__ int32_t sh[kWarps][16][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
@@ -220,6 +222,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
 // Output: double partial[cta][4][32].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
+    pdl_wait_release();
     __shared__ double sh[kWarps][4][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);

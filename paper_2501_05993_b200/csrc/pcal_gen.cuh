@@ -147,6 +147,7 @@ constexpr size_t gen_smem_bytes() {
 
 template <int KIND>
 __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
+    pdl_wait_release();
     constexpr int SPT = GenTraits<KIND>::SPT;
     constexpr int LB = GenCfg<KIND>::LB, LPT = GenCfg<KIND>::LPT, RUN = GenCfg<KIND>::RUN, DEPTH = GenCfg<KIND>::DEPTH;
     constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration
