@@ -112,6 +112,17 @@ int pcal_set_k_shift(pcal_ctx *ctx, int k);
 int pcal_set_start_index(pcal_ctx *ctx, uint64_t n_start);
 
 /*
+ * Promise about the sample buffers (default 0).  The kernels of a context are chained by programmatic
+ * dependent launch.  With ready != 0 the caller guarantees that every dev_samples buffer handed to
+ * pcal_extract / pcal_extract_series is completely written BEFORE the call (e.g. by an earlier,
+ * synchronised transfer; data resident in HBM) -- not produced by work that may still be running on
+ * cuda_stream.  The streaming kernel then reads its input while the small kernels of the previous
+ * segment are still finishing (it still waits for them before it writes anything).  With 0 it first
+ * waits for all earlier work of the stream, like any kernel.  Results are identical either way.
+ */
+int pcal_set_input_ready(pcal_ctx *ctx, int ready);
+
+/*
  * Rotate + fold one segment (eq. 2.3 + eq. 2.2) into the context's accumulators.
  *   dev_samples    [device] 16-byte aligned, caller-owned, valid until the stream work completes
  *   n_samples      samples PER CHANNEL in this segment; n_samples*bits*n_channels must be a

@@ -75,6 +75,7 @@ def lib():
             "pcal_set_rotator": (i32, [vp, i32]),
             "pcal_set_k_shift": (i32, [vp, i32]),
             "pcal_set_start_index": (i32, [vp, u64]),
+            "pcal_set_input_ready": (i32, [vp, i32]),
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
@@ -144,6 +145,9 @@ class Pcal:
 
     def set_k_shift(self, k: int):
         _check(lib().pcal_set_k_shift(self._h, k), "pcal_set_k_shift")
+
+    def set_input_ready(self, ready: bool):
+        _check(lib().pcal_set_input_ready(self._h, int(ready)), "pcal_set_input_ready")
 
     def set_start_index(self, n_start: int):
         _check(lib().pcal_set_start_index(self._h, n_start), "pcal_set_start_index")

@@ -69,6 +69,7 @@ struct pcal_ctx {
     void *d_partial, *d_stage;
     double* d_val;                  // [q][F][32] replica sums (stage 1 of pcal_post.cuh)
     uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
+    bool input_ready;               // pcal_set_input_ready: sample buffers are complete when extract is called
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
     double *d_summary, *h_ana;      // analysis outputs: [C][8] + band-pass [C][N] complex
@@ -238,6 +239,12 @@ extern "C" int pcal_set_k_shift(pcal_ctx* c, int k) {
     return PCAL_OK;
 }
 
+extern "C" int pcal_set_input_ready(pcal_ctx* c, int ready) {
+    if (!c) return PCAL_ERR_INVALID;
+    c->input_ready = ready != 0;
+    return PCAL_OK;
+}
+
 extern "C" int pcal_set_start_index(pcal_ctx* c, uint64_t n_start) {
     if (!c) return PCAL_ERR_INVALID;
     if (c->started) return PCAL_ERR_STATE;
@@ -388,6 +395,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         fp.n_iter = (uint32_t)it; fp.partial = c->d_partial;
         const uint64_t grid_threads = (uint64_t)c->R * kWarps * c->q * 32u;
         fp.n_quot = (uint32_t)(n_vec / grid_threads); fp.n_rem = n_vec % grid_threads;
+        fp.input_ready = c->input_ready ? 1 : 0;
         prof_mark(c, st);
         if (c->kind == KIND_2BIT) launch_chain(c->fold2, c->grid, kThreads, 0, st, fp);
         else if (c->kind == KIND_I8) launch_chain(fold_i8_kernel, c->grid, kThreads, 0, st, fp);
@@ -440,6 +448,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
         gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
+        gp.input_ready = c->input_ready ? 1 : 0;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
         if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
@@ -543,7 +552,10 @@ extern "C" int pcal_extract_host(pcal_ctx* c, const void* host_samples, uint64_t
         const uint64_t bytes = total - off < kStageBytes ? total - off : kStageBytes;
         uint8_t* d = reinterpret_cast<uint8_t*>(c->d_stage) + (size_t)buf * kStageBytes;
         CU(cudaMemcpyAsync(d, h + off, bytes, cudaMemcpyHostToDevice, st));
+        const bool promised = c->input_ready;
+        c->input_ready = false;                        // the staging buffer is being written on this very stream
         const int r = pcal_extract(c, d, bytes * 8 / bits_per_t, st);
+        c->input_ready = promised;
         if (r != PCAL_OK) return r;
     }
     CU(cudaStreamSynchronize(st));

@@ -25,13 +25,16 @@ __device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
     return r;
 }
 
-// First statement of every kernel of the per-step chain (see launch_chain in pcal_api.cu): wait
-// until the predecessor grid has completed and its writes are visible, then allow the successor's
-// CTAs to be scheduled behind this grid.  A no-op when the kernel was launched in plain stream order.
-__device__ __forceinline__ void pdl_wait_release() {
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-}
+// Programmatic dependent launch (see launch_chain in pcal_api.cu).  pdl_release(): first statement of
+// every kernel of the per-step chain -- the successor's CTAs may be scheduled behind this grid.
+// pdl_wait(): returns once the predecessor grid has COMPLETED and its writes are visible; a kernel
+// calls it before its first access to memory that any earlier kernel of the chain reads or writes.
+// Since a grid cannot complete before its own pdl_wait() has returned, completion is transitive along
+// the chain no matter how early the release is issued.  The streaming kernels (fold_*, gen_kernel)
+// only read the caller's input before the wait, so their load phase overlaps the small kernels of the
+// previous step/segment.  Both are no-ops when the kernel was launched in plain stream order.
+__device__ __forceinline__ void pdl_release() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __device__ __forceinline__ uint32_t lop3_xor3(uint32_t a, uint32_t b, uint32_t c) {
     uint32_t r;

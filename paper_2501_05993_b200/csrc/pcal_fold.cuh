@@ -32,6 +32,7 @@ struct FoldParams {
     uint32_t n_quot;        // n_vec / (threads in the grid): loads every thread makes ...
     uint64_t n_rem;         // ... plus one for the threads whose first vector index is < n_vec % threads
     void* partial;          // [device] per-CTA partial sums, layout [cta][field][lane]
+    int input_ready;        // caller promised the input is complete: stream it before pdl_wait()
 };
 
 __device__ __forceinline__ uint64_t fold_first_vec(const FoldParams& P, int w, int lane) {
@@ -56,7 +57,8 @@ constexpr int kFoldGroup = 16;   // loads per complete counter cascade
 
 template <bool SIGN_MAG, int U, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P) {
-    pdl_wait_release();
+    pdl_release();
+    if (!P.input_ready) pdl_wait();
     static_assert(U == 4 || U == 8, "block of 4 or 8 loads");
     __shared__ uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -161,6 +163,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
         }
     }
     __syncthreads();
+    pdl_wait();   // the partials of the previous launch may still be read by its reduce kernel
     uint16_t* out = reinterpret_cast<uint16_t*>(P.partial) + (size_t)blockIdx.x * 64 * 32;
 #pragma unroll
     for (int x = tid; x < 32 * 32; x += kThreads) {
@@ -179,7 +182,8 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
 // Output: int32 partial[cta][16][32].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
-    pdl_wait_release();
+    pdl_release();
+    if (!P.input_ready) pdl_wait();
     __shared__ int32_t sh[kWarps][16][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
@@ -206,6 +210,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
 #pragma unroll
     for (int k = 0; k < 16; ++k) sh[w][k][lane] = acc[k];
     __syncthreads();
+    pdl_wait();
     int32_t* out = reinterpret_cast<int32_t*>(P.partial) + (size_t)blockIdx.x * 16 * 32;
     for (int e = threadIdx.x; e < 16 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;
@@ -222,7 +227,8 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
 // Output: double partial[cta][4][32].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
-    pdl_wait_release();
+    pdl_release();
+    if (!P.input_ready) pdl_wait();
     __shared__ double sh[kWarps][4][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
@@ -253,6 +259,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
 #pragma unroll
     for (int k = 0; k < 4; ++k) sh[w][k][lane] = tot[k];
     __syncthreads();
+    pdl_wait();
     double* out = reinterpret_cast<double*>(P.partial) + (size_t)blockIdx.x * 4 * 32;
     for (int e = threadIdx.x; e < 4 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;

@@ -41,6 +41,7 @@ struct GenParams {
     double2* partial;        // [device] [cta][n_bins]
     uint32_t n_bins;
     int sign_mag;
+    int input_ready;              // caller promised the input is complete: stream it before pdl_wait()
     uint32_t dec_mask, dec_one;   // 0x00600000, 0x3F800000 (2-bit decode, see lop3_and_or)
 };
 
@@ -147,7 +148,8 @@ constexpr size_t gen_smem_bytes() {
 
 template <int KIND>
 __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
-    pdl_wait_release();
+    pdl_release();
+    if (!P.input_ready) pdl_wait();
     constexpr int SPT = GenTraits<KIND>::SPT;
     constexpr int LB = GenCfg<KIND>::LB, LPT = GenCfg<KIND>::LPT, RUN = GenCfg<KIND>::RUN, DEPTH = GenCfg<KIND>::DEPTH;
     constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration
@@ -276,6 +278,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
 #pragma unroll
     for (int k = 0; k < SPT; ++k) { pos_re[tid * SPT + k] = zr[k]; pos_im[tid * SPT + k] = zi[k]; }
     __syncthreads();
+    pdl_wait();   // the partial bins of the previous launch may still be read by its post kernel
     for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
         double re = 0.0, im = 0.0;
         for (uint32_t pos = sb; pos < SPAN; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }

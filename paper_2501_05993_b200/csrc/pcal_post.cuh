@@ -44,7 +44,8 @@ __device__ __forceinline__ Tacc replica_sum(const Tin* src, size_t stride, uint3
 // the host so that a slice has at most ~8 replicas): thread = (slice, element), consecutive
 // threads read consecutive elements (coalesced); the slice sums are then added in slice order.
 __global__ void __launch_bounds__(kPostThreads) reduce_replicas_kernel(ReplicaParams P) {
-    pdl_wait_release();
+    pdl_release();
+    pdl_wait();
     __shared__ double sd[kPostThreads];
     __shared__ long long si[kPostThreads];
     const uint32_t E = P.F * 32u, total = P.q * E;          // total is a multiple of 256
@@ -110,7 +111,8 @@ __device__ __forceinline__ double decode_tail(int kind, int sign_mag, const uint
 // thread u adds its elements j = u, u + tpp, ... in order (four look-ups in flight), then the
 // lane sums are combined by a fixed butterfly (and, for tpp = 256, the 8 warp sums in warp order).
 __global__ void __launch_bounds__(kPostThreads) rotate_fold_kernel(RotateParams P) {
-    pdl_wait_release();
+    pdl_release();
+    pdl_wait();
     __shared__ double sre[kPostThreads / 32], sim[kPostThreads / 32];
     __shared__ long long sint[kPostThreads / 32];
     const uint32_t tid = threadIdx.x, lane = tid & 31u, w = tid >> 5;
@@ -214,7 +216,8 @@ struct GenPostParams {
 // One CTA per 32 consecutive bins: warp w sums the CTAs w, w+8, ... (coalesced 512-byte rows),
 // the 8 warp sums are added in warp order, then the ragged tail with exactly reduced phases.
 __global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G) {
-    pdl_wait_release();
+    pdl_release();
+    pdl_wait();
     __shared__ double sre[kPostThreads / 32][32], sim[kPostThreads / 32][32];
     const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
     const uint32_t b = blockIdx.x * 32u + lane;
@@ -258,7 +261,8 @@ constexpr int kDftThreads = 256;
 __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restrict__ P, const double2* __restrict__ W,
                                                           double2* __restrict__ T, double2* __restrict__ T_host,
                                                           uint32_t N, uint32_t k_shift) {
-    pdl_wait_release();
+    pdl_release();
+    pdl_wait();
     extern __shared__ double2 dft_sm[];  // [N] bins of this channel, [N] twiddles
     double2* sp = dft_sm;
     double2* sw = dft_sm + N;

@@ -244,3 +244,38 @@ def test_segments_longer_than_one_launch(oracle, idx, n, rot, monkeypatch):
     p2, T2, _ = gpu_run(w, dev, rotator=rot)
     assert p2.info().kernel_launches < p.info().kernel_launches
     assert_close(T, T2, f"cfg{idx} pieces vs single launch")
+
+
+@pytest.mark.parametrize("idx,n,rot", [(2, 3_000_004, None), (4, 300_003, None), (5, 2_000_003, None), (3, 2_000_004, "generator")])
+def test_input_ready_promise_changes_nothing(oracle, idx, n, rot):
+    """pcal_set_input_ready(1) lets the streaming kernel read its input before the previous segment's small
+    kernels have finished (programmatic dependent launch); many back-to-back segments and resets must give
+    bit-identical results to the conservative order, and match the oracle."""
+    w, dev, host = make(idx, n)
+    if rot:
+        w = synth.replace(w, rotator=rot)
+    from paper_2501_05993_b200 import binding
+    outs = []
+    for ready in (False, True):
+        p = binding.from_workload(w)
+        p.set_input_ready(ready)
+        res = []
+        pinned = torch.empty((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory()
+        for rep in range(6):                      # reset + extract + finalize_async back to back, no sync
+            p.reset()
+            p.extract(dev, n)
+            p.finalize_async(pinned)
+        torch.cuda.synchronize()
+        res.append(pinned.numpy().copy())
+        p.reset()
+        bytes_per_t = w.bits * w.n_channels // 8 if w.bits * w.n_channels >= 8 else None
+        half = (n // 2) // 64 * 64
+        flat = dev.view(-1).view(dtype=torch.uint8)
+        cut = half * w.bits * w.n_channels // 8
+        p.extract(flat[:cut], half)
+        p.extract(flat[cut:], n - half)
+        res.append(p.finalize())
+        outs.append(res)
+        p.destroy()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert_close(outs[1][0][0], oracle_tones(oracle, w, host, 0), f"cfg{idx} input_ready")
