@@ -279,3 +279,30 @@ def test_input_ready_promise_changes_nothing(oracle, idx, n, rot):
         p.destroy()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     assert_close(outs[1][0][0], oracle_tones(oracle, w, host, 0), f"cfg{idx} input_ready")
+
+
+@pytest.mark.parametrize("C,enc", [(2, 0), (4, 1), (8, 0), (16, 1)])
+def test_every_power_of_two_channel_count(oracle, C, enc):
+    """Demultiplexing ("several baseband channels"): one field of 2C bits per time sample, packed
+    LSB-first; channel c in bits 2c..2c+1 of its field.  Random codes, mixed zero / non-zero offsets."""
+    from paper_2501_05993_b200 import binding
+    n = 300_004
+    rs = np.random.RandomState(4200 + C)
+    codes = rs.randint(0, 4, size=(n, C)).astype(np.uint8)
+    flat = codes.reshape(-1, 4)
+    packed = (flat[:, 0] | (flat[:, 1] << 2) | (flat[:, 2] << 4) | (flat[:, 3] << 6)).astype(np.uint8)
+    offs = [0.0 if c % 3 == 0 else 10e3 * (1 + c) for c in range(C)]
+    p = binding.Pcal(64e6, 1e6, 0.0, 2, enc, C)
+    p.set_channel_offsets(offs)
+    dev = torch.from_numpy(packed).cuda()
+    p.extract(dev, n)
+    T, P = p.finalize(), p.get_folded()
+    fmt = oracle.TWO_BIT_SIGN_MAG if enc else oracle.TWO_BIT_OFFSET_BINARY
+    for c in range(C):
+        pr, pi = oracle.fold_ld(packed, fmt, C, c, 0, 1, n, 0, 64e6, 1e6, offs[c], tabulated=True)
+        assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"C={C} ch{c} folded")
+        assert_close(T[c], oracle.dft(pr, pi), f"C={C} ch{c} tones")
+        if offs[c] == 0.0:
+            want = oracle.fold_i64(packed, fmt, C, c, 0, 1, n, 0, 64)
+            assert np.array_equal(P[c].real, want.astype(np.float64)) and not P[c].imag.any()
+    p.destroy()
