@@ -132,7 +132,7 @@ def time_oracle(w, n_sample: int, steps: int = 1):
 
 def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do_e2e: bool = True,
             rotator: str | None = None, n_override: int | None = None, min_warm_s: float = 0.5,
-            no_graph: bool = False):
+            no_graph: bool = False, exchange: bool = False):
     """Run config idx on this rank's GPU; returns the measurement dict (device timing is per rank)."""
     import torch
     import torch.distributed as dist
@@ -152,19 +152,19 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     p.set_input_ready(True)      # inputs are resident in HBM and complete before the timed region starts
     out_pinned = torch.empty((C, nb), dtype=torch.complex128).pin_memory()
     local = torch.empty(C * nb * 2, dtype=torch.float64, device=device)
+    gathered = torch.empty(world * C * nb * 2, dtype=torch.float64, device=device)
+
+    exchange = exchange or world > 1
 
     def step(i):
         p.reset()
-        if world > 1:
+        if exchange:
             p.set_start_index(rank * n)
         p.extract(bufs[i % ncopies], n)
-        if world > 1:  # the one exchange step: all-gather the bins, add them in rank order
+        if exchange:  # the one exchange step: all-gather the bins, add them in rank order
             p.get_folded_dev(local)
-            parts = [torch.empty_like(local) for _ in range(world)]
-            dist.all_gather(parts, local)
-            p.reset()
-            for part in parts:
-                p.add_folded_dev(part)
+            dist.all_gather_into_tensor(gathered, local)
+            p.set_folded_sum_dev(gathered, world)
         p.finalize_async(out_pinned)
 
     # clocks are sampled from the start of the warm-up to the end of the timed region (a timed
@@ -187,7 +187,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     # launch, so each kernel is scheduled while its predecessor still runs; (b) one CUDA-graph replay per
     # step (each distinct input copy gets its step captured once).  Multi-GPU steps (NCCL exchange)
     # launch directly.
-    use_graph = (world == 1) and not no_graph
+    use_graph = (world == 1) and not no_graph and not exchange
     graphs, per_step_launches = [], None
     if use_graph:
         side = torch.cuda.Stream()
@@ -334,6 +334,8 @@ def main():
     ap.add_argument("--samples", type=int, default=0, help="override samples per channel (debug)")
     ap.add_argument("--rotator", default=None, choices=["lut", "generator"], help="force the rotator variant (config 3 runs both)")
     ap.add_argument("--no-graph", action="store_true", help="launch every step directly instead of replaying a CUDA graph")
+    ap.add_argument("--force-exchange", action="store_true",
+                    help="testing: run the multi-GPU exchange path (NCCL all-gather + rank-order sum) even with one rank")
     ap.add_argument("--quick", action="store_true",
                     help="profiling mode (ncu): exactly W warm-up steps, no e2e / cpu_baseline / per-config table")
     args = ap.parse_args()
@@ -367,10 +369,12 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
-    if world > 1:
+    if world > 1 or args.force_exchange:
+        if "RANK" not in os.environ:
+            os.environ.update({"RANK": "0", "WORLD_SIZE": "1", "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": "29533"})
         dist.init_process_group("nccl", device_id=device)
     res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None,
-                     rotator=args.rotator, no_graph=args.no_graph, do_e2e=not args.quick, min_warm_s=0.0 if args.quick else 0.5)
+                     rotator=args.rotator, no_graph=args.no_graph, exchange=args.force_exchange, do_e2e=not args.quick, min_warm_s=0.0 if args.quick else 0.5)
     line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": res["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
@@ -402,7 +406,7 @@ def main():
             line["all_configs"] = table
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if world > 1 or args.force_exchange:
         dist.destroy_process_group()
 
 

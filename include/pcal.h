@@ -200,6 +200,11 @@ int pcal_add_folded(pcal_ctx *ctx, const double *bins);
 int pcal_get_folded_dev(pcal_ctx *ctx, double *dev_bins);
 int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
 
+/* The exchange step in one launch: accumulators <- sum over r of dev_parts[r] (r = 0..n_parts-1, in that
+ * order: deterministic), dev_parts = [device] n_parts contiguous blocks in the layout of pcal_get_folded_dev
+ * (e.g. the output of an NCCL all-gather of every rank's bins).  Replaces the previous contents. */
+int pcal_set_folded_sum_dev(pcal_ctx *ctx, const double *dev_parts, uint32_t n_parts);
+
 /* Timing hook for the roofline report: when enabled, every launch of the hot kernel (the fused
  * load/decode/fold kernel of the LUT path or the generator kernel) is bracketed by CUDA events on
  * the launching stream.  pcal_get_profile synchronises the stream and returns the summed event time

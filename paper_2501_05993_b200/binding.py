@@ -79,6 +79,7 @@ def lib():
             "pcal_extract": (i32, [vp, vp, u64, vp]),
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
+            "pcal_set_folded_sum_dev": (i32, [vp, vp, ctypes.c_uint32]),
             "pcal_generator_study": (i32, [vp, ctypes.c_uint32, u64, ctypes.c_uint32, vp]),
             "pcal_extract_series": (i32, [vp, vp, u64, ctypes.c_uint32, vp, vp, vp]),
             "pcal_analyze": (i32, [vp, vp, vp]),
@@ -229,6 +230,10 @@ class Pcal:
         """Calibration: enqueue a pure streaming read of the whole device tensor (roofline report)."""
         nbytes = dev_buf.numel() * dev_buf.element_size()
         _check(lib().pcal_read_probe(self._h, dev_buf.data_ptr(), nbytes, _stream_handle(stream)), "pcal_read_probe")
+
+    def set_folded_sum_dev(self, dev_parts, n_parts: int):
+        """Accumulators <- sum of n_parts gathered bin blocks (rank order); dev_parts: CUDA float64 tensor."""
+        _check(lib().pcal_set_folded_sum_dev(self._h, dev_parts.data_ptr(), n_parts), "pcal_set_folded_sum_dev")
 
     def set_profiling(self, enable: bool):
         _check(lib().pcal_set_profiling(self._h, int(enable)), "pcal_set_profiling")

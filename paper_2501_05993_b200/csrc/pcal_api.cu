@@ -699,6 +699,16 @@ extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
     return PCAL_OK;
 }
 
+extern "C" int pcal_set_folded_sum_dev(pcal_ctx* c, const double* dev_parts, uint32_t n_parts) {
+    if (!c || !dev_parts || n_parts == 0) return PCAL_ERR_INVALID;
+    const uint32_t n = c->n_bins * (uint32_t)c->C;
+    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_parts), n, n_parts);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->zero_pending = false;      // the accumulators now hold exactly the sum
+    return PCAL_OK;
+}
+
 extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, void* cuda_stream) {
     if (!c || !dev) return PCAL_ERR_INVALID;
     if ((uintptr_t)dev & 15u) return PCAL_ERR_ALIGNMENT;

@@ -301,6 +301,15 @@ __global__ void zero_kernel(double2* P, long long* Pint, uint32_t n) {
     if (i < n) { P[i] = make_double2(0.0, 0.0); Pint[i] = 0; }
 }
 
+// P[i] = sum_r parts[r][i], r = 0 .. n_parts-1 in that order (the exchange step of a time-sharded run)
+__global__ void sum_parts_kernel(double2* P, const double2* parts, uint32_t n, uint32_t n_parts) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double re = 0.0, im = 0.0;
+    for (uint32_t r = 0; r < n_parts; ++r) { const double2 v = parts[(size_t)r * n + i]; re += v.x; im += v.y; }
+    P[i] = make_double2(re, im);
+}
+
 __global__ void add_bins_kernel(double2* P, const double2* add, uint32_t n) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) { P[i].x += add[i].x; P[i].y += add[i].y; }

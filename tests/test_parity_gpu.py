@@ -306,3 +306,29 @@ def test_every_power_of_two_channel_count(oracle, C, enc):
             want = oracle.fold_i64(packed, fmt, C, c, 0, 1, n, 0, 64)
             assert np.array_equal(P[c].real, want.astype(np.float64)) and not P[c].imag.any()
     p.destroy()
+
+
+def test_exchange_step_in_one_launch(oracle):
+    """What bench.py does per step with N ranks, emulated on one GPU: every "rank" folds its time shard at
+    its absolute start index, the bins are gathered into one buffer (stand-in for the NCCL all-gather) and
+    pcal_set_folded_sum_dev adds them in rank order."""
+    from paper_2501_05993_b200 import binding
+    w, dev, host = make(2, 1_200_000)
+    world, per = 3, 400_000
+    flat = dev.view(torch.uint8)
+    gathered = torch.empty(world * w.n_bins * 2, dtype=torch.float64, device=DEV)
+    ctxs = []
+    for r in range(world):
+        p = binding.from_workload(w)
+        p.set_start_index(r * per)
+        p.extract(flat[r * per // 4:(r + 1) * per // 4], per)
+        p.get_folded_dev(gathered[r * w.n_bins * 2:(r + 1) * w.n_bins * 2])
+        ctxs.append(p)
+    torch.cuda.synchronize()
+    outs = []
+    for p in ctxs:                                  # every rank ends with the same bits
+        p.reset()
+        p.set_folded_sum_dev(gathered, world)
+        outs.append(p.finalize())
+    assert all(np.array_equal(outs[0], o) for o in outs[1:])
+    assert_close(outs[0][0], oracle_tones(oracle, w, host, 0), "gathered exchange")
