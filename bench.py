@@ -148,24 +148,45 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     # distinct input copies so that every step reads from DRAM, not from the 126 MB L2
     ncopies = 1 if w.n_bytes >= (300 << 20) else min(8, -(-(300 << 20) // w.n_bytes))
     bufs = [synth.generate(replace(w, seed=w.seed + 100 * i + 7 * rank), device) for i in range(ncopies)]
-    p = binding.from_workload(w)
-    p.set_input_ready(True)      # inputs are resident in HBM and complete before the timed region starts
-    out_pinned = torch.empty((C, nb), dtype=torch.complex128).pin_memory()
-    local = torch.empty(C * nb * 2, dtype=torch.float64, device=device)
-    gathered = torch.empty(world * C * nb * 2, dtype=torch.float64, device=device)
-
     exchange = exchange or world > 1
+    # Multi-GPU: two contexts ("lanes") alternate, so that the all-gather of integration k is in flight
+    # (on NCCL's stream) while integration k+1 is being folded and integration k-1 is being finished.
+    ctxs = [binding.from_workload(w) for _ in range(2 if exchange else 1)]
+    for q_ in ctxs:
+        q_.set_input_ready(True)  # inputs are resident in HBM and complete before the timed region starts
+    p = ctxs[0]
+    out_pinned = torch.empty((C, nb), dtype=torch.complex128).pin_memory()
+    lanes = [{"p": q_, "work": None,
+              "local": torch.empty(C * nb * 2, dtype=torch.float64, device=device),
+              "gathered": torch.empty(world * C * nb * 2, dtype=torch.float64, device=device),
+              "out": torch.empty((C, nb), dtype=torch.complex128).pin_memory()} for q_ in ctxs]
+
+    def complete(L):
+        """The one exchange step, second half: rank-order sum of the gathered bins, DFT, result to the host."""
+        if L["work"] is not None:
+            L["work"].wait()                              # the current stream waits for the all-gather
+            L["p"].set_folded_sum_dev(L["gathered"], world)
+            L["p"].finalize_async(L["out"])
+            L["work"] = None
+
+    def drain():
+        for L in lanes:
+            complete(L)
 
     def step(i):
-        p.reset()
-        if exchange:
-            p.set_start_index(rank * n)
-        p.extract(bufs[i % ncopies], n)
-        if exchange:  # the one exchange step: all-gather the bins, add them in rank order
-            p.get_folded_dev(local)
-            dist.all_gather_into_tensor(gathered, local)
-            p.set_folded_sum_dev(gathered, world)
-        p.finalize_async(out_pinned)
+        if not exchange:
+            p.reset()
+            p.extract(bufs[i % ncopies], n)
+            p.finalize_async(out_pinned)
+            return
+        L = lanes[i % 2]
+        complete(L)                                       # this lane's previous integration, if still open
+        L["p"].reset()
+        L["p"].set_start_index(rank * n)                  # time shard of rank r starts at r*n
+        L["p"].extract(bufs[i % ncopies], n)
+        L["p"].get_folded_dev(L["local"])
+        L["work"] = dist.all_gather_into_tensor(L["gathered"], L["local"], async_op=True)
+        complete(lanes[(i + 1) % 2])                      # finish the other lane under this all-gather
 
     # clocks are sampled from the start of the warm-up to the end of the timed region (a timed
     # region of K short steps alone can be shorter than one nvidia-smi period); the warm-up runs
@@ -180,6 +201,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         i += 1
         if i % 16 == 0:
             torch.cuda.synchronize()
+    drain()
     torch.cuda.synchronize()
     # Single GPU: the step (reset + extract + finalize_async: 3-4 kernels) is launch-bound for the small
     # configs.  Two ways to issue it are calibrated after the warm-up and the faster one is used for the
@@ -216,7 +238,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         t_graph = min(timed(lambda k: graphs[k % ncopies].replay(), reps) for _ in range(2))
         t_direct = min(timed(step, reps) for _ in range(2))
         use_graph = t_graph <= t_direct
-    launches0 = p.info().kernel_launches
+    launches0 = sum(q_.info().kernel_launches for q_ in ctxs)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -227,20 +249,26 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
             graphs[i % ncopies].replay()
         else:
             step(i)
+    drain()
     e1.record()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     ms = e0.elapsed_time(e1)
-    launches = per_step_launches * steps if use_graph else p.info().kernel_launches - launches0
+    launches = per_step_launches * steps if use_graph else sum(q_.info().kernel_launches for q_ in ctxs) - launches0
     # second pass over the same K steps, launched directly, with the hot kernel bracketed by CUDA
     # events on the launching stream (pcal_set_profiling): the roofline numerator
-    p.set_profiling(True)
+    for q_ in ctxs:
+        q_.set_profiling(True)
     for i in range(steps):
         step(i)
+    drain()
     torch.cuda.synchronize()
-    hot_ms, hot_launches = p.get_profile()
-    p.set_profiling(False)
+    hot_ms, hot_launches = 0.0, 0
+    for q_ in ctxs:
+        ms_q, n_q = q_.get_profile()
+        hot_ms, hot_launches = hot_ms + ms_q, hot_launches + n_q
+        q_.set_profiling(False)
     clocks = sampler.stop() if rank == 0 else None
     del graphs
     if world > 1:
@@ -317,7 +345,8 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
                       "d2h_bytes_per_step": C * nb * 16, "steps": e2e_steps,
                       "api": "pcal_reset + pcal_extract_host (pinned host buffer) + pcal_finalize"}
         del host
-    p.destroy()
+    for q_ in ctxs:
+        q_.destroy()
     del bufs
     torch.cuda.empty_cache()
     return res, w
