@@ -222,40 +222,54 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
                     step(k)
                 per_step_launches = p.info().kernel_launches - l0
                 graphs.append(g)
+            big = torch.cuda.CUDAGraph()              # ncopies consecutive steps in ONE graph
+            with torch.cuda.graph(big, stream=side):
+                for k in range(ncopies):
+                    step(k)
         torch.cuda.current_stream().wait_stream(side)
-        def timed(fn, reps):
-            for k in range(3):
-                fn(k)
+
+    def run_steps(mode, count):
+        if mode == "graph_per_step":
+            for k in range(count):
+                graphs[k % ncopies].replay()
+        elif mode == "graph_of_steps":
+            for _ in range(count // ncopies):
+                big.replay()
+            for k in range(count % ncopies):
+                step(k)
+        else:
+            for k in range(count):
+                step(k)
+        drain()
+
+    mode = "direct"
+    if use_graph:
+        def timed(m, reps):
+            run_steps(m, ncopies)
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
-            for k in range(reps):
-                fn(k)
+            run_steps(m, reps)
             b.record()
             torch.cuda.synchronize()
             return a.elapsed_time(b) / reps
-        reps = max(10, steps)
-        t_graph = min(timed(lambda k: graphs[k % ncopies].replay(), reps) for _ in range(2))
-        t_direct = min(timed(step, reps) for _ in range(2))
-        use_graph = t_graph <= t_direct
+        reps = max(2 * ncopies, steps)
+        cal = {m: min(timed(m, reps) for _ in range(2)) for m in ("direct", "graph_per_step", "graph_of_steps")}
+        mode = min(cal, key=cal.get)
     launches0 = sum(q_.info().kernel_launches for q_ in ctxs)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for i in range(steps):
-        if use_graph:
-            graphs[i % ncopies].replay()
-        else:
-            step(i)
-    drain()
+    run_steps(mode, steps)
     e1.record()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     ms = e0.elapsed_time(e1)
     launches = per_step_launches * steps if use_graph else sum(q_.info().kernel_launches for q_ in ctxs) - launches0
+    use_graph = mode != "direct"
     # second pass over the same K steps, launched directly, with the hot kernel bracketed by CUDA
     # events on the launching stream (pcal_set_profiling): the roofline numerator
     for q_ in ctxs:
@@ -271,6 +285,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         q_.set_profiling(False)
     clocks = sampler.stop() if rank == 0 else None
     del graphs
+    big = None
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device=device)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -284,8 +299,11 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         "input_gbs": world * w.n_bytes * steps / (ms * 1e-3) / 1e9,
         "hot_kernel_us": 1e3 * hot_ms / max(hot_launches, 1), "hot_kernel_launches": int(hot_launches),
         "gpu_launches": int(launches),
-        "launch_mode": "cuda_graph: one graph replay per step (reset + extract + finalize_async captured once per input copy)"
-        if use_graph else "direct launches (kernels chained by programmatic dependent launch)",
+        "launch_mode": {"direct": "direct launches (kernels chained by programmatic dependent launch)",
+                        "graph_per_step": "cuda_graph: one graph replay per step (reset + extract + finalize_async captured once per input copy)",
+                        "graph_of_steps": f"cuda_graph: one replay per {ncopies} consecutive steps (one per input copy), kernels chained "
+                                          "by programmatic dependent launch inside the graph; remainder steps launched directly"}[mode],
+        "launch_mode_calibration_us": {k_: 1e3 * v_ for k_, v_ in cal.items()} if world == 1 and not no_graph and not exchange else None,
         "l2_policy": f"rotating {ncopies} distinct input copies "
         f"({ncopies * w.n_bytes / 2**20:.0f} MiB total vs 126 MB L2)" if ncopies > 1 else "input larger than L2",
         "clocks": clocks,
@@ -413,7 +431,8 @@ def main():
                        "n_channels": res["n_channels"], "bits": res["bits"], "n_bins": res["n_bins"],
                        "rotator": res["rotator"], "input_bytes_per_gpu": res["input_bytes"],
                        "parallelism": f"time-sharded x{world}" if world > 1 else "single GPU",
-                       "l2": res["l2_policy"], "launch_mode": res["launch_mode"]},
+                       "l2": res["l2_policy"], "launch_mode": res["launch_mode"],
+                       "launch_mode_calibration_us": res["launch_mode_calibration_us"]},
             "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
             "roofline": res["roofline"], "hot_kernel_us": res["hot_kernel_us"]}
     if world == 1 and rank == 0 and not args.quick:
