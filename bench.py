@@ -449,6 +449,7 @@ def main():
                 r, _ = measure(idx, 5 if idx == 5 else 10, 3, 0, 1, device, do_e2e=False, rotator=rot)
                 key = f"cfg{idx}" + (f"_{rot}" if rot else "")
                 table[key] = {k: r[k] for k in ("workload", "rotator", "value", "input_gbs", "ms_per_step", "hot_kernel_us")}
+                table[key]["sm_mhz"] = (r.get("clocks") or {}).get("sm_mhz")
                 table[key]["roofline_frac"] = r["roofline"]["frac"]
                 table[key]["roofline_achieved_gbs"] = r["roofline"]["achieved"]
             line["all_configs"] = table

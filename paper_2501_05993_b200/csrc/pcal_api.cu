@@ -445,6 +445,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.E = mulmod_host(kTileSamples, Fo, Fs);
         gp.D = mulmod_host(c->gen_grid, gp.E, Fs);
         gp.rho = phasor_neg_host(mulmod_host((uint64_t)kThreads * spt, Fo, Fs), Fs);
+        gp.rho2 = phasor_neg_host(mulmod_host(2ull * kThreads * spt, Fo, Fs), Fs);
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
         gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;

@@ -37,6 +37,7 @@ struct GenParams {
     uint64_t Fs, k0, E, D;   // micro-hertz sample rate; (n0*Foff)%Fs; (tile*Foff)%Fs; (grid*E)%Fs
     uint64_t Foff;
     double2 rho;             // exp(-j w * kThreads*SPT): oscillator step per CTA iteration
+    double2 rho2;            // rho^2 (from the exactly reduced phase of two steps)
     double2 tw[16];          // exp(-j w k), k = 0..15: post-twiddle within a load
     double2* partial;        // [device] [cta][n_bins]
     uint32_t n_bins;
@@ -192,49 +193,58 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
 #pragma unroll
     for (int k2 = 0; k2 < SPT / 2; ++k2) { ar[k2] = make_float2(0.f, 0.f); ai[k2] = make_float2(0.f, 0.f); }
 
+    static_assert(DEPTH % 2 == 0 && LPT % 2 == 0, "loads are committed and consumed in pairs");
 #pragma unroll
     for (int j = 0; j < DEPTH; ++j) {                        // prologue: the first DEPTH loads of tile 0
         if (nt > 0 && off + j * LOAD_STRIDE < end_off)
             cp_async_own<LB>(my_ring + (size_t)j * LOAD_STRIDE, gdata + off + j * LOAD_STRIDE);
-        cp_async_commit();
+        if (j & 1) cp_async_commit();                        // one commit group per pair of loads
     }
+    const float rho_c = (float)P.rho.x, rho_s = (float)P.rho.y;
 
-    // one tile; CHECK = false when this tile and the next one are complete (no per-load tests)
+    // one tile; CHECK = false when this tile and the next one are complete (no per-load tests).
+    // Loads are consumed in pairs: one wait, two ring reads, two refills, one commit.  The fp64
+    // oscillator advances by rho^2 per pair; the second load's phasor is the first one turned by rho
+    // in fp32 (one step, ~1e-7, never fed back into the fp64 state).
     auto tile_body = [&](auto check_tag, double2 ph, bool next_exists) {
         constexpr bool CHECK = decltype(check_tag)::value;
+        auto mac = [&](const Vec& v, float c, float sn) {
+            float x[SPT];
+            if constexpr (KIND == KIND_2BIT) gen_decode_2bit(v, x, P.sign_mag, dec_mask, dec_one);
+            else gen_decode<KIND>(v, x, P.sign_mag);
+            const float2 cc = make_float2(c, c), ss = make_float2(sn, sn);
 #pragma unroll
-        for (int j = 0; j < LPT; ++j) {
-            constexpr int dummy = 0; (void)dummy;
-            const int slot = j % DEPTH;                      // compile-time after unrolling
-            cp_async_wait<DEPTH - 1>();
-            const Vec v = *reinterpret_cast<const Vec*>(my_ring + (size_t)slot * LOAD_STRIDE);
-            const float c = (float)ph.x, sn = (float)ph.y;
-            bool ok = true;
-            if (CHECK) ok = off + j * LOAD_STRIDE < end_off;
-            if (ok) {
-                float x[SPT];
-                if constexpr (KIND == KIND_2BIT) gen_decode_2bit(v, x, P.sign_mag, dec_mask, dec_one);
-                else gen_decode<KIND>(v, x, P.sign_mag);
-                const float2 cc = make_float2(c, c), ss = make_float2(sn, sn);
+            for (int k2 = 0; k2 < SPT / 2; ++k2) {
+                const float2 xx = make_float2(x[2 * k2], x[2 * k2 + 1]);
+                ffma2(ar[k2], xx, cc);
+                ffma2(ai[k2], xx, ss);
+            }
+        };
+        auto refill = [&](int j, int slot) {                 // load j + DEPTH: same tile or the next one
+            const uint64_t o = (j + DEPTH < LPT) ? off + (uint64_t)(j + DEPTH) * LOAD_STRIDE
+                                                 : off + tile_stride + (uint64_t)(j + DEPTH - LPT) * LOAD_STRIDE;
+            bool go = true;
+            if (CHECK) go = ((j + DEPTH < LPT) || next_exists) && o < end_off;
+            if (go) cp_async_own<LB>(my_ring + (size_t)slot * LOAD_STRIDE, gdata + o);
+        };
 #pragma unroll
-                for (int k2 = 0; k2 < SPT / 2; ++k2) {
-                    const float2 xx = make_float2(x[2 * k2], x[2 * k2 + 1]);
-                    ffma2(ar[k2], xx, cc);
-                    ffma2(ai[k2], xx, ss);
-                }
-            }
-            // refill the slot just consumed with the load DEPTH ahead (same tile or the next one)
-            {
-                const uint64_t o = (j + DEPTH < LPT) ? off + (uint64_t)(j + DEPTH) * LOAD_STRIDE
-                                                     : off + tile_stride + (uint64_t)(j + DEPTH - LPT) * LOAD_STRIDE;
-                bool go = true;
-                if (CHECK) go = ((j + DEPTH < LPT) || next_exists) && o < end_off;
-                if (go) cp_async_own<LB>(my_ring + (size_t)slot * LOAD_STRIDE, gdata + o);
-                cp_async_commit();
-            }
-            // coupled-form oscillator step (eq. 2.6): ph *= rho, fp64
-            const double nx = ph.x * P.rho.x - ph.y * P.rho.y;
-            const double ny = ph.x * P.rho.y + ph.y * P.rho.x;
+        for (int j = 0; j < LPT; j += 2) {
+            const int s0 = j % DEPTH, s1 = (j + 1) % DEPTH;  // compile-time after unrolling
+            cp_async_wait<DEPTH / 2 - 1>();
+            const Vec v0 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s0 * LOAD_STRIDE);
+            const Vec v1 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s1 * LOAD_STRIDE);
+            const float c0 = (float)ph.x, sn0 = (float)ph.y;
+            const float c1 = __fmaf_rn(c0, rho_c, -sn0 * rho_s), sn1 = __fmaf_rn(c0, rho_s, sn0 * rho_c);
+            bool ok0 = true, ok1 = true;
+            if (CHECK) { ok0 = off + j * LOAD_STRIDE < end_off; ok1 = off + (j + 1) * LOAD_STRIDE < end_off; }
+            if (ok0) mac(v0, c0, sn0);
+            if (ok1) mac(v1, c1, sn1);
+            refill(j, s0);
+            refill(j + 1, s1);
+            cp_async_commit();
+            // coupled-form oscillator step (eq. 2.6) over two loads: ph *= rho^2, fp64
+            const double nx = ph.x * P.rho2.x - ph.y * P.rho2.y;
+            const double ny = ph.x * P.rho2.y + ph.y * P.rho2.x;
             ph.x = nx; ph.y = ny;
         }
     };
