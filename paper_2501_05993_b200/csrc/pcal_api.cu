@@ -29,6 +29,8 @@ constexpr uint64_t kMaxLutEntries = 1ull << 22;
 constexpr uint32_t kMaxBins = 4096;
 constexpr uint32_t kMaxIterPerLaunch = 2048;      // keeps the 16-bit lanes of fold_2bit exact
 constexpr size_t kStageBytes = 128ull << 20;
+constexpr uint64_t kMaxTailEntries = 1ull << 17;  // fused tail: q * C * N_bins per-group bins at most (2 MiB)
+constexpr uint32_t kTailMaxReplicas = 32;         // fused tail: the fold period is doubled until R <= this
 
 uint64_t gcd64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
 // lcm with saturation
@@ -68,6 +70,14 @@ struct pcal_ctx {
     uint32_t *d_lut_off, *d_lut_len;
     void *d_partial, *d_stage;
     double* d_val;                  // [q][F][32] replica sums (stage 1 of pcal_post.cuh)
+    bool fused;                     // reduction + rotation run inside the fold kernel (pcal_tail.cuh)
+    uint32_t* d_cnt;                // [slot][q+1] arrival counters of the fused tail
+    double2* d_G;                   // [slot][q][C*n_bins] per-group bins of the fused tail
+    uint32_t* d_done;               // [kTailSlots] completed uses of each slot
+    unsigned long long* d_tick;     // [kTailSlots] tickets taken on each slot
+    uint32_t fold_seq;              // fold launches so far (slot = fold_seq mod kTailSlots)
+    size_t partial_slot_bytes;
+    uint32_t tail_tpp;              // threads per (channel, bin) pair in stage B of the fused tail
     uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
     bool input_ready;               // pcal_set_input_ready: sample buffers are complete when extract is called
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
@@ -75,7 +85,7 @@ struct pcal_ctx {
     double *d_summary, *h_ana;      // analysis outputs: [C][8] + band-pass [C][N] complex
     double2* d_B;
     uint64_t launches;
-    void (*fold2)(FoldParams);      // the fold_2bit_kernel instantiation in use
+    void (*fold2)(const FoldParams);      // the fold_2bit_kernel instantiation in use
     // profiling hook
     bool profiling;
     std::vector<cudaEvent_t>* ev;   // pairs (start, stop) recorded so far
@@ -125,7 +135,8 @@ static void launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t
 static void free_tables(pcal_ctx* c) {
     cudaFree(c->d_lut); cudaFree(c->d_lut_off); cudaFree(c->d_lut_len);
     cudaFree(c->d_partial); cudaFree(c->d_gen_partial);
-    cudaFree(c->d_val);
+    cudaFree(c->d_val); cudaFree(c->d_cnt); cudaFree(c->d_G); cudaFree(c->d_done); cudaFree(c->d_tick);
+    c->d_cnt = nullptr; c->d_G = nullptr; c->d_done = nullptr; c->d_tick = nullptr;
     c->d_lut = nullptr; c->d_lut_off = c->d_lut_len = nullptr;
     c->d_partial = nullptr; c->d_gen_partial = nullptr;
     c->d_val = nullptr;
@@ -272,7 +283,7 @@ extern "C" int pcal_info(const pcal_ctx* c, pcal_info_t* info) {
 
 // fold_2bit_kernel instantiations: <SIGN_MAG, loads per block, CTAs per SM>.  The default was
 // chosen on the B200 (profiles/); PCAL_FOLD2_VARIANT=u4b3|u4b4|u8b2 overrides it for tuning runs.
-typedef void (*fold2_fn)(FoldParams);
+typedef void (*fold2_fn)(const FoldParams);
 static fold2_fn pick_fold2(bool sm) {
     const char* v = getenv("PCAL_FOLD2_VARIANT");
     if (v && !strcmp(v, "u4b4")) return sm ? fold_2bit_kernel<true, 4, 4> : fold_2bit_kernel<false, 4, 4>;
@@ -333,10 +344,39 @@ static int prepare(pcal_ctx* c) {
         else { occ = occupancy_of(fold_f32_kernel, 0); elem = 8; }
         if (occ < 1) return PCAL_ERR_DEVICE;
         const uint32_t slots = (uint32_t)(c->sm_count * occ);
+        // Fused tail (pcal_tail.cuh): one CTA sums the R replicas of a slot group, so R is kept small by
+        // folding modulo a larger multiple of L (any multiple is a valid period): more, smaller groups.
+        const uint64_t pairs = (uint64_t)c->n_bins * c->C;
+        const char* nf = getenv("PCAL_NO_FUSED_TAIL");
+        c->fused = !(nf && nf[0] == '1') && (uint64_t)q * pairs <= kMaxTailEntries;
+        while (c->fused && slots / q > kTailMaxReplicas) {
+            const uint64_t M2 = M * 2, S2 = M2 / c->spv, q2 = S2 / gcd64(S2, 32);
+            if (M2 > kMaxFoldPeriod || q2 > kMaxSlotGroups || q2 * pairs > kMaxTailEntries) break;
+            M = M2; q = (uint32_t)q2;
+        }
         c->q = q; c->M = M;
         c->R = slots / q ? slots / q : 1;
+        if (c->fused) {
+            // leave room for the CTAs of the two previous launches that are still in their tail (q+1 each)
+            // and for a DFT kernel: the next launch must become resident in one wave
+            const uint32_t reserve = 2 * (q + 1) + 8;
+            if (slots > reserve + q) c->R = (slots - reserve) / q;
+            const uint32_t W = 32u * c->spv, per = W / c->n_bins ? W / c->n_bins : 1u;
+            uint32_t tpp = 1; while (tpp * 2 <= per && tpp < 32) tpp *= 2;
+            c->tail_tpp = tpp;
+            const size_t ns = kTailSlots;
+            CU(cudaMalloc(&c->d_cnt, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
+            CU(cudaMemset(c->d_cnt, 0, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
+            CU(cudaMalloc(&c->d_G, ns * (size_t)c->q * pairs * sizeof(double2)));
+            CU(cudaMalloc(&c->d_done, ns * sizeof(uint32_t)));
+            CU(cudaMemset(c->d_done, 0, ns * sizeof(uint32_t)));
+            CU(cudaMalloc(&c->d_tick, ns * sizeof(unsigned long long)));
+            CU(cudaMemset(c->d_tick, 0, ns * sizeof(unsigned long long)));
+            c->fold_seq = 0;
+        }
         c->grid = c->q * c->R;
-        CU(cudaMalloc(&c->d_partial, (size_t)c->grid * c->F * 32 * elem));
+        c->partial_slot_bytes = (size_t)c->grid * c->F * 32 * elem;
+        CU(cudaMalloc(&c->d_partial, c->partial_slot_bytes * (c->fused ? kTailSlots : 1)));
         CU(cudaMalloc(&c->d_val, (size_t)c->q * c->F * 32 * sizeof(double)));
         // rotate_fold_kernel: a warp per (channel, bin) pair, or the whole CTA when a pair has many elements
         const uint64_t per_pair = (uint64_t)c->q * 32u * c->spv / c->n_bins;
@@ -392,16 +432,43 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         const uint64_t NC = (n_vec + 31) / 32, NSR = (NC + c->q - 1) / c->q;
         uint64_t it = (NSR + (uint64_t)c->R * kWarps - 1) / ((uint64_t)c->R * kWarps);
         it = (it + kFoldGroup - 1) / kFoldGroup * kFoldGroup;
-        fp.n_iter = (uint32_t)it; fp.partial = c->d_partial;
+        fp.n_iter = (uint32_t)it;
+        const uint32_t slot = c->fused ? c->fold_seq % kTailSlots : 0u;   // ring of the fused tail (pcal_tail.cuh)
+        fp.partial = reinterpret_cast<uint8_t*>(c->d_partial) + (size_t)slot * c->partial_slot_bytes;
         const uint64_t grid_threads = (uint64_t)c->R * kWarps * c->q * 32u;
         fp.n_quot = (uint32_t)(n_vec / grid_threads); fp.n_rem = n_vec % grid_threads;
         fp.input_ready = c->input_ready ? 1 : 0;
+        TailParams& tp = fp.tail;
+        memset(&tp, 0, sizeof(tp));
+        if (c->fused) {
+            tp.enabled = 1;
+            tp.cnt = c->d_cnt + (size_t)slot * (c->q + 1);
+            tp.G = c->d_G + (size_t)slot * c->q * c->n_bins * c->C;
+            tp.tick = c->d_tick + slot; tp.done = c->d_done + slot;
+            if (const char* d = getenv("PCAL_TAIL_DEBUG")) tp.dbg = atoi(d);
+            c->fold_seq += 1;
+            tp.lut = c->d_lut; tp.lut_off = c->d_lut_off; tp.lut_len = c->d_lut_len;
+            tp.P = c->d_P; tp.Pint = c->d_Pint; tp.tail = data + n_vec * 16;
+            tp.n0 = c->n_processed; tp.NT = n_vec * c->spv; tp.n_total = n;
+            tp.n0_mod_bins = (uint32_t)(c->n_processed % c->n_bins);
+            for (int i = 0; i < c->C; ++i) tp.n0_mod_L[i] = (uint32_t)(c->n_processed % c->nrot[i]);
+            tp.cnt_quot = (uint32_t)(n_vec / ((uint64_t)c->q * 32u)); tp.cnt_rem = (uint32_t)(n_vec % ((uint64_t)c->q * 32u));
+            tp.C = (uint32_t)c->C; tp.spv = c->spv; tp.spv_log2 = log2_u32(c->spv); tp.n_bins = c->n_bins;
+            tp.tpp = c->tail_tpp; tp.kind = c->kind; tp.sign_mag = c->sign_mag;
+            tp.integer_exact = (c->all_zero && c->kind != KIND_F32) ? 1 : 0;
+            tp.overwrite = c->zero_pending ? 1 : 0;
+        }
         prof_mark(c, st);
         if (c->kind == KIND_2BIT) launch_chain(c->fold2, c->grid, kThreads, 0, st, fp);
         else if (c->kind == KIND_I8) launch_chain(fold_i8_kernel, c->grid, kThreads, 0, st, fp);
         else launch_chain(fold_f32_kernel, c->grid, kThreads, 0, st, fp);
         prof_mark(c, st);
         c->launches += 1;
+        if (c->fused) {               // the fold kernel's last CTAs did the reduction, the rotation and the tail
+            c->zero_pending = false;
+            CU(cudaGetLastError());
+            return PCAL_OK;
+        }
     }
     if (n_vec) {
         ReplicaParams rr;
@@ -715,8 +782,17 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
     if ((uintptr_t)dev & 15u) return PCAL_ERR_ALIGNMENT;
     int occ = occupancy_of(read_probe_kernel, 0);
     if (occ < 1) return PCAL_ERR_DEVICE;
-    read_probe_kernel<<<c->sm_count * occ, kThreads, 0, (cudaStream_t)cuda_stream>>>(
-        reinterpret_cast<const uint4*>(dev), n_bytes / 16, reinterpret_cast<uint32_t*>(c->d_tmp));
+    uint32_t grid = (uint32_t)(c->sm_count * occ);
+    if (const char* g = getenv("PCAL_PROBE_GRID")) grid = (uint32_t)atoi(g);      // tuning runs only
+    const char* pp = getenv("PCAL_PROBE_PDL");
+    uint32_t spin_ns = 0;
+    if (const char* sp = getenv("PCAL_PROBE_SPIN_NS")) spin_ns = (uint32_t)atoi(sp);
+    if (pp && pp[0] == '1')
+        launch_chain(read_probe_kernel, grid, kThreads, 0, (cudaStream_t)cuda_stream,
+                     reinterpret_cast<const uint4*>(dev), (uint64_t)(n_bytes / 16), reinterpret_cast<uint32_t*>(c->d_tmp), spin_ns);
+    else
+        read_probe_kernel<<<grid, kThreads, 0, (cudaStream_t)cuda_stream>>>(
+            reinterpret_cast<const uint4*>(dev), n_bytes / 16, reinterpret_cast<uint32_t*>(c->d_tmp), spin_ns);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;

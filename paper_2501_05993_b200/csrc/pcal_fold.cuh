@@ -20,6 +20,7 @@
 // i the CTAs together read one contiguous range of the input (grid-stride, fully coalesced).
 #pragma once
 #include "pcal_common.cuh"
+#include "pcal_tail.cuh"
 
 namespace pcal {
 
@@ -33,6 +34,7 @@ struct FoldParams {
     uint64_t n_rem;         // ... plus one for the threads whose first vector index is < n_vec % threads
     void* partial;          // [device] per-CTA partial sums, layout [cta][field][lane]
     int input_ready;        // caller promised the input is complete: stream it before pdl_wait()
+    TailParams tail;        // fused reduction + rotation by the CTAs that finish last (pcal_tail.cuh)
 };
 
 __device__ __forceinline__ uint64_t fold_first_vec(const FoldParams& P, int w, int lane) {
@@ -56,11 +58,11 @@ __device__ __forceinline__ uint64_t fold_first_vec(const FoldParams& P, int w, i
 constexpr int kFoldGroup = 16;   // loads per complete counter cascade
 
 template <bool SIGN_MAG, int U, int MINB>
-__global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P) {
-    pdl_release();
+__global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
     static_assert(U == 4 || U == 8, "block of 4 or 8 loads");
-    __shared__ uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
+    __shared__ uint32_t s_gen[2];
+    __shared__ __align__(16) uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint64_t first = fold_first_vec(P, w, lane);
     const uint64_t stride = (uint64_t)P.R * kWarps * P.q * 32u;
@@ -137,6 +139,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
 
     uint4 bufA[U], bufB[U];
     load_block(bufA, 0);
+    fold_ticket_and_release(P.tail, s_gen);   // first loads are in flight
     uint32_t groups_since_flush = 0;
     for (uint32_t i = 0; i < P.n_iter; i += kFoldGroup) {
 #pragma unroll
@@ -163,7 +166,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
         }
     }
     __syncthreads();
-    pdl_wait();   // the partials of the previous launch may still be read by its reduce kernel
+    fold_wait_slot(P.tail, s_gen);
     uint16_t* out = reinterpret_cast<uint16_t*>(P.partial) + (size_t)blockIdx.x * 64 * 32;
 #pragma unroll
     for (int x = tid; x < 32 * 32; x += kThreads) {
@@ -175,16 +178,18 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(FoldParams P)
         out[f * 32 + ln] = (uint16_t)(s & 0xFFFFu);
         out[(f + 8) * 32 + ln] = (uint16_t)(s >> 16);
     }
+    if (P.tail.enabled) fold_tail<KIND_2BIT>(P.tail, P.partial, P.q, P.R, reinterpret_cast<double*>(&hlf[0][0]), s_gen[0]);
 }
 
 // ---------------------------------------------------------------------------------------------
 // int8 samples: 16 fields per vector, exact int32 sums via DP4A with a one-hot byte selector.
 // Output: int32 partial[cta][16][32].
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
-    pdl_release();
+__global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
-    __shared__ int32_t sh[kWarps][16][32];
+    __shared__ uint32_t s_gen[2];
+    __shared__ __align__(16) int32_t sh[kWarps][16][32];   // also the (double) scratch of the fused tail
+    fold_ticket_and_release(P.tail, s_gen);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
     const uint64_t stride = (uint64_t)P.R * kWarps * P.q * 32u;
@@ -210,7 +215,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
 #pragma unroll
     for (int k = 0; k < 16; ++k) sh[w][k][lane] = acc[k];
     __syncthreads();
-    pdl_wait();
+    fold_wait_slot(P.tail, s_gen);
     int32_t* out = reinterpret_cast<int32_t*>(P.partial) + (size_t)blockIdx.x * 16 * 32;
     for (int e = threadIdx.x; e < 16 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;
@@ -219,6 +224,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
         for (int ww = 0; ww < kWarps; ++ww) s += sh[ww][f][ln];
         out[f * 32 + ln] = s;
     }
+    if (P.tail.enabled) fold_tail<KIND_I8>(P.tail, P.partial, P.q, P.R, reinterpret_cast<double*>(&sh[0][0][0]), s_gen[0]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -226,13 +232,14 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(FoldParams P) {
 // (runs <= 64 keep every bin within 1.3e-6 relative).
 // Output: double partial[cta][4][32].
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
-    pdl_release();
+__global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
-    __shared__ double sh[kWarps][4][32];
+    __shared__ uint32_t s_gen[2];
+    __shared__ __align__(16) double sh[kWarps][4][32];   // 1024 doubles: also the scratch of the fused tail
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
     const uint64_t stride = (uint64_t)P.R * kWarps * P.q * 32u;
+    fold_ticket_and_release(P.tail, s_gen);
     double tot[4] = {0.0, 0.0, 0.0, 0.0};
     for (uint32_t i = 0; i < P.n_iter; i += 2 * kUnroll) {
         float run[4] = {0.f, 0.f, 0.f, 0.f};
@@ -259,7 +266,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
 #pragma unroll
     for (int k = 0; k < 4; ++k) sh[w][k][lane] = tot[k];
     __syncthreads();
-    pdl_wait();
+    fold_wait_slot(P.tail, s_gen);
     double* out = reinterpret_cast<double*>(P.partial) + (size_t)blockIdx.x * 4 * 32;
     for (int e = threadIdx.x; e < 4 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;
@@ -268,6 +275,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(FoldParams P) {
         for (int ww = 0; ww < kWarps; ++ww) s += sh[ww][f][ln];  // fixed warp order: deterministic
         out[f * 32 + ln] = s;
     }
+    if (P.tail.enabled) fold_tail<KIND_F32>(P.tail, P.partial, P.q, P.R, &sh[0][0][0], s_gen[0]);
 }
 
 }  // namespace pcal

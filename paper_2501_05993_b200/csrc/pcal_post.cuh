@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
     double2* sw = dft_sm + N;
     const uint32_t c = blockIdx.y;
     for (uint32_t t = threadIdx.x; t < N; t += kDftThreads) {
-        sp[t] = P[(size_t)c * N + t];
+        sp[t] = __ldcg(P + (size_t)c * N + t);      // L2: the producer grid may have overlapped this one
         sw[t] = W[t];
     }
     __syncthreads();

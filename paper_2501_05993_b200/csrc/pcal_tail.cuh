@@ -1,0 +1,274 @@
+// pcal_tail.cuh -- the reduction behind the fold kernels, run INSIDE the fold kernel by the CTAs that
+// finish last ("fused tail"): a5 of SURVEY section 8 (deterministic reduction of per-block partials;
+// the step the paper leaves to the host CPU) plus the one-off rotation by the
+// table of eq. 2.4 after the reordering of PAPER.md:200.
+//
+// Same arithmetic as reduce_replicas_kernel + rotate_fold_kernel (pcal_post.cuh), which remain as the
+// un-fused path for geometries the tail does not take (see tail_ok in pcal_api.cu).  Three stages, each
+// entered by exactly one CTA per group, elected by an arrival counter (every CTA: write partial,
+// __threadfence, barrier, one atomicAdd; the CTA that observes count-1 is last and reads what the
+// others wrote):
+//   A  last CTA of slot group p: sum the R replica partials of the group (replica order), code sums
+//      -> level sums, into shared memory                                   [F*32 values]
+//   B  same CTA: multiply by the rotator table and fold the group's 32*spv time samples into per-group
+//      bins G[p][c][b]   (fixed thread -> element map + fixed butterfly: deterministic)
+//   C  last CTA of the grid: P[c][b] (+)= sum_p G[p][c][b] in group order, ragged tail (< 1 vector)
+//      added, integer bins kept when the data is integer and unrotated; counters reset for the next
+//      launch.
+// A step of the LUT path is thereby ONE launch (plus the DFT of pcal_finalize).
+//
+// Pipelining across launches.  Partials, counters and G live in a ring of kTailSlots slots; the host
+// hands consecutive launches consecutive slots.  A fold kernel never executes griddepcontrol.wait
+// before its partial writes.  Instead every CTA takes a ticket of its slot (64-bit atomicAdd) BEFORE
+// it lets the dependent grid be scheduled; a dependent grid starts only after every CTA of its
+// predecessor has done so, hence all tickets of launch s are taken before any CTA of a later launch
+// runs, and ticket / gridDim.x is the number g of earlier uses of the slot -- derived on the device, so
+// launches replayed from a CUDA graph (frozen parameters) stay correct.  Before its partial writes a
+// CTA checks (acquire load, spinning if ever needed) that done[slot] == g, i.e. that the stage-C CTA of
+// the slot's previous user -- a grid dispatched long before -- has finished reading it; that CTA
+// publishes g + 1 after its last read.  Only the ONE CTA that runs stage C executes
+// griddepcontrol.wait (predecessor grid complete, hence -- transitively -- every earlier grid, incl. the
+// DFT kernel that reads P) before it touches P.  Consecutive launches therefore overlap completely
+// except for stage C, and HBM never drains at a kernel boundary.
+#pragma once
+#include "pcal_post.cuh"
+
+namespace pcal {
+
+struct TailParams {
+    uint32_t* cnt;            // [device] q+1 arrival counters, zero between launches
+    double2* G;               // [device] per-group bins [q][C*n_bins]
+    const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
+    const uint32_t* lut_off;  // [device] per channel: first entry
+    const uint32_t* lut_len;  // [device] per channel: N_rotator,c (1 => no rotation)
+    double2* P;               // [device] folded bins [C][N_bins]
+    long long* Pint;          // [device] exact integer bins [C][N_bins]
+    const uint8_t* tail;      // [device] first byte after the last complete vector
+    uint64_t n0, NT, n_total; // absolute index of the first sample; samples in whole vectors; samples in the piece
+    uint32_t n0_mod_bins;     // n0 mod N_bins
+    uint32_t n0_mod_L[kMaxChannels];   // n0 mod N_rotator,c
+    uint32_t cnt_quot, cnt_rem;   // vectors per slot: cnt_quot + (p*32 + lane < cnt_rem)
+    uint32_t C, spv, spv_log2, n_bins;
+    uint32_t tpp;             // threads per (channel, bin) pair in stage B: power of two <= 32
+    int kind, sign_mag, integer_exact, overwrite;
+    int enabled;              // 0: the caller launches reduce_replicas_kernel + rotate_fold_kernel instead
+    unsigned long long* tick; // [device] ticket counter of this launch's slot
+    uint32_t* done;           // [device] completed uses of this launch's slot
+    int dbg;                  // tuning runs only (PCAL_TAIL_DEBUG): 1 = stage C without griddepcontrol.wait, 2 = no tail at all
+};
+
+constexpr uint32_t kTailSlots = 8;
+
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(uint32_t* p, uint32_t v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Arrival on an election counter: release (everything this CTA wrote before the preceding barrier) and
+// acquire (what the earlier arrivals released) in one instruction, issued by one thread per CTA.
+__device__ __forceinline__ uint32_t arrive_acq_rel(uint32_t* p) {
+    uint32_t v;
+    asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Called by every thread of a fold kernel once its first loads are in flight: slot ticket, then the
+// dependent grid may be scheduled.  *s_gen (shared) = number of earlier uses of the slot.
+// s_gen[1] = 1 when the slot was already free at that time (the usual case: no check needed later).
+__device__ __forceinline__ void fold_ticket_and_release(const TailParams& T, uint32_t* s_gen) {
+    if (T.enabled) {
+        if (threadIdx.x == 0) {
+            const uint32_t seen = ld_acquire_u32(T.done);
+            const uint32_t g = (uint32_t)(atomicAdd(T.tick, 1ull) / gridDim.x);
+            s_gen[0] = g; s_gen[1] = (seen == g) ? 1u : 0u;
+        }
+        __syncthreads();      // thread 0 holds the ticket (it stored the quotient) before any thread releases
+    }
+    pdl_release();
+}
+
+// Called by every thread of a fold kernel after its loads and before its partial writes.
+__device__ __forceinline__ void fold_wait_slot(const TailParams& T, const uint32_t* s_gen) {
+    if (T.enabled) {
+        if (threadIdx.x == 0 && !s_gen[1] && !(T.dbg & 6))
+            while (ld_acquire_u32(T.done) != s_gen[0]) __nanosleep(64);
+        __syncthreads();
+    } else {
+        pdl_wait();   // the partials of the previous launch may still be read by its reduce kernel
+    }
+}
+
+// `scratch` = shared memory the caller no longer needs: max(2*F*32, 512) doubles, 16-byte aligned.
+template <int KIND>
+__device__ __noinline__ void fold_tail(const TailParams& T, const void* partial, uint32_t q, uint32_t R, double* scratch, uint32_t gen) {
+    __shared__ uint32_t s_prev;
+    const uint32_t tid = threadIdx.x;
+    const uint32_t p = blockIdx.x % q;
+    constexpr uint32_t F = KIND == KIND_2BIT ? 64u : (KIND == KIND_I8 ? 16u : 4u);
+    constexpr uint32_t E = F * 32u;
+
+    if (T.dbg & 2) return;
+    __syncthreads();          // every thread's partial writes happen before thread 0's release below
+    if (tid == 0) s_prev = arrive_acq_rel(T.cnt + p);
+    __syncthreads();
+    if (s_prev != R - 1u || (T.dbg & 4)) return;
+
+    // ---- stage A: replica sums of group p ---------------------------------------------------
+    if (KIND == KIND_2BIT) {
+        // thread t owns elements 8t .. 8t+7 (one 16-byte word of eight uint16 per replica)
+        const uint4* src = reinterpret_cast<const uint4*>(partial) + (size_t)p * (E / 8u) + tid;
+        const size_t stride = (size_t)q * (E / 8u);
+        uint32_t a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (uint32_t r0 = 0; r0 < R; r0 += 8u) {
+            uint4 v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = (r0 + k < R) ? __ldcg(src + (size_t)(r0 + k) * stride) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                a[0] += v[k].x & 0xFFFFu; a[1] += v[k].x >> 16; a[2] += v[k].y & 0xFFFFu; a[3] += v[k].y >> 16;
+                a[4] += v[k].z & 0xFFFFu; a[5] += v[k].z >> 16; a[6] += v[k].w & 0xFFFFu; a[7] += v[k].w >> 16;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const uint32_t e = 8u * tid + k, vslot = p * 32u + (e & 31u);
+            const long long cnt = (long long)(T.cnt_quot + (vslot < T.cnt_rem ? 1u : 0u));
+            scratch[e] = (double)(2ll * (long long)a[k] - 3ll * cnt);      // code sum -> level sum
+        }
+    } else {
+        for (uint32_t e = tid; e < E; e += kThreads) {
+            const size_t stride = (size_t)q * E;
+            if (KIND == KIND_I8) {
+                const int32_t* src = reinterpret_cast<const int32_t*>(partial) + (size_t)p * E + e;
+                scratch[e] = (double)replica_sum<int32_t, long long>(src, stride, 0u, 1u, R);
+            } else {
+                const double* src = reinterpret_cast<const double*>(partial) + (size_t)p * E + e;
+                scratch[e] = replica_sum<double, double>(src, stride, 0u, 1u, R);
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- stage B: rotate, fold the group's W = 32*spv time samples into G[p] -----------------
+    // B1: thread t multiplies the elements t, t+256, ... by their phasors -- all table loads of a thread
+    //     in flight at once -- and leaves the products in shared memory (in place of the sums);
+    // B2: tpp threads per (channel, bin) pair add the pair's products in a fixed order.
+    const uint32_t pairs = T.C * T.n_bins, W = 32u * T.spv, tpp = T.tpp;
+    const uint32_t base_b = (uint32_t)((T.n0_mod_bins + (uint64_t)p * W) % T.n_bins);
+    {
+        constexpr uint32_t EPT = (E + kThreads - 1) / kThreads;       // 8, 2, 1
+        double v[EPT];
+        double2 ph[EPT];
+#pragma unroll
+        for (uint32_t j = 0; j < EPT; ++j) {
+            const uint32_t e = tid + j * kThreads;
+            v[j] = 0.0; ph[j] = make_double2(1.0, 0.0);
+            if (e < E) {
+                const uint32_t f = e >> 5, ln = e & 31u, t = f / T.C, c = f % T.C;
+                const uint32_t L = T.lut_len[c];
+                v[j] = scratch[e];
+                if (L > 1) ph[j] = __ldg(T.lut + T.lut_off[c] + (T.n0_mod_L[c] + p * W + ln * T.spv + t) % L);
+            }
+        }
+        __syncthreads();
+        double2* prod = reinterpret_cast<double2*>(scratch);
+#pragma unroll
+        for (uint32_t j = 0; j < EPT; ++j) {
+            const uint32_t e = tid + j * kThreads;
+            if (e < E) prod[e] = make_double2(v[j] * ph[j].x, v[j] * ph[j].y);
+        }
+        __syncthreads();
+    }
+    double2* Gp = T.G + (size_t)p * pairs;
+    for (uint32_t s0 = 0; s0 < pairs * tpp; s0 += kThreads) {          // uniform trip count: shuffles below
+        const uint32_t slot = s0 + tid;
+        const bool active = slot < pairs * tpp;
+        const uint32_t pp = active ? slot / tpp : 0u, u = slot % tpp;
+        const uint32_t c = pp / T.n_bins, b = pp % T.n_bins;
+        double are = 0.0, aim = 0.0;
+        if (active) {
+            const double2* prod = reinterpret_cast<const double2*>(scratch);
+            const uint32_t d0 = (b + T.n_bins - base_b) % T.n_bins;
+            const uint32_t dstep = tpp * T.n_bins;
+            for (uint32_t d = d0 + u * T.n_bins; d < W; d += dstep) {
+                const double2 x = prod[(((d & (T.spv - 1u)) * T.C + c) << 5) + (d >> T.spv_log2)];
+                are += x.x; aim += x.y;
+            }
+        }
+        for (uint32_t sh = tpp >> 1; sh > 0; sh >>= 1) {
+            are += __shfl_xor_sync(0xFFFFFFFFu, are, sh);
+            aim += __shfl_xor_sync(0xFFFFFFFFu, aim, sh);
+        }
+        if (active && u == 0) Gp[pp] = make_double2(are, aim);
+    }
+
+    __syncthreads();
+    if (tid == 0) s_prev = arrive_acq_rel(T.cnt + q);
+    __syncthreads();
+    if (s_prev != q - 1u) return;
+
+    // ---- stage C: groups in order, ragged tail, accumulate into the context ------------------
+    if (!(T.dbg & 1)) pdl_wait();   // every earlier grid (incl. a DFT kernel reading P) has completed
+    // thread = (slice sl of the groups, pair): slice sums first (all loads of a thread in flight at
+    // once where possible), then the slices in order.
+    const uint32_t ppc = pairs < (uint32_t)kThreads ? pairs : (uint32_t)kThreads;
+    const uint32_t ns = (uint32_t)kThreads / ppc;            // >= 1; > 1 only when pairs < 256
+    const uint32_t sl = tid / ppc, e0 = tid % ppc;
+    const uint32_t n_tail = (uint32_t)(T.n_total - T.NT);
+    double* s_re = scratch;                                  // [kThreads]
+    double* s_im = scratch + kThreads;                       // [kThreads]
+    for (uint32_t pp0 = 0; pp0 < pairs; pp0 += ppc) {        // uniform trip count (one trip when pairs <= 256)
+        const uint32_t pp = pp0 + e0;
+        double are = 0.0, aim = 0.0;
+        if (sl < ns && pp < pairs) {
+            for (uint32_t g0 = sl; g0 < q; g0 += 8u * ns) {
+                double2 g[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) g[k] = (g0 + k * ns < q) ? __ldcg(T.G + (size_t)(g0 + k * ns) * pairs + pp) : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { are += g[k].x; aim += g[k].y; }
+            }
+        }
+        if (ns > 1) {
+            __syncthreads();
+            s_re[tid] = are; s_im[tid] = aim;
+            __syncthreads();
+            are = 0.0; aim = 0.0;
+            if (sl == 0) for (uint32_t k = 0; k < ns; ++k) { are += s_re[k * ppc + e0]; aim += s_im[k * ppc + e0]; }
+        }
+        if (sl != 0 || pp >= pairs) continue;
+        const uint32_t c = pp / T.n_bins, b = pp % T.n_bins;
+        if (n_tail) {   // samples NT .. n_total-1 (fewer than one vector)
+            const uint32_t L = T.lut_len[c];
+            const double2* lut = T.lut + T.lut_off[c];
+            uint32_t bb = (uint32_t)((T.n0 + T.NT) % T.n_bins);
+            uint32_t k = L > 1 ? (uint32_t)((T.n0 + T.NT) % L) : 0;
+            for (uint32_t t = 0; t < n_tail; ++t) {
+                if (bb == b) {
+                    const double v = decode_tail(T.kind, T.sign_mag, T.tail, t, c, T.C);
+                    if (L > 1) { const double2 ph = lut[k]; are += v * ph.x; aim += v * ph.y; }
+                    else are += v;
+                }
+                if (++bb == T.n_bins) bb = 0;
+                if (L > 1 && ++k == L) k = 0;
+            }
+        }
+        long long ai = (long long)are;     // exact: unrotated integer sums are integers below 2^53
+        if (!T.overwrite) {
+            const double2 cur = __ldcg(T.P + pp);          // L2: written by another SM under an overlapping grid
+            are += cur.x; aim += cur.y;
+            if (T.integer_exact) ai += __ldcg(T.Pint + pp);
+        }
+        T.P[pp] = make_double2(are, aim);
+        if (T.integer_exact) T.Pint[pp] = ai;
+    }
+    for (uint32_t i = tid; i <= q; i += kThreads) T.cnt[i] = 0u;       // ready for the slot's next launch
+    __syncthreads();
+    if (tid == 0) st_release_u32(T.done, gen + 1u);                    // the slot may be written again
+}
+
+}  // namespace pcal

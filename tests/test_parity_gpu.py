@@ -236,7 +236,7 @@ def test_segments_longer_than_one_launch(oracle, idx, n, rot, monkeypatch):
     monkeypatch.setenv("PCAL_SMALL_PIECES", "1")
     w, dev, host = make(idx, n)
     p, T, P = gpu_run(w, dev, rotator=rot)
-    n_fold = 3 if rot is None and idx != 5 else 2          # kernels per piece: fold+reduce+rotate / gen+post
+    n_fold = 1 if rot is None and idx != 5 else 2          # kernels per piece: fold with fused tail / gen+post
     assert p.info().kernel_launches >= 2 * n_fold + 1, p.info().kernel_launches
     for c in range(0, w.n_channels, 6):
         assert_close(T[c], oracle_tones(oracle, w, host, c, threads=8), f"cfg{idx} ch{c} multi-launch")
@@ -244,6 +244,31 @@ def test_segments_longer_than_one_launch(oracle, idx, n, rot, monkeypatch):
     p2, T2, _ = gpu_run(w, dev, rotator=rot)
     assert p2.info().kernel_launches < p.info().kernel_launches
     assert_close(T, T2, f"cfg{idx} pieces vs single launch")
+
+
+@pytest.mark.parametrize("idx,n", [(1, 1_300_001), (2, 1_300_004), (3, 2_600_036), (4, 200_003), (6, 1_300_004),
+                                   (7, 1_300_003), (8, 1_300_001), (2, 60), (4, 7)])
+def test_unfused_reduction_kernels_agree_with_the_fused_tail(oracle, idx, n, monkeypatch):
+    """The LUT path reduces, rotates and accumulates inside the fold kernel (pcal_tail.cuh: the CTAs that
+    finish last).  PCAL_NO_FUSED_TAIL=1 selects the separate reduce_replicas/rotate_fold kernels instead
+    (also the fall-back for geometries with very many slot groups); both must match the oracle, and each
+    other to fp64 rounding (bit-identical integer bins)."""
+    w, dev, host = make(idx, n)
+    p1, T1, P1 = gpu_run(w, dev)
+    monkeypatch.setenv("PCAL_NO_FUSED_TAIL", "1")
+    p2, T2, P2 = gpu_run(w, dev)
+    monkeypatch.delenv("PCAL_NO_FUSED_TAIL")
+    if n > 1000:
+        assert p2.info().kernel_launches == p1.info().kernel_launches + 2
+        for c in range(0, w.n_channels, 5):
+            want = oracle_tones(oracle, w, host, c)
+            assert_close(T1[c], want, f"fused cfg{idx} ch{c}")
+            assert_close(T2[c], want, f"unfused cfg{idx} ch{c}")
+    scale = np.abs(P1).max()
+    # float32 input: the fused geometry folds modulo a larger period, which regroups the short fp32 runs
+    assert np.abs(P1 - P2).max() <= (1e-6 if idx in (1, 8) else 1e-11) * scale
+    if idx in (6, 7):
+        assert np.array_equal(p1.get_folded_i64(), p2.get_folded_i64())
 
 
 @pytest.mark.parametrize("idx,n,rot", [(2, 3_000_004, None), (4, 300_003, None), (5, 2_000_003, None), (3, 2_000_004, "generator")])
