@@ -11,8 +11,8 @@ One JSON line on stdout (rank 0):
   value      whole-job samples/s, inputs resident in HBM, device-timed over K steps (max over ranks)
   e2e        same metric through pcal_extract_host: pinned HOST buffer -> device inside the timed
              region, result read back to the host every step
-  roofline   the fused fold (or generator) kernel: algorithmic input bytes / its average duration,
-             measured live with CUDA events on the launching stream (pcal_set_profiling)
+  roofline   the fused fold (or generator) kernel: algorithmic input bytes / its average launch duration
+             over the timed region (CUDA events on the launching stream; launches overlap under PDL)
   cpu_baseline  the CPU oracle timed on this box's host cores on a bounded sample of the workload
 `--impl reference` times the oracle (the only "reference implementation" this paper-only task has).
 With N > 1 (torchrun) the stream is time-sharded: each rank folds its own 2^28-sample range at its
@@ -175,9 +175,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
 
     def step(i):
         if not exchange:
-            p.reset()
-            p.extract(bufs[i % ncopies], n)
-            p.finalize_async(out_pinned)
+            p.integrate(bufs[i % ncopies], n, out_pinned)     # pcal_reset + pcal_extract + pcal_finalize_async
             return
         L = lanes[i % 2]
         complete(L)                                       # this lane's previous integration, if still open
@@ -211,6 +209,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     # launch directly.
     use_graph = (world == 1) and not no_graph and not exchange
     graphs, per_step_launches = [], None
+    n_big = ncopies * max(1, min(steps, 40) // ncopies)      # steps in the big graph (whole rounds over the copies)
     if use_graph:
         side = torch.cuda.Stream()
         side.wait_stream(torch.cuda.current_stream())
@@ -222,9 +221,9 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
                     step(k)
                 per_step_launches = p.info().kernel_launches - l0
                 graphs.append(g)
-            big = torch.cuda.CUDAGraph()              # ncopies consecutive steps in ONE graph
+            big = torch.cuda.CUDAGraph()              # n_big consecutive steps in ONE graph
             with torch.cuda.graph(big, stream=side):
-                for k in range(ncopies):
+                for k in range(n_big):
                     step(k)
         torch.cuda.current_stream().wait_stream(side)
 
@@ -233,9 +232,9 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
             for k in range(count):
                 graphs[k % ncopies].replay()
         elif mode == "graph_of_steps":
-            for _ in range(count // ncopies):
+            for _ in range(count // n_big):
                 big.replay()
-            for k in range(count % ncopies):
+            for k in range(count % n_big):
                 step(k)
         else:
             for k in range(count):
@@ -245,7 +244,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     mode = "direct"
     if use_graph:
         def timed(m, reps):
-            run_steps(m, ncopies)
+            run_steps(m, n_big)
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
@@ -253,7 +252,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
             b.record()
             torch.cuda.synchronize()
             return a.elapsed_time(b) / reps
-        reps = max(2 * ncopies, steps)
+        reps = max(2 * n_big, steps)
         cal = {m: min(timed(m, reps) for _ in range(2)) for m in ("direct", "graph_per_step", "graph_of_steps")}
         mode = min(cal, key=cal.get)
     launches0 = sum(q_.info().kernel_launches for q_ in ctxs)
@@ -301,7 +300,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         "gpu_launches": int(launches),
         "launch_mode": {"direct": "direct launches (kernels chained by programmatic dependent launch)",
                         "graph_per_step": "cuda_graph: one graph replay per step (reset + extract + finalize_async captured once per input copy)",
-                        "graph_of_steps": f"cuda_graph: one replay per {ncopies} consecutive steps (one per input copy), kernels chained "
+                        "graph_of_steps": f"cuda_graph: one replay per {n_big} consecutive steps (cycling over the input copies), kernels chained "
                                           "by programmatic dependent launch inside the graph; remainder steps launched directly"}[mode],
         "launch_mode_calibration_us": {k_: 1e3 * v_ for k_, v_ in cal.items()} if world == 1 and not no_graph and not exchange else None,
         "l2_policy": f"rotating {ncopies} distinct input copies "
@@ -309,37 +308,48 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         "clocks": clocks,
     }
     peak, peak_src = load_peaks()
-    # calibration: a pure streaming read of the same buffers, same grid/loads, bracketed by events
-    # on the same stream in the same way as the hot kernel above
+    # calibration: a pure streaming read of the same buffers (no decode, no fold), launched back to back
+    # like the steps above (launches may overlap under programmatic dependent launch), timed the same way
     floor_us = None
     if rank == 0:
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        for i in range(3):
+        for i in range(ncopies):
             p.read_probe(bufs[i % ncopies])
-        for i, (a, b) in enumerate(evs):
-            a.record(); p.read_probe(bufs[i % ncopies]); b.record()
         torch.cuda.synchronize()
-        floor_us = 1e3 * sum(a.elapsed_time(b) for a, b in evs) / len(evs)
-    # algorithmic bytes per launch = input bytes of one launch (bits/8 per sample, read once)
-    bytes_per_launch = w.n_bytes * steps / max(hot_launches, 1)
-    hot_s = 1e-3 * hot_ms / max(hot_launches, 1)
-    achieved = bytes_per_launch / hot_s / 1e9 if hot_ms > 0 else 0.0
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for i in range(max(steps, 2 * ncopies)):
+            p.read_probe(bufs[i % ncopies])
+        b.record()
+        torch.cuda.synchronize()
+        floor_us = 1e3 * a.elapsed_time(b) / max(steps, 2 * ncopies)
+    # The dominant kernel's average launch duration over the timed region: consecutive launches overlap
+    # (programmatic dependent launch), so it is the region's device time / the kernel's launches in it --
+    # an upper bound, the small DFT kernel of every step is inside.  `isolated_kernel_us` is the same kernel
+    # bracketed by events launch by launch (which serialises the launches: its latency, not its cost).
+    fold_launches = steps * max(1, round(hot_launches / steps)) if hot_launches else steps
+    bytes_per_launch = w.n_bytes * steps / fold_launches
+    hot_s = 1e-3 * ms / fold_launches
+    achieved = bytes_per_launch / hot_s / 1e9
     gen = inf.rotator_in_effect == 2
     res["roofline"] = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                        "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                       "kernel": "gen_kernel (generator path)" if gen else "fold_*_kernel (LUT path)",
-                       "algorithmic_bytes_per_launch": bytes_per_launch}
+                       "kernel": "gen_kernel (generator path)" if gen else "fold_*_kernel incl. fused tail (LUT path)",
+                       "algorithmic_bytes_per_launch": bytes_per_launch,
+                       "avg_launch_us": hot_s * 1e6, "launches_in_timed_region": fold_launches,
+                       "isolated_kernel_us": 1e3 * hot_ms / max(hot_launches, 1),
+                       "how": "device time of the timed region (CUDA events on the launching stream) / launches of the kernel in it"}
     res["roofline"]["traffic"] = load_traffic(w.name, res["rotator"]) if not n_override else None
+    res["hot_kernel_us"], res["hot_kernel_isolated_us"] = hot_s * 1e6, 1e3 * hot_ms / max(hot_launches, 1)
     if floor_us:
         res["roofline"]["read_floor"] = {
             "us": floor_us, "gbs": w.n_bytes / floor_us / 1e3, "frac_of_floor": floor_us / (hot_s * 1e6),
-            "what": "pcal_read_probe: pure streaming read of the same buffer (no decode/fold), same event bracketing"}
+            "what": "pcal_read_probe: pure streaming read of the same buffers (no decode/fold), back-to-back launches timed like the steps"}
     if gen and w.bits == 2:
         # 2-bit generator variant: >= 3 thread-instructions per sample (shift, LOP3, one FFMA2 lane-op)
         # against the issue rate 148 SMs x 4 schedulers x 32 lanes x f_SM
         sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         alu_peak = 148 * 4 * 32 * sm_mhz * 1e6 / 1e9                     # G thread-instr/s
-        alu_ach = 3.0 * (n * C * steps / max(hot_launches, 1)) / hot_s / 1e9
+        alu_ach = 3.0 * (n * C * steps / fold_launches) / hot_s / 1e9
         res["roofline"].update({"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Ginstr/s",
                                 "frac": alu_ach / alu_peak, "peak_source": "derived: 148 SMs x 4 x 32 lanes x sm_max_mhz",
                                 "hbm_frac": achieved / peak, "hbm_achieved_gbs": achieved})
@@ -373,7 +383,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config (1-based); default configs[1]")
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
@@ -446,9 +456,9 @@ def main():
         if not args.no_all:
             table = {}
             for idx, rot in [(1, None), (2, None), (3, "lut"), (3, "generator"), (4, None), (5, None)]:
-                r, _ = measure(idx, 5 if idx == 5 else 10, 3, 0, 1, device, do_e2e=False, rotator=rot)
+                r, _ = measure(idx, 20 if idx == 5 else 100, 3, 0, 1, device, do_e2e=False, rotator=rot)
                 key = f"cfg{idx}" + (f"_{rot}" if rot else "")
-                table[key] = {k: r[k] for k in ("workload", "rotator", "value", "input_gbs", "ms_per_step", "hot_kernel_us")}
+                table[key] = {k: r[k] for k in ("workload", "rotator", "value", "input_gbs", "ms_per_step", "hot_kernel_us", "hot_kernel_isolated_us")}
                 table[key]["sm_mhz"] = (r.get("clocks") or {}).get("sm_mhz")
                 table[key]["roofline_frac"] = r["roofline"]["frac"]
                 table[key]["roofline_achieved_gbs"] = r["roofline"]["achieved"]

@@ -162,8 +162,19 @@ int pcal_extract_host(pcal_ctx *ctx, const void *host_samples, uint64_t n_sample
 int pcal_finalize(pcal_ctx *ctx, double *out_tones);
 
 /* As pcal_finalize but only enqueues (DFT + async copy into out_tones, which should be pinned
- * host memory) on the context's stream; the caller synchronises. */
+ * host memory) on the context's stream; the caller synchronises.  When out_tones is device-visible
+ * pinned memory the DFT kernel writes it directly; that property is looked up when the pointer changes
+ * from the previous call, so a buffer must not be freed and re-created at the same address with a
+ * different kind of memory between two calls. */
 int pcal_finalize_async(pcal_ctx *ctx, double *out_tones);
+
+/*
+ * One integration period in one call ("single integration ... 10 seconds"; the caller's
+ * loop over periods): pcal_reset, pcal_extract(dev_samples, n_samples, cuda_stream) and
+ * pcal_finalize_async(out_tones), with the argument rules of those calls.  Nothing else is added; it
+ * exists so that a host loop over short periods costs one library call per period.  Asynchronous.
+ */
+int pcal_integrate(pcal_ctx *ctx, const void *dev_samples, uint64_t n_samples, void *cuda_stream, double *out_tones);
 
 /*
  * PCal data analysis on the device (R23-R25): enqueues the DFT and
@@ -234,7 +245,8 @@ int pcal_generator_study(const pcal_gen_case_t *cases, uint32_t n_cases, uint64_
 
 /* Calibration for the roofline report: enqueue a pure streaming read (no decode, no fold) of
  * n_bytes from dev ([device], 16-byte aligned) on cuda_stream, with the load instruction, block
- * size and pipelining of the fold kernels.  Asynchronous; computes nothing; the caller times it.
+ * size and pipelining of the fold kernels; consecutive probes may overlap (programmatic dependent
+ * launch), like consecutive fold kernels.  Asynchronous; computes nothing; the caller times it.
  * What it reaches on a given size is the practical ceiling of a read-once kernel of that size. */
 int pcal_read_probe(pcal_ctx *ctx, const void *dev, uint64_t n_bytes, void *cuda_stream);
 

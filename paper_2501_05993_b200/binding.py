@@ -85,6 +85,7 @@ def lib():
             "pcal_analyze": (i32, [vp, vp, vp]),
             "pcal_finalize": (i32, [vp, vp]),
             "pcal_finalize_async": (i32, [vp, vp]),
+            "pcal_integrate": (i32, [vp, vp, u64, vp, vp]),
             "pcal_get_folded": (i32, [vp, vp]),
             "pcal_get_folded_i64": (i32, [vp, vp]),
             "pcal_add_folded": (i32, [vp, vp]),
@@ -197,6 +198,11 @@ class Pcal:
     def finalize_async(self, out_pinned):
         """Enqueue DFT + copy into a pinned complex128 host tensor; caller synchronises."""
         _check(lib().pcal_finalize_async(self._h, out_pinned.data_ptr()), "pcal_finalize_async")
+
+    def integrate(self, dev_samples, n_samples: int, out_pinned, stream=None):
+        """One integration period: reset + extract + finalize_async in one library call (asynchronous)."""
+        _check(lib().pcal_integrate(self._h, dev_samples.data_ptr(), n_samples, _stream_handle(stream),
+                                    out_pinned.data_ptr()), "pcal_integrate")
 
     def analyze(self, bandpass: bool = True):
         """(summary float64 [n_channels, 8], corrected band-pass complex128 [n_channels, N_bins] or None)."""

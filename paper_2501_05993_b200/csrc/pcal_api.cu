@@ -73,15 +73,15 @@ struct pcal_ctx {
     bool fused;                     // reduction + rotation run inside the fold kernel (pcal_tail.cuh)
     uint32_t* d_cnt;                // [slot][q+1] arrival counters of the fused tail
     double2* d_G;                   // [slot][q][C*n_bins] per-group bins of the fused tail
-    uint32_t* d_done;               // [kTailSlots] completed uses of each slot
-    unsigned long long* d_tick;     // [kTailSlots] tickets taken on each slot
-    uint32_t fold_seq;              // fold launches so far (slot = fold_seq mod kTailSlots)
+    TailState* d_tail_state;        // tickets and progress counters of the fused tail
     size_t partial_slot_bytes;
     uint32_t tail_tpp;              // threads per (channel, bin) pair in stage B of the fused tail
     uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
     bool input_ready;               // pcal_set_input_ready: sample buffers are complete when extract is called
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
+    const double* last_out;         // pcal_finalize_async: last host buffer seen and its device mapping (or null)
+    double2* last_out_mapped;
     double *d_summary, *h_ana;      // analysis outputs: [C][8] + band-pass [C][N] complex
     double2* d_B;
     uint64_t launches;
@@ -135,8 +135,8 @@ static void launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t
 static void free_tables(pcal_ctx* c) {
     cudaFree(c->d_lut); cudaFree(c->d_lut_off); cudaFree(c->d_lut_len);
     cudaFree(c->d_partial); cudaFree(c->d_gen_partial);
-    cudaFree(c->d_val); cudaFree(c->d_cnt); cudaFree(c->d_G); cudaFree(c->d_done); cudaFree(c->d_tick);
-    c->d_cnt = nullptr; c->d_G = nullptr; c->d_done = nullptr; c->d_tick = nullptr;
+    cudaFree(c->d_val); cudaFree(c->d_cnt); cudaFree(c->d_G); cudaFree(c->d_tail_state);
+    c->d_cnt = nullptr; c->d_G = nullptr; c->d_tail_state = nullptr;
     c->d_lut = nullptr; c->d_lut_off = c->d_lut_len = nullptr;
     c->d_partial = nullptr; c->d_gen_partial = nullptr;
     c->d_val = nullptr;
@@ -302,6 +302,8 @@ static int occupancy_of(K kernel, size_t smem) {
     return occ;
 }
 
+static uint32_t dft_ctas(const pcal_ctx* c);
+
 static int prepare(pcal_ctx* c) {
     if (c->prepared) return PCAL_OK;
     free_tables(c);
@@ -358,8 +360,8 @@ static int prepare(pcal_ctx* c) {
         c->R = slots / q ? slots / q : 1;
         if (c->fused) {
             // leave room for the CTAs of the two previous launches that are still in their tail (q+1 each)
-            // and for a DFT kernel: the next launch must become resident in one wave
-            const uint32_t reserve = 2 * (q + 1) + 8;
+            // and for the CTAs of a DFT kernel: the next launch must become resident in one wave
+            const uint32_t reserve = 2 * (q + 1) + dft_ctas(c) + 8;
             if (slots > reserve + q) c->R = (slots - reserve) / q;
             const uint32_t W = 32u * c->spv, per = W / c->n_bins ? W / c->n_bins : 1u;
             uint32_t tpp = 1; while (tpp * 2 <= per && tpp < 32) tpp *= 2;
@@ -368,11 +370,8 @@ static int prepare(pcal_ctx* c) {
             CU(cudaMalloc(&c->d_cnt, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
             CU(cudaMemset(c->d_cnt, 0, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
             CU(cudaMalloc(&c->d_G, ns * (size_t)c->q * pairs * sizeof(double2)));
-            CU(cudaMalloc(&c->d_done, ns * sizeof(uint32_t)));
-            CU(cudaMemset(c->d_done, 0, ns * sizeof(uint32_t)));
-            CU(cudaMalloc(&c->d_tick, ns * sizeof(unsigned long long)));
-            CU(cudaMemset(c->d_tick, 0, ns * sizeof(unsigned long long)));
-            c->fold_seq = 0;
+            CU(cudaMalloc(&c->d_tail_state, sizeof(TailState)));
+            CU(cudaMemset(c->d_tail_state, 0, sizeof(TailState)));
         }
         c->grid = c->q * c->R;
         c->partial_slot_bytes = (size_t)c->grid * c->F * 32 * elem;
@@ -433,8 +432,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         uint64_t it = (NSR + (uint64_t)c->R * kWarps - 1) / ((uint64_t)c->R * kWarps);
         it = (it + kFoldGroup - 1) / kFoldGroup * kFoldGroup;
         fp.n_iter = (uint32_t)it;
-        const uint32_t slot = c->fused ? c->fold_seq % kTailSlots : 0u;   // ring of the fused tail (pcal_tail.cuh)
-        fp.partial = reinterpret_cast<uint8_t*>(c->d_partial) + (size_t)slot * c->partial_slot_bytes;
+        fp.partial = c->d_partial;            // fused tail: slot 0 of the ring; the kernel picks its slot
         const uint64_t grid_threads = (uint64_t)c->R * kWarps * c->q * 32u;
         fp.n_quot = (uint32_t)(n_vec / grid_threads); fp.n_rem = n_vec % grid_threads;
         fp.input_ready = c->input_ready ? 1 : 0;
@@ -442,11 +440,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         memset(&tp, 0, sizeof(tp));
         if (c->fused) {
             tp.enabled = 1;
-            tp.cnt = c->d_cnt + (size_t)slot * (c->q + 1);
-            tp.G = c->d_G + (size_t)slot * c->q * c->n_bins * c->C;
-            tp.tick = c->d_tick + slot; tp.done = c->d_done + slot;
-            if (const char* d = getenv("PCAL_TAIL_DEBUG")) tp.dbg = atoi(d);
-            c->fold_seq += 1;
+            tp.cnt = c->d_cnt; tp.G = c->d_G; tp.st = c->d_tail_state; tp.partial_stride = c->partial_slot_bytes;
             tp.lut = c->d_lut; tp.lut_off = c->d_lut_off; tp.lut_len = c->d_lut_len;
             tp.P = c->d_P; tp.Pint = c->d_Pint; tp.tail = data + n_vec * 16;
             tp.n0 = c->n_processed; tp.NT = n_vec * c->spv; tp.n_total = n;
@@ -489,6 +483,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     rp.kind = c->kind; rp.sign_mag = c->sign_mag;
     rp.integer_exact = (c->all_zero && c->kind != KIND_F32) ? 1 : 0;
     rp.overwrite = c->zero_pending ? 1 : 0;
+    rp.release_late = c->fused ? 1 : 0;       // (fused context, piece without a complete vector)
     const uint32_t pairs = c->n_bins * (uint32_t)c->C, ppc = (uint32_t)kPostThreads / c->rot_tpp;
     launch_chain(rotate_fold_kernel, (pairs + ppc - 1) / ppc, kPostThreads, 0, st, rp);
     c->zero_pending = false;
@@ -632,13 +627,26 @@ extern "C" int pcal_extract_host(pcal_ctx* c, const void* host_samples, uint64_t
 
 // The DFT kernel writes T both to d_T and, when `host_out` is device-visible pinned host memory
 // (cudaHostAlloc / cudaHostRegister under unified addressing), straight into it: no copy node.
+// outputs per warp of dft_kernel: as many as keep the grid at <= 32 CTAs, at most 4096 terms per warp
+static uint32_t dft_opw(const pcal_ctx* c) {
+    const uint32_t per_cta = kDftThreads / 32;
+    uint32_t opw = 1;
+    while ((uint64_t)c->C * ((c->n_bins + per_cta * opw - 1) / (per_cta * opw)) > 32 && (uint64_t)c->n_bins * opw * 2 <= 4096) opw *= 2;
+    return opw;
+}
+static uint32_t dft_ctas(const pcal_ctx* c) {
+    const uint32_t per_cta = kDftThreads / 32 * dft_opw(c);
+    return (uint32_t)c->C * ((c->n_bins + per_cta - 1) / per_cta);
+}
+
 static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const int rz = ensure_zeroed(c);
     if (rz != PCAL_OK) return rz;
     const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
-    const uint32_t per_cta = kDftThreads / 32;
+    const uint32_t opw = dft_opw(c), per_cta = kDftThreads / 32 * opw;
     launch_chain(dft_kernel, dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream,
-                 (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift);
+                 (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift, opw,
+                 c->rot_eff == PCAL_ROT_LUT && c->fused ? c->d_tail_state : (TailState*)nullptr);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
@@ -646,16 +654,28 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
 
 extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
-    double2* mapped = nullptr;
-    cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
-        mapped = reinterpret_cast<double2*>(at.devicePointer);
-    cudaGetLastError();
+    if (out != c->last_out) {     // the attribute query costs more than a launch: remember the answer
+        c->last_out = out; c->last_out_mapped = nullptr;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+            c->last_out_mapped = reinterpret_cast<double2*>(at.devicePointer);
+        cudaGetLastError();
+    }
+    double2* mapped = c->last_out_mapped;
     const int r = enqueue_dft(c, mapped);
     if (r != PCAL_OK) return r;
     if (!mapped)
         CU(cudaMemcpyAsync(out, c->d_T, (size_t)c->n_bins * c->C * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
     return PCAL_OK;
+}
+
+extern "C" int pcal_integrate(pcal_ctx* c, const void* dev_samples, uint64_t n_samples, void* cuda_stream, double* out) {
+    int r = pcal_reset(c);
+    if (r != PCAL_OK) return r;
+    r = pcal_extract(c, dev_samples, n_samples, cuda_stream);
+    if (r != PCAL_OK) return r;
+    c->stream = (cudaStream_t)cuda_stream;
+    return pcal_finalize_async(c, out);
 }
 
 extern "C" int pcal_finalize(pcal_ctx* c, double* out) {
@@ -787,7 +807,7 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
     const char* pp = getenv("PCAL_PROBE_PDL");
     uint32_t spin_ns = 0;
     if (const char* sp = getenv("PCAL_PROBE_SPIN_NS")) spin_ns = (uint32_t)atoi(sp);
-    if (pp && pp[0] == '1')
+    if (!(pp && pp[0] == '0'))      // default: consecutive probes may overlap, like the fold kernels
         launch_chain(read_probe_kernel, grid, kThreads, 0, (cudaStream_t)cuda_stream,
                      reinterpret_cast<const uint4*>(dev), (uint64_t)(n_bytes / 16), reinterpret_cast<uint32_t*>(c->d_tmp), spin_ns);
     else

@@ -61,7 +61,7 @@ template <bool SIGN_MAG, int U, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
     static_assert(U == 4 || U == 8, "block of 4 or 8 loads");
-    __shared__ uint32_t s_gen[2];
+    __shared__ uint32_t s_gen[3];
     __shared__ __align__(16) uint32_t hlf[32][kThreads];   // weight-16 sums in 16-bit lanes: [8j + f8] = fields f8, f8+8 of word j
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint64_t first = fold_first_vec(P, w, lane);
@@ -167,7 +167,8 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(const __grid_
     }
     __syncthreads();
     fold_wait_slot(P.tail, s_gen);
-    uint16_t* out = reinterpret_cast<uint16_t*>(P.partial) + (size_t)blockIdx.x * 64 * 32;
+    void* partial = fold_partial_of(P.tail, P.partial, s_gen);
+    uint16_t* out = reinterpret_cast<uint16_t*>(partial) + (size_t)blockIdx.x * 64 * 32;
 #pragma unroll
     for (int x = tid; x < 32 * 32; x += kThreads) {
         const int h = x >> 5, ln = x & 31;
@@ -178,7 +179,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(const __grid_
         out[f * 32 + ln] = (uint16_t)(s & 0xFFFFu);
         out[(f + 8) * 32 + ln] = (uint16_t)(s >> 16);
     }
-    if (P.tail.enabled) fold_tail<KIND_2BIT>(P.tail, P.partial, P.q, P.R, reinterpret_cast<double*>(&hlf[0][0]), s_gen[0]);
+    if (P.tail.enabled) fold_tail<KIND_2BIT>(P.tail, partial, P.q, P.R, reinterpret_cast<double*>(&hlf[0][0]), s_gen[0], s_gen[1]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -187,7 +188,7 @@ __global__ void __launch_bounds__(kThreads, MINB) fold_2bit_kernel(const __grid_
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
-    __shared__ uint32_t s_gen[2];
+    __shared__ uint32_t s_gen[3];
     __shared__ __align__(16) int32_t sh[kWarps][16][32];   // also the (double) scratch of the fused tail
     fold_ticket_and_release(P.tail, s_gen);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -216,7 +217,8 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_const
     for (int k = 0; k < 16; ++k) sh[w][k][lane] = acc[k];
     __syncthreads();
     fold_wait_slot(P.tail, s_gen);
-    int32_t* out = reinterpret_cast<int32_t*>(P.partial) + (size_t)blockIdx.x * 16 * 32;
+    void* partial = fold_partial_of(P.tail, P.partial, s_gen);
+    int32_t* out = reinterpret_cast<int32_t*>(partial) + (size_t)blockIdx.x * 16 * 32;
     for (int e = threadIdx.x; e < 16 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;
         int32_t s = 0;
@@ -224,7 +226,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_const
         for (int ww = 0; ww < kWarps; ++ww) s += sh[ww][f][ln];
         out[f * 32 + ln] = s;
     }
-    if (P.tail.enabled) fold_tail<KIND_I8>(P.tail, P.partial, P.q, P.R, reinterpret_cast<double*>(&sh[0][0][0]), s_gen[0]);
+    if (P.tail.enabled) fold_tail<KIND_I8>(P.tail, partial, P.q, P.R, reinterpret_cast<double*>(&sh[0][0][0]), s_gen[0], s_gen[1]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -234,7 +236,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_const
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_constant__ FoldParams P) {
     if (!P.input_ready) pdl_wait();
-    __shared__ uint32_t s_gen[2];
+    __shared__ uint32_t s_gen[3];
     __shared__ __align__(16) double sh[kWarps][4][32];   // 1024 doubles: also the scratch of the fused tail
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint64_t idx = fold_first_vec(P, w, lane);
@@ -267,7 +269,8 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_cons
     for (int k = 0; k < 4; ++k) sh[w][k][lane] = tot[k];
     __syncthreads();
     fold_wait_slot(P.tail, s_gen);
-    double* out = reinterpret_cast<double*>(P.partial) + (size_t)blockIdx.x * 4 * 32;
+    void* partial = fold_partial_of(P.tail, P.partial, s_gen);
+    double* out = reinterpret_cast<double*>(partial) + (size_t)blockIdx.x * 4 * 32;
     for (int e = threadIdx.x; e < 4 * 32; e += kThreads) {
         const int f = e >> 5, ln = e & 31;
         double s = 0.0;
@@ -275,7 +278,7 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_cons
         for (int ww = 0; ww < kWarps; ++ww) s += sh[ww][f][ln];  // fixed warp order: deterministic
         out[f * 32 + ln] = s;
     }
-    if (P.tail.enabled) fold_tail<KIND_F32>(P.tail, P.partial, P.q, P.R, &sh[0][0][0], s_gen[0]);
+    if (P.tail.enabled) fold_tail<KIND_F32>(P.tail, partial, P.q, P.R, &sh[0][0][0], s_gen[0], s_gen[1]);
 }
 
 }  // namespace pcal

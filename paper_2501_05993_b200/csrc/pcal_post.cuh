@@ -13,6 +13,16 @@ namespace pcal {
 
 constexpr int kPostThreads = 256;
 
+// Progress counters of a context whose fold kernels run the fused tail (pcal_tail.cuh, "Pipelining").
+struct TailState {
+    unsigned long long tick;  // tickets taken (one per CTA of every fold launch)
+    uint32_t n_done;          // fold launches whose stage C has finished
+    uint32_t dft_started;     // CTAs of DFT kernels that have started ...
+    uint32_t dft_finished;    // ... and that have finished reading P
+    uint32_t pad;
+};
+
+
 // ---- stage 1: sum the R replicas of every slot group -------------------------------------------
 // in : elem partial[(rho*q + p)][F][32]          out: double val[p][F][32]
 // For 2-bit data the partials are code sums; val = 2*sum - 3*(vectors folded into this slot) is the
@@ -94,6 +104,7 @@ struct RotateParams {
     int sign_mag;
     int integer_exact;        // every channel unrotated and integer input: keep Pint
     int overwrite;            // first piece after reset: P = new instead of P += new
+    int release_late;         // do not let the dependent grid start early (its stage C reads P without a grid-wide wait)
 };
 
 __device__ __forceinline__ double decode_tail(int kind, int sign_mag, const uint8_t* tail, uint32_t t, uint32_t c, uint32_t C) {
@@ -111,7 +122,7 @@ __device__ __forceinline__ double decode_tail(int kind, int sign_mag, const uint
 // thread u adds its elements j = u, u + tpp, ... in order (four look-ups in flight), then the
 // lane sums are combined by a fixed butterfly (and, for tpp = 256, the 8 warp sums in warp order).
 __global__ void __launch_bounds__(kPostThreads) rotate_fold_kernel(RotateParams P) {
-    pdl_release();
+    if (!P.release_late) pdl_release();
     pdl_wait();
     __shared__ double sre[kPostThreads / 32], sim[kPostThreads / 32];
     __shared__ long long sint[kPostThreads / 32];
@@ -254,13 +265,18 @@ __global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G)
 
 // ---- DFT of the folded period ------------------------------------------------------------------
 // T[c][i] = sum_b P[c][b] * W[(i'*b) mod N], i' = (i - k_shift) mod N, W[k] = exp(-j 2 pi k/N)
-// (twiddle table built on the host in long double).  One warp per output: lane l sums the terms
-// b = l, l+32, ... in order, then a fixed xor-butterfly adds the 32 lane sums.  The twiddle index
-// is stepped in integers, never formed as a floating-point angle.
+// (twiddle table built on the host in long double).  One warp per output (opw outputs in turn, so
+// that the grid stays small: its CTAs share the SMs with the streaming kernel of the next step): lane l
+// sums the terms b = l, l+32, ... in order, then a fixed xor-butterfly adds the 32 lane sums.  The
+// twiddle index is stepped in integers, never formed as a floating-point angle.
 constexpr int kDftThreads = 256;
 __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restrict__ P, const double2* __restrict__ W,
                                                           double2* __restrict__ T, double2* __restrict__ T_host,
-                                                          uint32_t N, uint32_t k_shift) {
+                                                          uint32_t N, uint32_t k_shift, uint32_t opw, TailState* st) {
+    if (st) {   // counted before the dependents may start: a later fold kernel waits for these CTAs to have read P
+        if (threadIdx.x == 0) atomicAdd(&st->dft_started, 1u);
+        __syncthreads();
+    }
     pdl_release();
     pdl_wait();
     extern __shared__ double2 dft_sm[];  // [N] bins of this channel, [N] twiddles
@@ -272,27 +288,29 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
         sw[t] = W[t];
     }
     __syncthreads();
+    if (st && threadIdx.x == 0) { __threadfence(); atomicAdd(&st->dft_finished, 1u); }   // P has been read
     const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t i = blockIdx.x * (kDftThreads / 32) + (threadIdx.x >> 5);
-    if (i >= N) return;                                   // whole warp leaves together
-    const uint32_t ii = (i + N - k_shift % N) % N;
-    uint32_t k = (uint32_t)(((uint64_t)ii * lane) % N);
-    const uint32_t kstep = (uint32_t)(((uint64_t)ii * 32u) % N);
-    double re = 0.0, im = 0.0;
-    for (uint32_t b = lane; b < N; b += 32u) {
-        const double2 p = sp[b], w = sw[k];
-        re += p.x * w.x - p.y * w.y;
-        im += p.x * w.y + p.y * w.x;
-        k += kstep; if (k >= N) k -= N;
-    }
+    const uint32_t i0 = (blockIdx.x * (kDftThreads / 32) + (threadIdx.x >> 5)) * opw;
+    for (uint32_t i = i0; i < i0 + opw && i < N; ++i) {       // whole warp together
+        const uint32_t ii = (i + N - k_shift % N) % N;
+        uint32_t k = (uint32_t)(((uint64_t)ii * lane) % N);
+        const uint32_t kstep = (uint32_t)(((uint64_t)ii * 32u) % N);
+        double re = 0.0, im = 0.0;
+        for (uint32_t b = lane; b < N; b += 32u) {
+            const double2 p = sp[b], w = sw[k];
+            re += p.x * w.x - p.y * w.y;
+            im += p.x * w.y + p.y * w.x;
+            k += kstep; if (k >= N) k -= N;
+        }
 #pragma unroll
-    for (uint32_t s = 16; s > 0; s >>= 1) {
-        re += __shfl_xor_sync(0xFFFFFFFFu, re, s);
-        im += __shfl_xor_sync(0xFFFFFFFFu, im, s);
-    }
-    if (lane == 0) {
-        T[(size_t)c * N + i] = make_double2(re, im);
-        if (T_host) T_host[(size_t)c * N + i] = make_double2(re, im);   // mapped pinned host memory
+        for (uint32_t s = 16; s > 0; s >>= 1) {
+            re += __shfl_xor_sync(0xFFFFFFFFu, re, s);
+            im += __shfl_xor_sync(0xFFFFFFFFu, im, s);
+        }
+        if (lane == 0) {
+            T[(size_t)c * N + i] = make_double2(re, im);
+            if (T_host) T_host[(size_t)c * N + i] = make_double2(re, im);   // mapped pinned host memory
+        }
     }
 }
 

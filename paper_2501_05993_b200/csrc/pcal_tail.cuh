@@ -17,27 +17,31 @@
 //      launch.
 // A step of the LUT path is thereby ONE launch (plus the DFT of pcal_finalize).
 //
-// Pipelining across launches.  Partials, counters and G live in a ring of kTailSlots slots; the host
-// hands consecutive launches consecutive slots.  A fold kernel never executes griddepcontrol.wait
-// before its partial writes.  Instead every CTA takes a ticket of its slot (64-bit atomicAdd) BEFORE
-// it lets the dependent grid be scheduled; a dependent grid starts only after every CTA of its
-// predecessor has done so, hence all tickets of launch s are taken before any CTA of a later launch
-// runs, and ticket / gridDim.x is the number g of earlier uses of the slot -- derived on the device, so
-// launches replayed from a CUDA graph (frozen parameters) stay correct.  Before its partial writes a
-// CTA checks (acquire load, spinning if ever needed) that done[slot] == g, i.e. that the stage-C CTA of
-// the slot's previous user -- a grid dispatched long before -- has finished reading it; that CTA
-// publishes g + 1 after its last read.  Only the ONE CTA that runs stage C executes
-// griddepcontrol.wait (predecessor grid complete, hence -- transitively -- every earlier grid, incl. the
-// DFT kernel that reads P) before it touches P.  Consecutive launches therefore overlap completely
-// except for stage C, and HBM never drains at a kernel boundary.
+// Pipelining across launches.  Partials, counters and G live in a ring of kTailSlots slots and a fold
+// kernel never executes griddepcontrol.wait.  Every CTA takes a ticket (64-bit atomicAdd on the
+// context's TailState) BEFORE it lets the dependent grid be scheduled; a dependent grid starts only
+// after every CTA of its predecessor has done so, hence all tickets of one launch are taken before any
+// CTA of a later launch runs and s = ticket / gridDim.x is the launch's sequence number -- derived on the
+// device, so launches replayed from a CUDA graph (frozen parameters) stay correct.  Launch s uses slot
+// s mod kTailSlots.  Three conditions replace the grid-wide wait, each checked by one thread with an
+// acquire load (spinning only if ever needed; the grids waited for were dispatched earlier, so they
+// make progress):
+//   before the partial writes   n_done >= s - kTailSlots + 1   (the slot's previous user finished stage C)
+//   before stage C              n_done == s                    (P holds every earlier launch, in order)
+//   before stage C              dft_finished >= X              (every earlier DFT kernel has read P; X =
+//                               dft_started as seen before this CTA released its dependents, i.e. the
+//                               CTAs of all DFT kernels that precede this launch in the stream)
+// and stage C ends by publishing n_done = s + 1.  Consecutive launches therefore overlap completely
+// except for stage C, and HBM never drains at a kernel boundary.  Kernels that follow in plain stream
+// order (and the DFT kernel, which waits for its predecessor grid) see the finished accumulators.
 #pragma once
 #include "pcal_post.cuh"
 
 namespace pcal {
 
 struct TailParams {
-    uint32_t* cnt;            // [device] q+1 arrival counters, zero between launches
-    double2* G;               // [device] per-group bins [q][C*n_bins]
+    uint32_t* cnt;            // [device] [slot][q+1] arrival counters, zero between launches
+    double2* G;               // [device] [slot][q][C*n_bins] per-group bins
     const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
     const uint32_t* lut_off;  // [device] per channel: first entry
     const uint32_t* lut_len;  // [device] per channel: N_rotator,c (1 => no rotation)
@@ -52,9 +56,8 @@ struct TailParams {
     uint32_t tpp;             // threads per (channel, bin) pair in stage B: power of two <= 32
     int kind, sign_mag, integer_exact, overwrite;
     int enabled;              // 0: the caller launches reduce_replicas_kernel + rotate_fold_kernel instead
-    unsigned long long* tick; // [device] ticket counter of this launch's slot
-    uint32_t* done;           // [device] completed uses of this launch's slot
-    int dbg;                  // tuning runs only (PCAL_TAIL_DEBUG): 1 = stage C without griddepcontrol.wait, 2 = no tail at all
+    TailState* st;            // [device] tickets and progress counters of the context
+    uint64_t partial_stride;  // bytes between the partial buffers of consecutive slots
 };
 
 constexpr uint32_t kTailSlots = 8;
@@ -76,15 +79,17 @@ __device__ __forceinline__ uint32_t arrive_acq_rel(uint32_t* p) {
     return v;
 }
 
-// Called by every thread of a fold kernel once its first loads are in flight: slot ticket, then the
-// dependent grid may be scheduled.  *s_gen (shared) = number of earlier uses of the slot.
-// s_gen[1] = 1 when the slot was already free at that time (the usual case: no check needed later).
+// Called by every thread of a fold kernel once its first loads are in flight: ticket, then the dependent
+// grid may be scheduled.  s_gen (shared): [0] = sequence number s of this launch, [1] = X (see above),
+// [2] = 1 when the slot was already free at that time (the usual case: nothing to check later).
 __device__ __forceinline__ void fold_ticket_and_release(const TailParams& T, uint32_t* s_gen) {
     if (T.enabled) {
         if (threadIdx.x == 0) {
-            const uint32_t seen = ld_acquire_u32(T.done);
-            const uint32_t g = (uint32_t)(atomicAdd(T.tick, 1ull) / gridDim.x);
-            s_gen[0] = g; s_gen[1] = (seen == g) ? 1u : 0u;
+            const uint32_t done = ld_acquire_u32(&T.st->n_done);
+            const uint32_t x = ld_acquire_u32(&T.st->dft_started);
+            const uint32_t seq = (uint32_t)(atomicAdd(&T.st->tick, 1ull) / gridDim.x);
+            s_gen[0] = seq; s_gen[1] = x;
+            s_gen[2] = ((int32_t)(done - (seq - kTailSlots + 1u)) >= 0) ? 1u : 0u;
         }
         __syncthreads();      // thread 0 holds the ticket (it stored the quotient) before any thread releases
     }
@@ -94,28 +99,35 @@ __device__ __forceinline__ void fold_ticket_and_release(const TailParams& T, uin
 // Called by every thread of a fold kernel after its loads and before its partial writes.
 __device__ __forceinline__ void fold_wait_slot(const TailParams& T, const uint32_t* s_gen) {
     if (T.enabled) {
-        if (threadIdx.x == 0 && !s_gen[1] && !(T.dbg & 6))
-            while (ld_acquire_u32(T.done) != s_gen[0]) __nanosleep(64);
+        if (threadIdx.x == 0 && !s_gen[2])
+            while ((int32_t)(ld_acquire_u32(&T.st->n_done) - (s_gen[0] - kTailSlots + 1u)) < 0) __nanosleep(64);
         __syncthreads();
     } else {
         pdl_wait();   // the partials of the previous launch may still be read by its reduce kernel
     }
 }
 
+// this launch's partial buffer
+__device__ __forceinline__ void* fold_partial_of(const TailParams& T, void* base, const uint32_t* s_gen) {
+    return T.enabled ? reinterpret_cast<uint8_t*>(base) + (uint64_t)(s_gen[0] % kTailSlots) * T.partial_stride : base;
+}
+
 // `scratch` = shared memory the caller no longer needs: max(2*F*32, 512) doubles, 16-byte aligned.
 template <int KIND>
-__device__ __noinline__ void fold_tail(const TailParams& T, const void* partial, uint32_t q, uint32_t R, double* scratch, uint32_t gen) {
+__device__ __noinline__ void fold_tail(const TailParams& T, const void* partial, uint32_t q, uint32_t R, double* scratch,
+                                       uint32_t seq, uint32_t dft_x) {
     __shared__ uint32_t s_prev;
     const uint32_t tid = threadIdx.x;
     const uint32_t p = blockIdx.x % q;
+    const uint32_t slot = seq % kTailSlots;
+    uint32_t* cnt = T.cnt + (size_t)slot * (q + 1u);
     constexpr uint32_t F = KIND == KIND_2BIT ? 64u : (KIND == KIND_I8 ? 16u : 4u);
     constexpr uint32_t E = F * 32u;
 
-    if (T.dbg & 2) return;
     __syncthreads();          // every thread's partial writes happen before thread 0's release below
-    if (tid == 0) s_prev = arrive_acq_rel(T.cnt + p);
+    if (tid == 0) s_prev = arrive_acq_rel(cnt + p);
     __syncthreads();
-    if (s_prev != R - 1u || (T.dbg & 4)) return;
+    if (s_prev != R - 1u) return;
 
     // ---- stage A: replica sums of group p ---------------------------------------------------
     if (KIND == KIND_2BIT) {
@@ -183,7 +195,8 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         }
         __syncthreads();
     }
-    double2* Gp = T.G + (size_t)p * pairs;
+    const double2* G = T.G + (size_t)slot * q * pairs;
+    double2* Gp = T.G + ((size_t)slot * q + p) * pairs;
     for (uint32_t s0 = 0; s0 < pairs * tpp; s0 += kThreads) {          // uniform trip count: shuffles below
         const uint32_t slot = s0 + tid;
         const bool active = slot < pairs * tpp;
@@ -207,12 +220,16 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     }
 
     __syncthreads();
-    if (tid == 0) s_prev = arrive_acq_rel(T.cnt + q);
+    if (tid == 0) s_prev = arrive_acq_rel(cnt + q);
     __syncthreads();
     if (s_prev != q - 1u) return;
 
     // ---- stage C: groups in order, ragged tail, accumulate into the context ------------------
-    if (!(T.dbg & 1)) pdl_wait();   // every earlier grid (incl. a DFT kernel reading P) has completed
+    if (tid == 0) {
+        while (ld_acquire_u32(&T.st->n_done) != seq) __nanosleep(32);                          // P is up to date
+        while ((int32_t)(ld_acquire_u32(&T.st->dft_finished) - dft_x) < 0) __nanosleep(32);   // and no longer being read
+    }
+    __syncthreads();
     // thread = (slice sl of the groups, pair): slice sums first (all loads of a thread in flight at
     // once where possible), then the slices in order.
     const uint32_t ppc = pairs < (uint32_t)kThreads ? pairs : (uint32_t)kThreads;
@@ -228,7 +245,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
             for (uint32_t g0 = sl; g0 < q; g0 += 8u * ns) {
                 double2 g[8];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) g[k] = (g0 + k * ns < q) ? __ldcg(T.G + (size_t)(g0 + k * ns) * pairs + pp) : make_double2(0.0, 0.0);
+                for (int k = 0; k < 8; ++k) g[k] = (g0 + k * ns < q) ? __ldcg(G + (size_t)(g0 + k * ns) * pairs + pp) : make_double2(0.0, 0.0);
 #pragma unroll
                 for (int k = 0; k < 8; ++k) { are += g[k].x; aim += g[k].y; }
             }
@@ -266,9 +283,9 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         T.P[pp] = make_double2(are, aim);
         if (T.integer_exact) T.Pint[pp] = ai;
     }
-    for (uint32_t i = tid; i <= q; i += kThreads) T.cnt[i] = 0u;       // ready for the slot's next launch
+    for (uint32_t i = tid; i <= q; i += kThreads) cnt[i] = 0u;         // ready for the slot's next launch
     __syncthreads();
-    if (tid == 0) st_release_u32(T.done, gen + 1u);                    // the slot may be written again
+    if (tid == 0) st_release_u32(&T.st->n_done, seq + 1u);             // P is final for this launch; the slot is free
 }
 
 }  // namespace pcal
