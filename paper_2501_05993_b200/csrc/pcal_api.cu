@@ -14,6 +14,7 @@
 #include "../../include/pcal.h"
 #include "pcal_fold.cuh"
 #include "pcal_gen.cuh"
+#include "pcal_gen_mma.cuh"
 #include "pcal_post.cuh"
 #include "pcal_analysis.cuh"
 #include "pcal_genstudy.cuh"
@@ -61,6 +62,7 @@ struct pcal_ctx {
     uint64_t M, nrot[PCAL_MAX_CHANNELS], lut_len[PCAL_MAX_CHANNELS];
     // generator-mode geometry
     uint32_t gen_grid, gen_spt;
+    bool gen_mma;                   // integer samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
     size_t gen_smem;
     // device
     int device, sm_count;
@@ -329,7 +331,9 @@ static int prepare(pcal_ctx* c) {
         lut_ok = qq <= kMaxSlotGroups;
         q = (uint32_t)qq;
     }
-    const bool gen_ok = c->C == 1 && (kThreads * c->gen_spt) % c->n_bins == 0;
+    const char* gm = getenv("PCAL_GEN_MMA");       // =0: FFMA2 kernel of pcal_gen.cuh for every sample type (A/B runs, tests)
+    c->gen_mma = c->C == 1 && c->kind != KIND_F32 && kMmaSpan % c->n_bins == 0 && !(gm && gm[0] == '0');
+    const bool gen_ok = c->C == 1 && (c->gen_mma || (kThreads * c->gen_spt) % c->n_bins == 0);
     int mode;
     if (c->all_zero) mode = PCAL_ROT_LUT;
     else if (c->rot_req == PCAL_ROT_LUT) mode = lut_ok ? PCAL_ROT_LUT : 0;
@@ -396,7 +400,9 @@ static int prepare(pcal_ctx* c) {
         CU(cudaMemcpy(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
     } else {
         int occ = 0;
-        if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
+        if (c->gen_mma && c->kind == KIND_2BIT) { c->gen_smem = gen_mma_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_2BIT>, c->gen_smem); }
+        else if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8>, c->gen_smem); }
+        else if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
         else if (c->kind == KIND_I8) { c->gen_smem = gen_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_I8>, c->gen_smem); }
         else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
         if (occ < 1) return PCAL_ERR_DEVICE;
@@ -496,7 +502,8 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     const uint32_t spt = c->gen_spt;
     const uint64_t load_bytes = c->kind == KIND_2BIT ? 4 : 16;
     const uint64_t n_bytes = n * (uint64_t)c->bits / 8;
-    const uint64_t n_loads = n_bytes / load_bytes;
+    uint64_t n_loads = n_bytes / load_bytes;
+    if (c->gen_mma) n_loads -= n_loads % (kMmaSpan / spt);        // whole 2048-sample rows; the rest goes to the post kernel
     const uint64_t Fs = c->Fs, Fo = c->Feff[0];
     if (n_loads) {
         GenParams gp;
@@ -514,7 +521,9 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.input_ready = c->input_ready ? 1 : 0;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
-        if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
+        if (c->gen_mma && c->kind == KIND_2BIT) launch_chain(gen_mma_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
+        else if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
+        else if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
         else if (c->kind == KIND_I8) launch_chain(gen_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
         else launch_chain(gen_kernel<KIND_F32>, c->gen_grid, kThreads, smem, st, gp);
         prof_mark(c, st);

@@ -125,7 +125,9 @@ __device__ __forceinline__ void gen_decode_2bit(uint32_t v, float* x, int sign_m
 template <int BYTES>
 __device__ __forceinline__ void cp_async_own(void* smem_dst, const void* gsrc) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    static_assert(BYTES == 16 || BYTES == 8 || BYTES == 4, "cp.async sizes");
     if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+    else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
     else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }

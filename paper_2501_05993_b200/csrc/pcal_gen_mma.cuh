@@ -1,0 +1,287 @@
+// pcal_gen_mma.cuh -- generator path for integer samples (int8, 2-bit) as a dense contraction on the
+// tensor cores (eq. 2.3 + 2.2 with the phasor of eq. 2.5).
+//
+// With the sample index written as n = n0 + 2^16 tile + 2048 row + pos (pos < 2048, row < 32),
+//     P[b] = sum_{pos = b mod N_bins} e^{-j w pos} * sum_{tile,row} x[tile,row,pos] * rho[tile,row],
+//     rho[tile,row] = e^{-j w (n0 + 2^16 tile)} * e^{-j w 2048 row}
+// (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is
+// a matrix product  X^T (2048 positions x rows)  *  R (rows x {Re, Im})  -- a contraction over TIME with a
+// two-column right-hand side.  It runs as integer tensor-core MMAs (mma.sync m16n8k16, s8 x s8 -> s32):
+// the phasor is quantised to 23-bit fixed point, round(rho 2^22) = d0 + 2^8 d1 + 2^16 d2 with signed 8-bit
+// digits, and the six digit columns (3 for Re, 3 for Im) fill the n = 8 side of the MMA.  All sums are exact
+// integers (int32 per digit column; |sum| < 2^31 for the <= 256 tiles a CTA sees per launch), recombined
+// and converted to fp64 once per launch.  The only approximation is the 2^-23 phasor quantisation
+// (relative error of a bin ~1e-7).
+//
+// Generator and resync.  rho[tile,row]: the tile factor comes from the exactly reduced INTEGER phase
+// ((n0 + 2^16 tile) F_off mod F_s, the "fp64 phase resync every 2^16 samples" of BASELINE.json config 5),
+// the row factor from a 32-entry table of exact stride phasors e^{-j w 2048 row} (stride stepping as in
+// eq. 2.8); one coupled-form complex multiply (eq. 2.6) per row in fp64, never more than 31 strides from
+// a resync point.  Each warp builds its own copy of the 32 x 8 digit matrix per tile (lane = row).
+//
+// Data movement.  A row is 2048 positions (2048 B of int8, 512 B of 2-bit codes); warp w owns positions
+// 256 w .. 256 w + 255.  Thread (g = lane/4, t = lane%4) owns, for its 8 rows 16h + 4t + j, 32 positions:
+// int8: the two 16-byte blocks c = 0, 1 at 256 w + 128 c + 16 g; 2-bit: the 8 bytes (two 16-sample words) at
+// byte 64 w + 8 g of the row.  Its own cp.async ring (no barrier), every byte used by exactly one thread.  The MMA wants
+// four consecutive ROWS of one position in a register, memory has positions consecutive: a 4x4 byte
+// transpose (8 PRMT per 16 samples) turns 4 row words into 4 position words.  2-bit words are first spread
+// into bytes (shift + mask per 4 samples) and stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho)
+// term, which does not depend on the data, is added once at the end from the same quantised phasors.
+// Rows past the end of the segment get zero digits, so whatever their ring slots hold contributes nothing.
+// ~1 instruction per sample instead of 3-4 for the FFMA2 kernel of pcal_gen.cuh: HBM-bound at any SM clock.
+#pragma once
+#include "pcal_gen.cuh"
+
+namespace pcal {
+
+constexpr uint32_t kMmaSpan = 2048;                    // positions per row
+constexpr uint32_t kMmaRows = kTileSamples / kMmaSpan; // 32 rows per tile
+
+template <int KIND> struct GenMmaCfg;
+// LB bytes per load; GPT commit groups (of 4 loads: 4 consecutive rows) per tile; DG groups in flight per thread
+template <> struct GenMmaCfg<KIND_I8>   { static constexpr int LB = 16, GPT = 4, DG = 4; };   // groups (h, block c)
+template <> struct GenMmaCfg<KIND_2BIT> { static constexpr int LB = 8,  GPT = 2, DG = 8; };   // groups h; 8 B = 2 words = 32 samples
+
+template <int KIND>
+constexpr size_t gen_mma_smem_bytes() {
+    const size_t ring = (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
+    const size_t fin = (size_t)kMmaSpan * sizeof(double2);              // final per-position values alias the ring
+    return (size_t)kGenMaxTiles * sizeof(double2) + kMmaRows * sizeof(double2) + (size_t)kWarps * 256 + (ring > fin ? ring : fin);
+}
+
+__device__ __forceinline__ void mma_s8_k16(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a0), "r"(a1), "r"(b0));
+}
+
+// rows r0..r3 (bytes = 4 positions each) -> o[p] = (r0.p, r1.p, r2.p, r3.p), byte 0 = row 0
+__device__ __forceinline__ void transpose4x4_bytes(uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3, uint32_t (&o)[4]) {
+    const uint32_t x01l = __byte_perm(r0, r1, 0x5140), x01h = __byte_perm(r0, r1, 0x7362);
+    const uint32_t x23l = __byte_perm(r2, r3, 0x5140), x23h = __byte_perm(r2, r3, 0x7362);
+    o[0] = __byte_perm(x01l, x23l, 0x5410); o[1] = __byte_perm(x01l, x23l, 0x7632);
+    o[2] = __byte_perm(x01h, x23h, 0x5410); o[3] = __byte_perm(x01h, x23h, 0x7632);
+}
+
+// signed base-256 digits of v (|v| <= 2^22): v = d0 + 256 d1 + 65536 d2
+__device__ __forceinline__ void digits3(int v, int& d0, int& d1, int& d2) {
+    d0 = ((v + 128) & 0xFF) - 128; v = (v - d0) >> 8;
+    d1 = ((v + 128) & 0xFF) - 128; d2 = (v - d1) >> 8;
+}
+
+template <int LB>
+__device__ __forceinline__ void cp_async_pred(void* smem_dst, const void* gsrc, bool ok) {
+    if (ok) cp_async_own<LB>(smem_dst, gsrc);
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_constant__ GenParams P) {
+    pdl_release();
+    if (!P.input_ready) pdl_wait();
+    constexpr int LB = GenMmaCfg<KIND>::LB, DG = GenMmaCfg<KIND>::DG;
+    constexpr uint32_t ROW_BYTES = KIND == KIND_I8 ? kMmaSpan : kMmaSpan / 4;
+    constexpr uint32_t TILE_BYTES = ROW_BYTES * kMmaRows;
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    double2* base = reinterpret_cast<double2*>(gen_smem);                       // [kGenMaxTiles] tile-start phasors
+    double2* rtab = base + kGenMaxTiles;                                         // [32] exp(-j w 2048 row)
+    unsigned char* bt_all = reinterpret_cast<unsigned char*>(rtab + kMmaRows);   // [warp][8 digit columns][32 rows]
+    unsigned char* ring = bt_all + kWarps * 256;                                 // [DG*4][kThreads][LB]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    unsigned char* bt = bt_all + warp * 256;
+
+    const uint64_t n_rows = P.n_loads / (kMmaSpan / 16);                         // host loads = 16 samples; whole rows only (host guarantees a multiple)
+    const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    // this thread's loads of one tile, in consumption order: group-major, 4 consecutive rows per group
+    //   int8 : l = 8h + 4c + j -> row 16h + 4t + j, block c        2-bit: l = 4h + j -> row 16h + 4t + j
+    constexpr int GPT = GenMmaCfg<KIND>::GPT;
+    const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
+    const uint32_t col_off = (uint32_t)(warp * (ROW_BYTES / kWarps) + g * LB);
+    auto row_of = [&](int l) -> uint32_t {
+        return KIND == KIND_I8 ? (uint32_t)(16 * (l >> 3) + 4 * t + (l & 3)) : (uint32_t)(16 * (l >> 2) + 4 * t + (l & 3));
+    };
+    auto load_off = [&](int l) -> uint32_t {                  // byte offset inside a tile
+        const uint32_t c = KIND == KIND_I8 ? (uint32_t)((l >> 2) & 1) : 0u;
+        return row_of(l) * ROW_BYTES + col_off + c * (ROW_BYTES / 16);
+    };
+    // ring slot of this thread inside its warp's 32*LB bytes: lanes that read consecutive global addresses
+    // (same t, g = 0..7) sit in one contiguous run, so a cp.async of the warp writes whole shared-memory
+    // lines; the run is permuted (g ^ 2t for 16-byte loads, g ^ 4(t/2) for 8-byte loads) so that every
+    // LDS.128 quarter-warp / LDS.64 half-warp lands on distinct bank groups.
+    const uint32_t chunk = (uint32_t)t * 8u + (LB == 16 ? (uint32_t)(g ^ (2 * t)) : (uint32_t)(g ^ (4 * (t >> 1))));
+    unsigned char* my_ring = ring + ((size_t)warp * 32 + chunk) * LB;
+    constexpr size_t SLOT = (size_t)kThreads * LB;
+    const uint64_t tile_stride = (uint64_t)gridDim.x * TILE_BYTES;
+    uint64_t tile_byte0 = (uint64_t)blockIdx.x * TILE_BYTES;                     // first byte of this CTA's tile i
+    uint64_t tile_row0 = (uint64_t)blockIdx.x * kMmaRows;
+    const uint64_t row_stride = (uint64_t)gridDim.x * kMmaRows;
+
+    // issue the loads of commit group `grp` of the tile that starts at (byte0, row0)
+    auto issue_group = [&](uint64_t byte0, uint64_t row0, bool tile_exists, int grp, int slot_grp) {
+        const uint32_t lim = (tile_exists && row0 < n_rows) ? (uint32_t)(n_rows - row0 < kMmaRows ? n_rows - row0 : kMmaRows) : 0u;
+        const unsigned char* src = gdata + byte0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int l = grp * 4 + j;
+            cp_async_pred<LB>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT, src + load_off(l), row_of(l) < lim);
+        }
+        cp_async_commit();
+    };
+    // prologue: DG groups = DG/GPT tiles ahead
+    static_assert(DG % GPT == 0, "whole tiles in flight");
+#pragma unroll
+    for (int d = 0; d < DG; ++d) {
+        const uint32_t ti = d / GPT;
+        issue_group(tile_byte0 + ti * tile_stride, tile_row0 + ti * row_stride, ti < nt, d % GPT, d);
+    }
+
+    // (the first loads are in flight: now the tables)
+    {   // resync table: the exactly reduced integer phase of every tile start of this CTA -> fp64 phasor
+        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
+        if (k_cta >= P.Fs) k_cta -= P.Fs;
+        for (uint32_t i = tid; i < nt; i += kThreads) {
+            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
+            if (k >= P.Fs) k -= P.Fs;
+            base[i] = phasor_neg(k, P.Fs);
+        }
+        if (tid < (int)kMmaRows) rtab[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * kMmaSpan, P.Fs), P.Fs);
+    }
+    __syncthreads();
+
+    int acc[2][2][4][4];          // [block c (int8) / word (2-bit)][word half or field half w2][byte b][C fragment]
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int w2 = 0; w2 < 2; ++w2)
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc[c][w2][b][k] = 0;
+    long long s_re = 0, s_im = 0;     // sum over valid rows of the quantised phasors (2-bit: the -3 sum(rho) term)
+
+    for (uint32_t i = 0; i < nt; ++i, tile_byte0 += tile_stride, tile_row0 += row_stride) {
+        // ---- digit matrix of this tile: lane = row ----
+        {
+            const double2 b0 = base[i], r = rtab[lane];
+            const bool valid = tile_row0 + lane < n_rows;
+            const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
+            const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
+            int d0, d1, d2, e0, e1, e2;
+            digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
+            __syncwarp();             // every lane is done with the previous tile's digits
+            bt[0 * 32 + lane] = (unsigned char)d0; bt[1 * 32 + lane] = (unsigned char)d1; bt[2 * 32 + lane] = (unsigned char)d2;
+            bt[3 * 32 + lane] = (unsigned char)e0; bt[4 * 32 + lane] = (unsigned char)e1; bt[5 * 32 + lane] = (unsigned char)e2;
+            bt[6 * 32 + lane] = 0; bt[7 * 32 + lane] = 0;
+            if (KIND == KIND_2BIT) { s_re += vre; s_im += vim; }      // this lane's rows; summed over the warp at the end
+            __syncwarp();
+        }
+        const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt);
+        const uint32_t bf[2] = {bt32[g * 8 + t], bt32[g * 8 + 4 + t]};        // rows 4t.., 16+4t.. of digit column g
+
+#pragma unroll
+        for (int grp = 0; grp < GPT; ++grp) {
+            const int h = KIND == KIND_I8 ? (grp >> 1) : grp;
+            const int slot_grp = (int)((i * (uint32_t)GPT + grp) % DG);
+            cp_async_wait<DG - 1>();
+            auto refill = [&]() {     // the ring slot group just read: the same group, DG/GPT tiles ahead
+                const uint32_t ta = DG / GPT;
+                issue_group(tile_byte0 + ta * tile_stride, tile_row0 + ta * row_stride, i + ta < nt, grp, slot_grp);
+            };
+            if constexpr (KIND == KIND_I8) {
+                const int c = grp & 1;
+                uint32_t T[4][4];     // [word][byte]: 4 rows of one position
+                uint4 v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) v[j] = *reinterpret_cast<const uint4*>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT);
+#pragma unroll
+                for (int w = 0; w < 4; ++w) transpose4x4_bytes(word_of(v[0], w), word_of(v[1], w), word_of(v[2], w), word_of(v[3], w), T[w]);
+                refill();
+#pragma unroll
+                for (int w2 = 0; w2 < 2; ++w2)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) mma_s8_k16(acc[c][w2][b], T[w2][b], T[w2 + 2][b], bf[h]);
+            } else {
+                uint2 v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    v[j] = *reinterpret_cast<const uint2*>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT);
+                    if (P.sign_mag) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
+                }
+                refill();
+#pragma unroll
+                for (int w = 0; w < 2; ++w) {
+                    uint32_t T[4][4]; // [field][byte]: 4 rows of sample 4 b + f of word w
+                    const uint32_t r0 = w ? v[0].y : v[0].x, r1 = w ? v[1].y : v[1].x, r2 = w ? v[2].y : v[2].x, r3 = w ? v[3].y : v[3].x;
+#pragma unroll
+                    for (int f = 0; f < 4; ++f)
+                        transpose4x4_bytes((r0 >> (2 * f)) & 0x03030303u, (r1 >> (2 * f)) & 0x03030303u,
+                                           (r2 >> (2 * f)) & 0x03030303u, (r3 >> (2 * f)) & 0x03030303u, T[f]);
+#pragma unroll
+                    for (int f2 = 0; f2 < 2; ++f2)
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) mma_s8_k16(acc[w][f2][b], T[f2][b], T[f2 + 2][b], bf[h]);
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+    __syncthreads();                  // the ring is free: it becomes the per-position result array
+
+    // ---- digits -> fp64, post-twiddle by exp(-j w pos), positions -> bins ------------------------
+    double* pos_re = reinterpret_cast<double*>(ring);      // [2048]
+    double* pos_im = pos_re + kMmaSpan;
+    double2* tw256 = rtab;                                  // [8] exp(-j w 256 k): the row table is no longer needed
+    if (tid < 8) tw256[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * 256u, P.Fs), P.Fs);
+    if (KIND == KIND_2BIT) {
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) { s_re += __shfl_xor_sync(0xFFFFFFFFu, s_re, s); s_im += __shfl_xor_sync(0xFFFFFFFFu, s_im, s); }
+    }
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int w2 = 0; w2 < 2; ++w2)
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {      // matrix row g (half 0) / g + 8 (half 1)
+                    const long long c0 = acc[c][w2][b][2 * half], c1 = acc[c][w2][b][2 * half + 1];
+                    // digit columns held by this lane: 2t, 2t+1 (0..2 = Re digits, 3..5 = Im digits)
+                    long long pre = 0, pim = 0;
+                    if (t == 0) pre = c0 + 256 * c1;
+                    else if (t == 1) { pre = 65536 * c0; pim = c1; }
+                    else if (t == 2) pim = 256 * c0 + 65536 * c1;
+#pragma unroll
+                    for (int s = 1; s <= 2; s <<= 1) { pre += __shfl_xor_sync(0xFFFFFFFFu, pre, s); pim += __shfl_xor_sync(0xFFFFFFFFu, pim, s); }
+                    const int idx = ((c * 2 + w2) * 4 + b) * 2 + half;          // 0..31: lane t of the quad stores idx % 4 == t
+                    if ((idx & 3) == t) {
+                        const int wsel = w2 + 2 * half;                           // word (int8) / field (2-bit) of the block
+                        uint32_t pos;
+                        if (KIND == KIND_I8) pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
+                        else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8-byte load
+                        if (KIND == KIND_2BIT) { pre = 2 * pre - 3 * s_re; pim = 2 * pim - 3 * s_im; }
+                        pos_re[pos] = (double)pre * (1.0 / 4194304.0);
+                        pos_im[pos] = (double)pim * (1.0 / 4194304.0);
+                    }
+                }
+    __syncthreads();
+    {   // exp(-j w pos), pos = tid + 256 k: one exactly reduced phasor per thread times the 8-entry stride table
+        const double2 tw0 = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid, P.Fs), P.Fs);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const double2 s8 = tw256[k];
+            const double twx = tw0.x * s8.x - tw0.y * s8.y, twy = tw0.x * s8.y + tw0.y * s8.x;
+            const uint32_t pos = (uint32_t)tid + 256u * k;
+            const double re = pos_re[pos], im = pos_im[pos];
+            pos_re[pos] = re * twx - im * twy;
+            pos_im[pos] = re * twy + im * twx;
+        }
+    }
+    __syncthreads();
+    pdl_wait();   // the partial bins of the previous launch may still be read by its post kernel
+    for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
+        double re = 0.0, im = 0.0;
+        for (uint32_t pos = sb; pos < kMmaSpan; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
+        P.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
+    }
+}
+
+}  // namespace pcal

@@ -249,14 +249,11 @@ __global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G)
     for (int ww = 0; ww < kPostThreads / 32; ++ww) { re += sre[ww][lane]; im += sim[ww][lane]; }
     const uint32_t n_tail = (uint32_t)(G.n_total - G.n_done);
     if (n_tail) {
-        uint32_t bb = (uint32_t)((G.n0 + G.n_done) % G.n_bins);
-        for (uint32_t t = 0; t < n_tail; ++t) {
-            if (bb == b) {
-                const double v = decode_tail(G.kind, G.sign_mag, G.tail, t, 0, 1);
-                const double2 ph = phasor_neg(mulmod_u64(G.Foff, G.n0 + G.n_done + t, G.Fs), G.Fs);
-                re += v * ph.x; im += v * ph.y;
-            }
-            if (++bb == G.n_bins) bb = 0;
+        const uint32_t bb0 = (uint32_t)((G.n0 + G.n_done) % G.n_bins);        // bin of tail sample 0
+        for (uint32_t t = (b + G.n_bins - bb0) % G.n_bins; t < n_tail; t += G.n_bins) {   // this bin's tail samples, in order
+            const double v = decode_tail(G.kind, G.sign_mag, G.tail, t, 0, 1);
+            const double2 ph = phasor_neg(mulmod_u64(G.Foff, G.n0 + G.n_done + t, G.Fs), G.Fs);
+            re += v * ph.x; im += v * ph.y;
         }
     }
     if (!G.overwrite) { const double2 cur = G.P[b]; re += cur.x; im += cur.y; }

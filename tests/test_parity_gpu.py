@@ -90,6 +90,29 @@ def test_generator_on_every_sample_type(oracle, idx, n):
         assert_close(T[0], oracle_tones(oracle, w2, host, 0), "gen sign-mag")
 
 
+@pytest.mark.parametrize("idx,n,enc", [(5, 1_300_003, None), (7, 700_001, None), (2, 900_004, 0), (2, 900_004, 1), (3, 2_000_004, 0),
+                                       (5, 2047, None), (5, 2048 * 33 + 5, None), (2, 8192 * 3 + 64, 0)])
+def test_both_generator_kernels(oracle, idx, n, enc, monkeypatch):
+    """Integer samples with N_bins | 2048 run the tensor-core generator kernel (pcal_gen_mma.cuh: integer MMAs over
+    23-bit fixed-point phasor digits); PCAL_GEN_MMA=0 selects the FFMA2 kernel of pcal_gen.cuh (the path of float32
+    input).  Both must match the oracle; lengths around one 2048-sample row and one 2^16-sample tile included."""
+    w, dev, host = make(idx, n)
+    if idx == 7:
+        w = synth.replace(w, f_offset_hz=[1234.567])
+    if enc is not None:
+        w = synth.replace(w, encoding=enc)
+    want = oracle_tones(oracle, w, host, 0)
+    floor = 0.05 if n < 100_000 else 0.0          # very short integrations: see test_series_gpu.py
+    p1, T1, _ = gpu_run(w, dev, rotator="generator")
+    assert p1.info().rotator_in_effect == 2
+    assert_close(T1[0], want, f"mma generator cfg{idx}", floor_frac=floor)
+    monkeypatch.setenv("PCAL_GEN_MMA", "0")
+    p2, T2, _ = gpu_run(w, dev, rotator="generator")
+    monkeypatch.delenv("PCAL_GEN_MMA")
+    assert_close(T2[0], want, f"ffma2 generator cfg{idx}", floor_frac=floor)
+    assert np.abs(T1 - T2).max() <= 2e-6 * np.abs(want).max()
+
+
 @pytest.mark.parametrize("idx,n,splits", [
     (2, 1_000_004, [64, 64 * 1000, 64 * 9001]),
     (5, 800_003, [16, 16 * 4099, 16 * 30000]),
