@@ -400,8 +400,8 @@ static int prepare(pcal_ctx* c) {
         CU(cudaMemcpy(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
     } else {
         int occ = 0;
-        if (c->gen_mma && c->kind == KIND_2BIT) { c->gen_smem = gen_mma_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_2BIT>, c->gen_smem); }
-        else if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8>, c->gen_smem); }
+        if (c->gen_mma && c->kind == KIND_2BIT) { c->gen_smem = gen_mma_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_2BIT, false>, c->gen_smem); }
+        else if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8, false>, c->gen_smem); }
         else if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
         else if (c->kind == KIND_I8) { c->gen_smem = gen_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_I8>, c->gen_smem); }
         else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
@@ -521,8 +521,9 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.input_ready = c->input_ready ? 1 : 0;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
-        if (c->gen_mma && c->kind == KIND_2BIT) launch_chain(gen_mma_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
-        else if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
+        if (c->gen_mma && c->kind == KIND_2BIT && c->sign_mag) launch_chain(gen_mma_kernel<KIND_2BIT, true>, c->gen_grid, kThreads, smem, st, gp);
+        else if (c->gen_mma && c->kind == KIND_2BIT) launch_chain(gen_mma_kernel<KIND_2BIT, false>, c->gen_grid, kThreads, smem, st, gp);
+        else if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8, false>, c->gen_grid, kThreads, smem, st, gp);
         else if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
         else if (c->kind == KIND_I8) launch_chain(gen_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
         else launch_chain(gen_kernel<KIND_F32>, c->gen_grid, kThreads, smem, st, gp);

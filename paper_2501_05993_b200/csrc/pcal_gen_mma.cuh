@@ -25,7 +25,7 @@
 // byte 64 w + 8 g of the row.  Its own cp.async ring (no barrier), every byte used by exactly one thread.  The MMA wants
 // four consecutive ROWS of one position in a register, memory has positions consecutive: a 4x4 byte
 // transpose (8 PRMT per 16 samples) turns 4 row words into 4 position words.  2-bit words are first spread
-// into bytes (shift + mask per 4 samples) and stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho)
+// into bytes (after the transpose: shift + mask per 4 samples) and stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho)
 // term, which does not depend on the data, is added once at the end from the same quantised phasors.
 // Rows past the end of the segment get zero digits, so whatever their ring slots hold contributes nothing.
 // ~1 instruction per sample instead of 3-4 for the FFMA2 kernel of pcal_gen.cuh: HBM-bound at any SM clock.
@@ -55,6 +55,13 @@ __device__ __forceinline__ void mma_s8_k16(int (&d)[4], uint32_t a0, uint32_t a1
                  : "r"(a0), "r"(a1), "r"(b0));
 }
 
+// the same with an UNSIGNED left operand: 2-bit fields are used where they sit in the byte (code << 2f <= 192)
+__device__ __forceinline__ void mma_u8_k16(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a0), "r"(a1), "r"(b0));
+}
+
 // rows r0..r3 (bytes = 4 positions each) -> o[p] = (r0.p, r1.p, r2.p, r3.p), byte 0 = row 0
 __device__ __forceinline__ void transpose4x4_bytes(uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3, uint32_t (&o)[4]) {
     const uint32_t x01l = __byte_perm(r0, r1, 0x5140), x01h = __byte_perm(r0, r1, 0x7362);
@@ -74,7 +81,7 @@ __device__ __forceinline__ void cp_async_pred(void* smem_dst, const void* gsrc, 
     if (ok) cp_async_own<LB>(smem_dst, gsrc);
 }
 
-template <int KIND>
+template <int KIND, bool SIGN_MAG>
 __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_constant__ GenParams P) {
     pdl_release();
     if (!P.input_ready) pdl_wait();
@@ -96,13 +103,13 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     constexpr int GPT = GenMmaCfg<KIND>::GPT;
     const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
     const uint32_t col_off = (uint32_t)(warp * (ROW_BYTES / kWarps) + g * LB);
-    auto row_of = [&](int l) -> uint32_t {
-        return KIND == KIND_I8 ? (uint32_t)(16 * (l >> 3) + 4 * t + (l & 3)) : (uint32_t)(16 * (l >> 2) + 4 * t + (l & 3));
-    };
-    auto load_off = [&](int l) -> uint32_t {                  // byte offset inside a tile
+    // row (without the thread's 4t) and byte offset (without the thread's part) of load l: compile-time after unrolling
+    auto row_c = [](int l) -> int { return KIND == KIND_I8 ? 16 * (l >> 3) + (l & 3) : 16 * (l >> 2) + (l & 3); };
+    auto off_c = [&](int l) -> uint32_t {
         const uint32_t c = KIND == KIND_I8 ? (uint32_t)((l >> 2) & 1) : 0u;
-        return row_of(l) * ROW_BYTES + col_off + c * (ROW_BYTES / 16);
+        return (uint32_t)row_c(l) * ROW_BYTES + c * (ROW_BYTES / 16);
     };
+    const uint32_t thread_off = (uint32_t)(4 * t) * ROW_BYTES + col_off;
     // ring slot of this thread inside its warp's 32*LB bytes: lanes that read consecutive global addresses
     // (same t, g = 0..7) sit in one contiguous run, so a cp.async of the warp writes whole shared-memory
     // lines; the run is permuted (g ^ 2t for 16-byte loads, g ^ 4(t/2) for 8-byte loads) so that every
@@ -111,27 +118,34 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     unsigned char* my_ring = ring + ((size_t)warp * 32 + chunk) * LB;
     constexpr size_t SLOT = (size_t)kThreads * LB;
     const uint64_t tile_stride = (uint64_t)gridDim.x * TILE_BYTES;
-    uint64_t tile_byte0 = (uint64_t)blockIdx.x * TILE_BYTES;                     // first byte of this CTA's tile i
-    uint64_t tile_row0 = (uint64_t)blockIdx.x * kMmaRows;
-    const uint64_t row_stride = (uint64_t)gridDim.x * kMmaRows;
+    const long long row_stride = (long long)gridDim.x * kMmaRows;
+    long long rows_left = (long long)n_rows - (long long)blockIdx.x * kMmaRows;  // rows from the start of this CTA's tile i on
 
-    // issue the loads of commit group `grp` of the tile that starts at (byte0, row0)
-    auto issue_group = [&](uint64_t byte0, uint64_t row0, bool tile_exists, int grp, int slot_grp) {
-        const uint32_t lim = (tile_exists && row0 < n_rows) ? (uint32_t)(n_rows - row0 < kMmaRows ? n_rows - row0 : kMmaRows) : 0u;
-        const unsigned char* src = gdata + byte0;
+    // issue the loads of commit group `grp` of a tile: src = the thread's first byte of that tile,
+    // lim_t = (valid rows of that tile, 0..32) - 4t, so that load l is inside the data iff row_c(l) < lim_t
+    auto issue_group = [&](const unsigned char* src, int lim_t, int grp, int slot_grp) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int l = grp * 4 + j;
-            cp_async_pred<LB>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT, src + load_off(l), row_of(l) < lim);
+            cp_async_pred<LB>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT, src + off_c(l), row_c(l) < lim_t);
         }
         cp_async_commit();
     };
+    auto lim_of = [&](long long left, bool exists) -> int {
+        const int v = !exists || left <= 0 ? 0 : (left < (long long)kMmaRows ? (int)left : (int)kMmaRows);
+        return v - 4 * t;
+    };
     // prologue: DG groups = DG/GPT tiles ahead
     static_assert(DG % GPT == 0, "whole tiles in flight");
+    constexpr uint32_t TA = DG / GPT;
+    const unsigned char* ahead = gdata + (uint64_t)blockIdx.x * TILE_BYTES + thread_off;   // tile i + TA after the prologue
+    long long ahead_left = rows_left;
 #pragma unroll
-    for (int d = 0; d < DG; ++d) {
-        const uint32_t ti = d / GPT;
-        issue_group(tile_byte0 + ti * tile_stride, tile_row0 + ti * row_stride, ti < nt, d % GPT, d);
+    for (uint32_t ti = 0; ti < TA; ++ti) {
+        const int lim_t = lim_of(ahead_left, ti < nt);
+#pragma unroll
+        for (int gq = 0; gq < GPT; ++gq) issue_group(ahead, lim_t, gq, (int)(ti * GPT + gq));
+        ahead += tile_stride; ahead_left -= row_stride;
     }
 
     // (the first loads are in flight: now the tables)
@@ -158,11 +172,12 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
                 for (int k = 0; k < 4; ++k) acc[c][w2][b][k] = 0;
     long long s_re = 0, s_im = 0;     // sum over valid rows of the quantised phasors (2-bit: the -3 sum(rho) term)
 
-    for (uint32_t i = 0; i < nt; ++i, tile_byte0 += tile_stride, tile_row0 += row_stride) {
+    for (uint32_t i = 0; i < nt; ++i, rows_left -= row_stride, ahead += tile_stride, ahead_left -= row_stride) {
+        const int ahead_lim_t = lim_of(ahead_left, i + TA < nt);
         // ---- digit matrix of this tile: lane = row ----
         {
             const double2 b0 = base[i], r = rtab[lane];
-            const bool valid = tile_row0 + lane < n_rows;
+            const bool valid = (long long)lane < rows_left;
             const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
             const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
             int d0, d1, d2, e0, e1, e2;
@@ -182,10 +197,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             const int h = KIND == KIND_I8 ? (grp >> 1) : grp;
             const int slot_grp = (int)((i * (uint32_t)GPT + grp) % DG);
             cp_async_wait<DG - 1>();
-            auto refill = [&]() {     // the ring slot group just read: the same group, DG/GPT tiles ahead
-                const uint32_t ta = DG / GPT;
-                issue_group(tile_byte0 + ta * tile_stride, tile_row0 + ta * row_stride, i + ta < nt, grp, slot_grp);
-            };
+            auto refill = [&]() { issue_group(ahead, ahead_lim_t, grp, slot_grp); };   // the slot group just read: same group, TA tiles ahead
             if constexpr (KIND == KIND_I8) {
                 const int c = grp & 1;
                 uint32_t T[4][4];     // [word][byte]: 4 rows of one position
@@ -204,21 +216,21 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     v[j] = *reinterpret_cast<const uint2*>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT);
-                    if (P.sign_mag) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
+                    if (SIGN_MAG) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
                 }
                 refill();
 #pragma unroll
                 for (int w = 0; w < 2; ++w) {
-                    uint32_t T[4][4]; // [field][byte]: 4 rows of sample 4 b + f of word w
-                    const uint32_t r0 = w ? v[0].y : v[0].x, r1 = w ? v[1].y : v[1].x, r2 = w ? v[2].y : v[2].x, r3 = w ? v[3].y : v[3].x;
-#pragma unroll
-                    for (int f = 0; f < 4; ++f)
-                        transpose4x4_bytes((r0 >> (2 * f)) & 0x03030303u, (r1 >> (2 * f)) & 0x03030303u,
-                                           (r2 >> (2 * f)) & 0x03030303u, (r3 >> (2 * f)) & 0x03030303u, T[f]);
+                    // transpose the PACKED bytes first (a byte = 4 samples of one row), then spread the fields:
+                    // Tp[b] = byte b of rows 0..3; field f of it = 4 rows of sample 4 b + f, used in place: the sums carry
+                    // a factor 4^f that is shifted out (exactly) at the end
+                    uint32_t Tp[4];
+                    transpose4x4_bytes(w ? v[0].y : v[0].x, w ? v[1].y : v[1].x, w ? v[2].y : v[2].x, w ? v[3].y : v[3].x, Tp);
 #pragma unroll
                     for (int f2 = 0; f2 < 2; ++f2)
 #pragma unroll
-                        for (int b = 0; b < 4; ++b) mma_s8_k16(acc[w][f2][b], T[f2][b], T[f2 + 2][b], bf[h]);
+                        for (int b = 0; b < 4; ++b)
+                            mma_u8_k16(acc[w][f2][b], Tp[b] & (0x03030303u << (2 * f2)), Tp[b] & (0x30303030u << (2 * f2)), bf[h]);
                 }
             }
         }
@@ -257,7 +269,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
                         uint32_t pos;
                         if (KIND == KIND_I8) pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
                         else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8-byte load
-                        if (KIND == KIND_2BIT) { pre = 2 * pre - 3 * s_re; pim = 2 * pim - 3 * s_im; }
+                        if (KIND == KIND_2BIT) { pre = 2 * (pre >> (2 * wsel)) - 3 * s_re; pim = 2 * (pim >> (2 * wsel)) - 3 * s_im; }   // undo 4^field
                         pos_re[pos] = (double)pre * (1.0 / 4194304.0);
                         pos_im[pos] = (double)pim * (1.0 / 4194304.0);
                     }
