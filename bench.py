@@ -173,9 +173,13 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
         for L in lanes:
             complete(L)
 
-    def step(i):
+    buf_ptrs, out_ptr = [b_.data_ptr() for b_ in bufs], out_pinned.data_ptr()
+    cur_stream = int(torch.cuda.current_stream().cuda_stream)
+
+    def step(i, stream=None):
         if not exchange:
-            p.integrate(bufs[i % ncopies], n, out_pinned)     # pcal_reset + pcal_extract + pcal_finalize_async
+            # pcal_reset + pcal_extract + pcal_finalize_async in one call; raw addresses, stream handle hoisted
+            p.integrate(buf_ptrs[i % ncopies], n, out_ptr, stream=stream)
             return
         L = lanes[i % 2]
         complete(L)                                       # this lane's previous integration, if still open
@@ -235,10 +239,10 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
             for _ in range(count // n_big):
                 big.replay()
             for k in range(count % n_big):
-                step(k)
+                step(k, cur_stream)
         else:
             for k in range(count):
-                step(k)
+                step(k, cur_stream)
         drain()
 
     mode = "direct"

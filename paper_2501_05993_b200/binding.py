@@ -200,9 +200,11 @@ class Pcal:
         _check(lib().pcal_finalize_async(self._h, out_pinned.data_ptr()), "pcal_finalize_async")
 
     def integrate(self, dev_samples, n_samples: int, out_pinned, stream=None):
-        """One integration period: reset + extract + finalize_async in one library call (asynchronous)."""
-        _check(lib().pcal_integrate(self._h, dev_samples.data_ptr(), n_samples, _stream_handle(stream),
-                                    out_pinned.data_ptr()), "pcal_integrate")
+        """One integration period: reset + extract + finalize_async in one library call (asynchronous).
+        Tensors or raw addresses (a host loop over short periods can hoist ``data_ptr()`` and the stream handle)."""
+        src = dev_samples.data_ptr() if hasattr(dev_samples, "data_ptr") else int(dev_samples)
+        dst = out_pinned.data_ptr() if hasattr(out_pinned, "data_ptr") else int(out_pinned)
+        _check(lib().pcal_integrate(self._h, src, n_samples, _stream_handle(stream), dst), "pcal_integrate")
 
     def analyze(self, bandpass: bool = True):
         """(summary float64 [n_channels, 8], corrected band-pass complex128 [n_channels, N_bins] or None)."""

@@ -82,6 +82,8 @@ struct pcal_ctx {
     bool input_ready;               // pcal_set_input_ready: sample buffers are complete when extract is called
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
+    double2* fuse_out;              // pcal_integrate: the fold kernel of this call also takes the DFT and writes T here (or null)
+    bool fuse_req;                  // ... requested for the piece being enqueued
     const double* last_out;         // pcal_finalize_async: last host buffer seen and its device mapping (or null)
     double2* last_out_mapped;
     double *d_summary, *h_ana;      // analysis outputs: [C][8] + band-pass [C][N] complex
@@ -447,6 +449,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         if (c->fused) {
             tp.enabled = 1;
             tp.cnt = c->d_cnt; tp.G = c->d_G; tp.st = c->d_tail_state; tp.partial_stride = c->partial_slot_bytes;
+            if (c->fuse_req) { tp.fuse_dft = 1; tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W; tp.T_dev = c->d_T; tp.T_host = c->fuse_out; }
             tp.lut = c->d_lut; tp.lut_off = c->d_lut_off; tp.lut_len = c->d_lut_len;
             tp.P = c->d_P; tp.Pint = c->d_Pint; tp.tail = data + n_vec * 16;
             tp.n0 = c->n_processed; tp.NT = n_vec * c->spv; tp.n_total = n;
@@ -544,12 +547,17 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
 
 static int enqueue_dft(pcal_ctx* c, double2* second_dst);
 
+// PCAL_SMALL_PIECES=1 (tests only): see extract_segment.  Read per call (tests toggle it), but cheaply.
+static bool small_pieces() {
+    const char* sp = getenv("PCAL_SMALL_PIECES");
+    return sp && sp[0] == '1';
+}
+
 // pieces: bounded per-thread trip count (LUT path) / bounded resync table (generator path)
 static int extract_segment(pcal_ctx* c, const uint8_t* p, uint64_t n_samples) {
     // PCAL_SMALL_PIECES=1 (tests only) shrinks both limits so that a few million samples already
     // span several launches; the arithmetic is unchanged.
-    const char* sp = getenv("PCAL_SMALL_PIECES");
-    const bool small = sp && sp[0] == '1';
+    const bool small = small_pieces();
     uint64_t piece;
     if (c->rot_eff == PCAL_ROT_LUT)
         piece = (uint64_t)(small ? 16u : kMaxIterPerLaunch) * c->R * kWarps * c->q * 32ull * c->spv;
@@ -649,6 +657,13 @@ static uint32_t dft_ctas(const pcal_ctx* c) {
     return (uint32_t)c->C * ((c->n_bins + per_cta - 1) / per_cta);
 }
 
+// stage C of the fold kernel can take the DFT itself: small N_bins, and C*N_bins complex values fit in its scratch
+static bool can_fuse_dft(const pcal_ctx* c) {
+    if (!(c->prepared && c->rot_eff == PCAL_ROT_LUT && c->fused) || c->n_bins > 64) return false;
+    const uint32_t cap = c->kind == KIND_2BIT ? 1792u : (c->kind == KIND_I8 ? 768u : 256u);   // (scratch doubles - 512) / 2
+    return c->n_bins * (uint32_t)c->C <= cap;
+}
+
 static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const int rz = ensure_zeroed(c);
     if (rz != PCAL_OK) return rz;
@@ -656,22 +671,17 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const uint32_t opw = dft_opw(c), per_cta = kDftThreads / 32 * opw;
     launch_chain(dft_kernel, dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream,
                  (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift, opw,
-                 c->rot_eff == PCAL_ROT_LUT && c->fused ? c->d_tail_state : (TailState*)nullptr);
+                 c->rot_eff == PCAL_ROT_LUT && c->fused ? c->d_tail_state : (TailState*)nullptr, can_fuse_dft(c) ? 1 : 0);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
 }
 
+static double2* mapped_of(pcal_ctx* c, double* out);
+
 extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
-    if (out != c->last_out) {     // the attribute query costs more than a launch: remember the answer
-        c->last_out = out; c->last_out_mapped = nullptr;
-        cudaPointerAttributes at;
-        if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
-            c->last_out_mapped = reinterpret_cast<double2*>(at.devicePointer);
-        cudaGetLastError();
-    }
-    double2* mapped = c->last_out_mapped;
+    double2* mapped = mapped_of(c, out);
     const int r = enqueue_dft(c, mapped);
     if (r != PCAL_OK) return r;
     if (!mapped)
@@ -679,13 +689,36 @@ extern "C" int pcal_finalize_async(pcal_ctx* c, double* out) {
     return PCAL_OK;
 }
 
+static double2* mapped_of(pcal_ctx* c, double* out) {
+    if (out != c->last_out) {     // the attribute query costs more than a launch: remember the answer
+        c->last_out = out; c->last_out_mapped = nullptr;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, out) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+            c->last_out_mapped = reinterpret_cast<double2*>(at.devicePointer);
+        cudaGetLastError();
+    }
+    return c->last_out_mapped;
+}
+
 extern "C" int pcal_integrate(pcal_ctx* c, const void* dev_samples, uint64_t n_samples, void* cuda_stream, double* out) {
+    if (!c || !out) return PCAL_ERR_INVALID;
     int r = pcal_reset(c);
     if (r != PCAL_OK) return r;
+    r = prepare(c);
+    if (r != PCAL_OK) return r;
+    // One launch for the whole period when the fold kernel can deliver T itself: a small DFT, the period is one
+    // piece with at least one complete vector, and out is device-visible pinned memory.
+    double2* mapped = mapped_of(c, out);
+    const uint64_t piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
+    c->fuse_req = mapped && can_fuse_dft(c) && !small_pieces() && n_samples <= piece &&
+                  n_samples * (uint64_t)c->bits * c->C / 8 >= 16 && dev_samples;
+    c->fuse_out = mapped;
     r = pcal_extract(c, dev_samples, n_samples, cuda_stream);
+    const bool fused_done = c->fuse_req;
+    c->fuse_req = false;
     if (r != PCAL_OK) return r;
     c->stream = (cudaStream_t)cuda_stream;
-    return pcal_finalize_async(c, out);
+    return fused_done ? PCAL_OK : pcal_finalize_async(c, out);
 }
 
 extern "C" int pcal_finalize(pcal_ctx* c, double* out) {

@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G)
 constexpr int kDftThreads = 256;
 __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restrict__ P, const double2* __restrict__ W,
                                                           double2* __restrict__ T, double2* __restrict__ T_host,
-                                                          uint32_t N, uint32_t k_shift, uint32_t opw, TailState* st) {
+                                                          uint32_t N, uint32_t k_shift, uint32_t opw, TailState* st, int finish_late) {
     if (st) {   // counted before the dependents may start: a later fold kernel waits for these CTAs to have read P
         if (threadIdx.x == 0) atomicAdd(&st->dft_started, 1u);
         __syncthreads();
@@ -285,7 +285,9 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
         sw[t] = W[t];
     }
     __syncthreads();
-    if (st && threadIdx.x == 0) { __threadfence(); atomicAdd(&st->dft_finished, 1u); }   // P has been read
+    // P has been read.  (finish_late: contexts whose fold kernel may itself deliver T count this CTA out only after
+    // its T writes, so that a later launch cannot be overtaken by them.)
+    if (st && !finish_late && threadIdx.x == 0) { __threadfence(); atomicAdd(&st->dft_finished, 1u); }
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t i0 = (blockIdx.x * (kDftThreads / 32) + (threadIdx.x >> 5)) * opw;
     for (uint32_t i = i0; i < i0 + opw && i < N; ++i) {       // whole warp together
@@ -308,6 +310,10 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
             T[(size_t)c * N + i] = make_double2(re, im);
             if (T_host) T_host[(size_t)c * N + i] = make_double2(re, im);   // mapped pinned host memory
         }
+    }
+    if (st && finish_late) {
+        __syncthreads();
+        if (threadIdx.x == 0) { __threadfence(); atomicAdd(&st->dft_finished, 1u); }
     }
 }
 

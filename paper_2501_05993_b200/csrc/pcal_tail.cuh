@@ -58,6 +58,12 @@ struct TailParams {
     int enabled;              // 0: the caller launches reduce_replicas_kernel + rotate_fold_kernel instead
     TailState* st;            // [device] tickets and progress counters of the context
     uint64_t partial_stride;  // bytes between the partial buffers of consecutive slots
+    // pcal_integrate on small periods: stage C also takes the N_bins-point DFT and delivers T
+    int fuse_dft;             // 1: N_bins <= 64 and C*N_bins complex values fit behind the first 512 doubles of scratch
+    uint32_t k_shift;
+    const double2* W;         // [device] exp(-j 2 pi k / N_bins), k < N_bins
+    double2* T_dev;           // [device] tone spectrum [C][N_bins]
+    double2* T_host;          // device-visible pinned host memory or null
 };
 
 constexpr uint32_t kTailSlots = 8;
@@ -225,11 +231,18 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     if (s_prev != q - 1u) return;
 
     // ---- stage C: groups in order, ragged tail, accumulate into the context ------------------
-    if (tid == 0) {
-        while (ld_acquire_u32(&T.st->n_done) != seq) __nanosleep(32);                          // P is up to date
-        while ((int32_t)(ld_acquire_u32(&T.st->dft_finished) - dft_x) < 0) __nanosleep(32);   // and no longer being read
-    }
-    __syncthreads();
+    // The group sums and the ragged tail do not depend on P: they are formed first, and only then does the CTA wait
+    // (first trip of the loop below) until P is up to date (n_done == seq) and no longer being read by a DFT kernel.
+    auto wait_for_P = [&]() {
+        if (tid == 0) {
+            uint32_t a = ld_acquire_u32(&T.st->n_done), b = ld_acquire_u32(&T.st->dft_finished);
+            while (a != seq || (int32_t)(b - dft_x) < 0) {
+                __nanosleep(32);
+                a = ld_acquire_u32(&T.st->n_done); b = ld_acquire_u32(&T.st->dft_finished);
+            }
+        }
+        __syncthreads();
+    };
     // thread = (slice sl of the groups, pair): slice sums first (all loads of a thread in flight at
     // once where possible), then the slices in order.
     const uint32_t ppc = pairs < (uint32_t)kThreads ? pairs : (uint32_t)kThreads;
@@ -257,9 +270,9 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
             are = 0.0; aim = 0.0;
             if (sl == 0) for (uint32_t k = 0; k < ns; ++k) { are += s_re[k * ppc + e0]; aim += s_im[k * ppc + e0]; }
         }
-        if (sl != 0 || pp >= pairs) continue;
-        const uint32_t c = pp / T.n_bins, b = pp % T.n_bins;
-        if (n_tail) {   // samples NT .. n_total-1 (fewer than one vector)
+        const bool mine = sl == 0 && pp < pairs;
+        const uint32_t c = mine ? pp / T.n_bins : 0u, b = mine ? pp % T.n_bins : 0u;
+        if (mine && n_tail) {   // samples NT .. n_total-1 (fewer than one vector)
             const uint32_t L = T.lut_len[c];
             const double2* lut = T.lut + T.lut_off[c];
             uint32_t bb = (uint32_t)((T.n0 + T.NT) % T.n_bins);
@@ -274,6 +287,8 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
                 if (L > 1 && ++k == L) k = 0;
             }
         }
+        if (pp0 == 0) wait_for_P();        // every thread of the CTA, once
+        if (!mine) continue;
         long long ai = (long long)are;     // exact: unrotated integer sums are integers below 2^53
         if (!T.overwrite) {
             const double2 cur = __ldcg(T.P + pp);          // L2: written by another SM under an overlapping grid
@@ -282,6 +297,26 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         }
         T.P[pp] = make_double2(are, aim);
         if (T.integer_exact) T.Pint[pp] = ai;
+        if (T.fuse_dft) reinterpret_cast<double2*>(scratch + 2 * kThreads)[pp] = make_double2(are, aim);
+    }
+    if (T.fuse_dft) {   // T[c][i] = sum_b P[c][b] W[(i' b) mod N], i' = (i - k_shift) mod N: one thread per output, b in order
+        __syncthreads();
+        const double2* sP = reinterpret_cast<const double2*>(scratch + 2 * kThreads);
+        const uint32_t N = T.n_bins;
+        for (uint32_t pp = tid; pp < pairs; pp += kThreads) {
+            const uint32_t c = pp / N, i = pp % N;
+            const uint32_t ii = (i + N - T.k_shift % N) % N;
+            uint32_t k = 0;
+            double re = 0.0, im = 0.0;
+            for (uint32_t b = 0; b < N; ++b) {
+                const double2 p = sP[c * N + b], w = __ldg(T.W + k);
+                re += p.x * w.x - p.y * w.y;
+                im += p.x * w.y + p.y * w.x;
+                k += ii; if (k >= N) k -= N;
+            }
+            T.T_dev[pp] = make_double2(re, im);
+            if (T.T_host) T.T_host[pp] = make_double2(re, im);
+        }
     }
     for (uint32_t i = tid; i <= q; i += kThreads) cnt[i] = 0u;         // ready for the slot's next launch
     __syncthreads();

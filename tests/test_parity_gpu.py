@@ -90,6 +90,35 @@ def test_generator_on_every_sample_type(oracle, idx, n):
         assert_close(T[0], oracle_tones(oracle, w2, host, 0), "gen sign-mag")
 
 
+@pytest.mark.parametrize("idx,n,k_shift", [(1, 1_300_001, 0), (2, 1_300_004, 0), (2, 1_300_004, 5), (4, 200_003, 0), (6, 600_004, 0),
+                                           (3, 2_600_036, 0), (5, 1_300_003, 0), (8, 500_001, 0), (2, 60, 0)])
+def test_integrate_is_reset_extract_finalize(oracle, idx, n, k_shift):
+    """pcal_integrate = pcal_reset + pcal_extract + pcal_finalize_async in one call.  For small N_bins on the LUT path the
+    fold kernel's stage C takes the DFT itself and writes T straight into the pinned buffer (one launch per period);
+    otherwise the DFT kernel follows.  Repeated periods on one context, against the oracle and against the three calls."""
+    from paper_2501_05993_b200 import binding
+    w, dev, host = make(idx, n)
+    p = binding.from_workload(w)
+    if k_shift:
+        p.set_k_shift(k_shift)
+    out = torch.empty((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory()
+    l0 = p.info().kernel_launches
+    for _ in range(3):                      # the context keeps integrating period after period
+        out.zero_()
+        p.integrate(dev, n, out)
+    torch.cuda.synchronize()
+    per_period = (p.info().kernel_launches - l0) // 3
+    T1 = out.numpy().copy()
+    p.reset(); p.extract(dev, n); T2 = p.finalize()
+    small = w.n_bins <= 64 and idx != 5 and n > 1000
+    assert per_period == (1 if small else (3 if idx == 5 else 2)), per_period
+    for c in range(0, w.n_channels, 5):
+        if n > 1000:
+            assert_close(T1[c], oracle_tones(oracle, w, host, c), f"integrate cfg{idx} ch{c}")
+    assert np.abs(T1 - T2).max() <= 1e-12 * np.abs(T2).max()
+    p.destroy()
+
+
 @pytest.mark.parametrize("idx,n,enc", [(5, 1_300_003, None), (7, 700_001, None), (2, 900_004, 0), (2, 900_004, 1), (3, 2_000_004, 0),
                                        (5, 2047, None), (5, 2048 * 33 + 5, None), (2, 8192 * 3 + 64, 0)])
 def test_both_generator_kernels(oracle, idx, n, enc, monkeypatch):
