@@ -193,6 +193,33 @@ int pcal_integrate(pcal_ctx *ctx, const void *dev_samples, uint64_t n_samples, v
 #define PCAL_N_SUMMARY 8
 int pcal_analyze(pcal_ctx *ctx, double *out_summary, double *out_bandpass);
 
+/*
+ * Multi-pass counter-rotation ("short integration times combined with multiple passes over the
+ * x[n] input data, iteratively counter-rotating the input data using the residual phase shift detected in the
+ * previous pass"; reading R27).
+ *
+ * pcal_residual_rotation: the residual phase shift of one pass.  dev_series_tones = [device] the output of
+ * pcal_extract_series ([n_periods][n_channels][N_bins] complex128).  Per channel,
+ *   S = sum_{m < n_periods-1} sum_{i in band} T_{m+1}[i] conj(T_m[i]),  band = tones 0 (1 when that channel's
+ *   f_offset is 0: that tone is sin(0)) .. N_bins/2 - 1,
+ * and out[c*PCAL_N_RESIDUAL + {0,1,2}] = arg S (radians per period; = 2 pi (f_true - f_rot) n_per_period/f_s),
+ * |S|, sum |T_{m+1}[i]| |T_m[i]| (|S| over it = coherence in [0,1]).  out: [host].  Synchronises the context's stream.
+ *
+ * pcal_refine_offset: the passes.  Single-channel contexts only (else PCAL_ERR_UNSUPPORTED).  Starting from the
+ * context's f_offset, each pass extracts n_periods short integrations of n_per_period samples from dev_samples
+ * ([device], the rules of pcal_extract_series) at the current rotator frequency, measures the residual phase
+ * shift and counter-rotates: f_rot <- f_rot + arg S / (2 pi T_int), T_int = n_per_period / f_s, on the 1 micro-hertz
+ * grid; stops when |arg S| <= tol_rad or after max_passes passes.  Unambiguous for |f_true - f_rot| < 1/(2 T_int).
+ *   out_f_offset_hz [host] the last rotator frequency set;  out_history [host] max_passes*4 doubles or NULL: per
+ *   pass (f_rot used, arg S, |S|, norm);  out_passes [host] passes run.
+ * On success the context is reset and ITS f_offset is replaced by the refined value, so that the caller can go on
+ * to the long coherent integration (pcal_extract + pcal_finalize / pcal_analyze).  Synchronous.
+ */
+#define PCAL_N_RESIDUAL 3
+int pcal_residual_rotation(pcal_ctx *ctx, const double *dev_series_tones, uint32_t n_periods, double *out);
+int pcal_refine_offset(pcal_ctx *ctx, const void *dev_samples, uint64_t n_per_period, uint32_t n_periods, void *cuda_stream,
+                       uint32_t max_passes, double tol_rad, double *out_f_offset_hz, double *out_history, uint32_t *out_passes);
+
 /* Folded period P before the DFT: [host] n_channels*N_bins*2 doubles (Re, Im).  Synchronises. */
 int pcal_get_folded(pcal_ctx *ctx, double *out_bins);
 

@@ -83,6 +83,9 @@ def lib():
             "pcal_generator_study": (i32, [vp, ctypes.c_uint32, u64, ctypes.c_uint32, vp]),
             "pcal_extract_series": (i32, [vp, vp, u64, ctypes.c_uint32, vp, vp, vp]),
             "pcal_analyze": (i32, [vp, vp, vp]),
+            "pcal_residual_rotation": (i32, [vp, vp, ctypes.c_uint32, vp]),
+            "pcal_refine_offset": (i32, [vp, vp, u64, ctypes.c_uint32, vp, ctypes.c_uint32, dbl, ctypes.POINTER(dbl), vp,
+                                         ctypes.POINTER(ctypes.c_uint32)]),
             "pcal_finalize": (i32, [vp, vp]),
             "pcal_finalize_async": (i32, [vp, vp]),
             "pcal_integrate": (i32, [vp, vp, u64, vp, vp]),
@@ -212,6 +215,21 @@ class Pcal:
         bp = np.empty((self.n_channels, self.n_bins), np.complex128) if bandpass else None
         _check(lib().pcal_analyze(self._h, summ.ctypes.data, bp.ctypes.data if bandpass else None), "pcal_analyze")
         return summ, bp
+
+    def residual_rotation(self, dev_series_tones, n_periods: int) -> np.ndarray:
+        """float64 [n_channels, 3]: (arg S, |S|, norm) of a pcal_extract_series output (CUDA complex128 tensor)."""
+        out = np.empty((self.n_channels, 3), np.float64)
+        _check(lib().pcal_residual_rotation(self._h, dev_series_tones.data_ptr(), n_periods, out.ctypes.data), "pcal_residual_rotation")
+        return out
+
+    def refine_offset(self, dev_samples, n_per_period: int, n_periods: int, max_passes: int = 4, tol_rad: float = 1e-6, stream=None):
+        """Multi-pass counter-rotation.  Returns (refined f_offset in Hz, history float64 [passes, 4]:
+        f_rot used, arg S, |S|, norm).  The context is reset and its f_offset replaced by the refined value."""
+        f, n = ctypes.c_double(), ctypes.c_uint32()
+        hist = np.zeros((max_passes, 4), np.float64)
+        _check(lib().pcal_refine_offset(self._h, dev_samples.data_ptr(), n_per_period, n_periods, _stream_handle(stream), max_passes,
+                                        tol_rad, ctypes.byref(f), hist.ctypes.data, ctypes.byref(n)), "pcal_refine_offset")
+        return f.value, hist[:n.value]
 
     def get_folded(self) -> np.ndarray:
         out = np.empty((self.n_channels, self.n_bins), np.complex128)

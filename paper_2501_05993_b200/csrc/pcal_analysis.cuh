@@ -127,4 +127,40 @@ __global__ void __launch_bounds__(kAnaThreads) analyze_kernel(AnalyzeParams A) {
     out[7] = K > first ? sqrt(__ddiv_rn(rss, n)) : 0.0;
 }
 
+// ---- residual rotation of a time series of short integrations ----------------
+// "... multiple passes over the x[n] input data, iteratively counter-rotating the input data
+// using the residual phase shift detected in the previous pass."  Reading (R27): if eq. 2.3 rotates
+// by f_rot while the comb sits at i f_comb + f_true, every tone phasor turns by 2 pi (f_true - f_rot) T_int
+// from one short integration to the next, so
+//     S = sum_{m < M-1} sum_{i in band} T_{m+1}[i] conj(T_m[i]),   residual phase shift = arg S.
+// One CTA per channel; thread t adds the terms e = t, t + 256, ... (e = m * band + i, the oracle's order within
+// a thread), then a fixed tree adds the 256 thread sums: deterministic.  out[c] = (arg S, |S|, sum |T_{m+1}||T_m|).
+constexpr int kNResidual = 3;   // == PCAL_N_RESIDUAL
+__global__ void __launch_bounds__(kAnaThreads) residual_rotation_kernel(const double2* __restrict__ T, uint32_t M, uint32_t N, uint32_t C,
+                                                                        uint32_t zero_offset_mask, double* __restrict__ out) {
+    __shared__ double s_re[kAnaThreads], s_im[kAnaThreads], s_nm[kAnaThreads];
+    const uint32_t c = blockIdx.x, tid = threadIdx.x;
+    const uint32_t i0 = (zero_offset_mask >> c) & 1u, band = N / 2 - i0;
+    const uint32_t total = (M > 0 ? M - 1 : 0) * band;
+    double re = 0.0, im = 0.0, nm = 0.0;
+    for (uint32_t e = tid; e < total; e += kAnaThreads) {
+        const uint32_t m = e / band, i = i0 + e % band;
+        const double2 a = T[((size_t)(m + 1) * C + c) * N + i], b = T[((size_t)m * C + c) * N + i];
+        re += a.x * b.x + a.y * b.y;
+        im += a.y * b.x - a.x * b.y;
+        nm += sqrt(a.x * a.x + a.y * a.y) * sqrt(b.x * b.x + b.y * b.y);
+    }
+    s_re[tid] = re; s_im[tid] = im; s_nm[tid] = nm;
+    __syncthreads();
+    for (uint32_t s = kAnaThreads / 2; s > 0; s >>= 1) {
+        if (tid < s) { s_re[tid] += s_re[tid + s]; s_im[tid] += s_im[tid + s]; s_nm[tid] += s_nm[tid + s]; }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        out[c * kNResidual + 0] = atan2(s_im[0], s_re[0]);
+        out[c * kNResidual + 1] = hypot(s_re[0], s_im[0]);
+        out[c * kNResidual + 2] = s_nm[0];
+    }
+}
+
 }  // namespace pcal

@@ -753,6 +753,63 @@ extern "C" int pcal_analyze(pcal_ctx* c, double* out_summary, double* out_bandpa
     return PCAL_OK;
 }
 
+// ---- multi-pass counter-rotation (R27) ----------------------------------------------
+static int residual_rotation_of(pcal_ctx* c, const double* dev_series, uint32_t n_periods, uint32_t zero_mask, double* out) {
+    double* d_out = c->d_summary;       // [C][kNSummary] >= [C][kNResidual]
+    residual_rotation_kernel<<<c->C, kAnaThreads, 0, c->stream>>>(reinterpret_cast<const double2*>(dev_series), n_periods, c->n_bins,
+                                                                   (uint32_t)c->C, zero_mask, d_out);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    const size_t bytes = (size_t)c->C * kNResidual * sizeof(double);
+    CU(cudaMemcpyAsync(c->h_ana, d_out, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    memcpy(out, c->h_ana, bytes);
+    return PCAL_OK;
+}
+
+extern "C" int pcal_residual_rotation(pcal_ctx* c, const double* dev_series_tones, uint32_t n_periods, double* out) {
+    if (!c || !dev_series_tones || !out || n_periods == 0) return PCAL_ERR_INVALID;
+    uint32_t zero_mask = 0;
+    for (int i = 0; i < c->C; ++i) if (c->Foff[i] == 0) zero_mask |= 1u << i;
+    return residual_rotation_of(c, dev_series_tones, n_periods, zero_mask, out);
+}
+
+extern "C" int pcal_refine_offset(pcal_ctx* c, const void* dev_samples, uint64_t n_per_period, uint32_t n_periods, void* cuda_stream,
+                                  uint32_t max_passes, double tol_rad, double* out_f, double* out_history, uint32_t* out_passes) {
+    if (!c || !dev_samples || !out_f || n_per_period == 0 || n_periods < 2 || max_passes == 0 || !(tol_rad >= 0)) return PCAL_ERR_INVALID;
+    if (c->C != 1) return PCAL_ERR_UNSUPPORTED;
+    const double fs = (double)c->Fs * 1e-6, fcomb = (double)c->Fcomb * 1e-6;
+    const double t_int = (double)n_per_period / fs;
+    const uint32_t zero_mask = c->Foff[0] == 0 ? 1u : 0u;    // the band is fixed by the starting offset (tone 0 is sin(0) there)
+    double f = (double)c->Foff[0] * 1e-6;
+    double2* d_series = nullptr;
+    CU(cudaMalloc(&d_series, (size_t)n_periods * c->n_bins * sizeof(double2)));
+    int rc = PCAL_OK;
+    uint32_t passes = 0;
+    for (uint32_t k = 0; k < max_passes && rc == PCAL_OK; ++k) {
+        pcal_ctx* p = nullptr;        // one context per pass: the rotator (table or generator) of this pass's frequency
+        rc = pcal_create(&p, fs, fcomb, f, c->bits, c->enc, 1);
+        if (rc == PCAL_OK) rc = pcal_set_rotator(p, c->rot_req);
+        if (rc == PCAL_OK) rc = pcal_extract_series(p, dev_samples, n_per_period, n_periods, cuda_stream, reinterpret_cast<double*>(d_series), nullptr);
+        double res[kNResidual] = {0.0, 0.0, 0.0};
+        if (rc == PCAL_OK) rc = residual_rotation_of(p, reinterpret_cast<const double*>(d_series), n_periods, zero_mask, res);
+        pcal_destroy(p);
+        if (rc != PCAL_OK) break;
+        passes = k + 1;
+        if (out_history) { out_history[4 * k] = f; out_history[4 * k + 1] = res[0]; out_history[4 * k + 2] = res[1]; out_history[4 * k + 3] = res[2]; }
+        if (fabs(res[0]) <= tol_rad) break;
+        const double fn = (double)llround((f + res[0] / (2.0 * M_PI * t_int)) * 1e6) * 1e-6;     // counter-rotate, 1 uHz grid
+        if (!(fn >= 0.0) || !(fn < fs)) { rc = PCAL_ERR_INVALID; break; }
+        f = fn;
+    }
+    cudaFree(d_series);
+    if (rc != PCAL_OK) return rc;
+    *out_f = f;
+    if (out_passes) *out_passes = passes;
+    pcal_reset(c);                    // started = false: the offset may be replaced
+    return pcal_set_channel_offsets(c, &f);
+}
+
 // exp(+-j 2 pi k b / N) applied on the host to (un)shift the folded period
 static void kshift_bins(const pcal_ctx* c, double* bins, int sign) {
     if (!c->k_shift) return;
