@@ -409,3 +409,51 @@ def test_exchange_step_in_one_launch(oracle):
         outs.append(p.finalize())
     assert all(np.array_equal(outs[0], o) for o in outs[1:])
     assert_close(outs[0][0], oracle_tones(oracle, w, host, 0), "gathered exchange")
+
+
+@pytest.mark.parametrize("idx,n", [(2, 2_000_004), (1, 700_001), (4, 150_003), (3, 1_500_004)])
+def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n):
+    """Consecutive fold launches overlap (device-side sequence numbers instead of grid-wide waits, pcal_tail.cuh).  Many
+    back-to-back integration periods over different inputs, each into its own pinned buffer, must equal the result of the
+    same period run alone, bit for bit -- launched directly and replayed from a CUDA graph (frozen parameters: the ring
+    slot and the ordering are derived on the device)."""
+    from dataclasses import replace
+    from paper_2501_05993_b200 import binding
+    w = synth.config(idx).scaled(n)
+    bufs = [synth.generate(replace(w, seed=w.seed + 31 * k), DEV) for k in range(3)]
+    p = binding.from_workload(w)
+    alone = []
+    ref = torch.zeros((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory()
+    for b in bufs:                                   # reference: the same call, one period at a time, synchronised
+        p.integrate(b, n, ref); torch.cuda.synchronize(); alone.append(ref.numpy().copy())
+    assert_close(alone[0][0], oracle_tones(oracle, w, bufs[0].cpu().numpy(), 0), f"cfg{idx} alone")
+    p.set_input_ready(True)
+    reps = 40
+    outs = [torch.zeros((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory() for _ in range(reps)]
+    for r in range(reps):
+        p.integrate(bufs[r % 3], n, outs[r])
+    torch.cuda.synchronize()
+    for r in range(reps):
+        assert np.array_equal(outs[r].numpy(), alone[r % 3]), f"direct launch {r}"
+    # the same through a CUDA graph: 6 periods captured once, replayed 7 times, interleaved with direct launches
+    gouts = [torch.zeros((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory() for _ in range(6)]
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            for k in range(6):
+                p.integrate(bufs[k % 3], n, gouts[k])
+    torch.cuda.current_stream().wait_stream(side)
+    for it in range(7):
+        for o in gouts:
+            o.zero_()
+        g.replay()
+        if it % 2:
+            p.integrate(bufs[1], n, outs[0])
+        torch.cuda.synchronize()
+        for k in range(6):
+            assert np.array_equal(gouts[k].numpy(), alone[k % 3]), f"replay {it} period {k}"
+        if it % 2:
+            assert np.array_equal(outs[0].numpy(), alone[1])
+    p.destroy()
