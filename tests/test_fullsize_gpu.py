@@ -1,5 +1,6 @@
-"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one
-pcal_extract over the whole resident buffer, then pcal_finalize).
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times: the whole resident buffer in
+one period, once as pcal_extract + pcal_finalize and once exactly as bench.py's step issues it (pcal_set_input_ready +
+pcal_integrate into a pinned buffer, twice back to back so that the launches overlap).
 
 Configs 1-4: every folded bin and every tone against the oracle (rotator tabulated, host threads over
 contiguous ranges).  Config 5 (4e9 samples): sampled folded bins the oracle can compute one by one
@@ -19,6 +20,17 @@ pytestmark = pytest.mark.gpu
 THREADS = min(32, os.cpu_count() or 1)
 
 
+def bench_step_agrees(p, w, dev, T):
+    """bench.py's step on the same context: two overlapping periods; both must reproduce T (already held to the oracle)."""
+    outs = [torch.zeros((w.n_channels, w.n_bins), dtype=torch.complex128).pin_memory() for _ in range(2)]
+    p.set_input_ready(True)
+    for o in outs:
+        p.integrate(dev, w.n_samples, o)
+    torch.cuda.synchronize()
+    for o in outs:
+        assert np.abs(o.numpy() - T).max() <= 1e-12 * np.abs(T).max()
+
+
 @pytest.mark.parametrize("idx,rot", [(1, None), (2, None), (3, "lut"), (3, "generator")])
 def test_fullsize_single_channel(oracle, idx, rot):
     w = synth.config(idx)
@@ -30,6 +42,7 @@ def test_fullsize_single_channel(oracle, idx, rot):
     rel, _ = assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"cfg{idx} {rot} folded")
     assert_close(T[0], oracle.dft(pr, pi), f"cfg{idx} {rot} tones")
     print(f"cfg{idx} {rot}: worst-bin relative error {rel:.3e}")
+    bench_step_agrees(p, w, dev, T)
 
 
 def test_fullsize_cfg4_sixteen_channels(oracle):
@@ -42,6 +55,7 @@ def test_fullsize_cfg4_sixteen_channels(oracle):
         pr, pi = oracle_folded(oracle, w, host, c, threads=THREADS)
         assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"cfg4 ch{c} folded")
         assert_close(T[c], oracle.dft(pr, pi), f"cfg4 ch{c} tones")
+    bench_step_agrees(p, w, dev, T)
 
 
 def test_fullsize_cfg5_sampled_bins(oracle):
@@ -49,6 +63,7 @@ def test_fullsize_cfg5_sampled_bins(oracle):
     dev = synth.generate(w, "cuda")
     p, T, P = gpu_run(w, dev)
     assert p.info().rotator_in_effect == 2 and p.info().n_processed == w.n_samples
+    bench_step_agrees(p, w, dev, T)
     host = dev.cpu().numpy()
     del dev
     torch.cuda.empty_cache()
