@@ -60,6 +60,7 @@ struct pcal_ctx {
     // LUT-mode geometry
     uint32_t spv, F, q, R, grid;
     uint64_t M, nrot[PCAL_MAX_CHANNELS], lut_len[PCAL_MAX_CHANNELS];
+    uint32_t lut_off_h[PCAL_MAX_CHANNELS];   // first table entry of every channel (host copy)
     // generator-mode geometry
     uint32_t gen_grid, gen_spt;
     bool gen_mma;                   // integer samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
@@ -390,7 +391,7 @@ static int prepare(pcal_ctx* c) {
         std::vector<double2> lut;
         std::vector<uint32_t> off(c->C), len(c->C);
         for (int i = 0; i < c->C; ++i) {
-            off[i] = (uint32_t)lut.size(); len[i] = (uint32_t)c->nrot[i];
+            off[i] = (uint32_t)lut.size(); len[i] = (uint32_t)c->nrot[i]; c->lut_off_h[i] = off[i];
             for (uint64_t r = 0; r < c->nrot[i]; ++r) lut.push_back(phasor_neg_host(mulmod_host(r, c->Feff[i], c->Fs), c->Fs));
             c->lut_len[i] = c->nrot[i];
         }
@@ -450,7 +451,8 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
             tp.enabled = 1;
             tp.cnt = c->d_cnt; tp.G = c->d_G; tp.st = c->d_tail_state; tp.partial_stride = c->partial_slot_bytes;
             if (c->fuse_req) { tp.fuse_dft = 1; tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W; tp.T_dev = c->d_T; tp.T_host = c->fuse_out; }
-            tp.lut = c->d_lut; tp.lut_off = c->d_lut_off; tp.lut_len = c->d_lut_len;
+            tp.lut = c->d_lut;
+            for (int i = 0; i < c->C; ++i) { tp.lut_off[i] = c->lut_off_h[i]; tp.lut_len[i] = (uint32_t)c->nrot[i]; }
             tp.P = c->d_P; tp.Pint = c->d_Pint; tp.tail = data + n_vec * 16;
             tp.n0 = c->n_processed; tp.NT = n_vec * c->spv; tp.n_total = n;
             tp.n0_mod_bins = (uint32_t)(c->n_processed % c->n_bins);
@@ -905,14 +907,12 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
     uint32_t grid = (uint32_t)(c->sm_count * occ);
     if (const char* g = getenv("PCAL_PROBE_GRID")) grid = (uint32_t)atoi(g);      // tuning runs only
     const char* pp = getenv("PCAL_PROBE_PDL");
-    uint32_t spin_ns = 0;
-    if (const char* sp = getenv("PCAL_PROBE_SPIN_NS")) spin_ns = (uint32_t)atoi(sp);
     if (!(pp && pp[0] == '0'))      // default: consecutive probes may overlap, like the fold kernels
         launch_chain(read_probe_kernel, grid, kThreads, 0, (cudaStream_t)cuda_stream,
-                     reinterpret_cast<const uint4*>(dev), (uint64_t)(n_bytes / 16), reinterpret_cast<uint32_t*>(c->d_tmp), spin_ns);
+                     reinterpret_cast<const uint4*>(dev), (uint64_t)(n_bytes / 16), reinterpret_cast<uint32_t*>(c->d_tmp));
     else
         read_probe_kernel<<<grid, kThreads, 0, (cudaStream_t)cuda_stream>>>(
-            reinterpret_cast<const uint4*>(dev), n_bytes / 16, reinterpret_cast<uint32_t*>(c->d_tmp), spin_ns);
+            reinterpret_cast<const uint4*>(dev), n_bytes / 16, reinterpret_cast<uint32_t*>(c->d_tmp));
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;

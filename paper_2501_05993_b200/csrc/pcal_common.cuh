@@ -93,7 +93,7 @@ __device__ __forceinline__ double2 phasor_neg(uint64_t k, uint64_t m) {
 // (bench.py reports it beside the roofline fraction).  The xor of all words lands in out[0] only
 // if it equals a magic value, so the loads cannot be optimised away.
 namespace pcal {
-__global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __restrict__ d, uint64_t n_vec, uint32_t* out, uint32_t spin_ns) {
+__global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __restrict__ d, uint64_t n_vec, uint32_t* out) {
     pdl_release();
     const uint64_t stride = (uint64_t)gridDim.x * kThreads;
     uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
@@ -110,10 +110,5 @@ __global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __
         for (int u = 0; u < 4; ++u) v[u] = w[u];
     }
     if (acc == 0x5ca1ab1eu) out[0] = acc;
-    if (spin_ns && blockIdx.x == 0) {      // tuning runs only: one CTA stays behind (models a serial tail)
-        uint64_t t0, t1;
-        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
-        do { __nanosleep(200); asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t1)); } while (t1 - t0 < spin_ns);
-    }
 }
 }  // namespace pcal

@@ -43,8 +43,8 @@ struct TailParams {
     uint32_t* cnt;            // [device] [slot][q+1] arrival counters, zero between launches
     double2* G;               // [device] [slot][q][C*n_bins] per-group bins
     const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
-    const uint32_t* lut_off;  // [device] per channel: first entry
-    const uint32_t* lut_len;  // [device] per channel: N_rotator,c (1 => no rotation)
+    uint32_t lut_off[kMaxChannels];  // per channel: first entry (by value: no dependent load in the serial tail)
+    uint32_t lut_len[kMaxChannels];  // per channel: N_rotator,c (1 => no rotation)
     double2* P;               // [device] folded bins [C][N_bins]
     long long* Pint;          // [device] exact integer bins [C][N_bins]
     const uint8_t* tail;      // [device] first byte after the last complete vector
