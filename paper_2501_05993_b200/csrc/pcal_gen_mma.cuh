@@ -40,11 +40,12 @@ constexpr uint32_t kMmaRows = kTileSamples / kMmaSpan; // 32 rows per tile
 template <int KIND> struct GenMmaCfg;
 // LB bytes per load; GPT commit groups (of 4 loads: 4 consecutive rows) per tile; DG groups in flight per thread
 template <> struct GenMmaCfg<KIND_I8>   { static constexpr int LB = 16, GPT = 4, DG = 4; };   // groups (h, block c)
-template <> struct GenMmaCfg<KIND_2BIT> { static constexpr int LB = 8,  GPT = 2, DG = 8; };   // groups h; 8 B = 2 words = 32 samples
+template <> struct GenMmaCfg<KIND_2BIT> { static constexpr int LB = 16, GPT = 1, DG = 4; };   // DG = tiles in the CTA's staging ring (see the kernel)
 
 template <int KIND>
 constexpr size_t gen_mma_smem_bytes() {
-    const size_t ring = (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
+    const size_t ring = KIND == KIND_2BIT ? (size_t)GenMmaCfg<KIND>::DG * kMmaRows * 544
+                                          : (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
     const size_t fin = (size_t)kMmaSpan * sizeof(double2);              // final per-position values alias the ring
     return (size_t)kGenMaxTiles * sizeof(double2) + kMmaRows * sizeof(double2) + (size_t)kWarps * 256 + (ring > fin ? ring : fin);
 }
@@ -98,6 +99,18 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
 
     const uint64_t n_rows = P.n_loads / (kMmaSpan / 16);                         // host loads = 16 samples; whole rows only (host guarantees a multiple)
     const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    int acc[2][2][4][4];          // [block c (int8) / word (2-bit)][word half or field half w2][byte b][C fragment]
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int w2 = 0; w2 < 2; ++w2)
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc[c][w2][b][k] = 0;
+    long long s_re = 0, s_im = 0;     // sum over valid rows of the quantised phasors (2-bit: the -3 sum(rho) term)
+
+    if constexpr (KIND == KIND_I8) {
     // this thread's loads of one tile, in consumption order: group-major, 4 consecutive rows per group
     //   int8 : l = 8h + 4c + j -> row 16h + 4t + j, block c        2-bit: l = 4h + j -> row 16h + 4t + j
     constexpr int GPT = GenMmaCfg<KIND>::GPT;
@@ -161,17 +174,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     }
     __syncthreads();
 
-    int acc[2][2][4][4];          // [block c (int8) / word (2-bit)][word half or field half w2][byte b][C fragment]
-#pragma unroll
-    for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int w2 = 0; w2 < 2; ++w2)
-#pragma unroll
-            for (int b = 0; b < 4; ++b)
-#pragma unroll
-                for (int k = 0; k < 4; ++k) acc[c][w2][b][k] = 0;
-    long long s_re = 0, s_im = 0;     // sum over valid rows of the quantised phasors (2-bit: the -3 sum(rho) term)
-
     for (uint32_t i = 0; i < nt; ++i, rows_left -= row_stride, ahead += tile_stride, ahead_left -= row_stride) {
         const int ahead_lim_t = lim_of(ahead_left, i + TA < nt);
         // ---- digit matrix of this tile: lane = row ----
@@ -211,34 +213,104 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
                 for (int w2 = 0; w2 < 2; ++w2)
 #pragma unroll
                     for (int b = 0; b < 4; ++b) mma_s8_k16(acc[c][w2][b], T[w2][b], T[w2 + 2][b], bf[h]);
-            } else {
-                uint2 v[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    v[j] = *reinterpret_cast<const uint2*>(my_ring + (size_t)(slot_grp * 4 + j) * SLOT);
-                    if (SIGN_MAG) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
-                }
-                refill();
-#pragma unroll
-                for (int w = 0; w < 2; ++w) {
-                    // transpose the PACKED bytes first (a byte = 4 samples of one row), then spread the fields:
-                    // Tp[b] = byte b of rows 0..3; field f of it = 4 rows of sample 4 b + f, used in place: the sums carry
-                    // a factor 4^f that is shifted out (exactly) at the end
-                    uint32_t Tp[4];
-                    transpose4x4_bytes(w ? v[0].y : v[0].x, w ? v[1].y : v[1].x, w ? v[2].y : v[2].x, w ? v[3].y : v[3].x, Tp);
-#pragma unroll
-                    for (int f2 = 0; f2 < 2; ++f2)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b)
-                            mma_u8_k16(acc[w][f2][b], Tp[b] & (0x03030303u << (2 * f2)), Tp[b] & (0x30303030u << (2 * f2)), bf[h]);
-                }
             }
         }
+    }
+    } else {
+    // ---- 2-bit: whole tiles staged by the CTA ----------------------------------------------------------------
+    // A tile (32 rows x 512 B) is 16 KB of CONTIGUOUS input.  Per-thread 8-byte loads of it would reach the memory
+    // system as half-line requests and stall at ~2.3 TB/s (measured), so the CTA copies the tile as it lies: warp w
+    // loads rows w, w+8, w+16, w+24, one full 512-byte row per cp.async instruction (16 B per lane), into a shared
+    // tile with a row pitch of 544 B; DEPTH-1 tiles are in flight, one barrier per tile.  A thread's MMA operand is
+    // then read with LDS.64; the k slot 16h + 4t + j of the MMA is given to row 16h + t + 4j (the digit matrix uses
+    // the same permutation), which together with the pitch makes those reads conflict-free.
+    constexpr uint32_t PITCH = 544, TILE_SM = kMmaRows * PITCH;
+    constexpr int DEPTH = GenMmaCfg<KIND_2BIT>::DG;
+    const unsigned char* gdata2 = reinterpret_cast<const unsigned char*>(P.data);
+    auto issue_tile = [&](uint32_t ti) {                      // ti = index among this CTA's tiles
+        if (ti < nt) {
+            const uint64_t tile = (uint64_t)blockIdx.x + (uint64_t)ti * gridDim.x;
+            const long long left = (long long)n_rows - (long long)tile * kMmaRows;
+            const uint32_t lim = left <= 0 ? 0u : (left < (long long)kMmaRows ? (uint32_t)left : kMmaRows);
+            const unsigned char* src = gdata2 + tile * TILE_BYTES + (uint32_t)lane * 16u;
+            unsigned char* dst = ring + (size_t)(ti % DEPTH) * TILE_SM + (uint32_t)lane * 16u;
+#pragma unroll
+            for (uint32_t k = 0; k < 4; ++k) {
+                const uint32_t row = (uint32_t)warp + 8u * k;
+                if (row < lim) cp_async_own<16>(dst + row * PITCH, src + row * ROW_BYTES);
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (uint32_t ti = 0; ti + 1 < (uint32_t)DEPTH; ++ti) issue_tile(ti);
+    // (the first loads are in flight: now the tables)
+    {   // resync table: the exactly reduced integer phase of every tile start of this CTA -> fp64 phasor
+        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
+        if (k_cta >= P.Fs) k_cta -= P.Fs;
+        for (uint32_t i = tid; i < nt; i += kThreads) {
+            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
+            if (k >= P.Fs) k -= P.Fs;
+            base[i] = phasor_neg(k, P.Fs);
+        }
+        if (tid < (int)kMmaRows) rtab[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * kMmaSpan, P.Fs), P.Fs);
+    }
+    __syncthreads();
+
+    for (uint32_t i = 0; i < nt; ++i) {
+        cp_async_wait<DEPTH - 2>();       // this thread's part of tile i has landed ...
+        __syncthreads();                  // ... everybody's has, and everybody is done with tile i-1
+        issue_tile(i + DEPTH - 1);        // into the buffer of tile i-1
+        const long long rows_left = (long long)n_rows - ((long long)blockIdx.x + (long long)i * gridDim.x) * kMmaRows;
+        {   // digit matrix of this tile: lane = row, stored at its k slot
+            const double2 b0 = base[i], r = rtab[lane];
+            const bool valid = (long long)lane < rows_left;
+            const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
+            const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
+            int d0, d1, d2, e0, e1, e2;
+            digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
+            const int ks = (lane & 16) + 4 * (lane & 3) + ((lane >> 2) & 3);      // row 16h + t + 4j -> slot 16h + 4t + j
+            __syncwarp();
+            bt[0 * 32 + ks] = (unsigned char)d0; bt[1 * 32 + ks] = (unsigned char)d1; bt[2 * 32 + ks] = (unsigned char)d2;
+            bt[3 * 32 + ks] = (unsigned char)e0; bt[4 * 32 + ks] = (unsigned char)e1; bt[5 * 32 + ks] = (unsigned char)e2;
+            bt[6 * 32 + ks] = 0; bt[7 * 32 + ks] = 0;
+            s_re += vre; s_im += vim;     // this lane's rows; summed over the warp at the end
+            __syncwarp();
+        }
+        const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt);
+        const uint32_t bf[2] = {bt32[g * 8 + t], bt32[g * 8 + 4 + t]};
+        const unsigned char* tile = ring + (size_t)(i % DEPTH) * TILE_SM + (uint32_t)(warp * 64 + g * 8);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            uint2 v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                v[j] = *reinterpret_cast<const uint2*>(tile + (uint32_t)(16 * h + t + 4 * j) * PITCH);
+                if (SIGN_MAG) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
+            }
+#pragma unroll
+            for (int w = 0; w < 2; ++w) {
+                // transpose the PACKED bytes first (a byte = 4 samples of one row), then use the fields where they sit:
+                // Tp[b] = byte b of the 4 rows; field f of it = 4 rows of sample 4 b + f, scaled by 4^f (shifted out at the end)
+                uint32_t Tp[4];
+                transpose4x4_bytes(w ? v[0].y : v[0].x, w ? v[1].y : v[1].x, w ? v[2].y : v[2].x, w ? v[3].y : v[3].x, Tp);
+#pragma unroll
+                for (int f2 = 0; f2 < 2; ++f2)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b)
+                        mma_u8_k16(acc[w][f2][b], Tp[b] & (0x03030303u << (2 * f2)), Tp[b] & (0x30303030u << (2 * f2)), bf[h]);
+            }
+        }
+    }
     }
     cp_async_wait<0>();
     __syncthreads();                  // the ring is free: it becomes the per-position result array
 
     // ---- digits -> fp64, post-twiddle by exp(-j w pos), positions -> bins ------------------------
+    // The three Re and three Im digit sums of a position sit in lanes t = 0, 1, 2 of a quad: every thread leaves its 64
+    // int32 sums in shared memory ([element][thread]: conflict-free), then lane t of the quad finishes the positions
+    // idx % 4 == t of its quad (eight each), all reads before the result array -- which aliases the dump -- is written.
+    int* dump = reinterpret_cast<int*>(ring);               // [64][kThreads]
     double* pos_re = reinterpret_cast<double*>(ring);      // [2048]
     double* pos_im = pos_re + kMmaSpan;
     double2* tw256 = rtab;                                  // [8] exp(-j w 256 k): the row table is no longer needed
@@ -254,26 +326,36 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
 #pragma unroll
             for (int b = 0; b < 4; ++b)
 #pragma unroll
-                for (int half = 0; half < 2; ++half) {      // matrix row g (half 0) / g + 8 (half 1)
-                    const long long c0 = acc[c][w2][b][2 * half], c1 = acc[c][w2][b][2 * half + 1];
-                    // digit columns held by this lane: 2t, 2t+1 (0..2 = Re digits, 3..5 = Im digits)
-                    long long pre = 0, pim = 0;
-                    if (t == 0) pre = c0 + 256 * c1;
-                    else if (t == 1) { pre = 65536 * c0; pim = c1; }
-                    else if (t == 2) pim = 256 * c0 + 65536 * c1;
+                for (int k = 0; k < 4; ++k) dump[((((c * 2 + w2) * 4 + b) * 4) + k) * kThreads + tid] = acc[c][w2][b][k];
+    __syncthreads();
+    long long fre[8], fim[8];
+    {
+        const int qb = tid & ~3;                            // lane 0 of this thread's quad
 #pragma unroll
-                    for (int s = 1; s <= 2; s <<= 1) { pre += __shfl_xor_sync(0xFFFFFFFFu, pre, s); pim += __shfl_xor_sync(0xFFFFFFFFu, pim, s); }
-                    const int idx = ((c * 2 + w2) * 4 + b) * 2 + half;          // 0..31: lane t of the quad stores idx % 4 == t
-                    if ((idx & 3) == t) {
-                        const int wsel = w2 + 2 * half;                           // word (int8) / field (2-bit) of the block
-                        uint32_t pos;
-                        if (KIND == KIND_I8) pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
-                        else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8-byte load
-                        if (KIND == KIND_2BIT) { pre = 2 * (pre >> (2 * wsel)) - 3 * s_re; pim = 2 * (pim >> (2 * wsel)) - 3 * s_im; }   // undo 4^field
-                        pos_re[pos] = (double)pre * (1.0 / 4194304.0);
-                        pos_im[pos] = (double)pim * (1.0 / 4194304.0);
-                    }
-                }
+        for (int m = 0; m < 8; ++m) {
+            const int idx = 4 * m + t;                      // ((c*2 + w2)*4 + b)*2 + half
+            const int half = idx & 1, e0 = (idx >> 1) * 4 + 2 * half;      // elements e0, e0+1 = C-fragment columns 2t', 2t'+1
+            // digit columns: lane 0 holds (Re0, Re1), lane 1 (Re2, Im0), lane 2 (Im1, Im2)
+            const long long r0 = dump[e0 * kThreads + qb], r1 = dump[(e0 + 1) * kThreads + qb];
+            const long long r2 = dump[e0 * kThreads + qb + 1], i0 = dump[(e0 + 1) * kThreads + qb + 1];
+            const long long i1 = dump[e0 * kThreads + qb + 2], i2 = dump[(e0 + 1) * kThreads + qb + 2];
+            fre[m] = r0 + 256 * r1 + 65536 * r2;
+            fim[m] = i0 + 256 * i1 + 65536 * i2;
+        }
+    }
+    __syncthreads();                                        // the dump has been read: the result array may overwrite it
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const int idx = 4 * m + t, half = idx & 1, b = (idx >> 1) & 3, w2 = (idx >> 3) & 1, c = idx >> 4;
+        const int wsel = w2 + 2 * half;                     // word (int8) / field (2-bit) of the block
+        uint32_t pos;
+        if (KIND == KIND_I8) pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
+        else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8 bytes
+        long long pre = fre[m], pim = fim[m];
+        if (KIND == KIND_2BIT) { pre = 2 * (pre >> (2 * wsel)) - 3 * s_re; pim = 2 * (pim >> (2 * wsel)) - 3 * s_im; }   // undo 4^field
+        pos_re[pos] = (double)pre * (1.0 / 4194304.0);
+        pos_im[pos] = (double)pim * (1.0 / 4194304.0);
+    }
     __syncthreads();
     {   // exp(-j w pos), pos = tid + 256 k: one exactly reduced phasor per thread times the 8-entry stride table
         const double2 tw0 = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid, P.Fs), P.Fs);
