@@ -20,15 +20,19 @@
 // a resync point.  Each warp builds its own copy of the 32 x 8 digit matrix per tile (lane = row).
 //
 // Data movement.  A row is 2048 positions (2048 B of int8, 512 B of 2-bit codes); warp w owns positions
-// 256 w .. 256 w + 255.  Thread (g = lane/4, t = lane%4) owns, for its 8 rows 16h + 4t + j, 32 positions:
-// int8: the two 16-byte blocks c = 0, 1 at 256 w + 128 c + 16 g; 2-bit: the 8 bytes (two 16-sample words) at
-// byte 64 w + 8 g of the row.  Its own cp.async ring (no barrier), every byte used by exactly one thread.  The MMA wants
-// four consecutive ROWS of one position in a register, memory has positions consecutive: a 4x4 byte
-// transpose (8 PRMT per 16 samples) turns 4 row words into 4 position words.  2-bit words are first spread
-// into bytes (after the transpose: shift + mask per 4 samples) and stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho)
-// term, which does not depend on the data, is added once at the end from the same quantised phasors.
-// Rows past the end of the segment get zero digits, so whatever their ring slots hold contributes nothing.
-// ~1 instruction per sample instead of 3-4 for the FFMA2 kernel of pcal_gen.cuh: HBM-bound at any SM clock.
+// 256 w .. 256 w + 255 and thread (g = lane/4, t = lane%4) 32 of them for 8 of the 32 rows.
+//   int8 : the two 16-byte blocks c = 0, 1 at 256 w + 128 c + 16 g of rows 16h + 4t + j, loaded by the thread itself into
+//          its own cp.async ring (no barrier; a warp instruction covers 4 rows x 128 contiguous bytes).
+//   2-bit: 8 bytes per row and thread would reach the memory system as half-line requests (measured: 2.3 TB/s), so the CTA
+//          stages whole tiles -- 16 KB of contiguous input, one full 512-byte row per cp.async instruction -- in shared
+//          memory (4 tiles, one barrier per tile) and the threads read their 8 bytes (two 16-sample words) with LDS.64.
+// The MMA wants four consecutive ROWS of one position in a register, memory has positions consecutive: a 4x4 byte
+// transpose (8 PRMT per 16 bytes) turns 4 row words into 4 position words.  2-bit words are transposed as PACKED bytes and
+// the fields are then used where they sit (unsigned operand, code * 4^field <= 192; the factor is shifted out exactly at
+// the end); they stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho) term, which does not depend on the data, is added
+// once at the end from the same quantised phasors.  Rows past the end of the segment get zero digits, so whatever their
+// shared-memory slots hold contributes nothing.  ~1 instruction per sample instead of 3-4 for the FFMA2 kernel of
+// pcal_gen.cuh: HBM-bound at any SM clock for int8.
 #pragma once
 #include "pcal_gen.cuh"
 
