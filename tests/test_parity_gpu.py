@@ -457,3 +457,57 @@ def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n):
         if it % 2:
             assert np.array_equal(outs[0].numpy(), alone[1])
     p.destroy()
+
+
+@pytest.mark.parametrize("f_s,f_comb,f_off,bits,enc,n", [
+    (50e6, 1e6, 10e3, 2, 0, 1_000_064),      # N_bins = 50 (not a power of two), L = 5000
+    (25e6, 1e6, 0.0, 2, 1, 800_000),          # N_bins = 25 (odd), zero offset: integer-exact
+    (48e6, 2e6, 30e3, 32, 3, 600_001),        # N_bins = 24, float32, L = 1600
+    (96e6, 1e6, 250e3, 8, 2, 900_003),        # N_bins = 96 (> 64: DFT kernel), int8 through the LUT path, L = 384
+])
+def test_bin_counts_that_are_not_powers_of_two(oracle, f_s, f_comb, f_off, bits, enc, n):
+    """The fold geometry, the fused tail and its DFT make no power-of-two assumption about N_bins."""
+    from paper_2501_05993_b200 import binding
+    w = synth.Workload("odd_bins", 1, f_s, f_comb, [f_off], bits, enc, n, 0.05 if bits != 8 else 1.0, 1.0 if bits != 8 else 20.0, [5e-9], 4242)
+    dev = synth.generate(w, DEV)
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev)
+    assert p.info().rotator_in_effect == 1
+    pr, pi = oracle_folded(oracle, w, host, 0)
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), "folded")
+    assert_close(T[0], oracle.dft(pr, pi), "tones")
+    if f_off == 0.0 and bits != 32:
+        want = oracle.fold_i64(host, oracle_fmt(oracle, w), 1, 0, 0, 1, n, 0, w.n_bins)
+        assert np.array_equal(p.get_folded_i64()[0], want)
+    out = torch.zeros((1, w.n_bins), dtype=torch.complex128).pin_memory()
+    p.integrate(dev, n, out)
+    torch.cuda.synchronize()
+    assert np.abs(out.numpy() - T).max() <= 1e-12 * np.abs(T).max()
+    p.destroy()
+
+
+def test_two_contexts_interleaved_on_one_stream(oracle):
+    """Contexts keep their own tickets and progress counters: alternating overlapping periods of two different
+    configurations on one stream (what the time-sharded bench does with its two lanes) leaves both exact."""
+    from paper_2501_05993_b200 import binding
+    wa, da, ha = make(2, 1_500_004)
+    wb, db, hb = make(4, 120_003)
+    pa, pb = binding.from_workload(wa), binding.from_workload(wb)
+    for p_ in (pa, pb):
+        p_.set_input_ready(True)
+    oa = [torch.zeros((wa.n_channels, wa.n_bins), dtype=torch.complex128).pin_memory() for _ in range(12)]
+    ob = [torch.zeros((wb.n_channels, wb.n_bins), dtype=torch.complex128).pin_memory() for _ in range(12)]
+    for k in range(12):
+        pa.integrate(da, wa.n_samples, oa[k])
+        pb.integrate(db, wb.n_samples, ob[k])
+        if k % 3 == 2:
+            pa.finalize_async(oa[k])              # a DFT kernel of one context between the folds of the other
+    torch.cuda.synchronize()
+    want_a = oracle_tones(oracle, wa, ha, 0)
+    for k in range(12):
+        assert np.array_equal(oa[k].numpy(), oa[0].numpy()) or np.abs(oa[k].numpy() - oa[0].numpy()).max() <= 1e-12 * np.abs(want_a).max()
+        assert np.array_equal(ob[k].numpy(), ob[0].numpy())
+    assert_close(oa[0].numpy()[0], want_a, "context A")
+    for c in (0, 7, 15):
+        assert_close(ob[0].numpy()[c], oracle_tones(oracle, wb, hb, c), f"context B ch{c}")
+    pa.destroy(); pb.destroy()
