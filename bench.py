@@ -447,6 +447,11 @@ def main():
             "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
             "roofline": res["roofline"], "hot_kernel_us": res["hot_kernel_us"]}
     if world == 1 and rank == 0 and not args.quick:
+        from paper_2501_05993_b200 import binding as _b
+        # measured issue-rate ceilings of this GPU; every reported roofline is HBM, these say how far the ALU side is
+        line["pipe_peaks"] = {"ffma_thread_instr_per_s": _b.pipe_probe(0), "lop3_thread_instr_per_s": _b.pipe_probe(1),
+                              "imma_m16n8k16_s8_warp_instr_per_s": _b.pipe_probe(2),
+                              "how": "pcal_pipe_probe: 8 independent chains per thread, 8 CTAs x 256 threads per SM, best of 3"}
         probe, cores, _ = time_oracle(w, 1 << 21)
         n_sample = int(min(w.n_samples, max(1 << 22, probe * 1.0)))
         n_sample -= n_sample % 64

@@ -277,6 +277,12 @@ int pcal_generator_study(const pcal_gen_case_t *cases, uint32_t n_cases, uint64_
  * What it reaches on a given size is the practical ceiling of a read-once kernel of that size. */
 int pcal_read_probe(pcal_ctx *ctx, const void *dev, uint64_t n_bytes, void *cuda_stream);
 
+/* Calibration for the roofline report: the measured issue rate of one pipe of the current device.
+ * kind 0 = FFMA (fp32 FMA pipe), 1 = LOP3 (integer/logic pipe), 2 = IMMA m16n8k16 s8 (the legacy tensor path of the
+ * generator kernel).  out_per_s [host]: thread-instructions per second (kind 0, 1) or warp-level MMA instructions per
+ * second (kind 2) with every SM busy.  Synchronous, default stream, no context needed. */
+int pcal_pipe_probe(int kind, double *out_per_s);
+
 /* Zero accumulators, sample index <- 0 (on the context's stream); parameters are kept. */
 int pcal_reset(pcal_ctx *ctx);
 

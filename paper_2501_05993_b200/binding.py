@@ -96,6 +96,7 @@ def lib():
             "pcal_add_folded_dev": (i32, [vp, vp]),
             "pcal_set_profiling": (i32, [vp, i32]),
             "pcal_get_profile": (i32, [vp, ctypes.POINTER(dbl), ctypes.POINTER(u64)]),
+            "pcal_pipe_probe": (i32, [i32, ctypes.POINTER(dbl)]),
             "pcal_reset": (i32, [vp]),
             "pcal_destroy": (None, [vp]),
             "pcal_info": (i32, [vp, ctypes.POINTER(InfoT)]),
@@ -305,6 +306,13 @@ def generator_study(cases, n_steps: int, n_chk: int) -> np.ndarray:
     _check(lib().pcal_generator_study(ctypes.cast(arr, ctypes.c_void_p), len(cases), n_steps, n_chk, out.ctypes.data),
            "pcal_generator_study")
     return out
+
+
+def pipe_probe(kind: int) -> float:
+    """Measured issue rate of one pipe (0 FFMA, 1 LOP3: thread-instructions/s; 2 IMMA m16n8k16: warp-level MMAs/s)."""
+    v = ctypes.c_double()
+    _check(lib().pcal_pipe_probe(kind, ctypes.byref(v)), "pcal_pipe_probe")
+    return v.value
 
 
 def from_workload(w) -> "Pcal":

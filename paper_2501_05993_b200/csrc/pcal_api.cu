@@ -918,6 +918,35 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
     return PCAL_OK;
 }
 
+extern "C" int pcal_pipe_probe(int kind, double* out_per_s) {
+    if (!out_per_s || kind < 0 || kind > 2) return PCAL_ERR_INVALID;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    uint32_t* d_out = nullptr;
+    CU(cudaMalloc(&d_out, sizeof(uint32_t)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const uint32_t iters = 4096, grid = (uint32_t)sms * 8;       // 8 CTAs of 256 threads per SM: every scheduler has 16 warps
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        if (kind == 0) pipe_probe_kernel<0><<<grid, kThreads>>>(iters, d_out);
+        else if (kind == 1) pipe_probe_kernel<1><<<grid, kThreads>>>(iters, d_out);
+        else pipe_probe_kernel<2><<<grid, kThreads>>>(iters, d_out);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    if (cudaGetLastError() != cudaSuccess || !(best < 1e29f)) return PCAL_ERR_DEVICE;
+    const double per_thread = (double)iters * 8.0, threads = (double)grid * kThreads;
+    *out_per_s = (kind == 2 ? per_thread * threads / 32.0 : per_thread * threads) / (best * 1e-3);
+    return PCAL_OK;
+}
+
 // Generator accuracy study: one device thread per case.
 extern "C" int pcal_generator_study(const pcal_gen_case_t* cases, uint32_t n_cases, uint64_t n_steps, uint32_t n_chk,
                                     double* out_err) {
