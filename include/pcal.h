@@ -112,13 +112,14 @@ int pcal_set_k_shift(pcal_ctx *ctx, int k);
 int pcal_set_start_index(pcal_ctx *ctx, uint64_t n_start);
 
 /*
- * Promise about the sample buffers (default 0).  The kernels of a context are chained by programmatic
+ * Promise about the sample buffers (default 0).  The kernels of a context are launched with programmatic
  * dependent launch.  With ready != 0 the caller guarantees that every dev_samples buffer handed to
- * pcal_extract / pcal_extract_series is completely written BEFORE the call (e.g. by an earlier,
- * synchronised transfer; data resident in HBM) -- not produced by work that may still be running on
- * cuda_stream.  The streaming kernel then reads its input while the small kernels of the previous
- * segment are still finishing (it still waits for them before it writes anything).  With 0 it first
- * waits for all earlier work of the stream, like any kernel.  Results are identical either way.
+ * pcal_extract / pcal_extract_series / pcal_integrate is completely written BEFORE the call (e.g. by an
+ * earlier, synchronised transfer; data resident in HBM) -- not produced by work that may still be running
+ * on cuda_stream.  The streaming kernel of a call then reads its input while the kernels of the previous
+ * call are still running (consecutive launches overlap; whatever it WRITES is ordered behind them on the
+ * device).  With 0 it first waits for all earlier work of the stream, like any
+ * kernel.  Results are identical either way.
  */
 int pcal_set_input_ready(pcal_ctx *ctx, int ready);
 
@@ -129,6 +130,7 @@ int pcal_set_input_ready(pcal_ctx *ctx, int ready);
  *                  multiple of 8 (whole bytes), else PCAL_ERR_ALIGNMENT.  0 is a no-op.
  *   cuda_stream    cudaStream_t (NULL = default stream).  Asynchronous: never synchronises.
  * Successive calls are one continuous stream: the result is invariant to the split points.
+ * All calls on one context must use one stream, or be ordered by the caller (a context is not thread-safe).
  */
 int pcal_extract(pcal_ctx *ctx, const void *dev_samples, uint64_t n_samples, void *cuda_stream);
 
