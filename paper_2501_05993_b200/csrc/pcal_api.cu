@@ -84,6 +84,7 @@ struct pcal_ctx {
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
     double2* fuse_out;              // pcal_integrate: the fold kernel of this call also takes the DFT and writes T here (or null)
+    double2 *fuse_T_dev, *fuse_P_copy;   // pcal_extract_series: device destinations of T and of a copy of P for the piece being enqueued
     bool fuse_req;                  // ... requested for the piece being enqueued
     const double* last_out;         // pcal_finalize_async: last host buffer seen and its device mapping (or null)
     double2* last_out_mapped;
@@ -450,7 +451,10 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         if (c->fused) {
             tp.enabled = 1;
             tp.cnt = c->d_cnt; tp.G = c->d_G; tp.st = c->d_tail_state; tp.partial_stride = c->partial_slot_bytes;
-            if (c->fuse_req) { tp.fuse_dft = 1; tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W; tp.T_dev = c->d_T; tp.T_host = c->fuse_out; }
+            if (c->fuse_req) {
+                tp.fuse_dft = 1; tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W;
+                tp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; tp.T_host = c->fuse_out; tp.P_copy = c->fuse_P_copy;
+            }
             tp.lut = c->d_lut;
             for (int i = 0; i < c->C; ++i) { tp.lut_off[i] = c->lut_off_h[i]; tp.lut_len[i] = (uint32_t)c->nrot[i]; }
             tp.P = c->d_P; tp.Pint = c->d_Pint; tp.tail = data + n_vec * 16;
@@ -548,6 +552,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
 }
 
 static int enqueue_dft(pcal_ctx* c, double2* second_dst);
+static bool can_fuse_dft(const pcal_ctx* c);
 
 // PCAL_SMALL_PIECES=1 (tests only): see extract_segment.  Read per call (tests toggle it), but cheaply.
 static bool small_pieces() {
@@ -608,10 +613,21 @@ extern "C" int pcal_extract_series(pcal_ctx* c, const void* dev_samples, uint64_
     c->stream = (cudaStream_t)cuda_stream;
     const size_t nb = (size_t)c->n_bins * c->C;
     const uint8_t* p = reinterpret_cast<const uint8_t*>(dev_samples);
+    // Small N_bins on the LUT path: the fold kernel of a period delivers T and the copy of P itself (one launch per
+    // period, consecutive periods overlap); otherwise the DFT kernel and a device-to-device copy follow every period.
+    const uint64_t piece = c->rot_eff == PCAL_ROT_LUT ? (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv : 0;
+    const bool fuse = can_fuse_dft(c) && !small_pieces() && n_per_period <= piece && bits_per_period >= 128;
     for (uint32_t k = 0; k < n_periods; ++k) {
         c->zero_pending = true;                       // the period's first post kernel overwrites the bins
+        if (fuse) {
+            c->fuse_req = true; c->fuse_out = nullptr;
+            c->fuse_T_dev = reinterpret_cast<double2*>(dev_out_tones) + (size_t)k * nb;
+            c->fuse_P_copy = dev_out_folded ? reinterpret_cast<double2*>(dev_out_folded) + (size_t)k * nb : nullptr;
+        }
         int r = extract_segment(c, p + (size_t)k * (bits_per_period / 8), n_per_period);
+        c->fuse_req = false; c->fuse_T_dev = nullptr; c->fuse_P_copy = nullptr;
         if (r != PCAL_OK) return r;
+        if (fuse) continue;
         r = enqueue_dft(c, reinterpret_cast<double2*>(dev_out_tones) + (size_t)k * nb);
         if (r != PCAL_OK) return r;
         if (dev_out_folded)
@@ -714,7 +730,7 @@ extern "C" int pcal_integrate(pcal_ctx* c, const void* dev_samples, uint64_t n_s
     const uint64_t piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
     c->fuse_req = mapped && can_fuse_dft(c) && !small_pieces() && n_samples <= piece &&
                   n_samples * (uint64_t)c->bits * c->C / 8 >= 16 && dev_samples;
-    c->fuse_out = mapped;
+    c->fuse_out = mapped; c->fuse_T_dev = nullptr; c->fuse_P_copy = nullptr;
     r = pcal_extract(c, dev_samples, n_samples, cuda_stream);
     const bool fused_done = c->fuse_req;
     c->fuse_req = false;

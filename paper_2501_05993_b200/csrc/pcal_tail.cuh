@@ -64,6 +64,7 @@ struct TailParams {
     const double2* W;         // [device] exp(-j 2 pi k / N_bins), k < N_bins
     double2* T_dev;           // [device] tone spectrum [C][N_bins]
     double2* T_host;          // device-visible pinned host memory or null
+    double2* P_copy;          // [device] second destination of the folded bins (time series output) or null
 };
 
 constexpr uint32_t kTailSlots = 8;
@@ -298,6 +299,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         T.P[pp] = make_double2(are, aim);
         if (T.integer_exact) T.Pint[pp] = ai;
         if (T.fuse_dft) reinterpret_cast<double2*>(scratch + 2 * kThreads)[pp] = make_double2(are, aim);
+        if (T.P_copy) T.P_copy[pp] = make_double2(are, aim);
     }
     if (T.fuse_dft) {   // T[c][i] = sum_b P[c][b] W[(i' b) mod N], i' = (i - k_shift) mod N: one thread per output, b in order
         __syncthreads();

@@ -37,8 +37,9 @@ def test_series_matches_per_period_oracle(oracle, idx, n_per, n_periods, rot):
                                     w.f_s_hz, w.f_comb_hz, w.f_offset_hz[c], tabulated=True, threads=1)
             assert_close(P[k, c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"cfg{idx} period {k} ch{c} folded", floor_frac=0.05)
             assert_close(T[k, c], oracle.dft(pr, pi), f"cfg{idx} period {k} ch{c} tones", floor_frac=0.05)
-    # the context is left with the last period: finalize repeats it bit for bit
-    assert np.array_equal(p.finalize(), T[-1])
+    # the context is left with the last period: finalize repeats it
+    Tl = p.finalize()                                # (the DFT kernel and the fold kernel's own DFT sum in different orders)
+    assert np.abs(Tl - T[-1]).max() <= 1e-12 * np.abs(Tl).max()
     p.destroy()
 
 
