@@ -69,7 +69,7 @@ __device__ __forceinline__ uint32_t word_of(const uint4& v, int j) {
 // Only used a handful of times per kernel (tails, per-CTA start phases).
 __device__ __forceinline__ uint64_t mulmod_u64(uint64_t a, uint64_t b, uint64_t m) {
     uint64_t r = 0;
-    a %= m;
+    if (a >= m) a %= m;                                     // callers usually pass an already reduced factor
     if (__umul64hi(a, b) == 0) return (a * b) % m;       // the product fits in 64 bits (the usual case: small multipliers)
     while (b) {
         if (b & 1) { r += a; if (r >= m) r -= m; }

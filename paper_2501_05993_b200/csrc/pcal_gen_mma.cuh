@@ -174,7 +174,8 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             if (k >= P.Fs) k -= P.Fs;
             base[i] = phasor_neg(k, P.Fs);
         }
-        if (tid < (int)kMmaRows) rtab[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * kMmaSpan, P.Fs), P.Fs);
+        // (the last 32 threads: the first ones are busy with the tile phasors above)
+        if (tid >= kThreads - (int)kMmaRows) { const int r = tid - (kThreads - (int)kMmaRows); rtab[r] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)r * kMmaSpan, P.Fs), P.Fs); }
     }
     __syncthreads();
 
@@ -257,7 +258,8 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             if (k >= P.Fs) k -= P.Fs;
             base[i] = phasor_neg(k, P.Fs);
         }
-        if (tid < (int)kMmaRows) rtab[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * kMmaSpan, P.Fs), P.Fs);
+        // (the last 32 threads: the first ones are busy with the tile phasors above)
+        if (tid >= kThreads - (int)kMmaRows) { const int r = tid - (kThreads - (int)kMmaRows); rtab[r] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)r * kMmaSpan, P.Fs), P.Fs); }
     }
     __syncthreads();
 
