@@ -67,6 +67,12 @@ __device__ __forceinline__ void mma_u8_k16(int (&d)[4], uint32_t a0, uint32_t a1
                  : "r"(a0), "r"(a1), "r"(b0));
 }
 
+__device__ __forceinline__ void mma_u8_k32(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
 // rows r0..r3 (bytes = 4 positions each) -> o[p] = (r0.p, r1.p, r2.p, r3.p), byte 0 = row 0
 __device__ __forceinline__ void transpose4x4_bytes(uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3, uint32_t (&o)[4]) {
     const uint32_t x01l = __byte_perm(r0, r1, 0x5140), x01h = __byte_perm(r0, r1, 0x7362);
@@ -286,26 +292,28 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt);
         const uint32_t bf[2] = {bt32[g * 8 + t], bt32[g * 8 + 4 + t]};
         const unsigned char* tile = ring + (size_t)(i % DEPTH) * TILE_SM + (uint32_t)(warp * 64 + g * 8);
+        // both k halves (rows 0..15 and 16..31) go into ONE m16n8k32 MMA: same issue cost as k16 on this GPU (8 cycles)
+        uint2 v[2][4];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            uint2 v[4];
+        for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                v[j] = *reinterpret_cast<const uint2*>(tile + (uint32_t)(16 * h + t + 4 * j) * PITCH);
-                if (SIGN_MAG) { v[j].x = signmag_to_offset_binary(v[j].x); v[j].y = signmag_to_offset_binary(v[j].y); }
+                v[h][j] = *reinterpret_cast<const uint2*>(tile + (uint32_t)(16 * h + t + 4 * j) * PITCH);
+                if (SIGN_MAG) { v[h][j].x = signmag_to_offset_binary(v[h][j].x); v[h][j].y = signmag_to_offset_binary(v[h][j].y); }
             }
 #pragma unroll
-            for (int w = 0; w < 2; ++w) {
-                // transpose the PACKED bytes first (a byte = 4 samples of one row), then use the fields where they sit:
-                // Tp[b] = byte b of the 4 rows; field f of it = 4 rows of sample 4 b + f, scaled by 4^f (shifted out at the end)
-                uint32_t Tp[4];
-                transpose4x4_bytes(w ? v[0].y : v[0].x, w ? v[1].y : v[1].x, w ? v[2].y : v[2].x, w ? v[3].y : v[3].x, Tp);
+        for (int w = 0; w < 2; ++w) {
+            // transpose the PACKED bytes first (a byte = 4 samples of one row), then use the fields where they sit:
+            // Tp[b] = byte b of the 4 rows; field f of it = 4 rows of sample 4 b + f, scaled by 4^f (shifted out at the end)
+            uint32_t T0[4], T1[4];
+            transpose4x4_bytes(w ? v[0][0].y : v[0][0].x, w ? v[0][1].y : v[0][1].x, w ? v[0][2].y : v[0][2].x, w ? v[0][3].y : v[0][3].x, T0);
+            transpose4x4_bytes(w ? v[1][0].y : v[1][0].x, w ? v[1][1].y : v[1][1].x, w ? v[1][2].y : v[1][2].x, w ? v[1][3].y : v[1][3].x, T1);
 #pragma unroll
-                for (int f2 = 0; f2 < 2; ++f2)
+            for (int f2 = 0; f2 < 2; ++f2)
 #pragma unroll
-                    for (int b = 0; b < 4; ++b)
-                        mma_u8_k16(acc[w][f2][b], Tp[b] & (0x03030303u << (2 * f2)), Tp[b] & (0x30303030u << (2 * f2)), bf[h]);
-            }
+                for (int b = 0; b < 4; ++b)
+                    mma_u8_k32(acc[w][f2][b], T0[b] & (0x03030303u << (2 * f2)), T0[b] & (0x30303030u << (2 * f2)),
+                               T1[b] & (0x03030303u << (2 * f2)), T1[b] & (0x30303030u << (2 * f2)), bf[0], bf[1]);
         }
     }
     }
