@@ -269,27 +269,32 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     }
     __syncthreads();
 
+    // digit matrix of this CTA's tile ti, built by ONE warp (lane = row, stored at its k slot) into buffer ti & 1; the
+    // per-tile barrier hands it to the other warps.  s_re/s_im collect the quantised phasors of the rows this lane built.
+    auto build_digits = [&](uint32_t ti) {
+        if (ti >= nt) return;
+        const long long rows_left = (long long)n_rows - ((long long)blockIdx.x + (long long)ti * gridDim.x) * kMmaRows;
+        const double2 b0 = base[ti], r = rtab[lane];
+        const bool valid = (long long)lane < rows_left;
+        const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
+        const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
+        int d0, d1, d2, e0, e1, e2;
+        digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
+        const int ks = (lane & 16) + 4 * (lane & 3) + ((lane >> 2) & 3);      // row 16h + t + 4j -> slot 16h + 4t + j
+        unsigned char* b = bt_all + (ti & 1u) * 256u;
+        b[0 * 32 + ks] = (unsigned char)d0; b[1 * 32 + ks] = (unsigned char)d1; b[2 * 32 + ks] = (unsigned char)d2;
+        b[3 * 32 + ks] = (unsigned char)e0; b[4 * 32 + ks] = (unsigned char)e1; b[5 * 32 + ks] = (unsigned char)e2;
+        b[6 * 32 + ks] = 0; b[7 * 32 + ks] = 0;
+        s_re += vre; s_im += vim;
+    };
+    if (warp == 0) build_digits(0);
+
     for (uint32_t i = 0; i < nt; ++i) {
         cp_async_wait<DEPTH - 2>();       // this thread's part of tile i has landed ...
-        __syncthreads();                  // ... everybody's has, and everybody is done with tile i-1
+        __syncthreads();                  // ... everybody's has, the digits of tile i are there, everybody is done with tile i-1
         issue_tile(i + DEPTH - 1);        // into the buffer of tile i-1
-        const long long rows_left = (long long)n_rows - ((long long)blockIdx.x + (long long)i * gridDim.x) * kMmaRows;
-        {   // digit matrix of this tile: lane = row, stored at its k slot
-            const double2 b0 = base[i], r = rtab[lane];
-            const bool valid = (long long)lane < rows_left;
-            const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
-            const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
-            int d0, d1, d2, e0, e1, e2;
-            digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
-            const int ks = (lane & 16) + 4 * (lane & 3) + ((lane >> 2) & 3);      // row 16h + t + 4j -> slot 16h + 4t + j
-            __syncwarp();
-            bt[0 * 32 + ks] = (unsigned char)d0; bt[1 * 32 + ks] = (unsigned char)d1; bt[2 * 32 + ks] = (unsigned char)d2;
-            bt[3 * 32 + ks] = (unsigned char)e0; bt[4 * 32 + ks] = (unsigned char)e1; bt[5 * 32 + ks] = (unsigned char)e2;
-            bt[6 * 32 + ks] = 0; bt[7 * 32 + ks] = 0;
-            s_re += vre; s_im += vim;     // this lane's rows; summed over the warp at the end
-            __syncwarp();
-        }
-        const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt);
+        if (warp == (int)((i + 1) % kWarps)) build_digits(i + 1);      // for the next tile, into the other digit buffer
+        const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt_all + (i & 1u) * 256u);
         const uint32_t bf[2] = {bt32[g * 8 + t], bt32[g * 8 + 4 + t]};
         const unsigned char* tile = ring + (size_t)(i % DEPTH) * TILE_SM + (uint32_t)(warp * 64 + g * 8);
         // both k halves (rows 0..15 and 16..31) go into ONE m16n8k32 MMA: same issue cost as k16 on this GPU (8 cycles)
@@ -329,9 +334,15 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     double* pos_im = pos_re + kMmaSpan;
     double2* tw256 = rtab;                                  // [8] exp(-j w 256 k): the row table is no longer needed
     if (tid < 8) tw256[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * 256u, P.Fs), P.Fs);
-    if (KIND == KIND_2BIT) {
+    if (KIND == KIND_2BIT) {              // every tile's digits were built by one warp: add lanes, then warps
+        __shared__ long long s_sum[2][kWarps];
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) { s_re += __shfl_xor_sync(0xFFFFFFFFu, s_re, s); s_im += __shfl_xor_sync(0xFFFFFFFFu, s_im, s); }
+        if (lane == 0) { s_sum[0][warp] = s_re; s_sum[1][warp] = s_im; }
+        __syncthreads();
+        s_re = 0; s_im = 0;
+#pragma unroll
+        for (int ww = 0; ww < kWarps; ++ww) { s_re += s_sum[0][ww]; s_im += s_sum[1][ww]; }
     }
 #pragma unroll
     for (int c = 0; c < 2; ++c)
