@@ -51,7 +51,7 @@ constexpr size_t gen_mma_smem_bytes() {
     const size_t ring = KIND == KIND_2BIT ? (size_t)GenMmaCfg<KIND>::DG * kMmaRows * 544
                                           : (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
     const size_t fin = (size_t)kMmaSpan * sizeof(double2);              // final per-position values alias the ring
-    return (size_t)kGenMaxTiles * sizeof(double2) + kMmaRows * sizeof(double2) + (size_t)kWarps * 256 + (ring > fin ? ring : fin);
+    return (size_t)kGenMaxTiles * sizeof(double2) + (kMmaRows + 128 + 16) * sizeof(double2) + (size_t)kWarps * 256 + (ring > fin ? ring : fin);
 }
 
 __device__ __forceinline__ void mma_s8_k16(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
@@ -102,7 +102,9 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     extern __shared__ __align__(16) unsigned char gen_smem[];
     double2* base = reinterpret_cast<double2*>(gen_smem);                       // [kGenMaxTiles] tile-start phasors
     double2* rtab = base + kGenMaxTiles;                                         // [32] exp(-j w 2048 row)
-    unsigned char* bt_all = reinterpret_cast<unsigned char*>(rtab + kMmaRows);   // [warp][8 digit columns][32 rows]
+    double2* twA = rtab + kMmaRows;                                              // [128] exp(-j w 16 a): position factor, coarse part
+    double2* twB = twA + 128;                                                    // [16]  exp(-j w b):    position factor, fine part
+    unsigned char* bt_all = reinterpret_cast<unsigned char*>(twB + 16);          // [warp][8 digit columns][32 rows]
     unsigned char* ring = bt_all + kWarps * 256;                                 // [DG*4][kThreads][LB]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     unsigned char* bt = bt_all + warp * 256;
@@ -182,6 +184,9 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         }
         // (the last 32 threads: the first ones are busy with the tile phasors above)
         if (tid >= kThreads - (int)kMmaRows) { const int r = tid - (kThreads - (int)kMmaRows); rtab[r] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)r * kMmaSpan, P.Fs), P.Fs); }
+        // position factors exp(-j w pos), pos = 16 a + b, for the epilogue: threads 64 .. 207, exactly reduced as well
+        if (tid >= 64 && tid < 64 + 128) twA[tid - 64] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 64) * 16u, P.Fs), P.Fs);
+        if (tid >= 192 && tid < 192 + 16) twB[tid - 192] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 192), P.Fs), P.Fs);
     }
     __syncthreads();
 
@@ -266,6 +271,9 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         }
         // (the last 32 threads: the first ones are busy with the tile phasors above)
         if (tid >= kThreads - (int)kMmaRows) { const int r = tid - (kThreads - (int)kMmaRows); rtab[r] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)r * kMmaSpan, P.Fs), P.Fs); }
+        // position factors exp(-j w pos), pos = 16 a + b, for the epilogue: threads 64 .. 207, exactly reduced as well
+        if (tid >= 64 && tid < 64 + 128) twA[tid - 64] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 64) * 16u, P.Fs), P.Fs);
+        if (tid >= 192 && tid < 192 + 16) twB[tid - 192] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 192), P.Fs), P.Fs);
     }
     __syncthreads();
 
@@ -332,8 +340,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     int* dump = reinterpret_cast<int*>(ring);               // [64][kThreads]
     double* pos_re = reinterpret_cast<double*>(ring);      // [2048]
     double* pos_im = pos_re + kMmaSpan;
-    double2* tw256 = rtab;                                  // [8] exp(-j w 256 k): the row table is no longer needed
-    if (tid < 8) tw256[tid] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * 256u, P.Fs), P.Fs);
     if (KIND == KIND_2BIT) {              // every tile's digits were built by one warp: add lanes, then warps
         __shared__ long long s_sum[2][kWarps];
 #pragma unroll
@@ -382,12 +388,12 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         pos_im[pos] = (double)pim * (1.0 / 4194304.0);
     }
     __syncthreads();
-    {   // exp(-j w pos), pos = tid + 256 k: one exactly reduced phasor per thread times the 8-entry stride table
-        const double2 tw0 = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid, P.Fs), P.Fs);
+    {   // exp(-j w pos), pos = tid + 256 k = 16 a + b: product of two exactly reduced table phasors (built in the prologue)
+        const double2 fb = twB[tid & 15];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            const double2 s8 = tw256[k];
-            const double twx = tw0.x * s8.x - tw0.y * s8.y, twy = tw0.x * s8.y + tw0.y * s8.x;
+            const double2 fa = twA[(tid >> 4) + 16 * k];
+            const double twx = fa.x * fb.x - fa.y * fb.y, twy = fa.x * fb.y + fa.y * fb.x;
             const uint32_t pos = (uint32_t)tid + 256u * k;
             const double re = pos_re[pos], im = pos_im[pos];
             pos_re[pos] = re * twx - im * twy;
