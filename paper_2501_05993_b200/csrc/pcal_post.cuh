@@ -236,11 +236,16 @@ __global__ void __launch_bounds__(kPostThreads) post_gen_kernel(GenPostParams G)
     const uint32_t shift = (uint32_t)(G.n0 % G.n_bins);
     const uint32_t s = ok ? (b + G.n_bins - shift) % G.n_bins : 0;
     double re = 0.0, im = 0.0;
-    if (ok)
-        for (uint32_t c = w; c < G.grid; c += kPostThreads / 32) {
-            const double2 v = G.partial[(size_t)c * G.n_bins + s];
-            re += v.x; im += v.y;
+    if (ok) {
+        constexpr uint32_t W = kPostThreads / 32;
+        for (uint32_t c0 = w; c0 < G.grid; c0 += 8u * W) {        // eight loads in flight, added in CTA order
+            double2 v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = (c0 + k * W < G.grid) ? __ldcg(G.partial + (size_t)(c0 + k * W) * G.n_bins + s) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { re += v[k].x; im += v[k].y; }
         }
+    }
     sre[w][lane] = re; sim[w][lane] = im;
     __syncthreads();
     if (w != 0 || !ok) return;
