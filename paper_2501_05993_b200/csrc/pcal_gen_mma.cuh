@@ -6,7 +6,7 @@
 //     rho[tile,row] = e^{-j w (n0 + 2^16 tile)} * e^{-j w 2048 row}
 // (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is
 // a matrix product  X^T (2048 positions x rows)  *  R (rows x {Re, Im})  -- a contraction over TIME with a
-// two-column right-hand side.  It runs as integer tensor-core MMAs (mma.sync m16n8k16, s8 x s8 -> s32):
+// two-column right-hand side.  It runs as integer tensor-core MMAs (mma.sync m16n8k16 / m16n8k32, s8|u8 x s8 -> s32):
 // the phasor is quantised to 23-bit fixed point, round(rho 2^22) = d0 + 2^8 d1 + 2^16 d2 with signed 8-bit
 // digits, and the six digit columns (3 for Re, 3 for Im) fill the n = 8 side of the MMA.  All sums are exact
 // integers (int32 per digit column; |sum| < 2^31 for the <= 256 tiles a CTA sees per launch), recombined
@@ -17,7 +17,8 @@
 // ((n0 + 2^16 tile) F_off mod F_s, the "fp64 phase resync every 2^16 samples" of BASELINE.json config 5),
 // the row factor from a 32-entry table of exact stride phasors e^{-j w 2048 row} (stride stepping as in
 // eq. 2.8); one coupled-form complex multiply (eq. 2.6) per row in fp64, never more than 31 strides from
-// a resync point.  Each warp builds its own copy of the 32 x 8 digit matrix per tile (lane = row).
+// a resync point.  The 32 x 8 digit matrix of a tile is built with lane = row (int8: by every warp for itself; 2-bit:
+// by one warp per CTA, handed over by the per-tile barrier).
 //
 // Data movement.  A row is 2048 positions (2048 B of int8, 512 B of 2-bit codes); warp w owns positions
 // 256 w .. 256 w + 255 and thread (g = lane/4, t = lane%4) 32 of them for 8 of the 32 rows.

@@ -4,18 +4,18 @@
 // table of eq. 2.4 after the reordering of PAPER.md:200.
 //
 // Same arithmetic as reduce_replicas_kernel + rotate_fold_kernel (pcal_post.cuh), which remain as the
-// un-fused path for geometries the tail does not take (see tail_ok in pcal_api.cu).  Three stages, each
-// entered by exactly one CTA per group, elected by an arrival counter (every CTA: write partial,
-// __threadfence, barrier, one atomicAdd; the CTA that observes count-1 is last and reads what the
-// others wrote):
+// un-fused path for geometries the tail does not take (`fused` in pcal_api.cu's prepare).  Three stages, each
+// entered by exactly one CTA per group, elected by an arrival counter (every CTA: write partial, barrier,
+// one atom.add.acq_rel by one thread; the CTA that observes count-1 is last and reads what the others
+// wrote):
 //   A  last CTA of slot group p: sum the R replica partials of the group (replica order), code sums
 //      -> level sums, into shared memory                                   [F*32 values]
 //   B  same CTA: multiply by the rotator table and fold the group's 32*spv time samples into per-group
 //      bins G[p][c][b]   (fixed thread -> element map + fixed butterfly: deterministic)
 //   C  last CTA of the grid: P[c][b] (+)= sum_p G[p][c][b] in group order, ragged tail (< 1 vector)
 //      added, integer bins kept when the data is integer and unrotated; counters reset for the next
-//      launch.
-// A step of the LUT path is thereby ONE launch (plus the DFT of pcal_finalize).
+//      launch; for pcal_integrate / pcal_extract_series with N_bins <= 64 also the DFT.
+// A step of the LUT path is thereby ONE launch (plus the DFT kernel of pcal_finalize for larger N_bins).
 //
 // Pipelining across launches.  Partials, counters and G live in a ring of kTailSlots slots and a fold
 // kernel never executes griddepcontrol.wait.  Every CTA takes a ticket (64-bit atomicAdd on the
