@@ -15,6 +15,7 @@
 #include "pcal_fold.cuh"
 #include "pcal_gen.cuh"
 #include "pcal_gen_mma.cuh"
+#include "pcal_gen2.cuh"
 #include "pcal_post.cuh"
 #include "pcal_analysis.cuh"
 #include "pcal_genstudy.cuh"
@@ -64,6 +65,12 @@ struct pcal_ctx {
     // generator-mode geometry
     uint32_t gen_grid, gen_spt;
     bool gen_mma;                   // integer samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
+    bool gen2;                      // 2-bit samples, <= 4 channels: warp-specialised tensor-core generator kernel (pcal_gen2.cuh)
+    uint32_t g2_span_t, g2_chunks;  // ... its row: time samples, 16-byte chunks
+    uint32_t g2_cpw, g2_rt;         // ... chunks per consumer warp (1, 2, 4), rows per tile (128, 64, 32)
+    double2 *d_g2_rtab, *d_g2_tw;   // ... stride phasors [C][32], position factors [C][span_t]
+    uint32_t* d_g2_ctr;             // ... [slot][2] batch and arrival counters
+    long long* d_g2_posacc;         // ... [slot][2*2048] exact per-position sums
     size_t gen_smem;
     // device
     int device, sm_count;
@@ -142,6 +149,8 @@ static void free_tables(pcal_ctx* c) {
     cudaFree(c->d_lut); cudaFree(c->d_lut_off); cudaFree(c->d_lut_len);
     cudaFree(c->d_partial); cudaFree(c->d_gen_partial);
     cudaFree(c->d_val); cudaFree(c->d_cnt); cudaFree(c->d_G); cudaFree(c->d_tail_state);
+    cudaFree(c->d_g2_rtab); cudaFree(c->d_g2_tw); cudaFree(c->d_g2_ctr); cudaFree(c->d_g2_posacc);
+    c->d_g2_rtab = c->d_g2_tw = nullptr; c->d_g2_ctr = nullptr; c->d_g2_posacc = nullptr;
     c->d_cnt = nullptr; c->d_G = nullptr; c->d_tail_state = nullptr;
     c->d_lut = nullptr; c->d_lut_off = c->d_lut_len = nullptr;
     c->d_partial = nullptr; c->d_gen_partial = nullptr;
@@ -204,9 +213,10 @@ extern "C" int pcal_create(pcal_ctx** out, double f_s_hz, double f_comb_hz, doub
     if (ok) {
         std::vector<double2> W(c->n_bins);
         for (uint32_t k = 0; k < c->n_bins; ++k) W[k] = phasor_neg_host(k, c->n_bins);
-        ok = cudaMemcpy(c->d_W, W.data(), W.size() * sizeof(double2), cudaMemcpyHostToDevice) == cudaSuccess &&
-             cudaMemset(c->d_P, 0, nb * sizeof(double2)) == cudaSuccess &&
-             cudaMemset(c->d_Pint, 0, nb * sizeof(long long)) == cudaSuccess;
+        // (synchronous copy from pageable memory: complete on return.  The accumulators are zeroed lazily, on the
+        //  stream of the first call that needs them: zero_pending.)
+        ok = cudaMemcpy(c->d_W, W.data(), W.size() * sizeof(double2), cudaMemcpyHostToDevice) == cudaSuccess;
+        c->zero_pending = true;
     }
     if (ok && 2 * (size_t)c->n_bins * sizeof(double2) > 48 * 1024)
         ok = cudaFuncSetAttribute(dft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -309,6 +319,33 @@ static int occupancy_of(K kernel, size_t smem) {
 }
 
 static uint32_t dft_ctas(const pcal_ctx* c);
+// N = N1 * N2 for the two-stage DFT of the fused tails: N1 = the largest divisor of N not above sqrt(N)
+static uint32_t dft_n1_of(uint32_t n) {
+    uint32_t best = 1;
+    for (uint32_t d = 1; d * d <= n; ++d) if (n % d == 0) best = d;
+    return best;
+}
+
+// the gen2_kernel instantiation of a context: <channels, SIGN_MAG, chunks per consumer warp>
+typedef void (*gen2_kfn)(const Gen2Params);
+template <int C, int CPW>
+static gen2_kfn gen2_pick_sm(bool sm) { return sm ? gen2_kernel<C, true, CPW> : gen2_kernel<C, false, CPW>; }
+template <int C>
+static gen2_kfn gen2_pick_cpw(uint32_t cpw, bool sm) {
+    return cpw == 1 ? gen2_pick_sm<C, 1>(sm) : (cpw == 2 ? gen2_pick_sm<C, 2>(sm) : gen2_pick_sm<C, 4>(sm));
+}
+static gen2_kfn gen2_kernel_of(const pcal_ctx* c) {
+    const bool sm = c->sign_mag != 0;
+    if (c->C == 1) return gen2_pick_cpw<1>(c->g2_cpw, sm);
+    if (c->C == 2) return gen2_pick_cpw<2>(c->g2_cpw, sm);
+    return gen2_pick_cpw<4>(c->g2_cpw, sm);
+}
+template <int C>
+static size_t gen2_smem_c(uint32_t cpw) { return cpw == 1 ? gen2_smem_bytes<C, 1>() : (cpw == 2 ? gen2_smem_bytes<C, 2>() : gen2_smem_bytes<C, 4>()); }
+static size_t gen2_smem_of(const pcal_ctx* c) {
+    return c->C == 1 ? gen2_smem_c<1>(c->g2_cpw) : (c->C == 2 ? gen2_smem_c<2>(c->g2_cpw) : gen2_smem_c<4>(c->g2_cpw));
+}
+static const void* gen2_fn(const pcal_ctx* c) { return reinterpret_cast<const void*>(gen2_kernel_of(c)); }
 
 static int prepare(pcal_ctx* c) {
     if (c->prepared) return PCAL_OK;
@@ -337,7 +374,26 @@ static int prepare(pcal_ctx* c) {
     }
     const char* gm = getenv("PCAL_GEN_MMA");       // =0: FFMA2 kernel of pcal_gen.cuh for every sample type (A/B runs, tests)
     c->gen_mma = c->C == 1 && c->kind != KIND_F32 && kMmaSpan % c->n_bins == 0 && !(gm && gm[0] == '0');
-    const bool gen_ok = c->C == 1 && (c->gen_mma || (kThreads * c->gen_spt) % c->n_bins == 0);
+    // 2-bit samples, up to 4 channels: pcal_gen2.cuh.  A row is a multiple of lcm(N_bins, time samples per 16 bytes)
+    // time samples and at most 2048 fields.  PCAL_GEN2=0 keeps the older kernels (A/B runs, tests).
+    c->gen2 = false;
+    {
+        const char* g2 = getenv("PCAL_GEN2");
+        if (c->kind == KIND_2BIT && c->C <= (int)kG2MaxCh && !(g2 && g2[0] == '0') && !(gm && gm[0] == '0')) {
+            const uint64_t lam = lcm_sat(c->n_bins, 64u / (uint32_t)c->C, 1u << 20);
+            if (lam * (uint64_t)c->C <= kG2Fields) {
+                // the shortest row with at least 8 chunks (one per consumer warp): few positions, few accumulators
+                const uint32_t lam_chunks = (uint32_t)(lam * (uint64_t)c->C / 64u);
+                const uint32_t m = lam_chunks >= 8u ? 1u : (8u + lam_chunks - 1u) / lam_chunks;
+                c->gen2 = true;
+                c->g2_span_t = (uint32_t)lam * m;
+                c->g2_chunks = lam_chunks * m;
+                c->g2_cpw = c->g2_chunks <= 8u ? 1u : (c->g2_chunks <= 16u ? 2u : 4u);
+                c->g2_rt = 32u * (4u / c->g2_cpw);
+            }
+        }
+    }
+    const bool gen_ok = c->gen2 || (c->C == 1 && (c->gen_mma || (kThreads * c->gen_spt) % c->n_bins == 0));
     int mode;
     if (c->all_zero) mode = PCAL_ROT_LUT;
     else if (c->rot_req == PCAL_ROT_LUT) mode = lut_ok ? PCAL_ROT_LUT : 0;
@@ -376,10 +432,10 @@ static int prepare(pcal_ctx* c) {
             c->tail_tpp = tpp;
             const size_t ns = kTailSlots;
             CU(cudaMalloc(&c->d_cnt, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
-            CU(cudaMemset(c->d_cnt, 0, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
+            CU(cudaMemsetAsync(c->d_cnt, 0, ns * ((size_t)c->q + 1) * sizeof(uint32_t), c->stream));
             CU(cudaMalloc(&c->d_G, ns * (size_t)c->q * pairs * sizeof(double2)));
             CU(cudaMalloc(&c->d_tail_state, sizeof(TailState)));
-            CU(cudaMemset(c->d_tail_state, 0, sizeof(TailState)));
+            CU(cudaMemsetAsync(c->d_tail_state, 0, sizeof(TailState), c->stream));
         }
         c->grid = c->q * c->R;
         c->partial_slot_bytes = (size_t)c->grid * c->F * 32 * elem;
@@ -399,11 +455,41 @@ static int prepare(pcal_ctx* c) {
         CU(cudaMalloc(&c->d_lut, lut.size() * sizeof(double2)));
         CU(cudaMalloc(&c->d_lut_off, c->C * sizeof(uint32_t)));
         CU(cudaMalloc(&c->d_lut_len, c->C * sizeof(uint32_t)));
-        CU(cudaMemcpy(c->d_lut, lut.data(), lut.size() * sizeof(double2), cudaMemcpyHostToDevice));
-        CU(cudaMemcpy(c->d_lut_off, off.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
-        CU(cudaMemcpy(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        CU(cudaMemcpyAsync(c->d_lut, lut.data(), lut.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_lut_off, off.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_lut_len, len.data(), c->C * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
     } else {
         int occ = 0;
+        if (c->gen2) {
+            // tables in long double from exactly reduced phases: stride phasors per row, position factors per time offset
+            const uint32_t C = (uint32_t)c->C, span = c->g2_span_t;
+            std::vector<double2> rtab((size_t)C * kG2TabStride), tw((size_t)C * span);
+            const uint64_t D = (uint64_t)kG2Batch * c->g2_rt * span;       // samples per batch
+            for (uint32_t ch = 0; ch < C; ++ch) {
+                double2* g = rtab.data() + (size_t)ch * kG2TabStride;
+                for (uint32_t r = 0; r < kG2TabRows; ++r) g[r] = phasor_neg_host(mulmod_host((uint64_t)r * span, c->Feff[ch], c->Fs), c->Fs);
+                for (uint32_t k = 0; k < kG2TabLo; ++k) g[kG2TabRows + k] = phasor_neg_host(mulmod_host(D * k % c->Fs, c->Feff[ch], c->Fs), c->Fs);
+                for (uint32_t k = 0; k < kG2TabHi; ++k) g[kG2TabRows + kG2TabLo + k] = phasor_neg_host(mulmod_host(D * 256 * k % c->Fs, c->Feff[ch], c->Fs), c->Fs);
+                for (uint32_t t = 0; t < span; ++t) tw[(size_t)ch * span + t] = phasor_neg_host(mulmod_host(t, c->Feff[ch], c->Fs), c->Fs);
+            }
+            CU(cudaMalloc(&c->d_g2_rtab, rtab.size() * sizeof(double2)));
+            CU(cudaMalloc(&c->d_g2_tw, tw.size() * sizeof(double2)));
+            CU(cudaMalloc(&c->d_g2_ctr, kTailSlots * 2 * sizeof(uint32_t)));
+            CU(cudaMalloc(&c->d_g2_posacc, (size_t)kTailSlots * 2 * kG2Fields * sizeof(long long)));
+            CU(cudaMalloc(&c->d_tail_state, sizeof(TailState)));
+            CU(cudaMemcpyAsync(c->d_g2_rtab, rtab.data(), rtab.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+            CU(cudaMemcpyAsync(c->d_g2_tw, tw.data(), tw.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+            CU(cudaMemsetAsync(c->d_g2_ctr, 0, kTailSlots * 2 * sizeof(uint32_t), c->stream));
+            CU(cudaMemsetAsync(c->d_g2_posacc, 0, (size_t)kTailSlots * 2 * kG2Fields * sizeof(long long), c->stream));
+            CU(cudaMemsetAsync(c->d_tail_state, 0, sizeof(TailState), c->stream));
+            c->gen_smem = gen2_smem_of(c);
+            const void* fn = gen2_fn(c);
+            CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem));
+            CU(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+            c->gen_grid = (uint32_t)c->sm_count;           // half-SM CTAs, one per SM: consecutive launches share the SMs
+            c->prepared = true;
+            return PCAL_OK;
+        }
         if (c->gen_mma && c->kind == KIND_2BIT) { c->gen_smem = gen_mma_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_2BIT, false>, c->gen_smem); }
         else if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8, false>, c->gen_smem); }
         else if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
@@ -507,7 +593,49 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     return PCAL_OK;
 }
 
+static int enqueue_dft(pcal_ctx* c, double2* second_dst);
+static bool can_fuse_dft(const pcal_ctx* c);
+
+// one launch of pcal_gen2.cuh over n time samples starting at data: rows, tail and accumulation in ONE kernel
+static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
+    Gen2Params gp;
+    memset(&gp, 0, sizeof(gp));
+    const uint64_t n_bytes = n * 2ull * c->C / 8;
+    gp.data = data;
+    gp.chunks = c->g2_chunks; gp.row_bytes = c->g2_chunks * 16u; gp.span_t = c->g2_span_t;
+    gp.pitch = gp.row_bytes + ((c->g2_chunks & 1u) ? 0u : 16u);      // an odd number of 16-byte chunks
+    gp.n_rows = n_bytes / gp.row_bytes;
+    gp.n_tiles = (uint32_t)((gp.n_rows + c->g2_rt - 1) / c->g2_rt);
+    gp.n_batches = (gp.n_tiles + kG2Batch - 1) / kG2Batch;
+    gp.n_static = (uint32_t)(3ull * gp.n_batches / (4ull * c->gen_grid));
+    if (const char* ns = getenv("PCAL_G2_NSTATIC")) gp.n_static = (uint32_t)atoi(ns);   // TEMP
+    if (gp.n_static < 1) gp.n_static = 1;
+    gp.Fs = c->Fs;
+    for (int i = 0; i < c->C; ++i) {
+        gp.Foff[i] = c->Feff[i];
+        gp.base0[i] = phasor_neg_host(mulmod_host(c->n_processed % c->Fs, c->Feff[i], c->Fs), c->Fs);
+    }
+    gp.gtab = c->d_g2_rtab; gp.tw = c->d_g2_tw; gp.ctr = c->d_g2_ctr; gp.posacc = c->d_g2_posacc; gp.st = c->d_tail_state;
+    gp.P = c->d_P; gp.tail = data + gp.n_rows * gp.row_bytes;
+    gp.n0 = c->n_processed; gp.n_body = gp.n_rows * c->g2_span_t; gp.n_total = n;
+    gp.n_bins = c->n_bins; gp.n0_mod_bins = (uint32_t)(c->n_processed % c->n_bins);
+    gp.overwrite = c->zero_pending ? 1 : 0; gp.input_ready = c->input_ready ? 1 : 0;
+    if (c->fuse_req) {
+        gp.fuse_dft = 1; gp.dft_n1 = dft_n1_of(c->n_bins); gp.k_shift = (uint32_t)c->k_shift; gp.W = c->d_W;
+        gp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; gp.T_host = c->fuse_out; gp.P_copy = c->fuse_P_copy;
+    }
+    { const char* d = getenv("PCAL_G2_DBG"); gp.dbg = d ? atoi(d) : 0; }
+    prof_mark(c, st);
+    launch_chain(gen2_kernel_of(c), c->gen_grid, kG2Threads, c->gen_smem, st, gp);
+    prof_mark(c, st);
+    c->zero_pending = false;
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
 static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
+    if (c->gen2) return extract_piece_gen2(c, data, n, st);
     const uint32_t spt = c->gen_spt;
     const uint64_t load_bytes = c->kind == KIND_2BIT ? 4 : 16;
     const uint64_t n_bytes = n * (uint64_t)c->bits / 8;
@@ -551,25 +679,23 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     return PCAL_OK;
 }
 
-static int enqueue_dft(pcal_ctx* c, double2* second_dst);
-static bool can_fuse_dft(const pcal_ctx* c);
-
 // PCAL_SMALL_PIECES=1 (tests only): see extract_segment.  Read per call (tests toggle it), but cheaply.
 static bool small_pieces() {
     const char* sp = getenv("PCAL_SMALL_PIECES");
     return sp && sp[0] == '1';
 }
 
-// pieces: bounded per-thread trip count (LUT path) / bounded resync table (generator path)
+// time samples per launch: bounded per-thread trip count (LUT path) / bounded resync table or claims per CTA (generator path).
+// PCAL_SMALL_PIECES=1 (tests only) shrinks the limits so that a few million samples already span several
+// launches; the arithmetic is unchanged.
+static uint64_t piece_samples(const pcal_ctx* c, bool small) {
+    if (c->rot_eff == PCAL_ROT_LUT) return (uint64_t)(small ? 16u : kMaxIterPerLaunch) * c->R * kWarps * c->q * 32ull * c->spv;
+    if (c->gen2) return (uint64_t)(small ? 2 : kG2CapBatches * kG2Batch / 2) * c->gen_grid * c->g2_rt * c->g2_span_t;   // <= half of what the CTAs may claim
+    return (uint64_t)(small ? 2 : kGenMaxTiles) * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
+}
+
 static int extract_segment(pcal_ctx* c, const uint8_t* p, uint64_t n_samples) {
-    // PCAL_SMALL_PIECES=1 (tests only) shrinks both limits so that a few million samples already
-    // span several launches; the arithmetic is unchanged.
-    const bool small = small_pieces();
-    uint64_t piece;
-    if (c->rot_eff == PCAL_ROT_LUT)
-        piece = (uint64_t)(small ? 16u : kMaxIterPerLaunch) * c->R * kWarps * c->q * 32ull * c->spv;
-    else
-        piece = (uint64_t)(small ? 2 : kGenMaxTiles) * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
+    const uint64_t piece = piece_samples(c, small_pieces());
     uint64_t done = 0;
     while (done < n_samples) {
         const uint64_t n = n_samples - done < piece ? n_samples - done : piece;
@@ -589,10 +715,10 @@ extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_sam
     if (!dev_samples) return PCAL_ERR_INVALID;
     if ((uintptr_t)dev_samples & 15u) return PCAL_ERR_ALIGNMENT;
     if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
+    c->stream = (cudaStream_t)cuda_stream;       // prepare() issues its set-up copies on the caller's stream
     const int rc = prepare(c);
     if (rc != PCAL_OK) return rc;
     c->started = true;
-    c->stream = (cudaStream_t)cuda_stream;
     return extract_segment(c, reinterpret_cast<const uint8_t*>(dev_samples), n_samples);
 }
 
@@ -607,15 +733,15 @@ extern "C" int pcal_extract_series(pcal_ctx* c, const void* dev_samples, uint64_
     const uint64_t bits_per_period = n_per_period * (uint64_t)c->bits * c->C;
     if (((uintptr_t)dev_samples & 15u) || bits_per_period % 128) return PCAL_ERR_ALIGNMENT;   // every period 16-byte aligned
     if (dev_out_folded && c->k_shift) return PCAL_ERR_STATE;
+    c->stream = (cudaStream_t)cuda_stream;
     const int rc = prepare(c);
     if (rc != PCAL_OK) return rc;
     c->started = true;
-    c->stream = (cudaStream_t)cuda_stream;
     const size_t nb = (size_t)c->n_bins * c->C;
     const uint8_t* p = reinterpret_cast<const uint8_t*>(dev_samples);
     // Small N_bins on the LUT path: the fold kernel of a period delivers T and the copy of P itself (one launch per
     // period, consecutive periods overlap); otherwise the DFT kernel and a device-to-device copy follow every period.
-    const uint64_t piece = c->rot_eff == PCAL_ROT_LUT ? (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv : 0;
+    const uint64_t piece = piece_samples(c, false);
     const bool fuse = can_fuse_dft(c) && !small_pieces() && n_per_period <= piece && bits_per_period >= 128;
     for (uint32_t k = 0; k < n_periods; ++k) {
         c->zero_pending = true;                       // the period's first post kernel overwrites the bins
@@ -677,6 +803,14 @@ static uint32_t dft_ctas(const pcal_ctx* c) {
 
 // stage C of the fold kernel can take the DFT itself: small N_bins, and C*N_bins complex values fit in its scratch
 static bool can_fuse_dft(const pcal_ctx* c) {
+    if (c->prepared && c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) {
+        // two-stage DFT in the last CTA: cheap enough to sit in the serial final stage, and P and the scratch fit behind the
+        // position sums in the tile ring
+        const uint32_t n1 = dft_n1_of(c->n_bins);
+        const size_t ring = (c->C == 4 ? 4u : 5u) * (size_t)kG2StageBytes;
+        return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) &&
+               ((size_t)c->n_bins * c->C + c->n_bins) * sizeof(double2) + 2 * kG2Fields * sizeof(long long) <= ring;
+    }
     if (!(c->prepared && c->rot_eff == PCAL_ROT_LUT && c->fused) || c->n_bins > 64) return false;
     const uint32_t cap = c->kind == KIND_2BIT ? 1792u : (c->kind == KIND_I8 ? 768u : 256u);   // (scratch doubles - 512) / 2
     return c->n_bins * (uint32_t)c->C <= cap;
@@ -689,7 +823,8 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const uint32_t opw = dft_opw(c), per_cta = kDftThreads / 32 * opw;
     launch_chain(dft_kernel, dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream,
                  (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift, opw,
-                 c->rot_eff == PCAL_ROT_LUT && c->fused ? c->d_tail_state : (TailState*)nullptr, can_fuse_dft(c) ? 1 : 0);
+                 (c->rot_eff == PCAL_ROT_LUT && c->fused) || (c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) ? c->d_tail_state : (TailState*)nullptr,
+                 can_fuse_dft(c) ? 1 : 0);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
@@ -722,12 +857,13 @@ extern "C" int pcal_integrate(pcal_ctx* c, const void* dev_samples, uint64_t n_s
     if (!c || !out) return PCAL_ERR_INVALID;
     int r = pcal_reset(c);
     if (r != PCAL_OK) return r;
+    c->stream = (cudaStream_t)cuda_stream;
     r = prepare(c);
     if (r != PCAL_OK) return r;
     // One launch for the whole period when the fold kernel can deliver T itself: a small DFT, the period is one
     // piece with at least one complete vector, and out is device-visible pinned memory.
     double2* mapped = mapped_of(c, out);
-    const uint64_t piece = (uint64_t)kMaxIterPerLaunch * c->R * kWarps * c->q * 32ull * c->spv;
+    const uint64_t piece = piece_samples(c, false);
     c->fuse_req = mapped && can_fuse_dft(c) && !small_pieces() && n_samples <= piece &&
                   n_samples * (uint64_t)c->bits * c->C / 8 >= 16 && dev_samples;
     c->fuse_out = mapped; c->fuse_T_dev = nullptr; c->fuse_P_copy = nullptr;

@@ -1,0 +1,600 @@
+// pcal_gen2.cuh -- generator path for 2-bit samples (1, 2 or 4 channels per word group): eq. 2.3 + 2.2 with the
+// phasor of eq. 2.5 as a dense contraction over TIME on the tensor cores, one launch per piece.
+//
+// Algebra (as in pcal_gen_mma.cuh, the int8 kernel).  A piece is cut into ROWS of span_t time samples; span_t is a multiple
+// of N_bins and of the samples per 16 bytes, so a field position keeps its bin from row to row.  With
+// n = n0 + span_t R + tau (R = row, tau < span_t),
+//     P_c[b] = sum_{tau = b - n0 mod N_bins} e^{-j w_c tau} * sum_R x_c[R, tau] * rho_c[R],     rho_c[R] = e^{-j w_c (n0 + span_t R)}
+// (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is the matrix
+// product X^T (positions x rows) * R (rows x digit columns): mma.sync m16n8k32 u8 x s8 -> s32 with the phasor quantised
+// to 23-bit fixed point, round(rho 2^22) = d0 + 2^8 d1 + 2^16 d2 (signed 8-bit digits; 3 Re + 3 Im columns).  Every
+// sum is an exact integer; the only approximation is the 2^-23 phasor quantisation (~1e-7 relative per bin).
+// Rows are SHORT (span_t = the smallest admissible multiple with at least 8 sixteen-byte chunks; config 3: 512 samples
+// = N_bins): few positions mean few accumulators (16 registers per thread instead of 64), a small epilogue and a small
+// cross-CTA reduction, at the price of more phasors (one per row).
+//
+// Generator and resync (eq. 2.5-2.8).  rho_c[R] = base0 * hi[B / 256] * lo[B % 256] * row[r] for row r of batch B (a batch
+// = 4 tiles = 512 rows at most, <= 2^18 samples): four table phasors, each evaluated in long double on the host from an
+// exactly reduced INTEGER phase, three coupled-form multiplies (eq. 2.6) deep in fp64.  Nothing is carried from batch to
+// batch or from row to row -- every row restarts from the tables ("fp64 phase resync", BASELINE.json config 5, at every
+// row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-23 quantisation.
+//
+// Structure (profiles/r2_ncu_full.md has the before/after against the round-1 kernel):
+//   * warp roles, no CTA-wide barrier in the loop.  Warp 1 (generator) owns the CTA's tile sequence -- its own batch
+//     first, then batches claimed from a device counter, each claim issued one batch ahead -- and writes the digit
+//     matrices into a ring of entries.  Warp 0 (loader) follows the sequence and copies each tile as it lies in memory
+//     (one cp.async instruction per 512 contiguous bytes) into a ring of padded tiles; completion arrives on the
+//     stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 2..9 (consumers) wait for "full", read their operands
+//     and release stage and digit entry on "empty" barriers.  Nobody waits for anybody else's loads.
+//   * the 4x4 byte transpose (four rows of one position into one register) is done by the load itself:
+//     ldmatrix.m16n16.trans.b8 (SASS LDSM.8.MT1616, new on sm_100) returns exactly the A fragment of m16n8k32, lane
+//     (g, t): byte column g / g + 8 of rows 4t..4t+3 (+16).  The row pitch is an odd number of 16-byte chunks, which keeps
+//     it conflict-free.  No PRMT.
+//   * the four 2-bit fields of a byte are separated by PREFIX masks: U0 = byte, U1 = byte & 0xFC, U2 = & 0xF0,
+//     U3 = & 0xC0 (3 LOP3 instead of 4; single channel), the field sums S_f are differences of the U sums, exact.
+//     With C = 2 / 4 channels field f belongs to channel f mod C and is masked accordingly (digits per channel).
+//   * dynamic tiles: a CTA that starts late simply takes fewer.  A CTA is half an SM (320 threads) and lets its dependent
+//     grid start when half of the batches are claimed: consecutive launches overlap pairwise and HBM keeps streaming
+//     while one of them is in its epilogue.
+//   * the per-position sums of a CTA are exact int64 and are added to the launch's accumulators with integer
+//     red.global.add -- associative, so the result is bit-identical whatever the tile assignment was.  The CTA that
+//     arrives last converts to fp64, applies the position factor, folds positions to bins in a fixed order, adds the
+//     ragged tail and accumulates into the context (same TailState protocol as pcal_tail.cuh; DFT for N_bins <= 64).
+#pragma once
+#include "pcal_gen.cuh"
+#include "pcal_tail.cuh"
+
+namespace pcal {
+
+constexpr int kG2Consumers = 8;                               // consumer warps
+constexpr int kG2Threads = (kG2Consumers + 2) * 32;           // + loader + generator
+constexpr uint32_t kG2StageBytes = 18432;                     // a padded tile: 128 rows x 144 B (8 chunks) ... 32 rows x 528 B (32 chunks)
+constexpr uint32_t kG2Fields = 2048;                          // fields (positions) per row at most
+constexpr uint32_t kG2Batch = 4;                              // tiles per claim
+constexpr uint32_t kG2CapBatches = 256;                       // claims per CTA per launch: <= 1032 tiles keep the int32 digit sums exact
+constexpr uint32_t kG2MaxCh = 4;
+constexpr uint32_t kG2Invalid = 0xFFFFFFFFu;
+constexpr uint32_t kG2TabRows = 512, kG2TabLo = 256, kG2TabHi = 128;      // generator tables per channel: rows of a batch, lo, hi
+constexpr uint32_t kG2TabStride = kG2TabRows + kG2TabLo + kG2TabHi;
+
+// ring depths: sample tiles / digit matrices (the generator runs that far ahead of the consumers)
+template <int C> struct G2Depth { static constexpr int TILES = C == 4 ? 4 : 5, DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4); };
+
+struct Gen2Params {
+    const unsigned char* data;     // [device] packed samples of this piece, 16-byte aligned
+    uint64_t n_rows;               // complete rows in the piece
+    uint32_t n_tiles, n_batches;   // ceil(n_rows / rows per tile), ceil(n_tiles / kG2Batch)
+    uint32_t n_static;             // batches every CTA takes without asking (>= 1): about 3/4 of the launch
+    uint32_t chunks, row_bytes;    // 16-byte chunks per row (8..32), 16 * chunks
+    uint32_t pitch;                // row pitch in shared memory: row_bytes (+16 if chunks is even)
+    uint32_t span_t;               // time samples per row (multiple of N_bins)
+    uint64_t Fs;
+    uint64_t Foff[kG2MaxCh];       // rotator frequency per channel (micro-hertz, k-shift included): ragged tail
+    double2 base0[kG2MaxCh];       // exp(-j w_c n0): phasor of the first sample of the piece (exactly reduced phase, long double on the host)
+    const double2* gtab;           // [device] [C][kG2TabStride] generator tables, each entry from an exactly reduced phase in long double:
+                                   //   [0..511] exp(-j w_c span_t r) rows of a batch; [512..767] exp(-j w_c D k), D = samples per batch;
+                                   //   [768..895] exp(-j w_c 256 D k)
+    const double2* tw;             // [device] [C][span_t] exp(-j w_c tau)
+    uint32_t* ctr;                 // [device] [slot][2]: batch counter, arrival counter; zero between launches
+    long long* posacc;             // [device] [slot][2 * kG2Fields] exact per-position sums (re, im) * 2^22; zero between launches
+    TailState* st;                 // [device] tickets and progress counters of the context
+    // final stage
+    double2* P;                    // [device] folded bins [C][N_bins]
+    const uint8_t* tail;           // [device] first byte after the last complete row
+    uint64_t n0, n_body, n_total;  // absolute index of the first sample; samples in complete rows; samples in the piece
+    uint32_t n_bins, n0_mod_bins;
+    int overwrite, input_ready;
+    int fuse_dft;                  // 1: the last CTA also takes the DFT, two stages N_bins = dft_n1 * N2 (pcal_post.cuh)
+    uint32_t dft_n1;
+    uint32_t k_shift;
+    const double2* W;              // [device] exp(-j 2 pi k / N_bins)
+    double2 *T_dev, *T_host, *P_copy;
+    int dbg;                       // TEMP experiments: 1 = no loads, 2 = no MMAs
+    unsigned long long* stamps;    // TEMP
+};
+
+template <int C, int CPW>
+constexpr size_t gen2_smem_bytes() {
+    return (size_t)G2Depth<C>::TILES * kG2StageBytes + (size_t)G2Depth<C>::DIGITS * C * (4 / CPW) * 256 + 1024;
+}
+
+// ---- mbarrier / cp.async / ldmatrix helpers -----------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "G2_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra G2_DONE;\n"
+        "bra G2_WAIT;\n"
+        "G2_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// the arrival happens when every cp.async this thread issued before has landed; counted in the barrier's init count
+__device__ __forceinline__ void cp_async_arrive_noinc(uint32_t bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 16 bytes global -> shared (SASS LDGSTS.E.BYPASS.128), offsets as immediates where they are compile-time constants
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+template <uint32_t DOFF, uint32_t SOFF>
+__device__ __forceinline__ void cp_async16_imm(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0 + %2], [%1 + %3], 16;" ::"r"(dst), "l"(src), "n"(DOFF), "n"(SOFF) : "memory");
+}
+// warp loads K0..K1-1 of a complete tile: load k covers the 512 contiguous bytes k*512.. of the tile; in shared memory they
+// are DSTEP bytes apart (512 bytes = a whole number of rows for 8, 16 or 32 chunks per row)
+template <uint32_t K0, uint32_t K1, uint32_t DSTEP>
+__device__ __forceinline__ void g2_copy_tile(uint32_t dst, const void* src) {
+    if constexpr (K0 < K1) {
+        cp_async16_imm<K0 * DSTEP, K0 * 512u>(dst, src);
+        g2_copy_tile<K0 + 1, K1, DSTEP>(dst, src);
+    }
+}
+// two 16 x 16 byte matrices, transposed: lanes 0..15 give the rows of the first, 16..31 of the second.  Lane (g, t)
+// receives r0 = byte column g of rows 4t..4t+3, r1 = byte column g + 8, r2 / r3 the same of the second matrix:
+// the A fragment of mma.m16n8k32 with M = byte column and K = row.
+__device__ __forceinline__ void ldsm_t8_x2(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void mma_u8s8_k32(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void red_add_s64(long long* p, long long v) {
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// signed base-256 digits of v (|v| <= 2^22): v = d0 + 256 d1 + 65536 d2
+__device__ __forceinline__ void g2_digits3(int v, int& d0, int& d1, int& d2) {
+    d0 = ((v + 128) & 0xFF) - 128; v = (v - d0) >> 8;
+    d1 = ((v + 128) & 0xFF) - 128; d2 = (v - d1) >> 8;
+}
+
+// prefix / channel masks of the four "combinations" u = 0..3 of a byte and the channel whose digits they meet
+template <int C> __device__ __forceinline__ constexpr uint32_t g2_mask(int u) {
+    return C == 1 ? (u == 0 ? 0xFFFFFFFFu : (u == 1 ? 0xFCFCFCFCu : (u == 2 ? 0xF0F0F0F0u : 0xC0C0C0C0u)))
+         : C == 2 ? (u == 0 ? 0x33333333u : (u == 1 ? 0xCCCCCCCCu : (u == 2 ? 0x30303030u : 0xC0C0C0C0u)))
+                  : (0x03030303u << (2 * u));
+}
+template <int C> __device__ __forceinline__ constexpr int g2_chan(int u) { return C == 1 ? 0 : (C == 2 ? (u & 1) : u); }
+
+#ifdef G2_PROFILE
+#define G2_STAMPL(i) do { if ((threadIdx.x & 31) == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[blockIdx.x * 8 + (i)] = t_; } } while (0)
+#define G2_STAMP(i) do { if (threadIdx.x == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[blockIdx.x * 8 + (i)] = t_; } } while (0)
+#else
+#define G2_STAMP(i) do { } while (0)
+#define G2_STAMPL(i) do { } while (0)
+#endif
+
+// CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
+template <int C, bool SIGN_MAG, int CPW>
+__global__ void __launch_bounds__(kG2Threads + 64, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
+const __grid_constant__ Gen2Params P) {
+    G2_STAMP(0);
+    if (!P.input_ready) pdl_wait();
+    constexpr int KG = 4 / CPW, RT = 32 * KG;                                 // row groups (K = 32 rows each) and rows per tile
+    constexpr int DEPTH = G2Depth<C>::TILES, DIGD = G2Depth<C>::DIGITS;
+    constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;                    // digit matrices of a tile: [C][KG][8 columns][32 rows]
+    extern __shared__ __align__(128) unsigned char g2_smem[];
+    unsigned char* ring = g2_smem;                                            // [DEPTH] padded sample tiles
+    unsigned char* dig = ring + (size_t)DEPTH * kG2StageBytes;                // [DIGD][C][KG][8][32]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(dig + (size_t)DIGD * DIG_BYTES);   // full, empty [DEPTH]; digfull, digempty [DIGD]; ticket
+    uint32_t* dig_tile = reinterpret_cast<uint32_t*>(bars + 2 * DEPTH + 2 * DIGD + 1);   // [DIGD] tile of a digit entry
+    uint32_t* s_gen = dig_tile + DIGD;                                         // [0] sequence number, [1] dft_started seen, [3] arrival, [4], [5] first claims
+    __shared__ long long s_rsum[kG2MaxCh][2];                                  // sum of the quantised phasors of this CTA's valid rows
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t full0 = smem_u32(bars), empty0 = full0 + 8 * DEPTH, dfull0 = empty0 + 8 * DEPTH,
+                   dempty0 = dfull0 + 8 * DIGD, seqbar = dempty0 + 8 * DIGD;
+
+    if (tid == 0) {
+        for (int s = 0; s < DEPTH; ++s) {
+            mbar_init(full0 + 8 * s, 33);                 // 32 cp.async arrivals of the loader + 1 plain arrival (it has seen the digits)
+            mbar_init(empty0 + 8 * s, kG2Consumers);
+        }
+        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, 1); mbar_init(dempty0 + 8 * e, kG2Consumers); }
+        mbar_init(seqbar, 1);
+    }
+    __syncthreads();
+
+    int acc[CPW][4][4];               // [chunk of this warp][combination u][C fragment]
+#pragma unroll
+    for (int c = 0; c < CPW; ++c)
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) acc[c][u][k] = 0;
+
+    if (warp == 1) {
+        // ---------------- generator: owns the CTA's tile sequence; digit matrices of a batch of tiles, lane = row ----------------
+        // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
+        // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
+        // batch number past the end.
+        // Lane l builds rows 4l .. 4l+3 of a tile (row group l / 8, K slots 4 (l % 8) ..): the four digit bytes of a column
+        // are one 32-bit word of the B fragment.  Digit bytes of v: v, (v + 128) >> 8, ((v + 128) >> 8 + 128) >> 8 (low bytes).
+        long long rs_re[C], rs_im[C];
+#pragma unroll
+        for (int c = 0; c < C; ++c) { rs_re[c] = 0; rs_im[c] = 0; }
+        auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
+        auto pack4 = [](int v0, int v1, int v2, int v3) {      // low bytes of four values, v0 in byte 0
+            return __byte_perm(__byte_perm((uint32_t)v0, (uint32_t)v1, 0x0040), __byte_perm((uint32_t)v2, (uint32_t)v3, 0x0040), 0x5410);
+        };
+        const bool g_active = 4 * lane < RT;                   // (KG < 4: the upper lanes have no rows)
+        const uint32_t g_word = (uint32_t)(lane >> 3) * 64u + (uint32_t)(lane & 7);       // word of (row group, column 0, K slots) in a channel's digits
+        for (uint32_t i = lane; i < (uint32_t)DIGD * C * KG * 16u; i += 32u) {              // digit columns 6, 7 are zero for good
+            const uint32_t m = i / 16u, w = i % 16u;
+            reinterpret_cast<uint32_t*>(dig)[m * 64u + 48u + w] = 0u;
+        }
+        __syncwarp();
+        // The CTA's batch sequence: positions 0 .. n_static-1 are its own (index + position * grid: most of the launch,
+        // no round trips), the rest are claims from the launch's counter.  Claims are two positions ahead -- the first two
+        // were made by the ticket thread -- so a claim has two batches' time to come back.
+        uint32_t it = 0, pos = 0;
+        uint32_t batch = blockIdx.x;
+        uint32_t pend[2] = {kG2Invalid, kG2Invalid};           // lane 0: claims in flight for positions pos + 1, pos + 2 (by parity)
+        bool have_seq = false;
+        uint32_t* ctr = nullptr;
+        const uint32_t dyn0 = P.n_static * gridDim.x;          // first claimed batch number
+        auto load_tabs = [&](uint32_t b, double2 (&thi)[C], double2 (&tlo)[C]) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                const double2* tab = P.gtab + (size_t)c * kG2TabStride;
+                thi[c] = __ldg(tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
+                tlo[c] = __ldg(tab + kG2TabRows + (b & 255u));
+            }
+        };
+        double2 thi[C], tlo[C];
+        load_tabs(batch, thi, tlo);
+        while (batch < P.n_batches) {
+            const uint32_t tile0 = batch * kG2Batch;
+            const uint32_t nt = P.n_tiles - tile0 < kG2Batch ? P.n_tiles - tile0 : kG2Batch;
+            double2 base[C];                                    // batch phasor, scaled by 2^22
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                base[c] = cmul(cmul(P.base0[c], thi[c]), tlo[c]);
+                base[c].x *= 4194304.0; base[c].y *= 4194304.0;
+            }
+            // the next batch of the sequence, and its table entries on their way while this batch is built
+            uint32_t nbatch;
+            if (pos + 1 < P.n_static) {
+                nbatch = blockIdx.x + (pos + 1) * gridDim.x;
+            } else {
+                if (!have_seq) {      // (the ticket and its two claims have long arrived by now)
+                    mbar_wait(seqbar, 0u);
+                    ctr = P.ctr + 2 * (s_gen[0] % kTailSlots);
+                    pend[0] = s_gen[4 + ((pos + 1) & 1u)]; pend[1] = s_gen[4 + ((pos + 2) & 1u)];
+                    if (pos + 1 != P.n_static) pend[1] = kG2Invalid;          // (n_static == 0 never happens: host)
+                    have_seq = true;
+                }
+                nbatch = __shfl_sync(0xFFFFFFFFu, pend[0], 0);
+                // a claimed batch is always processed: claiming stops with the first batch number past the end
+                pend[0] = pend[1]; pend[1] = kG2Invalid;
+                if (lane == 0 && nbatch < P.n_batches && pos + 3 - P.n_static < kG2CapBatches) pend[1] = dyn0 + atomicAdd(ctr, 1u);
+            }
+            load_tabs(nbatch, thi, tlo);
+            // UJ tiles at a time: their (independent) phasor chains overlap
+            constexpr uint32_t UJ = C == 1 ? 4u : (C == 2 ? 2u : 1u);
+#pragma unroll 1
+            for (uint32_t j0 = 0; j0 < nt; j0 += UJ) {
+                uint32_t w[UJ][C][6];
+                if (g_active) {
+#pragma unroll
+                    for (uint32_t ju = 0; ju < UJ; ++ju) {
+                        const uint32_t rb = (j0 + ju) * RT + 4u * (uint32_t)lane;             // first of this lane's rows in the batch
+                        const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
+                        const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
+#pragma unroll
+                        for (int c = 0; c < C; ++c) {
+                            int vr[4], vi[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const double2 rho = cmul(base[c], __ldg(P.gtab + (size_t)c * kG2TabStride + (rb + i) % kG2TabRows));
+                                vr[i] = (uint32_t)i < nv ? __double2int_rn(rho.x) : 0;
+                                vi[i] = (uint32_t)i < nv ? __double2int_rn(rho.y) : 0;
+                            }
+                            rs_re[c] += (long long)((vr[0] + vr[1]) + (vr[2] + vr[3]));
+                            rs_im[c] += (long long)((vi[0] + vi[1]) + (vi[2] + vi[3]));
+                            w[ju][c][0] = pack4(vr[0], vr[1], vr[2], vr[3]);
+                            w[ju][c][3] = pack4(vi[0], vi[1], vi[2], vi[3]);
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
+                            w[ju][c][1] = pack4(vr[0], vr[1], vr[2], vr[3]);
+                            w[ju][c][4] = pack4(vi[0], vi[1], vi[2], vi[3]);
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
+                            w[ju][c][2] = pack4(vr[0], vr[1], vr[2], vr[3]);
+                            w[ju][c][5] = pack4(vi[0], vi[1], vi[2], vi[3]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (uint32_t ju = 0; ju < UJ; ++ju) {
+                    const uint32_t j = j0 + ju;
+                    if (j < nt) {
+                        const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
+                        mbar_wait(dempty0 + 8 * e, ph ^ 1u);          // the consumers are done with the entry's previous tile
+                        if (g_active) {
+                            uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES) + g_word;
+#pragma unroll
+                            for (int c = 0; c < C; ++c)
+#pragma unroll
+                                for (int col = 0; col < 6; ++col) dg[c * KG * 64 + col * 8] = w[ju][c][col];
+                        }
+                        if (lane == 0) dig_tile[e] = tile0 + j;
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(dfull0 + 8 * e);
+                    }
+                }
+            }
+            it += nt;
+            batch = nbatch; ++pos;
+        }
+        G2_STAMPL(6);
+        {   // terminator: the entry after the last tile carries "no tile"
+            const uint32_t e = it % DIGD, ph = (it / DIGD) & 1u;
+            mbar_wait(dempty0 + 8 * e, ph ^ 1u);
+            if (lane == 0) { dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
+        }
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+#pragma unroll
+            for (int sh = 16; sh > 0; sh >>= 1) {
+                rs_re[c] += __shfl_xor_sync(0xFFFFFFFFu, rs_re[c], sh);
+                rs_im[c] += __shfl_xor_sync(0xFFFFFFFFu, rs_im[c], sh);
+            }
+            if (lane == 0) { s_rsum[c][0] = rs_re[c]; s_rsum[c][1] = rs_im[c]; }
+        }
+    } else if (warp == 0) {
+        // ---------------- loader: copy each tile as it lies, 512 contiguous bytes per instruction ----------------
+        // The ticket is taken: the next launch may become resident (its CTAs take the slots this launch leaves free or frees).
+        mbar_wait(seqbar, 0u);
+        pdl_release();
+        // this lane's 16 bytes of warp load 0: row and column in the padded tile
+        const uint32_t q0 = ((uint32_t)lane * 16u) / P.row_bytes, col0 = ((uint32_t)lane * 16u) % P.row_bytes;
+        const bool pow2 = P.chunks == 8u * CPW;                              // 8, 16 or 32 chunks: 512 bytes = a whole number of rows
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t e = it % DIGD, phe = (it / DIGD) & 1u;
+            const uint32_t s = it % DEPTH, ph = (it / DEPTH) & 1u;
+            mbar_wait(dfull0 + 8 * e, phe);
+            const uint32_t tile = dig_tile[e];
+            mbar_wait(empty0 + 8 * s, ph ^ 1u);
+            if (tile == kG2Invalid) {
+                cp_async_arrive_noinc(full0 + 8 * s);
+                if (lane == 0) mbar_arrive(full0 + 8 * s);
+                break;
+            }
+            const uint64_t row0 = (uint64_t)tile * RT;
+            const uint32_t rows = P.n_rows - row0 < (uint64_t)RT ? (uint32_t)(P.n_rows - row0) : (uint32_t)RT;
+            const uint32_t stage = smem_u32(ring) + s * kG2StageBytes;
+            const unsigned char* src = P.data + row0 * P.row_bytes + (uint32_t)lane * 16u;
+            if (P.dbg & 1) {
+            } else if (rows == (uint32_t)RT && pow2) {
+                // row_bytes = 128 CPW: a warp load covers 4 / CPW rows
+                g2_copy_tile<0, 32, (4u / CPW) * (128u * CPW + 16u)>(stage + q0 * (128u * CPW + 16u) + col0, src);
+            } else {
+                uint32_t q = q0, col = col0;
+                const uint32_t valid_bytes = rows * P.row_bytes;
+                for (uint32_t o = (uint32_t)lane * 16u; o < valid_bytes; o += 512u) {
+                    cp_async16(stage + q * P.pitch + col, src + (o - (uint32_t)lane * 16u));
+                    col += 512u;
+                    while (col >= P.row_bytes) { col -= P.row_bytes; ++q; }
+                }
+            }
+            cp_async_arrive_noinc(full0 + 8 * s);
+            if (lane == 0) mbar_arrive(full0 + 8 * s);              // (release: what this warp has seen -- the digits -- is visible to whoever sees "full")
+        }
+        G2_STAMPL(7);
+    } else {
+        // ---------------- consumers: warp cw owns chunks CPW cw .. CPW cw + CPW - 1 of every row ----------------
+        const int cw = warp - 2, g = lane >> 2, t = lane & 3;
+        if (warp == 2 && lane == 0) {
+            // ticket: sequence number of this launch, derived on the device (pcal_tail.cuh, "Pipelining"); taken before the
+            // loader lets the dependent grid start.  The slot's previous user (launch seq - kTailSlots) must have finished
+            // before the slot's counters are touched.
+            const uint32_t done = ld_acquire_u32(&P.st->n_done);
+            const uint32_t x = ld_acquire_u32(&P.st->dft_started);
+            const uint32_t sq = (uint32_t)(atomicAdd(&P.st->tick, 1ull) / gridDim.x);
+            s_gen[0] = sq; s_gen[1] = x;
+            if ((int32_t)(done - (sq - kTailSlots + 1u)) < 0)
+                while ((int32_t)(ld_acquire_u32(&P.st->n_done) - (sq - kTailSlots + 1u)) < 0) __nanosleep(64);
+            // the generator's first two claims (positions n_static, n_static + 1 of its sequence; slot by position parity)
+            uint32_t* ctr = P.ctr + 2 * (sq % kTailSlots);
+            const uint32_t d0 = P.n_static * gridDim.x + atomicAdd(ctr, 1u), d1 = P.n_static * gridDim.x + atomicAdd(ctr, 1u);
+            s_gen[4 + (P.n_static & 1u)] = d0; s_gen[4 + ((P.n_static + 1u) & 1u)] = d1;
+            mbar_arrive(seqbar);
+        }
+        __syncwarp();
+        const uint32_t first = (uint32_t)(cw * CPW);
+        const uint32_t my = smem_u32(ring) + (uint32_t)lane * P.pitch + first * 16u;
+        const uint32_t nch = P.chunks > first ? (P.chunks - first < (uint32_t)CPW ? P.chunks - first : (uint32_t)CPW) : 0u;   // this warp's chunks
+        const uint32_t kg_step = 32u * P.pitch;
+        // one chunk of one row group: byte column -> four masked operands -> four MMAs
+        auto chunk_mma = [&](int c, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, const uint32_t (&bf)[C][2]) {
+            if (SIGN_MAG) {
+                a0 = signmag_to_offset_binary(a0); a1 = signmag_to_offset_binary(a1);
+                a2 = signmag_to_offset_binary(a2); a3 = signmag_to_offset_binary(a3);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t m = g2_mask<C>(u);
+                const int ch = g2_chan<C>(u);
+                if (m == 0xFFFFFFFFu) mma_u8s8_k32(acc[c][u], a0, a1, a2, a3, bf[ch][0], bf[ch][1]);
+                else mma_u8s8_k32(acc[c][u], a0 & m, a1 & m, a2 & m, a3 & m, bf[ch][0], bf[ch][1]);
+            }
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t e = it % DIGD;
+            const uint32_t s = it % DEPTH, ph = (it / DEPTH) & 1u;
+            mbar_wait(full0 + 8 * s, ph);
+            const uint32_t tile = dig_tile[e];
+            const uint32_t* dg32 = reinterpret_cast<const uint32_t*>(dig + (size_t)e * DIG_BYTES);
+            uint32_t bf[KG][C][2];
+#pragma unroll
+            for (int kg = 0; kg < KG; ++kg)
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    bf[kg][c][0] = dg32[(c * KG + kg) * 64 + g * 8 + t];
+                    bf[kg][c][1] = dg32[(c * KG + kg) * 64 + g * 8 + 4 + t];
+                }
+            const uint32_t base = my + s * kG2StageBytes;
+            if (nch == (uint32_t)CPW) {
+                // complete rows (the usual case): every operand load of the tile is issued before the first MMA
+                uint32_t a[KG][CPW][4];
+#pragma unroll
+                for (int kg = 0; kg < KG; ++kg)
+#pragma unroll
+                    for (int c = 0; c < CPW; ++c) ldsm_t8_x2(base + kg * kg_step + 16u * c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3]);
+                if (tile == kG2Invalid) break;
+                if (!(P.dbg & 2)) {
+#pragma unroll
+                    for (int kg = 0; kg < KG; ++kg)
+#pragma unroll
+                        for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf[kg]);
+                }
+            } else {
+                if (tile == kG2Invalid) break;
+#pragma unroll
+                for (int kg = 0; kg < KG; ++kg)
+#pragma unroll
+                    for (int c = 0; c < CPW; ++c) {
+                        if ((uint32_t)c < nch) {
+                            uint32_t a0, a1, a2, a3;
+                            ldsm_t8_x2(base + kg * kg_step + 16u * c, a0, a1, a2, a3);
+                            chunk_mma(c, a0, a1, a2, a3, bf[kg]);
+                        }
+                    }
+            }
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(empty0 + 8 * s); mbar_arrive(dempty0 + 8 * e); }
+        }
+    }
+    G2_STAMP(1);
+    __syncthreads();                  // every role is done: the ring becomes the per-position result array
+    G2_STAMP(2);
+    const uint32_t seq = s_gen[0], slot = seq % kTailSlots;
+    uint32_t* ctr = P.ctr + 2 * slot;
+
+    // ---- epilogue: digit sums -> exact per-position int64 (re, im) * 2^22 -> red.add into the launch's accumulators ----
+    long long* pos_s = reinterpret_cast<long long*>(ring);                  // [kG2Fields][2]
+    if (warp >= 2) {
+        const int cw = warp - 2, g = lane >> 2, t = lane & 3;
+#pragma unroll
+        for (int c = 0; c < CPW; ++c) {
+            // field sums from the combination sums (exact: every U is a sum of non-negative multiples of the S)
+            int S[4][4];              // [field f][C fragment], field f scaled by 4^f
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (C == 1) {
+                    S[0][k] = acc[c][0][k] - acc[c][1][k]; S[1][k] = acc[c][1][k] - acc[c][2][k];
+                    S[2][k] = acc[c][2][k] - acc[c][3][k]; S[3][k] = acc[c][3][k];
+                } else if (C == 2) {
+                    S[0][k] = acc[c][0][k] - acc[c][2][k]; S[1][k] = acc[c][1][k] - acc[c][3][k];
+                    S[2][k] = acc[c][2][k]; S[3][k] = acc[c][3][k];
+                } else {
+                    S[0][k] = acc[c][0][k]; S[1][k] = acc[c][1][k]; S[2][k] = acc[c][2][k]; S[3][k] = acc[c][3][k];
+                }
+            }
+#pragma unroll
+            for (int f = 0; f < 4; ++f)
+#pragma unroll
+                for (int hi = 0; hi < 2; ++hi) {
+                    // C fragment: [2 hi], [2 hi + 1] = digit columns 2t, 2t+1 of M row g + 8 hi.  Columns 0..2 = Re digits,
+                    // 3..5 = Im digits: lane t = 0 owns Re (needs column 2 from t = 1), t = 1 owns Im (needs 4, 5 from t = 2).
+                    const int c0 = S[f][2 * hi] >> (2 * f), c1 = S[f][2 * hi + 1] >> (2 * f);
+                    const int x0 = __shfl_down_sync(0xFFFFFFFFu, c0, 1), x1 = __shfl_down_sync(0xFFFFFFFFu, c1, 1);
+                    const long long v = t == 0 ? (long long)c0 + ((long long)c1 << 8) + ((long long)x0 << 16)
+                                               : (long long)c1 + ((long long)x0 << 8) + ((long long)x1 << 16);
+                    if (t < 2) {
+                        const uint32_t bytecol = (uint32_t)(cw * CPW + c) * 16u + (uint32_t)g + 8u * hi;
+                        const uint32_t F = 4u * bytecol + (uint32_t)f;
+                        pos_s[2 * F + t] = 2 * v - 3 * s_rsum[f % C][t];     // codes 0..3 -> levels 2 code - 3
+                    }
+                }
+        }
+    }
+    __syncthreads();
+    const uint32_t nval = 2u * 64u * P.chunks;                              // values of the positions that exist
+    {
+        long long* dst = P.posacc + (size_t)slot * 2 * kG2Fields;
+        for (uint32_t i = tid; i < nval; i += kG2Threads) { const long long v = pos_s[i]; if (v) red_add_s64(dst + i, v); }
+    }
+    G2_STAMP(3);
+    __syncthreads();                  // every thread's reds happen before thread 0's release below
+    if (tid == 0) s_gen[3] = arrive_acq_rel(ctr + 1);
+    __syncthreads();
+    G2_STAMP(4);
+    if (s_gen[3] != gridDim.x - 1u) return;
+
+    // ---- final stage (the CTA that arrived last): positions -> bins, ragged tail, accumulate into the context ----
+    // (first the loads whose latency the rest can hide: the progress counters, the accumulators, the position factors)
+    uint32_t seen_done = 0, seen_dft = 0;
+    if (tid == 0) { seen_done = ld_acquire_u32(&P.st->n_done); seen_dft = ld_acquire_u32(&P.st->dft_finished); }
+    long long* gacc = P.posacc + (size_t)slot * 2 * kG2Fields;
+    for (uint32_t i = tid; i < nval; i += kG2Threads) { pos_s[i] = __ldcg(gacc + i); gacc[i] = 0; }     // and ready for the slot's next launch
+    const uint32_t pairs = (uint32_t)C * P.n_bins, n_tail = (uint32_t)(P.n_total - P.n_body);
+    double2* sP = reinterpret_cast<double2*>(ring + 2 * kG2Fields * sizeof(long long));               // [pairs] (fused DFT)
+    const uint32_t dft_x = s_gen[1];
+    __syncthreads();
+    bool waited = false;
+    auto wait_for_P = [&]() {
+        if (tid == 0) {
+            uint32_t a = seen_done, b = seen_dft;
+            while (a != seq || (int32_t)(b - dft_x) < 0) {
+                __nanosleep(32);
+                a = ld_acquire_u32(&P.st->n_done); b = ld_acquire_u32(&P.st->dft_finished);
+            }
+        }
+        __syncthreads();
+    };
+    for (uint32_t pp0 = 0; pp0 < pairs; pp0 += kG2Threads) {          // uniform trip count
+        const uint32_t pp = pp0 + tid;
+        const bool mine = pp < pairs;
+        const uint32_t c = mine ? pp / P.n_bins : 0u, b = mine ? pp % P.n_bins : 0u;
+        double re = 0.0, im = 0.0;
+        if (mine) {
+            const double2* tw = P.tw + (size_t)c * P.span_t;
+            for (uint32_t tau = (b + P.n_bins - P.n0_mod_bins) % P.n_bins; tau < P.span_t; tau += P.n_bins) {    // in order
+                const uint32_t F = tau * C + c;
+                const double xr = (double)pos_s[2 * F] * (1.0 / 4194304.0), xi = (double)pos_s[2 * F + 1] * (1.0 / 4194304.0);
+                const double2 w = __ldg(tw + tau);
+                re += xr * w.x - xi * w.y;
+                im += xr * w.y + xi * w.x;
+            }
+            if (n_tail) {     // samples n_body .. n_total-1 (less than one row), exactly reduced phases
+                const uint32_t bb0 = (uint32_t)((P.n0 + P.n_body) % P.n_bins);
+                for (uint32_t tt = (b + P.n_bins - bb0) % P.n_bins; tt < n_tail; tt += P.n_bins) {
+                    const double v = decode_tail(KIND_2BIT, SIGN_MAG ? 1 : 0, P.tail, tt, c, C);
+                    const double2 ph = phasor_neg(mulmod_u64(P.Foff[c], P.n0 + P.n_body + tt, P.Fs), P.Fs);
+                    re += v * ph.x; im += v * ph.y;
+                }
+            }
+        }
+        if (!waited) { wait_for_P(); waited = true; }
+        if (!mine) continue;
+        if (!P.overwrite) { const double2 cur = __ldcg(P.P + pp); re += cur.x; im += cur.y; }
+        P.P[pp] = make_double2(re, im);
+        if (P.fuse_dft) sP[pp] = make_double2(re, im);
+        if (P.P_copy) P.P_copy[pp] = make_double2(re, im);
+    }
+    if (P.fuse_dft) {   // T[c] = DFT(P[c]), channel by channel, from shared memory
+        __syncthreads();
+        double2* sY = sP + pairs;
+        for (uint32_t c = 0; c < (uint32_t)C; ++c)
+            dft_in_cta(sP + c * P.n_bins, sY, P.W, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev + c * P.n_bins,
+                       P.T_host ? P.T_host + c * P.n_bins : nullptr, kG2Threads);
+    }
+    if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
+    __syncthreads();
+    if (tid == 0) st_release_u32(&P.st->n_done, seq + 1u);             // P is final for this launch; the slot is free
+    G2_STAMP(5);
+}
+
+}  // namespace pcal
