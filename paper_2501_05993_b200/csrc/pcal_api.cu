@@ -68,6 +68,7 @@ struct pcal_ctx {
     bool gen2;                      // 2-bit samples, <= 4 channels: warp-specialised tensor-core generator kernel (pcal_gen2.cuh)
     uint32_t g2_span_t, g2_chunks;  // ... its row: time samples, 16-byte chunks
     uint32_t g2_cpw, g2_rt;         // ... chunks per consumer warp (1, 2, 4), rows per tile (128, 64, 32)
+    uint32_t g2_blocks;             // ... column blocks of a row (rows longer than 32 chunks are served 32 chunks per launch)
     double2 *d_g2_rtab, *d_g2_tw;   // ... stride phasors [C][32], position factors [C][span_t]
     uint32_t* d_g2_ctr;             // ... [slot][2] batch and arrival counters
     long long* d_g2_posacc;         // ... [slot][2*2048] exact per-position sums
@@ -334,6 +335,8 @@ template <int C>
 static gen2_kfn gen2_pick_cpw(uint32_t cpw, bool sm) {
     return cpw == 1 ? gen2_pick_sm<C, 1>(sm) : (cpw == 2 ? gen2_pick_sm<C, 2>(sm) : gen2_pick_sm<C, 4>(sm));
 }
+// (words of 8 / 16 channels are served four channels -- one byte of the time sample -- per launch)
+static int gen2_ck(const pcal_ctx* c) { return c->C < 4 ? c->C : 4; }
 static gen2_kfn gen2_kernel_of(const pcal_ctx* c) {
     const bool sm = c->sign_mag != 0;
     if (c->C == 1) return gen2_pick_cpw<1>(c->g2_cpw, sm);
@@ -379,15 +382,17 @@ static int prepare(pcal_ctx* c) {
     c->gen2 = false;
     {
         const char* g2 = getenv("PCAL_GEN2");
-        if (c->kind == KIND_2BIT && c->C <= (int)kG2MaxCh && !(g2 && g2[0] == '0') && !(gm && gm[0] == '0')) {
-            const uint64_t lam = lcm_sat(c->n_bins, 64u / (uint32_t)c->C, 1u << 20);
-            if (lam * (uint64_t)c->C <= kG2Fields) {
-                // the shortest row with at least 8 chunks (one per consumer warp): few positions, few accumulators
+        if (c->kind == KIND_2BIT && !(g2 && g2[0] == '0') && !(gm && gm[0] == '0')) {
+            const uint64_t lam = lcm_sat(c->n_bins, 64u / (uint32_t)c->C, 1u << 20);      // <= 4096 * 64 time samples
+            {
+                // the shortest row with at least 8 chunks (one per consumer warp): few positions, few accumulators.  A row of
+                // more than 32 chunks (2048 fields) is served in column blocks of 32 chunks, one launch each.
                 const uint32_t lam_chunks = (uint32_t)(lam * (uint64_t)c->C / 64u);
                 const uint32_t m = lam_chunks >= 8u ? 1u : (8u + lam_chunks - 1u) / lam_chunks;
                 c->gen2 = true;
                 c->g2_span_t = (uint32_t)lam * m;
                 c->g2_chunks = lam_chunks * m;
+                c->g2_blocks = (c->g2_chunks + 31u) / 32u;
                 c->g2_cpw = c->g2_chunks <= 8u ? 1u : (c->g2_chunks <= 16u ? 2u : 4u);
                 c->g2_rt = 32u * (4u / c->g2_cpw);
             }
@@ -596,40 +601,51 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
 static int enqueue_dft(pcal_ctx* c, double2* second_dst);
 static bool can_fuse_dft(const pcal_ctx* c);
 
-// one launch of pcal_gen2.cuh over n time samples starting at data: rows, tail and accumulation in ONE kernel
+// pcal_gen2.cuh over n time samples starting at data: rows, tail and accumulation in ONE kernel (one launch per group of
+// four channels for words of 8 / 16 channels)
 static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
-    Gen2Params gp;
-    memset(&gp, 0, sizeof(gp));
-    const uint64_t n_bytes = n * 2ull * c->C / 8;
-    gp.data = data;
-    gp.chunks = c->g2_chunks; gp.row_bytes = c->g2_chunks * 16u; gp.span_t = c->g2_span_t;
-    gp.pitch = gp.row_bytes + ((c->g2_chunks & 1u) ? 0u : 16u);      // an odd number of 16-byte chunks
-    gp.n_rows = n_bytes / gp.row_bytes;
-    gp.n_tiles = (uint32_t)((gp.n_rows + c->g2_rt - 1) / c->g2_rt);
-    gp.n_batches = (gp.n_tiles + kG2Batch - 1) / kG2Batch;
-    gp.n_static = (uint32_t)(3ull * gp.n_batches / (4ull * c->gen_grid));
-    if (const char* ns = getenv("PCAL_G2_NSTATIC")) gp.n_static = (uint32_t)atoi(ns);   // TEMP
-    if (gp.n_static < 1) gp.n_static = 1;
-    gp.Fs = c->Fs;
-    for (int i = 0; i < c->C; ++i) {
-        gp.Foff[i] = c->Feff[i];
-        gp.base0[i] = phasor_neg_host(mulmod_host(c->n_processed % c->Fs, c->Feff[i], c->Fs), c->Fs);
+    const int ck = gen2_ck(c);
+    const uint32_t n_cls = (uint32_t)c->C / (uint32_t)ck;
+    const bool was_pending = c->zero_pending;
+    for (uint32_t blk = 0; blk < c->g2_blocks; ++blk)
+    for (uint32_t cls = 0; cls < n_cls; ++cls) {
+        Gen2Params gp;
+        memset(&gp, 0, sizeof(gp));
+        const uint64_t n_bytes = n * 2ull * c->C / 8;
+        gp.data = data;
+        gp.chunks = c->g2_chunks - 32u * blk < 32u ? c->g2_chunks - 32u * blk : 32u;
+        gp.row_bytes = gp.chunks * 16u; gp.span_t = c->g2_span_t;
+        gp.row_stride = (uint64_t)c->g2_chunks * 16u; gp.col_off = 512ull * blk;
+        gp.tau0 = 2048u * blk / (uint32_t)c->C; gp.do_tail = blk == 0 ? 1 : 0;
+        gp.pitch = gp.row_bytes + ((gp.chunks & 1u) ? 0u : 16u);      // an odd number of 16-byte chunks
+        gp.cls_count = n_cls; gp.cls = cls; gp.c_real = (uint32_t)c->C; gp.c_base = cls * (uint32_t)ck;
+        gp.n_rows = n_bytes / gp.row_stride;
+        gp.n_tiles = (uint32_t)((gp.n_rows + c->g2_rt - 1) / c->g2_rt);
+        gp.n_batches = (gp.n_tiles + kG2Batch - 1) / kG2Batch;
+        gp.n_static = (uint32_t)(3ull * gp.n_batches / (4ull * c->gen_grid));
+        if (gp.n_static < 1) gp.n_static = 1;
+        gp.Fs = c->Fs;
+        for (int i = 0; i < ck; ++i) {
+            const int ch = (int)gp.c_base + i;
+            gp.Foff[i] = c->Feff[ch];
+            gp.base0[i] = phasor_neg_host(mulmod_host(c->n_processed % c->Fs, c->Feff[ch], c->Fs), c->Fs);
+        }
+        gp.gtab = c->d_g2_rtab + (size_t)gp.c_base * kG2TabStride; gp.tw = c->d_g2_tw + (size_t)gp.c_base * c->g2_span_t;
+        gp.ctr = c->d_g2_ctr; gp.posacc = c->d_g2_posacc; gp.st = c->d_tail_state;
+        gp.P = c->d_P; gp.tail = data + gp.n_rows * gp.row_stride;
+        gp.n0 = c->n_processed; gp.n_body = gp.n_rows * c->g2_span_t; gp.n_total = n;
+        gp.n_bins = c->n_bins; gp.n0_mod_bins = (uint32_t)(c->n_processed % c->n_bins);
+        gp.overwrite = was_pending && blk == 0 ? 1 : 0; gp.input_ready = c->input_ready ? 1 : 0;
+        if (c->fuse_req) {        // (single launch per piece only: can_fuse_dft)
+            gp.fuse_dft = 1; gp.dft_n1 = dft_n1_of(c->n_bins); gp.k_shift = (uint32_t)c->k_shift; gp.W = c->d_W;
+            gp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; gp.T_host = c->fuse_out; gp.P_copy = c->fuse_P_copy;
+        }
+        prof_mark(c, st);
+        launch_chain(gen2_kernel_of(c), c->gen_grid, kG2Threads, c->gen_smem, st, gp);
+        prof_mark(c, st);
+        c->launches += 1;
     }
-    gp.gtab = c->d_g2_rtab; gp.tw = c->d_g2_tw; gp.ctr = c->d_g2_ctr; gp.posacc = c->d_g2_posacc; gp.st = c->d_tail_state;
-    gp.P = c->d_P; gp.tail = data + gp.n_rows * gp.row_bytes;
-    gp.n0 = c->n_processed; gp.n_body = gp.n_rows * c->g2_span_t; gp.n_total = n;
-    gp.n_bins = c->n_bins; gp.n0_mod_bins = (uint32_t)(c->n_processed % c->n_bins);
-    gp.overwrite = c->zero_pending ? 1 : 0; gp.input_ready = c->input_ready ? 1 : 0;
-    if (c->fuse_req) {
-        gp.fuse_dft = 1; gp.dft_n1 = dft_n1_of(c->n_bins); gp.k_shift = (uint32_t)c->k_shift; gp.W = c->d_W;
-        gp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; gp.T_host = c->fuse_out; gp.P_copy = c->fuse_P_copy;
-    }
-    { const char* d = getenv("PCAL_G2_DBG"); gp.dbg = d ? atoi(d) : 0; }
-    prof_mark(c, st);
-    launch_chain(gen2_kernel_of(c), c->gen_grid, kG2Threads, c->gen_smem, st, gp);
-    prof_mark(c, st);
     c->zero_pending = false;
-    c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
 }
@@ -804,6 +820,7 @@ static uint32_t dft_ctas(const pcal_ctx* c) {
 // stage C of the fold kernel can take the DFT itself: small N_bins, and C*N_bins complex values fit in its scratch
 static bool can_fuse_dft(const pcal_ctx* c) {
     if (c->prepared && c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) {
+        if (c->C > 4 || c->g2_blocks > 1) return false;   // several launches per piece
         // two-stage DFT in the last CTA: cheap enough to sit in the serial final stage, and P and the scratch fit behind the
         // position sums in the tile ring
         const uint32_t n1 = dft_n1_of(c->n_bins);

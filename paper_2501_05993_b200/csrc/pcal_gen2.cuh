@@ -7,8 +7,9 @@
 //     P_c[b] = sum_{tau = b - n0 mod N_bins} e^{-j w_c tau} * sum_R x_c[R, tau] * rho_c[R],     rho_c[R] = e^{-j w_c (n0 + span_t R)}
 // (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is the matrix
 // product X^T (positions x rows) * R (rows x digit columns): mma.sync m16n8k32 u8 x s8 -> s32 with the phasor quantised
-// to 23-bit fixed point, round(rho 2^22) = d0 + 2^8 d1 + 2^16 d2 (signed 8-bit digits; 3 Re + 3 Im columns).  Every
-// sum is an exact integer; the only approximation is the 2^-23 phasor quantisation (~1e-7 relative per bin).
+// to 31-bit fixed point, round(rho 2^30) = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 (signed 8-bit digits; 4 Re + 4 Im columns =
+// the n = 8 side of the MMA).  Every sum is an exact integer; the only approximation is the 2^-31 phasor quantisation
+// (~5e-10 of a typical bin).
 // Rows are SHORT (span_t = the smallest admissible multiple with at least 8 sixteen-byte chunks; config 3: 512 samples
 // = N_bins): few positions mean few accumulators (16 registers per thread instead of 64), a small epilogue and a small
 // cross-CTA reduction, at the price of more phasors (one per row).
@@ -17,7 +18,7 @@
 // = 4 tiles = 512 rows at most, <= 2^18 samples): four table phasors, each evaluated in long double on the host from an
 // exactly reduced INTEGER phase, three coupled-form multiplies (eq. 2.6) deep in fp64.  Nothing is carried from batch to
 // batch or from row to row -- every row restarts from the tables ("fp64 phase resync", BASELINE.json config 5, at every
-// row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-23 quantisation.
+// row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-31 quantisation.
 //
 // Structure (profiles/r2_ncu_full.md has the before/after against the round-1 kernel):
 //   * warp roles, no CTA-wide barrier in the loop.  Warp 1 (generator) owns the CTA's tile sequence -- its own batch
@@ -65,9 +66,16 @@ struct Gen2Params {
     uint64_t n_rows;               // complete rows in the piece
     uint32_t n_tiles, n_batches;   // ceil(n_rows / rows per tile), ceil(n_tiles / kG2Batch)
     uint32_t n_static;             // batches every CTA takes without asking (>= 1): about 3/4 of the launch
-    uint32_t chunks, row_bytes;    // 16-byte chunks per row (8..32), 16 * chunks
+    uint32_t chunks, row_bytes;    // 16-byte chunks of a row that this launch serves (<= 32), 16 * chunks
+    uint64_t row_stride, col_off;  // bytes from row to row in memory; first byte of this launch's columns in a row (rows longer than 32
+                                   // chunks are served in column blocks, one launch each; else row_bytes, 0)
+    uint32_t tau0;                 // time offset of the first position of this launch's columns inside a row
+    int do_tail;                   // this launch also adds the ragged tail of the piece
     uint32_t pitch;                // row pitch in shared memory: row_bytes (+16 if chunks is even)
     uint32_t span_t;               // time samples per row (multiple of N_bins)
+    uint32_t cls_count, cls;       // words of 8 / 16 channels: a time sample is cls_count bytes, this launch serves byte `cls` of each
+                                   // (channels 4 cls .. 4 cls + 3; the other bytes' sums are not used); else 1, 0
+    uint32_t c_real, c_base;       // channels in the stream; first channel of this launch
     uint64_t Fs;
     uint64_t Foff[kG2MaxCh];       // rotator frequency per channel (micro-hertz, k-shift included): ragged tail
     double2 base0[kG2MaxCh];       // exp(-j w_c n0): phasor of the first sample of the piece (exactly reduced phase, long double on the host)
@@ -76,7 +84,7 @@ struct Gen2Params {
                                    //   [768..895] exp(-j w_c 256 D k)
     const double2* tw;             // [device] [C][span_t] exp(-j w_c tau)
     uint32_t* ctr;                 // [device] [slot][2]: batch counter, arrival counter; zero between launches
-    long long* posacc;             // [device] [slot][2 * kG2Fields] exact per-position sums (re, im) * 2^22; zero between launches
+    long long* posacc;             // [device] [slot][2 * kG2Fields] exact per-position sums (re, im) * 2^30; zero between launches
     TailState* st;                 // [device] tickets and progress counters of the context
     // final stage
     double2* P;                    // [device] folded bins [C][N_bins]
@@ -89,7 +97,6 @@ struct Gen2Params {
     uint32_t k_shift;
     const double2* W;              // [device] exp(-j 2 pi k / N_bins)
     double2 *T_dev, *T_host, *P_copy;
-    int dbg;                       // TEMP experiments: 1 = no loads, 2 = no MMAs
     unsigned long long* stamps;    // TEMP
 };
 
@@ -153,12 +160,6 @@ __device__ __forceinline__ void mma_u8s8_k32(int (&d)[4], uint32_t a0, uint32_t 
 __device__ __forceinline__ void red_add_s64(long long* p, long long v) {
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-// signed base-256 digits of v (|v| <= 2^22): v = d0 + 256 d1 + 65536 d2
-__device__ __forceinline__ void g2_digits3(int v, int& d0, int& d1, int& d2) {
-    d0 = ((v + 128) & 0xFF) - 128; v = (v - d0) >> 8;
-    d1 = ((v + 128) & 0xFF) - 128; d2 = (v - d1) >> 8;
-}
-
 // prefix / channel masks of the four "combinations" u = 0..3 of a byte and the channel whose digits they meet
 template <int C> __device__ __forceinline__ constexpr uint32_t g2_mask(int u) {
     return C == 1 ? (u == 0 ? 0xFFFFFFFFu : (u == 1 ? 0xFCFCFCFCu : (u == 2 ? 0xF0F0F0F0u : 0xC0C0C0C0u)))
@@ -219,7 +220,8 @@ const __grid_constant__ Gen2Params P) {
         // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
         // batch number past the end.
         // Lane l builds rows 4l .. 4l+3 of a tile (row group l / 8, K slots 4 (l % 8) ..): the four digit bytes of a column
-        // are one 32-bit word of the B fragment.  Digit bytes of v: v, (v + 128) >> 8, ((v + 128) >> 8 + 128) >> 8 (low bytes).
+        // are one 32-bit word of the B fragment.  Digit bytes of v: the low bytes of v, v1 = (v + 128) >> 8, v2 = (v1 + 128) >> 8,
+        // v3 = (v2 + 128) >> 8 (signed base-256 digits; columns 0..3 = Re, 4..7 = Im).
         long long rs_re[C], rs_im[C];
 #pragma unroll
         for (int c = 0; c < C; ++c) { rs_re[c] = 0; rs_im[c] = 0; }
@@ -229,11 +231,6 @@ const __grid_constant__ Gen2Params P) {
         };
         const bool g_active = 4 * lane < RT;                   // (KG < 4: the upper lanes have no rows)
         const uint32_t g_word = (uint32_t)(lane >> 3) * 64u + (uint32_t)(lane & 7);       // word of (row group, column 0, K slots) in a channel's digits
-        for (uint32_t i = lane; i < (uint32_t)DIGD * C * KG * 16u; i += 32u) {              // digit columns 6, 7 are zero for good
-            const uint32_t m = i / 16u, w = i % 16u;
-            reinterpret_cast<uint32_t*>(dig)[m * 64u + 48u + w] = 0u;
-        }
-        __syncwarp();
         // The CTA's batch sequence: positions 0 .. n_static-1 are its own (index + position * grid: most of the launch,
         // no round trips), the rest are claims from the launch's counter.  Claims are two positions ahead -- the first two
         // were made by the ticket thread -- so a claim has two batches' time to come back.
@@ -256,11 +253,11 @@ const __grid_constant__ Gen2Params P) {
         while (batch < P.n_batches) {
             const uint32_t tile0 = batch * kG2Batch;
             const uint32_t nt = P.n_tiles - tile0 < kG2Batch ? P.n_tiles - tile0 : kG2Batch;
-            double2 base[C];                                    // batch phasor, scaled by 2^22
+            double2 base[C];                                    // batch phasor, scaled by 2^30
 #pragma unroll
             for (int c = 0; c < C; ++c) {
                 base[c] = cmul(cmul(P.base0[c], thi[c]), tlo[c]);
-                base[c].x *= 4194304.0; base[c].y *= 4194304.0;
+                base[c].x *= 1073741824.0; base[c].y *= 1073741824.0;
             }
             // the next batch of the sequence, and its table entries on their way while this batch is built
             uint32_t nbatch;
@@ -284,7 +281,7 @@ const __grid_constant__ Gen2Params P) {
             constexpr uint32_t UJ = C == 1 ? 4u : (C == 2 ? 2u : 1u);
 #pragma unroll 1
             for (uint32_t j0 = 0; j0 < nt; j0 += UJ) {
-                uint32_t w[UJ][C][6];
+                uint32_t w[UJ][C][8];
                 if (g_active) {
 #pragma unroll
                     for (uint32_t ju = 0; ju < UJ; ++ju) {
@@ -300,18 +297,15 @@ const __grid_constant__ Gen2Params P) {
                                 vr[i] = (uint32_t)i < nv ? __double2int_rn(rho.x) : 0;
                                 vi[i] = (uint32_t)i < nv ? __double2int_rn(rho.y) : 0;
                             }
-                            rs_re[c] += (long long)((vr[0] + vr[1]) + (vr[2] + vr[3]));
-                            rs_im[c] += (long long)((vi[0] + vi[1]) + (vi[2] + vi[3]));
-                            w[ju][c][0] = pack4(vr[0], vr[1], vr[2], vr[3]);
-                            w[ju][c][3] = pack4(vi[0], vi[1], vi[2], vi[3]);
+                            rs_re[c] += ((long long)vr[0] + vr[1]) + ((long long)vr[2] + vr[3]);
+                            rs_im[c] += ((long long)vi[0] + vi[1]) + ((long long)vi[2] + vi[3]);
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
-                            w[ju][c][1] = pack4(vr[0], vr[1], vr[2], vr[3]);
-                            w[ju][c][4] = pack4(vi[0], vi[1], vi[2], vi[3]);
+                            for (int d = 0; d < 4; ++d) {
+                                w[ju][c][d] = pack4(vr[0], vr[1], vr[2], vr[3]);
+                                w[ju][c][4 + d] = pack4(vi[0], vi[1], vi[2], vi[3]);
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
-                            w[ju][c][2] = pack4(vr[0], vr[1], vr[2], vr[3]);
-                            w[ju][c][5] = pack4(vi[0], vi[1], vi[2], vi[3]);
+                                for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
+                            }
                         }
                     }
                 }
@@ -326,7 +320,7 @@ const __grid_constant__ Gen2Params P) {
 #pragma unroll
                             for (int c = 0; c < C; ++c)
 #pragma unroll
-                                for (int col = 0; col < 6; ++col) dg[c * KG * 64 + col * 8] = w[ju][c][col];
+                                for (int col = 0; col < 8; ++col) dg[c * KG * 64 + col * 8] = w[ju][c][col];
                         }
                         if (lane == 0) dig_tile[e] = tile0 + j;
                         __syncwarp();
@@ -359,7 +353,7 @@ const __grid_constant__ Gen2Params P) {
         pdl_release();
         // this lane's 16 bytes of warp load 0: row and column in the padded tile
         const uint32_t q0 = ((uint32_t)lane * 16u) / P.row_bytes, col0 = ((uint32_t)lane * 16u) % P.row_bytes;
-        const bool pow2 = P.chunks == 8u * CPW;                              // 8, 16 or 32 chunks: 512 bytes = a whole number of rows
+        const bool pow2 = P.chunks == 8u * CPW && P.row_stride == P.row_bytes;  // 8, 16 or 32 chunks, rows contiguous: 512 bytes = whole rows
         for (uint32_t it = 0;; ++it) {
             const uint32_t e = it % DIGD, phe = (it / DIGD) & 1u;
             const uint32_t s = it % DEPTH, ph = (it / DEPTH) & 1u;
@@ -374,16 +368,16 @@ const __grid_constant__ Gen2Params P) {
             const uint64_t row0 = (uint64_t)tile * RT;
             const uint32_t rows = P.n_rows - row0 < (uint64_t)RT ? (uint32_t)(P.n_rows - row0) : (uint32_t)RT;
             const uint32_t stage = smem_u32(ring) + s * kG2StageBytes;
-            const unsigned char* src = P.data + row0 * P.row_bytes + (uint32_t)lane * 16u;
-            if (P.dbg & 1) {
-            } else if (rows == (uint32_t)RT && pow2) {
+            const unsigned char* src = P.data + row0 * P.row_stride + P.col_off + (uint32_t)lane * 16u;
+            if (rows == (uint32_t)RT && pow2) {
                 // row_bytes = 128 CPW: a warp load covers 4 / CPW rows
                 g2_copy_tile<0, 32, (4u / CPW) * (128u * CPW + 16u)>(stage + q0 * (128u * CPW + 16u) + col0, src);
             } else {
                 uint32_t q = q0, col = col0;
                 const uint32_t valid_bytes = rows * P.row_bytes;
+                const unsigned char* rows_src = P.data + row0 * P.row_stride + P.col_off;
                 for (uint32_t o = (uint32_t)lane * 16u; o < valid_bytes; o += 512u) {
-                    cp_async16(stage + q * P.pitch + col, src + (o - (uint32_t)lane * 16u));
+                    cp_async16(stage + q * P.pitch + col, rows_src + (uint64_t)q * P.row_stride + col);
                     col += 512u;
                     while (col >= P.row_bytes) { col -= P.row_bytes; ++q; }
                 }
@@ -453,12 +447,10 @@ const __grid_constant__ Gen2Params P) {
 #pragma unroll
                     for (int c = 0; c < CPW; ++c) ldsm_t8_x2(base + kg * kg_step + 16u * c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3]);
                 if (tile == kG2Invalid) break;
-                if (!(P.dbg & 2)) {
 #pragma unroll
-                    for (int kg = 0; kg < KG; ++kg)
+                for (int kg = 0; kg < KG; ++kg)
 #pragma unroll
-                        for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf[kg]);
-                }
+                    for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf[kg]);
             } else {
                 if (tile == kG2Invalid) break;
 #pragma unroll
@@ -482,7 +474,7 @@ const __grid_constant__ Gen2Params P) {
     const uint32_t seq = s_gen[0], slot = seq % kTailSlots;
     uint32_t* ctr = P.ctr + 2 * slot;
 
-    // ---- epilogue: digit sums -> exact per-position int64 (re, im) * 2^22 -> red.add into the launch's accumulators ----
+    // ---- epilogue: digit sums -> exact per-position int64 (re, im) * 2^30 -> red.add into the launch's accumulators ----
     long long* pos_s = reinterpret_cast<long long*>(ring);                  // [kG2Fields][2]
     if (warp >= 2) {
         const int cw = warp - 2, g = lane >> 2, t = lane & 3;
@@ -506,16 +498,17 @@ const __grid_constant__ Gen2Params P) {
             for (int f = 0; f < 4; ++f)
 #pragma unroll
                 for (int hi = 0; hi < 2; ++hi) {
-                    // C fragment: [2 hi], [2 hi + 1] = digit columns 2t, 2t+1 of M row g + 8 hi.  Columns 0..2 = Re digits,
-                    // 3..5 = Im digits: lane t = 0 owns Re (needs column 2 from t = 1), t = 1 owns Im (needs 4, 5 from t = 2).
+                    // C fragment: [2 hi], [2 hi + 1] = digit columns 2t, 2t+1 of M row g + 8 hi.  Columns 0..3 = Re digits,
+                    // 4..7 = Im digits: lane t = 0 (2) holds the low half of Re (Im), lane t = 1 (3) the high half.
                     const int c0 = S[f][2 * hi] >> (2 * f), c1 = S[f][2 * hi + 1] >> (2 * f);
                     const int x0 = __shfl_down_sync(0xFFFFFFFFu, c0, 1), x1 = __shfl_down_sync(0xFFFFFFFFu, c1, 1);
-                    const long long v = t == 0 ? (long long)c0 + ((long long)c1 << 8) + ((long long)x0 << 16)
-                                               : (long long)c1 + ((long long)x0 << 8) + ((long long)x1 << 16);
-                    if (t < 2) {
+                    const long long v = (long long)c0 + ((long long)c1 << 8) + ((long long)x0 << 16) + ((long long)x1 << 24);
+                    const int ri = t >> 1;                                    // 0: Re, 1: Im (lanes t = 0 and t = 2 own the results)
+                    if (!(t & 1)) {
                         const uint32_t bytecol = (uint32_t)(cw * CPW + c) * 16u + (uint32_t)g + 8u * hi;
                         const uint32_t F = 4u * bytecol + (uint32_t)f;
-                        pos_s[2 * F + t] = 2 * v - 3 * s_rsum[f % C][t];     // codes 0..3 -> levels 2 code - 3
+                        const bool mine = bytecol % P.cls_count == P.cls;       // (8 / 16 channels: the bytes of this launch's channels)
+                        pos_s[2 * F + ri] = mine ? 2 * v - 3 * s_rsum[f % C][ri] : 0;    // codes 0..3 -> levels 2 code - 3
                     }
                 }
         }
@@ -560,18 +553,20 @@ const __grid_constant__ Gen2Params P) {
         const uint32_t c = mine ? pp / P.n_bins : 0u, b = mine ? pp % P.n_bins : 0u;
         double re = 0.0, im = 0.0;
         if (mine) {
-            const double2* tw = P.tw + (size_t)c * P.span_t;
-            for (uint32_t tau = (b + P.n_bins - P.n0_mod_bins) % P.n_bins; tau < P.span_t; tau += P.n_bins) {    // in order
-                const uint32_t F = tau * C + c;
-                const double xr = (double)pos_s[2 * F] * (1.0 / 4194304.0), xi = (double)pos_s[2 * F + 1] * (1.0 / 4194304.0);
+            const double2* tw = P.tw + (size_t)c * P.span_t + P.tau0;
+            const uint32_t n_tau = 64u * P.chunks / ((uint32_t)C * P.cls_count);       // time offsets in this launch's columns
+            // tau0 + tau = b - n0 (mod N_bins), in order
+            for (uint32_t tau = (b + 2u * P.n_bins - P.n0_mod_bins - P.tau0 % P.n_bins) % P.n_bins; tau < n_tau; tau += P.n_bins) {
+                const uint32_t F = (tau * P.cls_count + P.cls) * C + c;
+                const double xr = (double)pos_s[2 * F] * (1.0 / 1073741824.0), xi = (double)pos_s[2 * F + 1] * (1.0 / 1073741824.0);
                 const double2 w = __ldg(tw + tau);
                 re += xr * w.x - xi * w.y;
                 im += xr * w.y + xi * w.x;
             }
-            if (n_tail) {     // samples n_body .. n_total-1 (less than one row), exactly reduced phases
+            if (n_tail && P.do_tail) {     // samples n_body .. n_total-1 (less than one row), exactly reduced phases
                 const uint32_t bb0 = (uint32_t)((P.n0 + P.n_body) % P.n_bins);
                 for (uint32_t tt = (b + P.n_bins - bb0) % P.n_bins; tt < n_tail; tt += P.n_bins) {
-                    const double v = decode_tail(KIND_2BIT, SIGN_MAG ? 1 : 0, P.tail, tt, c, C);
+                    const double v = decode_tail(KIND_2BIT, SIGN_MAG ? 1 : 0, P.tail, tt, P.c_base + c, P.c_real);
                     const double2 ph = phasor_neg(mulmod_u64(P.Foff[c], P.n0 + P.n_body + tt, P.Fs), P.Fs);
                     re += v * ph.x; im += v * ph.y;
                 }
@@ -579,10 +574,11 @@ const __grid_constant__ Gen2Params P) {
         }
         if (!waited) { wait_for_P(); waited = true; }
         if (!mine) continue;
-        if (!P.overwrite) { const double2 cur = __ldcg(P.P + pp); re += cur.x; im += cur.y; }
-        P.P[pp] = make_double2(re, im);
+        const uint32_t po = P.c_base * P.n_bins + pp;             // (c_base + c, b) in the context's arrays
+        if (!P.overwrite) { const double2 cur = __ldcg(P.P + po); re += cur.x; im += cur.y; }
+        P.P[po] = make_double2(re, im);
         if (P.fuse_dft) sP[pp] = make_double2(re, im);
-        if (P.P_copy) P.P_copy[pp] = make_double2(re, im);
+        if (P.P_copy) P.P_copy[po] = make_double2(re, im);
     }
     if (P.fuse_dft) {   // T[c] = DFT(P[c]), channel by channel, from shared memory
         __syncthreads();

@@ -358,28 +358,42 @@ def test_input_ready_promise_changes_nothing(oracle, idx, n, rot):
     assert_close(outs[1][0][0], oracle_tones(oracle, w, host, 0), f"cfg{idx} input_ready")
 
 
+@pytest.mark.parametrize("rot", ["lut", "generator"])
 @pytest.mark.parametrize("C,enc", [(2, 0), (4, 1), (8, 0), (16, 1)])
-def test_every_power_of_two_channel_count(oracle, C, enc):
+def test_every_power_of_two_channel_count(oracle, C, enc, rot):
     """Demultiplexing ("several baseband channels"): one field of 2C bits per time sample, packed
-    LSB-first; channel c in bits 2c..2c+1 of its field.  Random codes, mixed zero / non-zero offsets."""
+    LSB-first; channel c in bits 2c..2c+1 of its field.  Random codes.  Table rotation: mixed zero / non-zero
+    offsets.  Generator rotation: a different offset with an impractical table per channel, one
+    channel left unrotated; two segments, the second one starting in the middle of a row."""
     from paper_2501_05993_b200 import binding
     n = 300_004
     rs = np.random.RandomState(4200 + C)
     codes = rs.randint(0, 4, size=(n, C)).astype(np.uint8)
     flat = codes.reshape(-1, 4)
     packed = (flat[:, 0] | (flat[:, 1] << 2) | (flat[:, 2] << 4) | (flat[:, 3] << 6)).astype(np.uint8)
-    offs = [0.0 if c % 3 == 0 else 10e3 * (1 + c) for c in range(C)]
+    gen = rot == "generator"
+    if gen:
+        offs = [0.0 if c == 1 else 1234.567 + 100321.0123 * c for c in range(C)]
+    else:
+        offs = [0.0 if c % 3 == 0 else 10e3 * (1 + c) for c in range(C)]
     p = binding.Pcal(64e6, 1e6, 0.0, 2, enc, C)
     p.set_channel_offsets(offs)
+    p.set_rotator(binding.ROT_GENERATOR if gen else binding.ROT_LUT)
     dev = torch.from_numpy(packed).cuda()
-    p.extract(dev, n)
+    if gen:
+        cut = 100_032 * 2 * C // 8       # bytes of the first 100 032 time samples (16-byte aligned for every C)
+        p.extract(dev[:cut], 100_032)
+        p.extract(dev[cut:], n - 100_032)
+        assert p.info().rotator_in_effect == binding.ROT_GENERATOR
+    else:
+        p.extract(dev, n)
     T, P = p.finalize(), p.get_folded()
     fmt = oracle.TWO_BIT_SIGN_MAG if enc else oracle.TWO_BIT_OFFSET_BINARY
     for c in range(C):
-        pr, pi = oracle.fold_ld(packed, fmt, C, c, 0, 1, n, 0, 64e6, 1e6, offs[c], tabulated=True)
+        pr, pi = oracle.fold_ld(packed, fmt, C, c, 0, 1, n, 0, 64e6, 1e6, offs[c], tabulated=not gen)
         assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"C={C} ch{c} folded")
         assert_close(T[c], oracle.dft(pr, pi), f"C={C} ch{c} tones")
-        if offs[c] == 0.0:
+        if offs[c] == 0.0 and not gen:
             want = oracle.fold_i64(packed, fmt, C, c, 0, 1, n, 0, 64)
             assert np.array_equal(P[c].real, want.astype(np.float64)) and not P[c].imag.any()
     p.destroy()
@@ -483,6 +497,28 @@ def test_bin_counts_that_are_not_powers_of_two(oracle, f_s, f_comb, f_off, bits,
     p.integrate(dev, n, out)
     torch.cuda.synchronize()
     assert np.abs(out.numpy() - T).max() <= 1e-12 * np.abs(T).max()
+    p.destroy()
+
+
+@pytest.mark.parametrize("f_s,f_comb,f_off,bits,enc,n", [
+    (50e6, 1e6, 1234.567, 2, 0, 1_000_064),    # N_bins = 50: rows of 1600 samples (25 sixteen-byte chunks)
+    (25e6, 1e6, 777.123456, 2, 1, 800_000),    # N_bins = 25 (odd), SIGN_MAG
+    (48e6, 2e6, 30e3 + 0.5, 2, 0, 600_004),    # N_bins = 24: rows of 576 samples (9 chunks)
+    (96e6, 1e6, 250e3 + 1e-3, 2, 0, 900_004),  # N_bins = 96
+    (2048e6, 1e6, 1234.567, 2, 0, 3_000_004),  # N_bins = 2048: the longest row (32 chunks)
+    (1000e6, 1e6, 1234.567, 2, 0, 2_000_004),  # N_bins = 1000: rows of 8000 samples, in column blocks
+])
+def test_generator_bin_counts_that_are_not_powers_of_two(oracle, f_s, f_comb, f_off, bits, enc, n):
+    """The generator path needs an integer N_bins only (eq. 2.2): offsets whose table is impractical."""
+    from paper_2501_05993_b200 import binding
+    w = synth.Workload("odd_bins_gen", 1, f_s, f_comb, [f_off], bits, enc, n, 0.05, 1.0, [5e-9], 4243, rotator="generator")
+    dev = synth.generate(w, DEV)
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev, splits=(300_032,))
+    assert p.info().rotator_in_effect == 2
+    pr, pi = oracle_folded(oracle, w, host, 0, tabulated=False)
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), "folded")
+    assert_close(T[0], oracle.dft(pr, pi), "tones")
     p.destroy()
 
 
