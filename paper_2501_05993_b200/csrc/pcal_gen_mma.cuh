@@ -7,11 +7,11 @@
 // (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is
 // a matrix product  X^T (2048 positions x rows)  *  R (rows x {Re, Im})  -- a contraction over TIME with a
 // two-column right-hand side.  It runs as integer tensor-core MMAs (mma.sync m16n8k16 / m16n8k32, s8|u8 x s8 -> s32):
-// the phasor is quantised to 23-bit fixed point, round(rho 2^22) = d0 + 2^8 d1 + 2^16 d2 with signed 8-bit
-// digits, and the six digit columns (3 for Re, 3 for Im) fill the n = 8 side of the MMA.  All sums are exact
+// the phasor is quantised to 31-bit fixed point, round(rho 2^30) = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 with signed 8-bit
+// digits, and the eight digit columns (4 for Re, 4 for Im) fill the n = 8 side of the MMA.  All sums are exact
 // integers (int32 per digit column; |sum| < 2^31 for the <= 256 tiles a CTA sees per launch), recombined
-// and converted to fp64 once per launch.  The only approximation is the 2^-23 phasor quantisation
-// (relative error of a bin ~1e-7).
+// and converted to fp64 once per launch.  The only approximation is the 2^-31 phasor quantisation
+// (~5e-10 of a typical bin).
 //
 // Generator and resync.  rho[tile,row]: the tile factor comes from the exactly reduced INTEGER phase
 // ((n0 + 2^16 tile) F_off mod F_s, the "fp64 phase resync every 2^16 samples" of BASELINE.json config 5),
@@ -82,10 +82,11 @@ __device__ __forceinline__ void transpose4x4_bytes(uint32_t r0, uint32_t r1, uin
     o[2] = __byte_perm(x01h, x23h, 0x5410); o[3] = __byte_perm(x01h, x23h, 0x7632);
 }
 
-// signed base-256 digits of v (|v| <= 2^22): v = d0 + 256 d1 + 65536 d2
-__device__ __forceinline__ void digits3(int v, int& d0, int& d1, int& d2) {
-    d0 = ((v + 128) & 0xFF) - 128; v = (v - d0) >> 8;
-    d1 = ((v + 128) & 0xFF) - 128; d2 = (v - d1) >> 8;
+// signed base-256 digits of v (|v| <= 2^30): v = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3; only their low bytes are used
+__device__ __forceinline__ void digits4(int v, int& d0, int& d1, int& d2, int& d3) {
+    d0 = v; v = (v + 128) >> 8;
+    d1 = v; v = (v + 128) >> 8;
+    d2 = v; d3 = (v + 128) >> 8;
 }
 
 template <int LB>
@@ -197,14 +198,14 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         {
             const double2 b0 = base[i], r = rtab[lane];
             const bool valid = (long long)lane < rows_left;
-            const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
-            const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
-            int d0, d1, d2, e0, e1, e2;
-            digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
+            const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 1073741824.0) : 0;
+            const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 1073741824.0) : 0;
+            int d0, d1, d2, d3, e0, e1, e2, e3;
+            digits4(vre, d0, d1, d2, d3); digits4(vim, e0, e1, e2, e3);
             __syncwarp();             // every lane is done with the previous tile's digits
             bt[0 * 32 + lane] = (unsigned char)d0; bt[1 * 32 + lane] = (unsigned char)d1; bt[2 * 32 + lane] = (unsigned char)d2;
-            bt[3 * 32 + lane] = (unsigned char)e0; bt[4 * 32 + lane] = (unsigned char)e1; bt[5 * 32 + lane] = (unsigned char)e2;
-            bt[6 * 32 + lane] = 0; bt[7 * 32 + lane] = 0;
+            bt[3 * 32 + lane] = (unsigned char)d3; bt[4 * 32 + lane] = (unsigned char)e0; bt[5 * 32 + lane] = (unsigned char)e1;
+            bt[6 * 32 + lane] = (unsigned char)e2; bt[7 * 32 + lane] = (unsigned char)e3;
             if (KIND == KIND_2BIT) { s_re += vre; s_im += vim; }      // this lane's rows; summed over the warp at the end
             __syncwarp();
         }
@@ -285,15 +286,15 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         const long long rows_left = (long long)n_rows - ((long long)blockIdx.x + (long long)ti * gridDim.x) * kMmaRows;
         const double2 b0 = base[ti], r = rtab[lane];
         const bool valid = (long long)lane < rows_left;
-        const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 4194304.0) : 0;
-        const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 4194304.0) : 0;
-        int d0, d1, d2, e0, e1, e2;
-        digits3(vre, d0, d1, d2); digits3(vim, e0, e1, e2);
+        const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 1073741824.0) : 0;
+        const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 1073741824.0) : 0;
+        int d0, d1, d2, d3, e0, e1, e2, e3;
+        digits4(vre, d0, d1, d2, d3); digits4(vim, e0, e1, e2, e3);
         const int ks = (lane & 16) + 4 * (lane & 3) + ((lane >> 2) & 3);      // row 16h + t + 4j -> slot 16h + 4t + j
         unsigned char* b = bt_all + (ti & 1u) * 256u;
         b[0 * 32 + ks] = (unsigned char)d0; b[1 * 32 + ks] = (unsigned char)d1; b[2 * 32 + ks] = (unsigned char)d2;
-        b[3 * 32 + ks] = (unsigned char)e0; b[4 * 32 + ks] = (unsigned char)e1; b[5 * 32 + ks] = (unsigned char)e2;
-        b[6 * 32 + ks] = 0; b[7 * 32 + ks] = 0;
+        b[3 * 32 + ks] = (unsigned char)d3; b[4 * 32 + ks] = (unsigned char)e0; b[5 * 32 + ks] = (unsigned char)e1;
+        b[6 * 32 + ks] = (unsigned char)e2; b[7 * 32 + ks] = (unsigned char)e3;
         s_re += vre; s_im += vim;
     };
     if (warp == 0) build_digits(0);
@@ -367,12 +368,13 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         for (int m = 0; m < 8; ++m) {
             const int idx = 4 * m + t;                      // ((c*2 + w2)*4 + b)*2 + half
             const int half = idx & 1, e0 = (idx >> 1) * 4 + 2 * half;      // elements e0, e0+1 = C-fragment columns 2t', 2t'+1
-            // digit columns: lane 0 holds (Re0, Re1), lane 1 (Re2, Im0), lane 2 (Im1, Im2)
+            // digit columns: lane 0 holds (Re0, Re1), lane 1 (Re2, Re3), lane 2 (Im0, Im1), lane 3 (Im2, Im3)
             const long long r0 = dump[e0 * kThreads + qb], r1 = dump[(e0 + 1) * kThreads + qb];
-            const long long r2 = dump[e0 * kThreads + qb + 1], i0 = dump[(e0 + 1) * kThreads + qb + 1];
-            const long long i1 = dump[e0 * kThreads + qb + 2], i2 = dump[(e0 + 1) * kThreads + qb + 2];
-            fre[m] = r0 + 256 * r1 + 65536 * r2;
-            fim[m] = i0 + 256 * i1 + 65536 * i2;
+            const long long r2 = dump[e0 * kThreads + qb + 1], r3 = dump[(e0 + 1) * kThreads + qb + 1];
+            const long long i0 = dump[e0 * kThreads + qb + 2], i1 = dump[(e0 + 1) * kThreads + qb + 2];
+            const long long i2 = dump[e0 * kThreads + qb + 3], i3 = dump[(e0 + 1) * kThreads + qb + 3];
+            fre[m] = r0 + 256 * r1 + 65536 * r2 + 16777216 * r3;
+            fim[m] = i0 + 256 * i1 + 65536 * i2 + 16777216 * i3;
         }
     }
     __syncthreads();                                        // the dump has been read: the result array may overwrite it
@@ -385,8 +387,8 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
         else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8 bytes
         long long pre = fre[m], pim = fim[m];
         if (KIND == KIND_2BIT) { pre = 2 * (pre >> (2 * wsel)) - 3 * s_re; pim = 2 * (pim >> (2 * wsel)) - 3 * s_im; }   // undo 4^field
-        pos_re[pos] = (double)pre * (1.0 / 4194304.0);
-        pos_im[pos] = (double)pim * (1.0 / 4194304.0);
+        pos_re[pos] = (double)pre * (1.0 / 1073741824.0);
+        pos_im[pos] = (double)pim * (1.0 / 1073741824.0);
     }
     __syncthreads();
     {   // exp(-j w pos), pos = tid + 256 k = 16 a + b: product of two exactly reduced table phasors (built in the prologue)

@@ -63,18 +63,29 @@ def gpu_run(w, dev_buf, splits=(), k_shift=0, rotator=None, start=0):
     return p, T, P
 
 
-def assert_close(got, want, what="", floor_frac=0.0):
-    """north_star's bar, per output.  ``floor_frac`` > 0 (short integrations only, where a noise bin
-    can fall near zero by chance and its relative error is ill-conditioned) measures the error of
-    such a bin against floor_frac * median |want| instead of its own magnitude."""
+SMALL_BIN = 1e-3    # DESIGN.md reading R28: a bin below SMALL_BIN * median |bin| is "small"
+
+
+def assert_close(got, want, what="", max_small=0):
+    """north_star's bar for every output: |got - want| <= 1e-5 |want| and phase within 1e-5 rad.
+
+    DESIGN.md reading R28 (the only relaxation, and only where a test passes ``max_small`` > 0): an output whose
+    magnitude is below SMALL_BIN * median |want| -- a bin of a short integration in which signal and noise cancel --
+    has no meaningful relative error.  At most ``max_small`` outputs may be that small (asserted); for those the
+    ABSOLUTE error must stay within 1e-5 * SMALL_BIN * median |want| (i.e. 1e-8 of a typical output), and their phase
+    within the bound that this absolute error implies, 1e-5 * SMALL_BIN * median / |want| rad.
+    Returns (largest relative error of the regular outputs, largest error / largest |want|)."""
     got = np.asarray(got)
     want = np.asarray(want)
     err = np.abs(got - want)
-    rel = err / np.maximum(np.maximum(np.abs(want), floor_frac * np.median(np.abs(want))), 1e-300)
+    mag = np.abs(want)
+    floor = SMALL_BIN * np.median(mag)
+    small = mag < floor if max_small else np.zeros(mag.shape, bool)
+    assert int(small.sum()) <= max_small, f"{what}: {int(small.sum())} outputs below {SMALL_BIN:g} x median (allowed {max_small})"
+    rel = err / np.maximum(np.where(small, floor, mag), 1e-300)
     worst = int(np.argmax(rel))
     assert rel.max() <= REL_TOL, f"{what}: rel err {rel.max():.3e} at {worst} (|want|={abs(want.flat[worst]):.3e})"
-    dphi = np.angle(got * np.conj(want))
-    if floor_frac:
-        dphi = dphi[np.abs(want) >= floor_frac * np.median(np.abs(want))]
-    assert np.abs(dphi).max() <= PHASE_TOL, f"{what}: phase err {np.abs(dphi).max():.3e} rad"
-    return float(rel.max()), float(err.max() / np.abs(want).max())
+    dphi = np.abs(np.angle(got * np.conj(want)))
+    bound = np.where(small, PHASE_TOL * floor / np.maximum(mag, 1e-300), PHASE_TOL)
+    assert np.all(dphi <= bound), f"{what}: phase err {dphi.max():.3e} rad"
+    return float(rel[~small].max() if (~small).any() else 0.0), float(err.max() / mag.max())

@@ -122,23 +122,24 @@ def test_integrate_is_reset_extract_finalize(oracle, idx, n, k_shift):
 @pytest.mark.parametrize("idx,n,enc", [(5, 1_300_003, None), (7, 700_001, None), (2, 900_004, 0), (2, 900_004, 1), (3, 2_000_004, 0),
                                        (5, 2047, None), (5, 2048 * 33 + 5, None), (2, 8192 * 3 + 64, 0)])
 def test_both_generator_kernels(oracle, idx, n, enc, monkeypatch):
-    """Integer samples with N_bins | 2048 run the tensor-core generator kernel (pcal_gen_mma.cuh: integer MMAs over
-    23-bit fixed-point phasor digits); PCAL_GEN_MMA=0 selects the FFMA2 kernel of pcal_gen.cuh (the path of float32
-    input).  Both must match the oracle; lengths around one 2048-sample row and one 2^16-sample tile included."""
+    """Integer samples run the tensor-core generator kernels (pcal_gen2.cuh for 2-bit, pcal_gen_mma.cuh for int8: integer
+    MMAs over 31-bit fixed-point phasor digits); PCAL_GEN_MMA=0 selects the FFMA2 kernel of pcal_gen.cuh (the path of
+    float32 input).  Both must match the oracle; lengths around one row and one 2^16-sample tile included."""
     w, dev, host = make(idx, n)
     if idx == 7:
         w = synth.replace(w, f_offset_hz=[1234.567])
     if enc is not None:
         w = synth.replace(w, encoding=enc)
     want = oracle_tones(oracle, w, host, 0)
-    floor = 0.05 if n < 100_000 else 0.0          # very short integrations: see test_series_gpu.py
     p1, T1, _ = gpu_run(w, dev, rotator="generator")
     assert p1.info().rotator_in_effect == 2
-    assert_close(T1[0], want, f"mma generator cfg{idx}", floor_frac=floor)
+    assert_close(T1[0], want, f"mma generator cfg{idx}")
     monkeypatch.setenv("PCAL_GEN_MMA", "0")
     p2, T2, _ = gpu_run(w, dev, rotator="generator")
     monkeypatch.delenv("PCAL_GEN_MMA")
-    assert_close(T2[0], want, f"ffma2 generator cfg{idx}", floor_frac=floor)
+    # (the FFMA2 kernel multiplies in fp32: ~1e-7 of a typical tone, which a tone of a very short integration
+    #  that happens to be small cannot meet per bin -- reading R28)
+    assert_close(T2[0], want, f"ffma2 generator cfg{idx}", max_small=1 if n < 100_000 else 0)
     assert np.abs(T1 - T2).max() <= 2e-6 * np.abs(want).max()
 
 
@@ -214,7 +215,14 @@ def test_tiny_and_ragged_lengths(oracle, idx, n):
     for c in range(w.n_channels):
         pr, pi = oracle_folded(oracle, w, host, c)
         want = pr.astype(np.float64) + 1j * pi.astype(np.float64)
-        assert np.abs(P[c] - want).max() <= 1e-9 * max(1.0, np.abs(want).max()), (idx, n, c)
+        empty = want == 0                                    # bins no sample fell into: exactly zero on both sides
+        assert not P[c][empty].any(), (idx, n, c)
+        if (~empty).any():
+            assert_close(P[c][~empty], want[~empty], f"cfg{idx} n={n} ch{c} folded")
+        wt = oracle.dft(pr, pi)
+        assert np.abs(T[c] - wt).max() <= 1e-5 * np.abs(wt).max() * 1e-3 + 1e-300, (idx, n, c)     # every tone to 1e-8 of the largest ...
+        big = np.abs(wt) >= 1e-3 * np.abs(wt).max()
+        assert_close(T[c][big], wt[big], f"cfg{idx} n={n} ch{c} tones")                              # ... and per tone where it is not a cancellation
 
 
 def test_impulse_and_reset(oracle):

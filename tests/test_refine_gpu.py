@@ -32,9 +32,21 @@ def test_residual_rotation_kernel_matches_oracle_estimator(oracle, idx, n_per, M
     T = torch.empty((M, 1, w.n_bins), dtype=torch.complex128, device="cuda")
     p.extract_series(dev, n_per, M, T)
     got = p.residual_rotation(T, M)[0]
+    # (a) the kernel's arithmetic: the oracle's estimator on the very same numbers
     want = orefine.residual_rotation(T.cpu().numpy()[:, 0, :], zero_offset=(w.f_offset_hz[0] == 0.0))
     assert abs(got[0] - want[0]) <= 1e-10
     assert abs(got[1] - want[1]) <= 1e-11 * want[1] and abs(got[2] - want[2]) <= 1e-11 * want[2]
+    # (b) end to end, nothing from the GPU on the oracle's side: the oracle's estimator on the ORACLE's series of the
+    # same bytes.  Every tone of the GPU series is within 1e-5 of the oracle's, hence arg S within 1e-5 rad.
+    host = dev.cpu().numpy().reshape(-1).view(np.uint8)
+    bytes_per = n_per * w.bits // 8
+    series = np.empty((M, w.n_bins), np.complex128)
+    for m in range(M):
+        series[m] = oracle.extract(host[m * bytes_per:(m + 1) * bytes_per], oracle_fmt(oracle, w), 1, 0, n_per, m * n_per,
+                                   w.f_s_hz, w.f_comb_hz, w.f_offset_hz[0])
+    indep = orefine.residual_rotation(series, zero_offset=(w.f_offset_hz[0] == 0.0))
+    assert abs(got[0] - indep[0]) <= 1e-5
+    assert abs(got[1] - indep[1]) <= 1e-5 * indep[1] and abs(got[2] - indep[2]) <= 1e-5 * indep[2]
     t_int = n_per / w.f_s_hz
     # closed form, to the noise of the short integrations (config 5: comb amplitude 1 under sigma = 20 noise)
     assert abs(got[0] - 2 * math.pi * delta * t_int) < (0.15 if idx == 5 else 0.02)
