@@ -245,14 +245,6 @@ int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
  * (e.g. the output of an NCCL all-gather of every rank's bins).  Replaces the previous contents. */
 int pcal_set_folded_sum_dev(pcal_ctx *ctx, const double *dev_parts, uint32_t n_parts);
 
-/* Timing hook for the roofline report: when enabled, every launch of the hot kernel (the fused
- * load/decode/fold kernel of the LUT path or the generator kernel) is bracketed by CUDA events on
- * the launching stream.  pcal_get_profile synchronises the stream and returns the summed event time
- * in milliseconds and the number of hot-kernel launches since profiling was enabled (or since the
- * last pcal_get_profile). */
-int pcal_set_profiling(pcal_ctx *ctx, int enable);
-int pcal_get_profile(pcal_ctx *ctx, double *hot_kernel_ms, uint64_t *hot_kernel_launches);
-
 /*
  * Accuracy of the sinewave generators over many cycles (eq. 2.6/2.7, PAPER.md:142-153
  * direct method, PAPER.md:97 k-shift; R26).  One device thread per case runs the
@@ -271,19 +263,6 @@ typedef struct pcal_gen_case_t {
 } pcal_gen_case_t;
 int pcal_generator_study(const pcal_gen_case_t *cases, uint32_t n_cases, uint64_t n_steps, uint32_t n_chk,
                          double *out_err);
-
-/* Calibration for the roofline report: enqueue a pure streaming read (no decode, no fold) of
- * n_bytes from dev ([device], 16-byte aligned) on cuda_stream, with the load instruction, block
- * size and pipelining of the fold kernels; consecutive probes may overlap (programmatic dependent
- * launch), like consecutive fold kernels.  Asynchronous; computes nothing; the caller times it.
- * What it reaches on a given size is the practical ceiling of a read-once kernel of that size. */
-int pcal_read_probe(pcal_ctx *ctx, const void *dev, uint64_t n_bytes, void *cuda_stream);
-
-/* Calibration for the roofline report: the measured issue rate of one pipe of the current device.
- * kind 0 = FFMA (fp32 FMA pipe), 1 = LOP3 (integer/logic pipe), 2 = IMMA m16n8k16 s8 (the legacy tensor path of the
- * generator kernel).  out_per_s [host]: thread-instructions per second (kind 0, 1) or warp-level MMA instructions per
- * second (kind 2) with every SM busy.  Synchronous, default stream, no context needed. */
-int pcal_pipe_probe(int kind, double *out_per_s);
 
 /* Zero accumulators, sample index <- 0 (on the context's stream); parameters are kept. */
 int pcal_reset(pcal_ctx *ctx);

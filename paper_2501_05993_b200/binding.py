@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpcal.so")
 _SRC_DIR = os.path.join(_HERE, "csrc")
-_INCLUDE = os.path.join(os.path.dirname(_HERE), "include", "pcal.h")
+_INCLUDE_DIR = os.path.join(os.path.dirname(_HERE), "include")
 
 PCAL_OK = 0
 ENC_OFFSET_BINARY, ENC_SIGN_MAG, ENC_TWOS_COMPLEMENT, ENC_IEEE_FLOAT = 0, 1, 2, 3
@@ -43,7 +43,8 @@ class InfoT(ctypes.Structure):
 
 
 def _sources():
-    return sorted(os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)) + [_INCLUDE]
+    return sorted(os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)) + \
+        sorted(os.path.join(_INCLUDE_DIR, f) for f in os.listdir(_INCLUDE_DIR))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -53,7 +54,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB_PATH, os.path.join(_SRC_DIR, "pcal_api.cu")]
+              ["-o", LIB_PATH, os.path.join(_SRC_DIR, "pcal_api.cu"), os.path.join(_SRC_DIR, "pcal_probe.cu")]
         subprocess.check_call(cmd)
     return LIB_PATH
 

@@ -87,58 +87,3 @@ __device__ __forceinline__ double2 phasor_neg(uint64_t k, uint64_t m) {
 }
 
 }  // namespace pcal
-
-// ---- calibration: a pure streaming read of `n_vec` 16-byte vectors (no decode, no fold) --------
-// Same load instruction, block size and software pipelining as the fold kernels; what it reaches
-// on a given buffer size is the practical ceiling for any read-once kernel of that size
-// (bench.py reports it beside the roofline fraction).  The xor of all words lands in out[0] only
-// if it equals a magic value, so the loads cannot be optimised away.
-namespace pcal {
-__global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __restrict__ d, uint64_t n_vec, uint32_t* out) {
-    pdl_release();
-    const uint64_t stride = (uint64_t)gridDim.x * kThreads;
-    uint64_t i = (uint64_t)blockIdx.x * kThreads + threadIdx.x;
-    uint32_t acc = 0;
-    uint4 v[4], w[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) { const uint64_t a = i + u * stride; v[u] = a < n_vec ? ldg_stream(d + a) : make_uint4(0, 0, 0, 0); }
-    for (i += 4 * stride; i < n_vec + 4 * stride; i += 4 * stride) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { const uint64_t a = i + u * stride; w[u] = a < n_vec ? ldg_stream(d + a) : make_uint4(0, 0, 0, 0); }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) v[u] = w[u];
-    }
-    if (acc == 0x5ca1ab1eu) out[0] = acc;
-}
-
-// ---- calibration: issue-rate ceilings of the pipes the kernels lean on ----------------
-// kind 0: FFMA (fp32 FMA pipe), 1: LOP3 (integer/logic pipe), 2: IMMA m16n8k16 s8 (legacy tensor path used by
-// gen_mma_kernel).  Eight independent dependency chains per thread, `iters` trips; the result is written so that
-// nothing is optimised away.  The host times the launch and reports instructions per second.
-template <int KIND_P>
-__global__ void __launch_bounds__(kThreads) pipe_probe_kernel(uint32_t iters, uint32_t* out) {
-    uint32_t a[8];
-    float f[8];
-    int d[8][4];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) { a[j] = threadIdx.x * 2654435761u + j; f[j] = 1.0f + j; d[j][0] = d[j][1] = d[j][2] = d[j][3] = 0; }
-    const float m = 1.0000001f, q = 1e-9f;
-    const uint32_t x = blockIdx.x | 0x01010101u, y = threadIdx.x * 0x01010101u;
-    for (uint32_t i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            if (KIND_P == 0) f[j] = __fmaf_rn(f[j], m, q);
-            else if (KIND_P == 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[j]) : "r"(x), "r"(y));
-            else asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
-                              : "+r"(d[j][0]), "+r"(d[j][1]), "+r"(d[j][2]), "+r"(d[j][3]) : "r"(x), "r"(y), "r"(a[j]));
-        }
-    }
-    uint32_t s = 0;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) s += a[j] + __float_as_uint(f[j]) + (uint32_t)(d[j][0] + d[j][1] + d[j][2] + d[j][3]);
-    if (s == 0x5ca1ab1eu) out[0] = s;
-}
-
-}  // namespace pcal
