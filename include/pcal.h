@@ -245,6 +245,14 @@ int pcal_add_folded_dev(pcal_ctx *ctx, const double *dev_bins);
  * (e.g. the output of an NCCL all-gather of every rank's bins).  Replaces the previous contents. */
 int pcal_set_folded_sum_dev(pcal_ctx *ctx, const double *dev_parts, uint32_t n_parts);
 
+/* The same for a time series of integrations with ONE exchange for all its periods: every rank folded
+ * its time shard of each of n_periods periods and the bins were gathered into dev_parts = [device]
+ * [n_parts][n_periods][n_channels][N_bins] complex128.  dev_out_folded [device] [n_periods][n_channels][N_bins] receives the
+ * rank-order sums (P of every period), dev_out_tones [device] (same shape) their DFT (layout of pcal_finalize per
+ * period).  Asynchronous on the context's stream; the context's own accumulators are not touched. */
+int pcal_finalize_series_sum_dev(pcal_ctx *ctx, const double *dev_parts, uint32_t n_parts, uint32_t n_periods,
+                                 double *dev_out_folded, double *dev_out_tones);
+
 /*
  * Accuracy of the sinewave generators over many cycles (eq. 2.6/2.7, PAPER.md:142-153
  * direct method, PAPER.md:97 k-shift; R26).  One device thread per case runs the

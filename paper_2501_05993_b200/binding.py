@@ -81,6 +81,7 @@ def lib():
             "pcal_extract_host": (i32, [vp, vp, u64, vp]),
             "pcal_read_probe": (i32, [vp, vp, u64, vp]),
             "pcal_set_folded_sum_dev": (i32, [vp, vp, ctypes.c_uint32]),
+            "pcal_finalize_series_sum_dev": (i32, [vp, vp, ctypes.c_uint32, ctypes.c_uint32, vp, vp]),
             "pcal_generator_study": (i32, [vp, ctypes.c_uint32, u64, ctypes.c_uint32, vp]),
             "pcal_extract_series": (i32, [vp, vp, u64, ctypes.c_uint32, vp, vp, vp]),
             "pcal_analyze": (i32, [vp, vp, vp]),
@@ -262,6 +263,11 @@ class Pcal:
     def set_folded_sum_dev(self, dev_parts, n_parts: int):
         """Accumulators <- sum of n_parts gathered bin blocks (rank order); dev_parts: CUDA float64 tensor."""
         _check(lib().pcal_set_folded_sum_dev(self._h, dev_parts.data_ptr(), n_parts), "pcal_set_folded_sum_dev")
+
+    def finalize_series_sum_dev(self, dev_parts, n_parts: int, n_periods: int, out_folded, out_tones):
+        """Rank-order sums + DFT of n_periods gathered periods (CUDA tensors); asynchronous."""
+        _check(lib().pcal_finalize_series_sum_dev(self._h, dev_parts.data_ptr(), n_parts, n_periods, out_folded.data_ptr(),
+                                                  out_tones.data_ptr()), "pcal_finalize_series_sum_dev")
 
     def set_profiling(self, enable: bool):
         _check(lib().pcal_set_profiling(self._h, int(enable)), "pcal_set_profiling")

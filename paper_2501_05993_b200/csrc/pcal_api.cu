@@ -965,6 +965,28 @@ extern "C" int pcal_set_folded_sum_dev(pcal_ctx* c, const double* dev_parts, uin
     return PCAL_OK;
 }
 
+// The exchange step of a time-sharded SERIES in one go: n_periods folded periods per rank were gathered into dev_parts
+// ([n_parts][n_periods][C][N_bins] complex); each period's bins are added in rank order, then its DFT is taken.
+extern "C" int pcal_finalize_series_sum_dev(pcal_ctx* c, const double* dev_parts, uint32_t n_parts, uint32_t n_periods,
+                                            double* dev_out_folded, double* dev_out_tones) {
+    if (!c || !dev_parts || !dev_out_folded || !dev_out_tones || n_parts == 0) return PCAL_ERR_INVALID;
+    if (n_periods == 0) return PCAL_OK;
+    const uint64_t n64 = (uint64_t)c->n_bins * c->C * n_periods;
+    if (n64 > (1ull << 30) || (uint64_t)c->C * n_periods > 65535) return PCAL_ERR_INVALID;
+    const uint32_t n = (uint32_t)n64;
+    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dev_out_folded),
+                                                             reinterpret_cast<const double2*>(dev_parts), n, n_parts);
+    // one DFT grid over (period, channel) rows: the series is laid out [period][channel][bin]
+    const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);
+    const uint32_t per_cta = kDftThreads / 32;
+    dft_kernel<<<dim3((c->n_bins + per_cta - 1) / per_cta, c->C * n_periods), kDftThreads, smem, c->stream>>>(
+        reinterpret_cast<const double2*>(dev_out_folded), (const double2*)c->d_W, reinterpret_cast<double2*>(dev_out_tones),
+        (double2*)nullptr, c->n_bins, (uint32_t)c->k_shift, 1u, (TailState*)nullptr, 0);
+    c->launches += 2;
+    CU(cudaGetLastError());
+    return PCAL_OK;
+}
+
 // Generator accuracy study: one device thread per case.
 extern "C" int pcal_generator_study(const pcal_gen_case_t* cases, uint32_t n_cases, uint64_t n_steps, uint32_t n_chk,
                                     double* out_err) {

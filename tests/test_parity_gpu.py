@@ -433,6 +433,76 @@ def test_exchange_step_in_one_launch(oracle):
     assert_close(outs[0][0], oracle_tones(oracle, w, host, 0), "gathered exchange")
 
 
+def test_sharding_package_on_one_gpu(oracle):
+    """sharding.ShardedIntegrator and sharding.series_sharded (what bench.py --gpus N and the gloo test run) with real
+    contexts: three "ranks" in one process, two lanes each, three periods; then a two-period series with one exchange."""
+    from paper_2501_05993_b200 import binding, sharding
+    w, dev, host = make(2, 1_200_000)
+    world, per = 3, 400_000
+    flat = dev.view(torch.uint8)
+    # every rank's gathered buffers must exist before anybody copies into them: one warm-up round builds them
+    want = oracle_tones(oracle, w, host, 0)
+    ranks = []
+    for r in range(world):
+        ctxs = [binding.from_workload(w), binding.from_workload(w)]
+        ranks.append({"ctxs": ctxs, "local": [torch.empty(w.n_bins * 2, dtype=torch.float64, device=DEV) for _ in range(3)]})
+    n2 = w.n_bins * 2
+    outs = [[torch.zeros((1, w.n_bins), dtype=torch.complex128).pin_memory() for _ in range(3)] for _ in range(world)]
+    # the exchange, in process: period k of every rank writes into one gathered tensor per period, shared by the ranks
+    shared = [torch.empty(world * n2, dtype=torch.float64, device=DEV) for _ in range(3)]
+
+    class Done:
+        def wait(self):
+            pass
+
+    integ = []
+    for r in range(world):
+        s = sharding.ShardedIntegrator(ranks[r]["ctxs"], 1, w.n_bins, world, DEV, gather=None)
+        integ.append(s)
+    for k in range(3):
+        for r in range(world):
+            s = integ[r]
+            lane = s.lanes[s.count % 2]
+
+            def gather(gathered, local, k=k, r=r, lane=lane):
+                shared[k][r * n2:(r + 1) * n2].copy_(local)
+                lane["gathered"] = shared[k]              # every rank reads the same gathered bins
+                return Done()
+            s.gather = gather
+            s.submit(flat[r * per // 4:(r + 1) * per // 4], per, r * per, outs[r][k])
+    for s in integ:
+        s.drain()
+    torch.cuda.synchronize()
+    for r in range(world):
+        for k in range(3):
+            assert np.array_equal(outs[r][k].numpy(), outs[0][0].numpy())     # every rank, every period: the same bits
+    assert_close(outs[0][0].numpy()[0], want, "sharded integrator")
+    # series: two periods of 600 000 samples, three ranks, ONE exchange
+    half, sh = 600_000, 200_000
+    big = torch.zeros(world * 2 * n2, dtype=torch.float64, device=DEV)
+    pf = torch.zeros((2, 1, w.n_bins), dtype=torch.complex128, device=DEV)
+    pt = torch.zeros_like(pf)
+    for r in range(world):
+        shards = [flat[(k * half + r * sh) // 4:(k * half + (r + 1) * sh) // 4] for k in range(2)]
+        starts = [k * half + r * sh for k in range(2)]
+
+        def gather(gathered, local, r=r):
+            big.view(world, -1)[r].copy_(local)
+            gathered.copy_(big)
+            return Done()
+        sharding.series_sharded(ranks[r]["ctxs"][0], shards, sh, starts, 1, w.n_bins, world, DEV, pf, pt, gather=gather)
+    torch.cuda.synchronize()                          # (the last rank saw every rank's bins)
+    hb = host.reshape(-1).view(np.uint8)
+    for k in range(2):
+        pr, pi = oracle.fold_ld(hb[k * half // 4:(k + 1) * half // 4], oracle.TWO_BIT_OFFSET_BINARY, 1, 0, 0, 1, half, k * half,
+                                w.f_s_hz, w.f_comb_hz, w.f_offset_hz[0])
+        assert_close(pf[k, 0].cpu().numpy(), pr.astype(np.float64) + 1j * pi.astype(np.float64), f"series period {k} folded")
+        assert_close(pt[k, 0].cpu().numpy(), oracle.dft(pr, pi), f"series period {k} tones")
+    for rk in ranks:
+        for c in rk["ctxs"]:
+            c.destroy()
+
+
 @pytest.mark.parametrize("idx,n", [(2, 2_000_004), (1, 700_001), (4, 150_003), (3, 1_500_004)])
 def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n):
     """Consecutive fold launches overlap (device-side sequence numbers instead of grid-wide waits, pcal_tail.cuh).  Many
