@@ -474,7 +474,8 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         rr.kind = c->kind;
         const uint32_t total = c->q * c->F * 32u;
         rr.ns = c->R <= 8 ? 1u : (c->R <= 16 ? 2u : (c->R <= 32 ? 4u : 8u));
-        launch_chain(reduce_replicas_kernel, total / ((uint32_t)kPostThreads / rr.ns), kPostThreads, 0, st, rr);
+        const uint32_t epc = (uint32_t)kPostThreads / rr.ns;
+        launch_chain(reduce_replicas_kernel, (total + epc - 1) / epc, kPostThreads, 0, st, rr);
         c->launches += 1;
     }
     RotateParams rp;
@@ -892,6 +893,13 @@ static void kshift_bins(const pcal_ctx* c, double* bins, int sign) {
         }
 }
 
+// the exact integer bins, where the context keeps them (integer samples, no rotation): the exchange calls maintain them too
+static long long* exact_bins_of(const pcal_ctx* c) {
+    if (c->kind == KIND_F32 || c->k_shift) return nullptr;
+    for (int i = 0; i < c->C; ++i) if (c->Foff[i]) return nullptr;
+    return c->d_Pint;
+}
+
 extern "C" int pcal_get_folded(pcal_ctx* c, double* out) {
     if (!c || !out) return PCAL_ERR_INVALID;
     { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
@@ -923,7 +931,7 @@ extern "C" int pcal_add_folded(pcal_ctx* c, const double* bins) {
     memcpy(c->h_pinned, bins, (size_t)n * sizeof(double2));
     kshift_bins(c, c->h_pinned, -1);
     CU(cudaMemcpyAsync(c->d_tmp, c->h_pinned, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
-    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, c->d_tmp, n);
+    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, exact_bins_of(c), c->d_tmp, n);
     c->launches += 1;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(c->stream));
@@ -949,7 +957,7 @@ extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
     if (!c || !dev_bins) return PCAL_ERR_INVALID;
     { const int rz = ensure_zeroed(c); if (rz != PCAL_OK) return rz; }
     const uint32_t n = c->n_bins * (uint32_t)c->C;
-    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_bins), n);
+    add_bins_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, exact_bins_of(c), reinterpret_cast<const double2*>(dev_bins), n);
     c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
@@ -958,7 +966,7 @@ extern "C" int pcal_add_folded_dev(pcal_ctx* c, const double* dev_bins) {
 extern "C" int pcal_set_folded_sum_dev(pcal_ctx* c, const double* dev_parts, uint32_t n_parts) {
     if (!c || !dev_parts || n_parts == 0) return PCAL_ERR_INVALID;
     const uint32_t n = c->n_bins * (uint32_t)c->C;
-    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, reinterpret_cast<const double2*>(dev_parts), n, n_parts);
+    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d_P, exact_bins_of(c), reinterpret_cast<const double2*>(dev_parts), n, n_parts);
     c->launches += 1;
     CU(cudaGetLastError());
     c->zero_pending = false;      // the accumulators now hold exactly the sum
@@ -974,7 +982,7 @@ extern "C" int pcal_finalize_series_sum_dev(pcal_ctx* c, const double* dev_parts
     const uint64_t n64 = (uint64_t)c->n_bins * c->C * n_periods;
     if (n64 > (1ull << 30) || (uint64_t)c->C * n_periods > 65535) return PCAL_ERR_INVALID;
     const uint32_t n = (uint32_t)n64;
-    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dev_out_folded),
+    sum_parts_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(reinterpret_cast<double2*>(dev_out_folded), (long long*)nullptr,
                                                              reinterpret_cast<const double2*>(dev_parts), n, n_parts);
     // one DFT grid over (period, channel) rows: the series is laid out [period][channel][bin]
     const size_t smem = 2 * (size_t)c->n_bins * sizeof(double2);

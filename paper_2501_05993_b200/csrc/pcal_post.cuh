@@ -58,15 +58,17 @@ __global__ void __launch_bounds__(kPostThreads) reduce_replicas_kernel(ReplicaPa
     pdl_wait();
     __shared__ double sd[kPostThreads];
     __shared__ long long si[kPostThreads];
-    const uint32_t E = P.F * 32u, total = P.q * E;          // total is a multiple of 256
+    const uint32_t E = P.F * 32u, total = P.q * E;          // a multiple of 128 (float32, odd q: not of 256)
     const uint32_t epc = kPostThreads / P.ns;                // elements per CTA
     const uint32_t sl = threadIdx.x / epc, e = threadIdx.x % epc;
     const uint32_t i = blockIdx.x * epc + e;
-    if (P.kind == KIND_F32) sd[threadIdx.x] = replica_sum<double, double>(reinterpret_cast<const double*>(P.partial) + i, total, sl, P.ns, P.R);
+    const bool in = i < total;                               // (the last CTA may be partly empty)
+    if (!in) { sd[threadIdx.x] = 0.0; si[threadIdx.x] = 0; }
+    else if (P.kind == KIND_F32) sd[threadIdx.x] = replica_sum<double, double>(reinterpret_cast<const double*>(P.partial) + i, total, sl, P.ns, P.R);
     else if (P.kind == KIND_I8) si[threadIdx.x] = replica_sum<int32_t, long long>(reinterpret_cast<const int32_t*>(P.partial) + i, total, sl, P.ns, P.R);
     else si[threadIdx.x] = replica_sum<uint16_t, long long>(reinterpret_cast<const uint16_t*>(P.partial) + i, total, sl, P.ns, P.R);
     __syncthreads();
-    if (sl != 0) return;
+    if (sl != 0 || !in) return;
     double v;
     if (P.kind == KIND_F32) {
         v = 0.0;
@@ -371,17 +373,20 @@ __global__ void zero_kernel(double2* P, long long* Pint, uint32_t n) {
 }
 
 // P[i] = sum_r parts[r][i], r = 0 .. n_parts-1 in that order (the exchange step of a time-sharded run)
-__global__ void sum_parts_kernel(double2* P, const double2* parts, uint32_t n, uint32_t n_parts) {
+// (Pint, when given: the exact integer bins of unrotated integer input -- the real parts are integers below 2^53, so the
+//  fp64 sums above are exact and llrint recovers them)
+__global__ void sum_parts_kernel(double2* P, long long* Pint, const double2* parts, uint32_t n, uint32_t n_parts) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double re = 0.0, im = 0.0;
     for (uint32_t r = 0; r < n_parts; ++r) { const double2 v = parts[(size_t)r * n + i]; re += v.x; im += v.y; }
     P[i] = make_double2(re, im);
+    if (Pint) Pint[i] = llrint(re);
 }
 
-__global__ void add_bins_kernel(double2* P, const double2* add, uint32_t n) {
+__global__ void add_bins_kernel(double2* P, long long* Pint, const double2* add, uint32_t n) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) { P[i].x += add[i].x; P[i].y += add[i].y; }
+    if (i < n) { P[i].x += add[i].x; P[i].y += add[i].y; if (Pint) Pint[i] = llrint(P[i].x); }
 }
 
 }  // namespace pcal

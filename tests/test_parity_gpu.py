@@ -433,6 +433,67 @@ def test_exchange_step_in_one_launch(oracle):
     assert_close(outs[0][0], oracle_tones(oracle, w, host, 0), "gathered exchange")
 
 
+@pytest.mark.parametrize("n_bins", [375, 1100, 363])
+@pytest.mark.parametrize("unfused", [False, True])
+def test_float32_odd_slot_group_counts(oracle, n_bins, unfused, monkeypatch):
+    """float32 vectors hold 4 samples, so a slot-group count q that is odd makes q * 4 * 32 replica sums -- not a multiple
+    of the 256 threads of reduce_replicas_kernel's CTAs (its last CTA is partly empty).  Both reduction paths."""
+    if unfused:
+        monkeypatch.setenv("PCAL_NO_FUSED_TAIL", "1")
+    w = synth.Workload("f32_odd_q", 1, n_bins * 1e6, 1e6, [0.0], 32, 3, 1_500_003, 0.05, 1.0, [5e-9], 4250)
+    dev = synth.generate(w, DEV)
+    host = dev.cpu().numpy()
+    p, T, P = gpu_run(w, dev)
+    pr, pi = oracle_folded(oracle, w, host, 0)
+    # (4000 samples per bin: one bin in which the comb's pulse and the noise cancel to 1e-5 of a typical bin -- reading R28)
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"N_bins={n_bins} folded", max_small=1)
+    assert_close(T[0][1:n_bins // 2], oracle.dft(pr, pi)[1:n_bins // 2], f"N_bins={n_bins} in-band tones")
+    p.destroy()
+
+
+def test_first_call_on_a_side_stream(oracle):
+    """Everything a context sets up lazily (tables, counters) is issued on the stream handed to pcal_extract: the very
+    first call may be made on a non-blocking side stream (every torch.cuda.Stream is one)."""
+    for idx, n, rot in [(2, 2_000_004, None), (3, 2_000_004, "generator"), (4, 300_003, None)]:
+        w, dev, host = make(idx, n)
+        if rot:
+            w = synth.replace(w, rotator=rot)
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            p = __import__("paper_2501_05993_b200.binding", fromlist=["x"]).from_workload(w)
+            p.extract(dev, n)
+            T = p.finalize()
+        assert_close(T[0], oracle_tones(oracle, w, host, 0), f"cfg{idx} first call on a side stream")
+        p.destroy()
+
+
+def test_exact_integer_bins_survive_the_exchange(oracle):
+    """Time-sharded integer input without rotation: after the exchange step (pcal_set_folded_sum_dev, pcal_add_folded_dev,
+    pcal_add_folded) pcal_get_folded_i64 still returns the exact bins of the WHOLE stream."""
+    from paper_2501_05993_b200 import binding
+    w, dev, host = make(6, 1_200_000)                  # config 2 with f_offset = 0
+    fmt = oracle.TWO_BIT_OFFSET_BINARY
+    want = oracle.fold_i64(host, fmt, 1, 0, 0, 1, w.n_samples, 0, w.n_bins)
+    flat = dev.view(torch.uint8)
+    world, per = 3, 400_000
+    gathered = torch.empty(world * w.n_bins * 2, dtype=torch.float64, device=DEV)
+    ctxs = []
+    for r in range(world):
+        p = binding.from_workload(w)
+        p.set_start_index(r * per)
+        p.extract(flat[r * per // 4:(r + 1) * per // 4], per)
+        p.get_folded_dev(gathered[r * w.n_bins * 2:(r + 1) * w.n_bins * 2])
+        ctxs.append(p)
+    ctxs[0].set_folded_sum_dev(gathered, world)
+    assert np.array_equal(ctxs[0].get_folded_i64()[0], want)
+    ctxs[1].add_folded_dev(gathered[0:w.n_bins * 2])                       # rank 1 + rank 0 + rank 2, one at a time
+    ctxs[1].add_folded(ctxs[2].get_folded())
+    assert np.array_equal(ctxs[1].get_folded_i64()[0], want)
+    for p in ctxs:
+        p.destroy()
+
+
 def test_sharding_package_on_one_gpu(oracle):
     """sharding.ShardedIntegrator and sharding.series_sharded (what bench.py --gpus N and the gloo test run) with real
     contexts: three "ranks" in one process, two lanes each, three periods; then a two-period series with one exchange."""
