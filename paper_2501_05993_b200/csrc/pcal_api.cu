@@ -333,8 +333,8 @@ static int prepare(pcal_ctx* c) {
             uint32_t tpp = 1; while (tpp * 2 <= per && tpp < 32) tpp *= 2;
             c->tail_tpp = tpp;
             const size_t ns = kTailSlots;
-            CU(cudaMalloc(&c->d_cnt, ns * ((size_t)c->q + 1) * sizeof(uint32_t)));
-            CU(cudaMemsetAsync(c->d_cnt, 0, ns * ((size_t)c->q + 1) * sizeof(uint32_t), c->stream));
+            CU(cudaMalloc(&c->d_cnt, ns * ((size_t)c->q + 2) * sizeof(uint32_t)));
+            CU(cudaMemsetAsync(c->d_cnt, 0, ns * ((size_t)c->q + 2) * sizeof(uint32_t), c->stream));
             CU(cudaMalloc(&c->d_G, ns * (size_t)c->q * pairs * sizeof(double2)));
             CU(cudaMalloc(&c->d_tail_state, sizeof(TailState)));
             CU(cudaMemsetAsync(c->d_tail_state, 0, sizeof(TailState), c->stream));
@@ -440,7 +440,7 @@ static int extract_piece_lut(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
             tp.enabled = 1;
             tp.cnt = c->d_cnt; tp.G = c->d_G; tp.st = c->d_tail_state; tp.partial_stride = c->partial_slot_bytes;
             if (c->fuse_req) {
-                tp.fuse_dft = 1; tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W;
+                tp.fuse_dft = 1; tp.dft_n1 = dft_n1_of(c->n_bins); tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W;
                 tp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; tp.T_host = c->fuse_out; tp.P_copy = c->fuse_P_copy;
             }
             tp.lut = c->d_lut;
@@ -724,11 +724,14 @@ static bool can_fuse_dft(const pcal_ctx* c) {
         const uint32_t n1 = dft_n1_of(c->n_bins);
         const size_t ring = (c->C == 4 ? 4u : 5u) * (size_t)kG2StageBytes;
         return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) &&
-               ((size_t)c->n_bins * c->C + c->n_bins) * sizeof(double2) + 2 * kG2Fields * sizeof(long long) <= ring;
+               2 * (size_t)c->n_bins * c->C * sizeof(double2) + 2 * kG2Fields * sizeof(long long) <= ring;
     }
-    if (!(c->prepared && c->rot_eff == PCAL_ROT_LUT && c->fused) || c->n_bins > 64) return false;
-    const uint32_t cap = c->kind == KIND_2BIT ? 1792u : (c->kind == KIND_I8 ? 768u : 256u);   // (scratch doubles - 512) / 2
-    return c->n_bins * (uint32_t)c->C <= cap;
+    if (!(c->prepared && c->rot_eff == PCAL_ROT_LUT && c->fused)) return false;
+    // the last finishing CTA of the fold kernel: two-stage DFT cheap enough for a serial stage, and 2 * C * N_bins complex
+    // values (P and as much scratch) fit in the kernel's shared scratch (4096 / 2048 / 1024 doubles)
+    const uint32_t n1 = dft_n1_of(c->n_bins);
+    const uint32_t cap = c->kind == KIND_2BIT ? 2048u : 512u;
+    return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) && 2u * c->n_bins * (uint32_t)c->C <= cap;
 }
 
 static int enqueue_dft(pcal_ctx* c, double2* second_dst) {

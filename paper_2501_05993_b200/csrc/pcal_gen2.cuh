@@ -583,9 +583,7 @@ const __grid_constant__ Gen2Params P) {
     if (P.fuse_dft) {   // T[c] = DFT(P[c]), channel by channel, from shared memory
         __syncthreads();
         double2* sY = sP + pairs;
-        for (uint32_t c = 0; c < (uint32_t)C; ++c)
-            dft_in_cta(sP + c * P.n_bins, sY, P.W, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev + c * P.n_bins,
-                       P.T_host ? P.T_host + c * P.n_bins : nullptr, kG2Threads);
+        dft_in_cta(sP, sY, P.W, (uint32_t)C, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev, P.T_host, kG2Threads);
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
     __syncthreads();

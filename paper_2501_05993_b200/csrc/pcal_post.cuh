@@ -325,42 +325,47 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
 }
 
 // ---- the same DFT inside a CTA that already holds P in shared memory (fused tails) ----------------------------
-// T[i] = X[(i - k_shift) mod N], X[k] = sum_b P[b] W[(k b) mod N], evaluated in two stages for N = N1 N2 (N1 = 1: the
-// plain sum): with b = N2 b1 + b2 and k = k1 + N1 k2,
+// T[c][i] = X_c[(i - k_shift) mod N], X_c[k] = sum_b P[c][b] W[(k b) mod N], evaluated in two stages for N = N1 N2 (N1 = 1:
+// the plain sum): with b = N2 b1 + b2 and k = k1 + N1 k2,
 //     Y[k1][b2] = W[(k1 b2) mod N] * sum_{b1 < N1} P[N2 b1 + b2] W[(N2 k1 b1) mod N]
 //     X[k1 + N1 k2] = sum_{b2 < N2} Y[k1][b2] W[(N1 k2 b2) mod N]
-// -- N (N1 + N2) complex MACs instead of N^2, every twiddle taken from the table at an index reduced in integers, every
-// sum in a fixed order.  sP, sY: [N] each in shared memory (sY is scratch, laid out [b2][k1]); all threads of the CTA call it.
-__device__ __forceinline__ void dft_in_cta(const double2* sP, double2* sY, const double2* __restrict__ W, uint32_t N, uint32_t N1,
-                                           uint32_t k_shift, double2* T_dev, double2* T_host, uint32_t nthreads) {
-    const uint32_t N2 = N / N1, tid = threadIdx.x;
-    for (uint32_t o = tid; o < N; o += nthreads) {
+// -- N (N1 + N2) complex MACs per channel instead of N^2, every twiddle taken from the table at an index reduced in
+// integers, every sum in a fixed order.  All n_ch channels at once (one thread per output).  sP, sY: [n_ch][N] each in
+// shared memory (sY is scratch, laid out [b2][k1] per channel); all threads of the CTA call it.
+__device__ __forceinline__ void dft_in_cta(const double2* sP, double2* sY, const double2* __restrict__ W, uint32_t n_ch, uint32_t N,
+                                           uint32_t N1, uint32_t k_shift, double2* T_dev, double2* T_host, uint32_t nthreads) {
+    const uint32_t N2 = N / N1, tid = threadIdx.x, total = n_ch * N;
+    for (uint32_t oo = tid; oo < total; oo += nthreads) {
+        const uint32_t c = oo / N, o = oo % N;
         const uint32_t k1 = o / N2, b2 = o % N2;
         const uint32_t step = (uint32_t)(((uint64_t)N2 * k1) % N);
+        const double2* p0 = sP + c * N + b2;
         uint32_t idx = 0;
         double re = 0.0, im = 0.0;
         for (uint32_t b1 = 0; b1 < N1; ++b1) {
-            const double2 p = sP[N2 * b1 + b2], w = __ldg(W + idx);
+            const double2 p = p0[N2 * b1], w = __ldg(W + idx);
             re += p.x * w.x - p.y * w.y;
             im += p.x * w.y + p.y * w.x;
             idx += step; if (idx >= N) idx -= N;
         }
         const double2 w = __ldg(W + (uint32_t)(((uint64_t)k1 * b2) % N));
-        sY[b2 * N1 + k1] = make_double2(re * w.x - im * w.y, re * w.y + im * w.x);
+        sY[c * N + b2 * N1 + k1] = make_double2(re * w.x - im * w.y, re * w.y + im * w.x);
     }
     __syncthreads();
-    for (uint32_t o = tid; o < N; o += nthreads) {
+    for (uint32_t oo = tid; oo < total; oo += nthreads) {
+        const uint32_t c = oo / N, o = oo % N;
         const uint32_t k1 = o % N1, k2 = o / N1;
         const uint32_t step = (uint32_t)(((uint64_t)N1 * k2) % N);
+        const double2* y0 = sY + c * N + k1;
         uint32_t idx = 0;
         double re = 0.0, im = 0.0;
         for (uint32_t b2 = 0; b2 < N2; ++b2) {
-            const double2 y = sY[b2 * N1 + k1], w = __ldg(W + idx);
+            const double2 y = y0[b2 * N1], w = __ldg(W + idx);
             re += y.x * w.x - y.y * w.y;
             im += y.x * w.y + y.y * w.x;
             idx += step; if (idx >= N) idx -= N;
         }
-        const uint32_t i = (o + k_shift) % N;
+        const uint32_t i = c * N + (o + k_shift) % N;
         T_dev[i] = make_double2(re, im);
         if (T_host) T_host[i] = make_double2(re, im);
     }

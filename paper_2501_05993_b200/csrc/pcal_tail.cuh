@@ -40,7 +40,7 @@
 namespace pcal {
 
 struct TailParams {
-    uint32_t* cnt;            // [device] [slot][q+1] arrival counters, zero between launches
+    uint32_t* cnt;            // [device] [slot][q+2] arrival counters (groups, grid, finishers), zero between launches
     double2* G;               // [device] [slot][q][C*n_bins] per-group bins
     const double2* lut;       // [device] concatenated per-channel rotator tables (eq. 2.4)
     uint32_t lut_off[kMaxChannels];  // per channel: first entry (by value: no dependent load in the serial tail)
@@ -59,7 +59,8 @@ struct TailParams {
     TailState* st;            // [device] tickets and progress counters of the context
     uint64_t partial_stride;  // bytes between the partial buffers of consecutive slots
     // pcal_integrate on small periods: stage C also takes the N_bins-point DFT and delivers T
-    int fuse_dft;             // 1: N_bins <= 64 and C*N_bins complex values fit behind the first 512 doubles of scratch
+    int fuse_dft;             // 1: the DFT is cheap in two stages and (C + 1) * N_bins complex values fit in the scratch
+    uint32_t dft_n1;          // N_bins = dft_n1 * N2 (dft_in_cta, pcal_post.cuh)
     uint32_t k_shift;
     const double2* W;         // [device] exp(-j 2 pi k / N_bins), k < N_bins
     double2* T_dev;           // [device] tone spectrum [C][N_bins]
@@ -68,6 +69,7 @@ struct TailParams {
 };
 
 constexpr uint32_t kTailSlots = 8;
+constexpr uint32_t kTailFinishers = 8;      // CTAs that share stage C of the fused tail
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
     uint32_t v;
@@ -127,7 +129,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     const uint32_t tid = threadIdx.x;
     const uint32_t p = blockIdx.x % q;
     const uint32_t slot = seq % kTailSlots;
-    uint32_t* cnt = T.cnt + (size_t)slot * (q + 1u);
+    uint32_t* cnt = T.cnt + (size_t)slot * (q + 2u);
     constexpr uint32_t F = KIND == KIND_2BIT ? 64u : (KIND == KIND_I8 ? 16u : 4u);
     constexpr uint32_t E = F * 32u;
 
@@ -229,9 +231,21 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     __syncthreads();
     if (tid == 0) s_prev = arrive_acq_rel(cnt + q);
     __syncthreads();
-    if (s_prev != q - 1u) return;
-
     // ---- stage C: groups in order, ragged tail, accumulate into the context ------------------
+    // The last S group CTAs to arrive share it: the one that arrives as number q - S + k takes slice k of the (channel, bin)
+    // pairs.  All but the very last wait (one thread, acquire loads) until every group has arrived -- the CTAs they wait for
+    // are running -- so that a 16-channel stream is not finished by a single CTA.  Which CTA takes which slice changes
+    // nothing in the arithmetic: every pair is summed by one thread in group order.
+    const uint32_t S_want = (pairs + 127u) / 128u < kTailFinishers ? (pairs + 127u) / 128u : kTailFinishers;    // >= 128 pairs each
+    const uint32_t S = q < S_want ? q : S_want;
+    if (s_prev < q - S) return;
+    const uint32_t slice = s_prev - (q - S);
+    if (s_prev != q - 1u) {
+        if (tid == 0) while (ld_acquire_u32(cnt + q) != q) __nanosleep(64);
+        __syncthreads();
+    }
+    const uint32_t per_slice = (pairs + S - 1u) / S;
+    const uint32_t pair_lo = slice * per_slice, pair_hi = pair_lo + per_slice < pairs ? pair_lo + per_slice : pairs;
     // The group sums and the ragged tail do not depend on P: they are formed first, and only then does the CTA wait
     // (first trip of the loop below) until P is up to date (n_done == seq) and no longer being read by a DFT kernel.
     auto wait_for_P = [&]() {
@@ -246,16 +260,18 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     };
     // thread = (slice sl of the groups, pair): slice sums first (all loads of a thread in flight at
     // once where possible), then the slices in order.
-    const uint32_t ppc = pairs < (uint32_t)kThreads ? pairs : (uint32_t)kThreads;
-    const uint32_t ns = (uint32_t)kThreads / ppc;            // >= 1; > 1 only when pairs < 256
+    const uint32_t my_pairs = pair_hi > pair_lo ? pair_hi - pair_lo : 0u;
+    const uint32_t ppc = my_pairs < (uint32_t)kThreads ? (my_pairs ? my_pairs : 1u) : (uint32_t)kThreads;
+    const uint32_t ns = (uint32_t)kThreads / ppc;            // >= 1; > 1 only when this CTA has fewer than 256 pairs
     const uint32_t sl = tid / ppc, e0 = tid % ppc;
     const uint32_t n_tail = (uint32_t)(T.n_total - T.NT);
     double* s_re = scratch;                                  // [kThreads]
     double* s_im = scratch + kThreads;                       // [kThreads]
-    for (uint32_t pp0 = 0; pp0 < pairs; pp0 += ppc) {        // uniform trip count (one trip when pairs <= 256)
+    bool waited = false;
+    for (uint32_t pp0 = pair_lo; pp0 < pair_hi || !waited; pp0 += ppc) {        // uniform trip count; at least one trip (the wait)
         const uint32_t pp = pp0 + e0;
         double are = 0.0, aim = 0.0;
-        if (sl < ns && pp < pairs) {
+        if (sl < ns && pp < pair_hi) {
             for (uint32_t g0 = sl; g0 < q; g0 += 8u * ns) {
                 double2 g[8];
 #pragma unroll
@@ -271,7 +287,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
             are = 0.0; aim = 0.0;
             if (sl == 0) for (uint32_t k = 0; k < ns; ++k) { are += s_re[k * ppc + e0]; aim += s_im[k * ppc + e0]; }
         }
-        const bool mine = sl == 0 && pp < pairs;
+        const bool mine = sl == 0 && pp < pair_hi;
         const uint32_t c = mine ? pp / T.n_bins : 0u, b = mine ? pp % T.n_bins : 0u;
         if (mine && n_tail) {   // samples NT .. n_total-1 (fewer than one vector)
             const uint32_t L = T.lut_len[c];
@@ -288,7 +304,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
                 if (L > 1 && ++k == L) k = 0;
             }
         }
-        if (pp0 == 0) wait_for_P();        // every thread of the CTA, once
+        if (!waited) { wait_for_P(); waited = true; }        // every thread of the CTA, once
         if (!mine) continue;
         long long ai = (long long)are;     // exact: unrotated integer sums are integers below 2^53
         if (!T.overwrite) {
@@ -298,29 +314,27 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         }
         T.P[pp] = make_double2(are, aim);
         if (T.integer_exact) T.Pint[pp] = ai;
-        if (T.fuse_dft) reinterpret_cast<double2*>(scratch + 2 * kThreads)[pp] = make_double2(are, aim);
         if (T.P_copy) T.P_copy[pp] = make_double2(are, aim);
+        if (S == 1u && T.fuse_dft) reinterpret_cast<double2*>(scratch + 2 * kThreads)[pp] = make_double2(are, aim);   // (<= 128 pairs)
     }
-    if (T.fuse_dft) {   // T[c][i] = sum_b P[c][b] W[(i' b) mod N], i' = (i - k_shift) mod N: one thread per output, b in order
+    // the finishing CTAs meet once more; the last of them takes the DFT (pcal_integrate / series on small periods), makes the
+    // slot ready for its next launch and publishes the result
+    __syncthreads();
+    if (S > 1u) {
+        if (tid == 0) s_prev = arrive_acq_rel(cnt + q + 1u);
         __syncthreads();
-        const double2* sP = reinterpret_cast<const double2*>(scratch + 2 * kThreads);
-        const uint32_t N = T.n_bins;
-        for (uint32_t pp = tid; pp < pairs; pp += kThreads) {
-            const uint32_t c = pp / N, i = pp % N;
-            const uint32_t ii = (i + N - T.k_shift % N) % N;
-            uint32_t k = 0;
-            double re = 0.0, im = 0.0;
-            for (uint32_t b = 0; b < N; ++b) {
-                const double2 p = sP[c * N + b], w = __ldg(T.W + k);
-                re += p.x * w.x - p.y * w.y;
-                im += p.x * w.y + p.y * w.x;
-                k += ii; if (k >= N) k -= N;
-            }
-            T.T_dev[pp] = make_double2(re, im);
-            if (T.T_host) T.T_host[pp] = make_double2(re, im);
-        }
+        if (s_prev != S - 1u) return;
     }
-    for (uint32_t i = tid; i <= q; i += kThreads) cnt[i] = 0u;         // ready for the slot's next launch
+    if (T.fuse_dft) {   // T[c] = DFT(P[c]), every channel at once, from shared memory
+        double2* sP = reinterpret_cast<double2*>(S > 1u ? scratch : scratch + 2 * kThreads);
+        double2* sY = sP + pairs;
+        if (S > 1u) {
+            for (uint32_t pp = tid; pp < pairs; pp += kThreads) sP[pp] = __ldcg(T.P + pp);      // (slices written by the other finishers: L2)
+            __syncthreads();
+        }
+        dft_in_cta(sP, sY, T.W, T.C, T.n_bins, T.dft_n1, T.k_shift % T.n_bins, T.T_dev, T.T_host, kThreads);
+    }
+    for (uint32_t i = tid; i <= q + 1u; i += kThreads) cnt[i] = 0u;    // ready for the slot's next launch
     __syncthreads();
     if (tid == 0) st_release_u32(&T.st->n_done, seq + 1u);             // P is final for this launch; the slot is free
 }

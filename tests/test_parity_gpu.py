@@ -93,9 +93,10 @@ def test_generator_on_every_sample_type(oracle, idx, n):
 @pytest.mark.parametrize("idx,n,k_shift", [(1, 1_300_001, 0), (2, 1_300_004, 0), (2, 1_300_004, 5), (4, 200_003, 0), (6, 600_004, 0),
                                            (3, 2_600_036, 0), (5, 1_300_003, 0), (8, 500_001, 0), (2, 60, 0)])
 def test_integrate_is_reset_extract_finalize(oracle, idx, n, k_shift):
-    """pcal_integrate = pcal_reset + pcal_extract + pcal_finalize_async in one call.  For small N_bins on the LUT path the
-    fold kernel's stage C takes the DFT itself and writes T straight into the pinned buffer (one launch per period);
-    otherwise the DFT kernel follows.  Repeated periods on one context, against the oracle and against the three calls."""
+    """pcal_integrate = pcal_reset + pcal_extract + pcal_finalize_async in one call.  On the LUT path and on the 2-bit
+    generator path the last CTA of the extract kernel takes the DFT itself (two stages) and writes T straight into the
+    pinned buffer: one launch per period; the int8 / float32 generator kernels are followed by their post and DFT
+    kernels.  Repeated periods on one context, against the oracle and against the three calls."""
     from paper_2501_05993_b200 import binding
     w, dev, host = make(idx, n)
     p = binding.from_workload(w)
@@ -110,8 +111,8 @@ def test_integrate_is_reset_extract_finalize(oracle, idx, n, k_shift):
     per_period = (p.info().kernel_launches - l0) // 3
     T1 = out.numpy().copy()
     p.reset(); p.extract(dev, n); T2 = p.finalize()
-    small = w.n_bins <= 64 and idx != 5 and n > 1000
-    assert per_period == (1 if small else (3 if idx == 5 else 2)), per_period
+    fused = idx != 5 and n > 1000
+    assert per_period == (1 if fused else (3 if idx == 5 else 2)), per_period
     for c in range(0, w.n_channels, 5):
         if n > 1000:
             assert_close(T1[c], oracle_tones(oracle, w, host, c), f"integrate cfg{idx} ch{c}")
@@ -445,8 +446,9 @@ def test_float32_odd_slot_group_counts(oracle, n_bins, unfused, monkeypatch):
     host = dev.cpu().numpy()
     p, T, P = gpu_run(w, dev)
     pr, pi = oracle_folded(oracle, w, host, 0)
-    # (4000 samples per bin: one bin in which the comb's pulse and the noise cancel to 1e-5 of a typical bin -- reading R28)
-    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"N_bins={n_bins} folded", max_small=1)
+    # (reading R28: without rotation the bins are REAL sums of ~4000 float32 samples each -- a Gaussian variable lies within
+    #  1 % of its median magnitude of zero with probability ~0.5 %, so a few of the N_bins bins are that small)
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"N_bins={n_bins} folded", max_small=n_bins // 64, small_bin=1e-2)
     assert_close(T[0][1:n_bins // 2], oracle.dft(pr, pi)[1:n_bins // 2], f"N_bins={n_bins} in-band tones")
     p.destroy()
 
