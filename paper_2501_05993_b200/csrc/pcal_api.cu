@@ -295,7 +295,13 @@ static int prepare(pcal_ctx* c) {
             }
         }
     }
-    const bool gen_ok = c->gen2 || (c->C == 1 && (c->gen_mma || (kThreads * c->gen_spt) % c->n_bins == 0));
+    // FFMA2 kernel (float32; int8 when N_bins does not divide 2048): a CTA iteration covers the largest multiple of
+    // lcm(N_bins, samples per load) that its 256 threads hold
+    {
+        const uint64_t unit = lcm_sat(c->n_bins, c->gen_spt, 1u << 20), cap = (uint64_t)kThreads * c->gen_spt;
+        c->gen_span = unit <= cap ? (uint32_t)(unit * (cap / unit)) : 0u;
+    }
+    const bool gen_ok = c->gen2 || (c->C == 1 && (c->gen_mma || c->gen_span != 0));
     int mode;
     if (c->all_zero) mode = PCAL_ROT_LUT;
     else if (c->rot_req == PCAL_ROT_LUT) mode = lut_ok ? PCAL_ROT_LUT : 0;
@@ -548,6 +554,9 @@ static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cuda
     return PCAL_OK;
 }
 
+// FFMA2 generator kernel: samples per tile (iterations per tile x samples per iteration)
+static uint64_t gen_tile_samples(const pcal_ctx* c) { return (uint64_t)(kTileSamples / (kThreads * c->gen_spt)) * c->gen_span; }
+
 static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
     if (c->gen2) return extract_piece_gen2(c, data, n, st);
     const uint32_t spt = c->gen_spt;
@@ -559,13 +568,17 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     if (n_loads) {
         GenParams gp;
         gp.data = data; gp.n_loads = n_loads;
-        gp.n_tiles = (n_loads * spt + kTileSamples - 1) / kTileSamples;
+        // FFMA2 kernel: a CTA iteration covers gen_span samples (a multiple of N_bins), a tile 2^16 / (kThreads * spt) iterations
+        const uint64_t span = c->gen_mma ? (uint64_t)kThreads * spt : c->gen_span;
+        const uint64_t tile = c->gen_mma ? kTileSamples : gen_tile_samples(c);
+        gp.span = (uint32_t)span;
+        gp.n_tiles = (n_loads * spt + tile - 1) / tile;
         gp.Fs = Fs; gp.Foff = Fo;
         gp.k0 = mulmod_host(c->n_processed % Fs, Fo, Fs);
-        gp.E = mulmod_host(kTileSamples, Fo, Fs);
+        gp.E = mulmod_host(tile, Fo, Fs);
         gp.D = mulmod_host(c->gen_grid, gp.E, Fs);
-        gp.rho = phasor_neg_host(mulmod_host((uint64_t)kThreads * spt, Fo, Fs), Fs);
-        gp.rho2 = phasor_neg_host(mulmod_host(2ull * kThreads * spt, Fo, Fs), Fs);
+        gp.rho = phasor_neg_host(mulmod_host(span, Fo, Fs), Fs);
+        gp.rho2 = phasor_neg_host(mulmod_host(2 * span, Fo, Fs), Fs);
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
         gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
         gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
@@ -605,7 +618,7 @@ static bool small_pieces() {
 static uint64_t piece_samples(const pcal_ctx* c, bool small) {
     if (c->rot_eff == PCAL_ROT_LUT) return (uint64_t)(small ? 16u : kMaxIterPerLaunch) * c->R * kWarps * c->q * 32ull * c->spv;
     if (c->gen2) return (uint64_t)(small ? 2 : kG2CapBatches * kG2Batch / 2) * c->gen_grid * c->g2_rt * c->g2_span_t;   // <= half of what the CTAs may claim
-    return (uint64_t)(small ? 2 : kGenMaxTiles) * c->gen_grid * kTileSamples;   // resync table: <= 256 tiles per CTA
+    return (uint64_t)(small ? 2 : kGenMaxTiles) * c->gen_grid * (c->gen_mma ? (uint64_t)kTileSamples : gen_tile_samples(c));   // resync table: <= 256 tiles per CTA
 }
 
 static int extract_segment(pcal_ctx* c, const uint8_t* p, uint64_t n_samples) {

@@ -34,6 +34,7 @@ struct GenParams {
     const void* data;        // [device] packed samples
     uint64_t n_loads;        // complete per-thread loads available (vectors of SPT samples)
     uint64_t n_tiles;
+    uint32_t span;           // samples per CTA iteration: the largest multiple of lcm(N_bins, SPT) <= kThreads*SPT (threads past it idle)
     uint64_t Fs, k0, E, D;   // micro-hertz sample rate; (n0*Foff)%Fs; (tile*Foff)%Fs; (grid*E)%Fs
     uint64_t Foff;
     double2 rho;             // exp(-j w * kThreads*SPT): oscillator step per CTA iteration
@@ -155,8 +156,9 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     if (!P.input_ready) pdl_wait();
     constexpr int SPT = GenTraits<KIND>::SPT;
     constexpr int LB = GenCfg<KIND>::LB, LPT = GenCfg<KIND>::LPT, RUN = GenCfg<KIND>::RUN, DEPTH = GenCfg<KIND>::DEPTH;
-    constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration
-    static_assert((uint32_t)LPT * SPAN == kTileSamples, "a tile is 2^16 samples");
+    constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration at most (a tile: LPT iterations, <= 2^16 samples)
+    static_assert((uint32_t)LPT * SPAN == kTileSamples, "a full tile is 2^16 samples");
+    const bool active = (uint32_t)threadIdx.x * SPT < P.span;   // N_bins that do not divide SPAN: the last threads have no samples
     using Vec = typename GenTraits<KIND>::Vec;
     extern __shared__ __align__(16) unsigned char gen_smem[];
     double2* acc = reinterpret_cast<double2*>(gen_smem);                 // [SPT][kThreads] (re, im)
@@ -184,9 +186,10 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
 
     const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
     unsigned char* my_ring = ring + (size_t)tid * LB;
+    constexpr size_t RING_STRIDE = (size_t)kThreads * LB;                // bytes between a thread's ring slots
     static_assert(LPT % DEPTH == 0, "ring slot of load j is j % DEPTH, a compile-time constant");
-    constexpr uint64_t LOAD_STRIDE = (uint64_t)kThreads * LB;            // bytes between a thread's loads
-    constexpr uint64_t TILE_BYTES = (uint64_t)LPT * LOAD_STRIDE;
+    const uint64_t LOAD_STRIDE = (uint64_t)(P.span / SPT) * LB;          // bytes between a thread's loads
+    const uint64_t TILE_BYTES = (uint64_t)LPT * LOAD_STRIDE;
     const uint64_t end_off = P.n_loads * LB;                              // first byte past the last complete load
     const uint64_t tile_stride = (uint64_t)gridDim.x * TILE_BYTES;
     uint64_t off = (uint64_t)blockIdx.x * TILE_BYTES + (uint64_t)tid * LB;   // this thread's load 0 of tile i
@@ -198,8 +201,8 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     static_assert(DEPTH % 2 == 0 && LPT % 2 == 0, "loads are committed and consumed in pairs");
 #pragma unroll
     for (int j = 0; j < DEPTH; ++j) {                        // prologue: the first DEPTH loads of tile 0
-        if (nt > 0 && off + j * LOAD_STRIDE < end_off)
-            cp_async_own<LB>(my_ring + (size_t)j * LOAD_STRIDE, gdata + off + j * LOAD_STRIDE);
+        if (active && nt > 0 && off + j * LOAD_STRIDE < end_off)
+            cp_async_own<LB>(my_ring + (size_t)j * RING_STRIDE, gdata + off + j * LOAD_STRIDE);
         if (j & 1) cp_async_commit();                        // one commit group per pair of loads
     }
     const float rho_c = (float)P.rho.x, rho_s = (float)P.rho.y;
@@ -227,20 +230,20 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
                                                  : off + tile_stride + (uint64_t)(j + DEPTH - LPT) * LOAD_STRIDE;
             bool go = true;
             if (CHECK) go = ((j + DEPTH < LPT) || next_exists) && o < end_off;
-            if (go) cp_async_own<LB>(my_ring + (size_t)slot * LOAD_STRIDE, gdata + o);
+            if (go && active) cp_async_own<LB>(my_ring + (size_t)slot * RING_STRIDE, gdata + o);
         };
 #pragma unroll
         for (int j = 0; j < LPT; j += 2) {
             const int s0 = j % DEPTH, s1 = (j + 1) % DEPTH;  // compile-time after unrolling
             cp_async_wait<DEPTH / 2 - 1>();
-            const Vec v0 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s0 * LOAD_STRIDE);
-            const Vec v1 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s1 * LOAD_STRIDE);
+            const Vec v0 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s0 * RING_STRIDE);
+            const Vec v1 = *reinterpret_cast<const Vec*>(my_ring + (size_t)s1 * RING_STRIDE);
             const float c0 = (float)ph.x, sn0 = (float)ph.y;
             const float c1 = __fmaf_rn(c0, rho_c, -sn0 * rho_s), sn1 = __fmaf_rn(c0, rho_s, sn0 * rho_c);
             bool ok0 = true, ok1 = true;
             if (CHECK) { ok0 = off + j * LOAD_STRIDE < end_off; ok1 = off + (j + 1) * LOAD_STRIDE < end_off; }
-            if (ok0) mac(v0, c0, sn0);
-            if (ok1) mac(v1, c1, sn1);
+            if (ok0 && active) mac(v0, c0, sn0);
+            if (ok1 && active) mac(v1, c1, sn1);
             refill(j, s0);
             refill(j + 1, s1);
             cp_async_commit();
@@ -293,7 +296,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
     pdl_wait();   // the partial bins of the previous launch may still be read by its post kernel
     for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
         double re = 0.0, im = 0.0;
-        for (uint32_t pos = sb; pos < SPAN; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
+        for (uint32_t pos = sb; pos < P.span; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
         P.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
     }
 }

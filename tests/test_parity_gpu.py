@@ -648,11 +648,16 @@ def test_bin_counts_that_are_not_powers_of_two(oracle, f_s, f_comb, f_off, bits,
     (96e6, 1e6, 250e3 + 1e-3, 2, 0, 900_004),  # N_bins = 96
     (2048e6, 1e6, 1234.567, 2, 0, 3_000_004),  # N_bins = 2048: the longest row (32 chunks)
     (1000e6, 1e6, 1234.567, 2, 0, 2_000_004),  # N_bins = 1000: rows of 8000 samples, in column blocks
+    (50e6, 1e6, 1234.567, 8, 2, 1_000_003),    # int8, N_bins = 50 does not divide 2048: FFMA2 kernel, 4000 samples per CTA iteration
+    (1000e6, 1e6, 777.123456, 8, 2, 2_000_001),  # int8, N_bins = 1000
+    (48e6, 2e6, 30e3 + 0.5, 32, 3, 600_001),   # float32, N_bins = 24: 1008 samples per CTA iteration
+    (1000e6, 1e6, 1234.567, 32, 3, 1_500_001), # float32, N_bins = 1000
 ])
 def test_generator_bin_counts_that_are_not_powers_of_two(oracle, f_s, f_comb, f_off, bits, enc, n):
     """The generator path needs an integer N_bins only (eq. 2.2): offsets whose table is impractical."""
     from paper_2501_05993_b200 import binding
-    w = synth.Workload("odd_bins_gen", 1, f_s, f_comb, [f_off], bits, enc, n, 0.05, 1.0, [5e-9], 4243, rotator="generator")
+    w = synth.Workload("odd_bins_gen", 1, f_s, f_comb, [f_off], bits, enc, n, 0.05 if bits != 8 else 1.0, 1.0 if bits != 8 else 20.0,
+                       [5e-9], 4243, rotator="generator")
     dev = synth.generate(w, DEV)
     host = dev.cpu().numpy()
     p, T, P = gpu_run(w, dev, splits=(300_032,))
