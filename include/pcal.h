@@ -9,9 +9,8 @@
  *     T[i]  = sum_b P[b] exp(-j 2 pi i b/N_bins) ("DFT(P)")
  * with N_bins = f_s / f_comb.  The rotator comes either from a precomputed look-up table of
  * length L = lcm(N_bins, N_rotator), N_rotator = f_s / gcd(f_s, f_offset) (eq. 2.4)
- * or from a recursive sinewave generator with constant phase increment (eq. 2.5-2.9,
- * PAPER.md:68-120) that is re-derived from the exactly reduced integer phase in fp64 at least
- * every 2^16 samples.
+ * or from a sinewave generator with constant phase increment (eq. 2.5-2.9) whose
+ * phasor is re-derived from exactly reduced integer phases at least every 2^16 samples (R14).
  *
  * Conventions: rotator sign exp(-j...) as eq. 2.3; forward unnormalised
  * DFT; sample index n = 0 at the first sample after create/reset and running across
@@ -96,8 +95,9 @@ int pcal_create(pcal_ctx **out, double f_s_hz, double f_comb_hz, double f_offset
 int pcal_set_channel_offsets(pcal_ctx *ctx, const double *f_offset_hz);
 
 /* Choose the rotator source.  AUTO = LUT when the fold period is practical, else GENERATOR.
- * LUT with an impractical period, or GENERATOR with n_channels > 1 -> PCAL_ERR_UNSUPPORTED
- * (reported by the next pcal_extract).  Legal only before the first pcal_extract after
+ * LUT with an impractical period -> PCAL_ERR_UNSUPPORTED (reported by the next pcal_extract).  GENERATOR serves every
+ * 2-bit layout (1..16 channels, each with its own offset) and every integer N_bins <= 4096 for 2-bit and int8 samples;
+ * float32 samples: N_bins <= 1024 (else PCAL_ERR_UNSUPPORTED).  Legal only before the first pcal_extract after
  * create/reset. */
 int pcal_set_rotator(pcal_ctx *ctx, int mode);
 

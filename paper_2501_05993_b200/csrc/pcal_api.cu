@@ -273,9 +273,9 @@ static int prepare(pcal_ctx* c) {
         q = (uint32_t)qq;
     }
     const char* gm = getenv("PCAL_GEN_MMA");       // =0: FFMA2 kernel of pcal_gen.cuh for every sample type (A/B runs, tests)
-    c->gen_mma = c->C == 1 && c->kind != KIND_F32 && kMmaSpan % c->n_bins == 0 && !(gm && gm[0] == '0');
-    // 2-bit samples, up to 4 channels: pcal_gen2.cuh.  A row is a multiple of lcm(N_bins, time samples per 16 bytes)
-    // time samples and at most 2048 fields.  PCAL_GEN2=0 keeps the older kernels (A/B runs, tests).
+    c->gen_mma = c->C == 1 && c->kind == KIND_I8 && kMmaSpan % c->n_bins == 0 && !(gm && gm[0] == '0');
+    // 2-bit samples: pcal_gen2.cuh.  A row is a multiple of lcm(N_bins, time samples per 16 bytes) time samples.
+    // PCAL_GEN2=0 or PCAL_GEN_MMA=0 selects the FFMA2 kernel instead (single channel; A/B runs, tests).
     c->gen2 = false;
     {
         const char* g2 = getenv("PCAL_GEN2");
@@ -398,8 +398,7 @@ static int prepare(pcal_ctx* c) {
             c->prepared = true;
             return PCAL_OK;
         }
-        if (c->gen_mma && c->kind == KIND_2BIT) { c->gen_smem = gen_mma_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_2BIT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_2BIT, false>, c->gen_smem); }
-        else if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8, false>, c->gen_smem); }
+        if (c->gen_mma) { c->gen_smem = gen_mma_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_mma_kernel<KIND_I8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_mma_kernel<KIND_I8, false>, c->gen_smem); }
         else if (c->kind == KIND_2BIT) { c->gen_smem = gen_smem_bytes<KIND_2BIT>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_2BIT>, c->gen_smem); }
         else if (c->kind == KIND_I8) { c->gen_smem = gen_smem_bytes<KIND_I8>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_I8>, c->gen_smem); }
         else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
@@ -585,9 +584,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.input_ready = c->input_ready ? 1 : 0;
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
-        if (c->gen_mma && c->kind == KIND_2BIT && c->sign_mag) launch_chain(gen_mma_kernel<KIND_2BIT, true>, c->gen_grid, kThreads, smem, st, gp);
-        else if (c->gen_mma && c->kind == KIND_2BIT) launch_chain(gen_mma_kernel<KIND_2BIT, false>, c->gen_grid, kThreads, smem, st, gp);
-        else if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8, false>, c->gen_grid, kThreads, smem, st, gp);
+        if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8, false>, c->gen_grid, kThreads, smem, st, gp);
         else if (c->kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, c->gen_grid, kThreads, smem, st, gp);
         else if (c->kind == KIND_I8) launch_chain(gen_kernel<KIND_I8>, c->gen_grid, kThreads, smem, st, gp);
         else launch_chain(gen_kernel<KIND_F32>, c->gen_grid, kThreads, smem, st, gp);

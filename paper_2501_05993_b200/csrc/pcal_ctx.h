@@ -25,8 +25,8 @@ struct pcal_ctx {
     uint32_t lut_off_h[PCAL_MAX_CHANNELS];   // first table entry of every channel (host copy)
     // generator-mode geometry
     uint32_t gen_grid, gen_spt, gen_span;   // (gen_span: samples per CTA iteration of the FFMA2 kernel, a multiple of N_bins)
-    bool gen_mma;                   // integer samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
-    bool gen2;                      // 2-bit samples, <= 4 channels: warp-specialised tensor-core generator kernel (pcal_gen2.cuh)
+    bool gen_mma;                   // int8 samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
+    bool gen2;                      // 2-bit samples: warp-specialised tensor-core generator kernel (pcal_gen2.cuh)
     uint32_t g2_span_t, g2_chunks;  // ... its row: time samples, 16-byte chunks
     uint32_t g2_cpw, g2_rt;         // ... chunks per consumer warp (1, 2, 4), rows per tile (128, 64, 32)
     uint32_t g2_blocks;             // ... column blocks of a row (rows longer than 32 chunks are served 32 chunks per launch)

@@ -21,8 +21,8 @@
 // row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-31 quantisation.
 //
 // Structure (profiles/r2_ncu_full.md has the before/after against the round-1 kernel):
-//   * warp roles, no CTA-wide barrier in the loop.  Warp 1 (generator) owns the CTA's tile sequence -- its own batch
-//     first, then batches claimed from a device counter, each claim issued one batch ahead -- and writes the digit
+//   * warp roles, no CTA-wide barrier in the loop.  Warp 1 (generator) owns the CTA's tile sequence -- its own batches
+//     first, then batches claimed from a device counter, each claim issued two batches ahead -- and writes the digit
 //     matrices into a ring of entries.  Warp 0 (loader) follows the sequence and copies each tile as it lies in memory
 //     (one cp.async instruction per 512 contiguous bytes) into a ring of padded tiles; completion arrives on the
 //     stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 2..9 (consumers) wait for "full", read their operands
@@ -34,13 +34,17 @@
 //   * the four 2-bit fields of a byte are separated by PREFIX masks: U0 = byte, U1 = byte & 0xFC, U2 = & 0xF0,
 //     U3 = & 0xC0 (3 LOP3 instead of 4; single channel), the field sums S_f are differences of the U sums, exact.
 //     With C = 2 / 4 channels field f belongs to channel f mod C and is masked accordingly (digits per channel).
-//   * dynamic tiles: a CTA that starts late simply takes fewer.  A CTA is half an SM (320 threads) and lets its dependent
-//     grid start when half of the batches are claimed: consecutive launches overlap pairwise and HBM keeps streaming
-//     while one of them is in its epilogue.
+//   * hybrid tile assignment: three quarters of the batches are a CTA's own (index + k * grid), the rest are claimed from a
+//     device counter -- a CTA that starts late simply takes fewer.  A CTA is half an SM (320 threads, 80 registers) and
+//     lets its dependent grid start as soon as its ticket is taken: consecutive launches share the SMs pairwise and HBM
+//     keeps streaming while one of them is in its epilogue.
 //   * the per-position sums of a CTA are exact int64 and are added to the launch's accumulators with integer
 //     red.global.add -- associative, so the result is bit-identical whatever the tile assignment was.  The CTA that
 //     arrives last converts to fp64, applies the position factor, folds positions to bins in a fixed order, adds the
-//     ragged tail and accumulates into the context (same TailState protocol as pcal_tail.cuh; DFT for N_bins <= 64).
+//     ragged tail and accumulates into the context (same TailState protocol as pcal_tail.cuh) and, for pcal_integrate /
+//     pcal_extract_series, takes the DFT in two stages (dft_in_cta).
+//   * words of 8 / 16 channels: four channels (one byte of the time sample) per launch; rows longer than 2048 fields: column
+//     blocks of 32 chunks, one launch each.
 #pragma once
 #include "pcal_gen.cuh"
 #include "pcal_tail.cuh"
@@ -97,7 +101,6 @@ struct Gen2Params {
     uint32_t k_shift;
     const double2* W;              // [device] exp(-j 2 pi k / N_bins)
     double2 *T_dev, *T_host, *P_copy;
-    unsigned long long* stamps;    // TEMP
 };
 
 template <int C, int CPW>
@@ -168,19 +171,10 @@ template <int C> __device__ __forceinline__ constexpr uint32_t g2_mask(int u) {
 }
 template <int C> __device__ __forceinline__ constexpr int g2_chan(int u) { return C == 1 ? 0 : (C == 2 ? (u & 1) : u); }
 
-#ifdef G2_PROFILE
-#define G2_STAMPL(i) do { if ((threadIdx.x & 31) == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[blockIdx.x * 8 + (i)] = t_; } } while (0)
-#define G2_STAMP(i) do { if (threadIdx.x == 0 && P.stamps) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.stamps[blockIdx.x * 8 + (i)] = t_; } } while (0)
-#else
-#define G2_STAMP(i) do { } while (0)
-#define G2_STAMPL(i) do { } while (0)
-#endif
-
 // CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
 template <int C, bool SIGN_MAG, int CPW>
 __global__ void __launch_bounds__(kG2Threads + 64, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
 const __grid_constant__ Gen2Params P) {
-    G2_STAMP(0);
     if (!P.input_ready) pdl_wait();
     constexpr int KG = 4 / CPW, RT = 32 * KG;                                 // row groups (K = 32 rows each) and rows per tile
     constexpr int DEPTH = G2Depth<C>::TILES, DIGD = G2Depth<C>::DIGITS;
@@ -331,7 +325,6 @@ const __grid_constant__ Gen2Params P) {
             it += nt;
             batch = nbatch; ++pos;
         }
-        G2_STAMPL(6);
         {   // terminator: the entry after the last tile carries "no tile"
             const uint32_t e = it % DIGD, ph = (it / DIGD) & 1u;
             mbar_wait(dempty0 + 8 * e, ph ^ 1u);
@@ -385,7 +378,6 @@ const __grid_constant__ Gen2Params P) {
             cp_async_arrive_noinc(full0 + 8 * s);
             if (lane == 0) mbar_arrive(full0 + 8 * s);              // (release: what this warp has seen -- the digits -- is visible to whoever sees "full")
         }
-        G2_STAMPL(7);
     } else {
         // ---------------- consumers: warp cw owns chunks CPW cw .. CPW cw + CPW - 1 of every row ----------------
         const int cw = warp - 2, g = lane >> 2, t = lane & 3;
@@ -468,9 +460,7 @@ const __grid_constant__ Gen2Params P) {
             if (lane == 0) { mbar_arrive(empty0 + 8 * s); mbar_arrive(dempty0 + 8 * e); }
         }
     }
-    G2_STAMP(1);
     __syncthreads();                  // every role is done: the ring becomes the per-position result array
-    G2_STAMP(2);
     const uint32_t seq = s_gen[0], slot = seq % kTailSlots;
     uint32_t* ctr = P.ctr + 2 * slot;
 
@@ -519,11 +509,9 @@ const __grid_constant__ Gen2Params P) {
         long long* dst = P.posacc + (size_t)slot * 2 * kG2Fields;
         for (uint32_t i = tid; i < nval; i += kG2Threads) { const long long v = pos_s[i]; if (v) red_add_s64(dst + i, v); }
     }
-    G2_STAMP(3);
     __syncthreads();                  // every thread's reds happen before thread 0's release below
     if (tid == 0) s_gen[3] = arrive_acq_rel(ctr + 1);
     __syncthreads();
-    G2_STAMP(4);
     if (s_gen[3] != gridDim.x - 1u) return;
 
     // ---- final stage (the CTA that arrived last): positions -> bins, ragged tail, accumulate into the context ----
@@ -588,7 +576,6 @@ const __grid_constant__ Gen2Params P) {
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
     __syncthreads();
     if (tid == 0) st_release_u32(&P.st->n_done, seq + 1u);             // P is final for this launch; the slot is free
-    G2_STAMP(5);
 }
 
 }  // namespace pcal

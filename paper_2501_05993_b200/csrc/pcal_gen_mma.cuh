@@ -1,39 +1,30 @@
-// pcal_gen_mma.cuh -- generator path for integer samples (int8, 2-bit) as a dense contraction on the
-// tensor cores (eq. 2.3 + 2.2 with the phasor of eq. 2.5).
+// pcal_gen_mma.cuh -- generator path for int8 samples as a dense contraction on the tensor cores (eq. 2.3 + 2.2 with the
+// phasor of eq. 2.5; BASELINE.json config 5).  (2-bit samples: pcal_gen2.cuh, the same algebra.)
 //
 // With the sample index written as n = n0 + 2^16 tile + 2048 row + pos (pos < 2048, row < 32),
 //     P[b] = sum_{pos = b mod N_bins} e^{-j w pos} * sum_{tile,row} x[tile,row,pos] * rho[tile,row],
 //     rho[tile,row] = e^{-j w (n0 + 2^16 tile)} * e^{-j w 2048 row}
 // (the k-shift algebra of PAPER.md:97: the position factor is applied once at the end).  The inner sum is
-// a matrix product  X^T (2048 positions x rows)  *  R (rows x {Re, Im})  -- a contraction over TIME with a
-// two-column right-hand side.  It runs as integer tensor-core MMAs (mma.sync m16n8k16 / m16n8k32, s8|u8 x s8 -> s32):
-// the phasor is quantised to 31-bit fixed point, round(rho 2^30) = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 with signed 8-bit
-// digits, and the eight digit columns (4 for Re, 4 for Im) fill the n = 8 side of the MMA.  All sums are exact
-// integers (int32 per digit column; |sum| < 2^31 for the <= 256 tiles a CTA sees per launch), recombined
-// and converted to fp64 once per launch.  The only approximation is the 2^-31 phasor quantisation
-// (~5e-10 of a typical bin).
+// a matrix product  X^T (2048 positions x rows)  *  R (rows x digit columns)  -- a contraction over TIME.  It runs as
+// integer tensor-core MMAs (mma.sync m16n8k16, s8 x s8 -> s32): the phasor is quantised to 31-bit fixed point,
+// round(rho 2^30) = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 with signed 8-bit digits, and the eight digit columns (4 for Re,
+// 4 for Im) fill the n = 8 side of the MMA.  All sums are exact integers (int32 per digit column; |sum| < 2^31 for the
+// <= 256 tiles a CTA sees per launch), recombined and converted to fp64 once per launch.  The only approximation is the
+// 2^-31 phasor quantisation (~5e-10 of a typical bin).
 //
 // Generator and resync.  rho[tile,row]: the tile factor comes from the exactly reduced INTEGER phase
 // ((n0 + 2^16 tile) F_off mod F_s, the "fp64 phase resync every 2^16 samples" of BASELINE.json config 5),
 // the row factor from a 32-entry table of exact stride phasors e^{-j w 2048 row} (stride stepping as in
 // eq. 2.8); one coupled-form complex multiply (eq. 2.6) per row in fp64, never more than 31 strides from
-// a resync point.  The 32 x 8 digit matrix of a tile is built with lane = row (int8: by every warp for itself; 2-bit:
-// by one warp per CTA, handed over by the per-tile barrier).
+// a resync point.  The 32 x 8 digit matrix of a tile is built by every warp for itself, lane = row.
 //
-// Data movement.  A row is 2048 positions (2048 B of int8, 512 B of 2-bit codes); warp w owns positions
-// 256 w .. 256 w + 255 and thread (g = lane/4, t = lane%4) 32 of them for 8 of the 32 rows.
-//   int8 : the two 16-byte blocks c = 0, 1 at 256 w + 128 c + 16 g of rows 16h + 4t + j, loaded by the thread itself into
-//          its own cp.async ring (no barrier; a warp instruction covers 4 rows x 128 contiguous bytes).
-//   2-bit: 8 bytes per row and thread would reach the memory system as half-line requests (measured: 2.3 TB/s), so the CTA
-//          stages whole tiles -- 16 KB of contiguous input, one full 512-byte row per cp.async instruction -- in shared
-//          memory (4 tiles, one barrier per tile) and the threads read their 8 bytes (two 16-sample words) with LDS.64.
-// The MMA wants four consecutive ROWS of one position in a register, memory has positions consecutive: a 4x4 byte
-// transpose (8 PRMT per 16 bytes) turns 4 row words into 4 position words.  2-bit words are transposed as PACKED bytes and
-// the fields are then used where they sit (unsigned operand, code * 4^field <= 192; the factor is shifted out exactly at
-// the end); they stay CODES 0..3: level = 2 code - 3, and the -3 sum(rho) term, which does not depend on the data, is added
-// once at the end from the same quantised phasors.  Rows past the end of the segment get zero digits, so whatever their
-// shared-memory slots hold contributes nothing.  ~1 instruction per sample instead of 3-4 for the FFMA2 kernel of
-// pcal_gen.cuh: HBM-bound at any SM clock for int8.
+// Data movement.  A row is 2048 positions (2048 B); warp w owns positions 256 w .. 256 w + 255 and thread
+// (g = lane/4, t = lane%4) 32 of them for 8 of the 32 rows: the two 16-byte blocks c = 0, 1 at 256 w + 128 c + 16 g of rows
+// 16h + 4t + j, loaded by the thread itself into its own cp.async ring (no barrier; a warp instruction covers 4 rows x
+// 128 contiguous bytes).  The MMA wants four consecutive ROWS of one position in a register, memory has positions
+// consecutive: a 4x4 byte transpose (8 PRMT per 16 bytes) turns 4 row words into 4 position words.  Rows past the end
+// of the segment get zero digits, so whatever their ring slots hold contributes nothing.  ~1.2 instructions per sample
+// instead of 3.75 for the FFMA2 kernel of pcal_gen.cuh: HBM-bound at any SM clock.
 #pragma once
 #include "pcal_gen.cuh"
 
@@ -45,12 +36,10 @@ constexpr uint32_t kMmaRows = kTileSamples / kMmaSpan; // 32 rows per tile
 template <int KIND> struct GenMmaCfg;
 // LB bytes per load; GPT commit groups (of 4 loads: 4 consecutive rows) per tile; DG groups in flight per thread
 template <> struct GenMmaCfg<KIND_I8>   { static constexpr int LB = 16, GPT = 4, DG = 4; };   // groups (h, block c)
-template <> struct GenMmaCfg<KIND_2BIT> { static constexpr int LB = 16, GPT = 1, DG = 4; };   // DG = tiles in the CTA's staging ring (see the kernel)
 
 template <int KIND>
 constexpr size_t gen_mma_smem_bytes() {
-    const size_t ring = KIND == KIND_2BIT ? (size_t)GenMmaCfg<KIND>::DG * kMmaRows * 544
-                                          : (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
+    const size_t ring = (size_t)GenMmaCfg<KIND>::DG * 4 * kThreads * GenMmaCfg<KIND>::LB;
     const size_t fin = (size_t)kMmaSpan * sizeof(double2);              // final per-position values alias the ring
     return (size_t)kGenMaxTiles * sizeof(double2) + (kMmaRows + 128 + 16) * sizeof(double2) + (size_t)kWarps * 256 + (ring > fin ? ring : fin);
 }
@@ -59,19 +48,6 @@ __device__ __forceinline__ void mma_s8_k16(int (&d)[4], uint32_t a0, uint32_t a1
     asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
                  : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
                  : "r"(a0), "r"(a1), "r"(b0));
-}
-
-// the same with an UNSIGNED left operand: 2-bit fields are used where they sit in the byte (code << 2f <= 192)
-__device__ __forceinline__ void mma_u8_k16(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
-                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
-                 : "r"(a0), "r"(a1), "r"(b0));
-}
-
-__device__ __forceinline__ void mma_u8_k32(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
-    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
-                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
 // rows r0..r3 (bytes = 4 positions each) -> o[p] = (r0.p, r1.p, r2.p, r3.p), byte 0 = row 0
@@ -94,7 +70,7 @@ __device__ __forceinline__ void cp_async_pred(void* smem_dst, const void* gsrc, 
     if (ok) cp_async_own<LB>(smem_dst, gsrc);
 }
 
-template <int KIND, bool SIGN_MAG>
+template <int KIND, bool SIGN_MAG>          // (KIND_I8, false: the only instantiation)
 __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_constant__ GenParams P) {
     pdl_release();
     if (!P.input_ready) pdl_wait();
@@ -113,7 +89,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
 
     const uint64_t n_rows = P.n_loads / (kMmaSpan / 16);                         // host loads = 16 samples; whole rows only (host guarantees a multiple)
     const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
-    int acc[2][2][4][4];          // [block c (int8) / word (2-bit)][word half or field half w2][byte b][C fragment]
+    int acc[2][2][4][4];          // [block c][word half w2][byte b][C fragment]
 #pragma unroll
     for (int c = 0; c < 2; ++c)
 #pragma unroll
@@ -122,11 +98,10 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             for (int b = 0; b < 4; ++b)
 #pragma unroll
                 for (int k = 0; k < 4; ++k) acc[c][w2][b][k] = 0;
-    long long s_re = 0, s_im = 0;     // sum over valid rows of the quantised phasors (2-bit: the -3 sum(rho) term)
 
     if constexpr (KIND == KIND_I8) {
     // this thread's loads of one tile, in consumption order: group-major, 4 consecutive rows per group
-    //   int8 : l = 8h + 4c + j -> row 16h + 4t + j, block c        2-bit: l = 4h + j -> row 16h + 4t + j
+    //   l = 8h + 4c + j -> row 16h + 4t + j, block c
     constexpr int GPT = GenMmaCfg<KIND>::GPT;
     const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
     const uint32_t col_off = (uint32_t)(warp * (ROW_BYTES / kWarps) + g * LB);
@@ -206,7 +181,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             bt[0 * 32 + lane] = (unsigned char)d0; bt[1 * 32 + lane] = (unsigned char)d1; bt[2 * 32 + lane] = (unsigned char)d2;
             bt[3 * 32 + lane] = (unsigned char)d3; bt[4 * 32 + lane] = (unsigned char)e0; bt[5 * 32 + lane] = (unsigned char)e1;
             bt[6 * 32 + lane] = (unsigned char)e2; bt[7 * 32 + lane] = (unsigned char)e3;
-            if (KIND == KIND_2BIT) { s_re += vre; s_im += vim; }      // this lane's rows; summed over the warp at the end
             __syncwarp();
         }
         const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt);
@@ -234,103 +208,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
             }
         }
     }
-    } else {
-    // ---- 2-bit: whole tiles staged by the CTA ----------------------------------------------------------------
-    // A tile (32 rows x 512 B) is 16 KB of CONTIGUOUS input.  Per-thread 8-byte loads of it would reach the memory
-    // system as half-line requests and stall at ~2.3 TB/s (measured), so the CTA copies the tile as it lies: warp w
-    // loads rows w, w+8, w+16, w+24, one full 512-byte row per cp.async instruction (16 B per lane), into a shared
-    // tile with a row pitch of 544 B; DEPTH-1 tiles are in flight, one barrier per tile.  A thread's MMA operand is
-    // then read with LDS.64; the k slot 16h + 4t + j of the MMA is given to row 16h + t + 4j (the digit matrix uses
-    // the same permutation), which together with the pitch makes those reads conflict-free.
-    constexpr uint32_t PITCH = 544, TILE_SM = kMmaRows * PITCH;
-    constexpr int DEPTH = GenMmaCfg<KIND_2BIT>::DG;
-    const unsigned char* gdata2 = reinterpret_cast<const unsigned char*>(P.data);
-    auto issue_tile = [&](uint32_t ti) {                      // ti = index among this CTA's tiles
-        if (ti < nt) {
-            const uint64_t tile = (uint64_t)blockIdx.x + (uint64_t)ti * gridDim.x;
-            const long long left = (long long)n_rows - (long long)tile * kMmaRows;
-            const uint32_t lim = left <= 0 ? 0u : (left < (long long)kMmaRows ? (uint32_t)left : kMmaRows);
-            const unsigned char* src = gdata2 + tile * TILE_BYTES + (uint32_t)lane * 16u;
-            unsigned char* dst = ring + (size_t)(ti % DEPTH) * TILE_SM + (uint32_t)lane * 16u;
-#pragma unroll
-            for (uint32_t k = 0; k < 4; ++k) {
-                const uint32_t row = (uint32_t)warp + 8u * k;
-                if (row < lim) cp_async_own<16>(dst + row * PITCH, src + row * ROW_BYTES);
-            }
-        }
-        cp_async_commit();
-    };
-#pragma unroll
-    for (uint32_t ti = 0; ti + 1 < (uint32_t)DEPTH; ++ti) issue_tile(ti);
-    // (the first loads are in flight: now the tables)
-    {   // resync table: the exactly reduced integer phase of every tile start of this CTA -> fp64 phasor
-        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
-        if (k_cta >= P.Fs) k_cta -= P.Fs;
-        for (uint32_t i = tid; i < nt; i += kThreads) {
-            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
-            if (k >= P.Fs) k -= P.Fs;
-            base[i] = phasor_neg(k, P.Fs);
-        }
-        // (the last 32 threads: the first ones are busy with the tile phasors above)
-        if (tid >= kThreads - (int)kMmaRows) { const int r = tid - (kThreads - (int)kMmaRows); rtab[r] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)r * kMmaSpan, P.Fs), P.Fs); }
-        // position factors exp(-j w pos), pos = 16 a + b, for the epilogue: threads 64 .. 207, exactly reduced as well
-        if (tid >= 64 && tid < 64 + 128) twA[tid - 64] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 64) * 16u, P.Fs), P.Fs);
-        if (tid >= 192 && tid < 192 + 16) twB[tid - 192] = phasor_neg(mulmod_u64(P.Foff, (uint64_t)(tid - 192), P.Fs), P.Fs);
-    }
-    __syncthreads();
-
-    // digit matrix of this CTA's tile ti, built by ONE warp (lane = row, stored at its k slot) into buffer ti & 1; the
-    // per-tile barrier hands it to the other warps.  s_re/s_im collect the quantised phasors of the rows this lane built.
-    auto build_digits = [&](uint32_t ti) {
-        if (ti >= nt) return;
-        const long long rows_left = (long long)n_rows - ((long long)blockIdx.x + (long long)ti * gridDim.x) * kMmaRows;
-        const double2 b0 = base[ti], r = rtab[lane];
-        const bool valid = (long long)lane < rows_left;
-        const int vre = valid ? __double2int_rn((b0.x * r.x - b0.y * r.y) * 1073741824.0) : 0;
-        const int vim = valid ? __double2int_rn((b0.x * r.y + b0.y * r.x) * 1073741824.0) : 0;
-        int d0, d1, d2, d3, e0, e1, e2, e3;
-        digits4(vre, d0, d1, d2, d3); digits4(vim, e0, e1, e2, e3);
-        const int ks = (lane & 16) + 4 * (lane & 3) + ((lane >> 2) & 3);      // row 16h + t + 4j -> slot 16h + 4t + j
-        unsigned char* b = bt_all + (ti & 1u) * 256u;
-        b[0 * 32 + ks] = (unsigned char)d0; b[1 * 32 + ks] = (unsigned char)d1; b[2 * 32 + ks] = (unsigned char)d2;
-        b[3 * 32 + ks] = (unsigned char)d3; b[4 * 32 + ks] = (unsigned char)e0; b[5 * 32 + ks] = (unsigned char)e1;
-        b[6 * 32 + ks] = (unsigned char)e2; b[7 * 32 + ks] = (unsigned char)e3;
-        s_re += vre; s_im += vim;
-    };
-    if (warp == 0) build_digits(0);
-
-    for (uint32_t i = 0; i < nt; ++i) {
-        cp_async_wait<DEPTH - 2>();       // this thread's part of tile i has landed ...
-        __syncthreads();                  // ... everybody's has, the digits of tile i are there, everybody is done with tile i-1
-        issue_tile(i + DEPTH - 1);        // into the buffer of tile i-1
-        if (warp == (int)((i + 1) % kWarps)) build_digits(i + 1);      // for the next tile, into the other digit buffer
-        const uint32_t* bt32 = reinterpret_cast<const uint32_t*>(bt_all + (i & 1u) * 256u);
-        const uint32_t bf[2] = {bt32[g * 8 + t], bt32[g * 8 + 4 + t]};
-        const unsigned char* tile = ring + (size_t)(i % DEPTH) * TILE_SM + (uint32_t)(warp * 64 + g * 8);
-        // both k halves (rows 0..15 and 16..31) go into ONE m16n8k32 MMA: same issue cost as k16 on this GPU (8 cycles)
-        uint2 v[2][4];
-#pragma unroll
-        for (int h = 0; h < 2; ++h)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                v[h][j] = *reinterpret_cast<const uint2*>(tile + (uint32_t)(16 * h + t + 4 * j) * PITCH);
-                if (SIGN_MAG) { v[h][j].x = signmag_to_offset_binary(v[h][j].x); v[h][j].y = signmag_to_offset_binary(v[h][j].y); }
-            }
-#pragma unroll
-        for (int w = 0; w < 2; ++w) {
-            // transpose the PACKED bytes first (a byte = 4 samples of one row), then use the fields where they sit:
-            // Tp[b] = byte b of the 4 rows; field f of it = 4 rows of sample 4 b + f, scaled by 4^f (shifted out at the end)
-            uint32_t T0[4], T1[4];
-            transpose4x4_bytes(w ? v[0][0].y : v[0][0].x, w ? v[0][1].y : v[0][1].x, w ? v[0][2].y : v[0][2].x, w ? v[0][3].y : v[0][3].x, T0);
-            transpose4x4_bytes(w ? v[1][0].y : v[1][0].x, w ? v[1][1].y : v[1][1].x, w ? v[1][2].y : v[1][2].x, w ? v[1][3].y : v[1][3].x, T1);
-#pragma unroll
-            for (int f2 = 0; f2 < 2; ++f2)
-#pragma unroll
-                for (int b = 0; b < 4; ++b)
-                    mma_u8_k32(acc[w][f2][b], T0[b] & (0x03030303u << (2 * f2)), T0[b] & (0x30303030u << (2 * f2)),
-                               T1[b] & (0x03030303u << (2 * f2)), T1[b] & (0x30303030u << (2 * f2)), bf[0], bf[1]);
-        }
-    }
     }
     cp_async_wait<0>();
     __syncthreads();                  // the ring is free: it becomes the per-position result array
@@ -342,16 +219,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     int* dump = reinterpret_cast<int*>(ring);               // [64][kThreads]
     double* pos_re = reinterpret_cast<double*>(ring);      // [2048]
     double* pos_im = pos_re + kMmaSpan;
-    if (KIND == KIND_2BIT) {              // every tile's digits were built by one warp: add lanes, then warps
-        __shared__ long long s_sum[2][kWarps];
-#pragma unroll
-        for (int s = 16; s > 0; s >>= 1) { s_re += __shfl_xor_sync(0xFFFFFFFFu, s_re, s); s_im += __shfl_xor_sync(0xFFFFFFFFu, s_im, s); }
-        if (lane == 0) { s_sum[0][warp] = s_re; s_sum[1][warp] = s_im; }
-        __syncthreads();
-        s_re = 0; s_im = 0;
-#pragma unroll
-        for (int ww = 0; ww < kWarps; ++ww) { s_re += s_sum[0][ww]; s_im += s_sum[1][ww]; }
-    }
 #pragma unroll
     for (int c = 0; c < 2; ++c)
 #pragma unroll
@@ -381,12 +248,9 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
         const int idx = 4 * m + t, half = idx & 1, b = (idx >> 1) & 3, w2 = (idx >> 3) & 1, c = idx >> 4;
-        const int wsel = w2 + 2 * half;                     // word (int8) / field (2-bit) of the block
-        uint32_t pos;
-        if (KIND == KIND_I8) pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
-        else pos = 4u * (uint32_t)(warp * 64 + g * 8 + c * 4 + b) + (uint32_t)wsel;      // c = word of the 8 bytes
-        long long pre = fre[m], pim = fim[m];
-        if (KIND == KIND_2BIT) { pre = 2 * (pre >> (2 * wsel)) - 3 * s_re; pim = 2 * (pim >> (2 * wsel)) - 3 * s_im; }   // undo 4^field
+        const int wsel = w2 + 2 * half;                     // word of the block
+        const uint32_t pos = (uint32_t)(warp * 256 + c * 128 + g * 16 + 4 * wsel + b);
+        const long long pre = fre[m], pim = fim[m];
         pos_re[pos] = (double)pre * (1.0 / 1073741824.0);
         pos_im[pos] = (double)pim * (1.0 / 1073741824.0);
     }
