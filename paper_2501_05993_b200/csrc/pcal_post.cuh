@@ -331,9 +331,11 @@ __global__ void __launch_bounds__(kDftThreads) dft_kernel(const double2* __restr
 //     X[k1 + N1 k2] = sum_{b2 < N2} Y[k1][b2] W[(N1 k2 b2) mod N]
 // -- N (N1 + N2) complex MACs per channel instead of N^2, every twiddle taken from the table at an index reduced in
 // integers, every sum in a fixed order.  All n_ch channels at once (one thread per output).  sP, sY: [n_ch][N] each in
-// shared memory (sY is scratch, laid out [b2][k1] per channel); all threads of the CTA call it.
+// shared memory (sY is scratch, laid out [b2][k1] per channel); all threads of the CTA call it.  With sOut != null the tones
+// are left there ([n_ch][N] in shared memory; may be sP) instead of being stored, for a caller that is not yet allowed to.
 __device__ __forceinline__ void dft_in_cta(const double2* sP, double2* sY, const double2* __restrict__ W, uint32_t n_ch, uint32_t N,
-                                           uint32_t N1, uint32_t k_shift, double2* T_dev, double2* T_host, uint32_t nthreads) {
+                                           uint32_t N1, uint32_t k_shift, double2* T_dev, double2* T_host, uint32_t nthreads,
+                                           double2* sOut = nullptr) {
     const uint32_t N2 = N / N1, tid = threadIdx.x, total = n_ch * N;
     for (uint32_t oo = tid; oo < total; oo += nthreads) {
         const uint32_t c = oo / N, o = oo % N;
@@ -366,6 +368,7 @@ __device__ __forceinline__ void dft_in_cta(const double2* sP, double2* sY, const
             idx += step; if (idx >= N) idx -= N;
         }
         const uint32_t i = c * N + (o + k_shift) % N;
+        if (sOut) { sOut[i] = make_double2(re, im); continue; }
         T_dev[i] = make_double2(re, im);
         if (T_host) T_host[i] = make_double2(re, im);
     }

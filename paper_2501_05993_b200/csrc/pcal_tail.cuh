@@ -267,6 +267,10 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     const uint32_t n_tail = (uint32_t)(T.n_total - T.NT);
     double* s_re = scratch;                                  // [kThreads]
     double* s_im = scratch + kThreads;                       // [kThreads]
+    // A single finisher that OVERWRITES the bins and takes the DFT (one integration period per launch: pcal_integrate, series)
+    // needs nothing from the earlier launches: it forms P and T first and only then waits for its turn to store them, so that
+    // consecutive periods are serialised on a handful of stores instead of on the whole stage.  (<= 128 pairs: one trip below.)
+    const bool early = S == 1u && T.overwrite && T.fuse_dft;
     bool waited = false;
     for (uint32_t pp0 = pair_lo; pp0 < pair_hi || !waited; pp0 += ppc) {        // uniform trip count; at least one trip (the wait)
         const uint32_t pp = pp0 + e0;
@@ -304,6 +308,22 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
                 if (L > 1 && ++k == L) k = 0;
             }
         }
+        if (early) {
+            double2* sP = reinterpret_cast<double2*>(scratch + 2 * kThreads);
+            if (mine) sP[pp] = make_double2(are, aim);
+            __syncthreads();
+            dft_in_cta(sP, sP + pairs, T.W, T.C, T.n_bins, T.dft_n1, T.k_shift % T.n_bins, nullptr, nullptr, kThreads, sP);
+            wait_for_P(); waited = true;
+            if (mine) {
+                T.P[pp] = make_double2(are, aim);
+                if (T.integer_exact) T.Pint[pp] = (long long)are;
+                if (T.P_copy) T.P_copy[pp] = make_double2(are, aim);
+                const double2 t = sP[pp];
+                T.T_dev[pp] = t;
+                if (T.T_host) T.T_host[pp] = t;
+            }
+            continue;
+        }
         if (!waited) { wait_for_P(); waited = true; }        // every thread of the CTA, once
         if (!mine) continue;
         long long ai = (long long)are;     // exact: unrotated integer sums are integers below 2^53
@@ -325,7 +345,7 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
         __syncthreads();
         if (s_prev != S - 1u) return;
     }
-    if (T.fuse_dft) {   // T[c] = DFT(P[c]), every channel at once, from shared memory
+    if (T.fuse_dft && !early) {   // T[c] = DFT(P[c]), every channel at once, from shared memory
         double2* sP = reinterpret_cast<double2*>(S > 1u ? scratch : scratch + 2 * kThreads);
         double2* sY = sP + pairs;
         if (S > 1u) {
