@@ -182,11 +182,11 @@ def test_start_index_and_add_folded_time_sharding(oracle):
     assert_close(a.finalize()[0], oracle_tones(oracle, w, host, 0), "time-sharded")
 
 
-@pytest.mark.parametrize("idx", [2, 5])
-def test_k_shift_unshifts_to_natural_order(oracle, idx):
+@pytest.mark.parametrize("idx,rot", [(2, None), (5, None), (2, "generator"), (3, "generator")])
+def test_k_shift_unshifts_to_natural_order(oracle, idx, rot):
     """rotate by w_off + k w_comb, reorder the bins back."""
-    w, dev, host = make(idx, 600_004 if idx == 2 else 500_000)
-    p, T, P = gpu_run(w, dev, k_shift=w.n_bins // 4)
+    w, dev, host = make(idx, 500_000 if idx == 5 else 600_004)
+    p, T, P = gpu_run(w, dev, k_shift=w.n_bins // 4, rotator=rot)
     assert p.info().k_shift == w.n_bins // 4
     pr, pi = oracle_folded(oracle, w, host, 0)
     assert_close(T[0], oracle.dft(pr, pi), f"k-shift cfg{idx}")
@@ -203,11 +203,40 @@ def test_bitwise_determinism():
         assert np.array_equal(P1.view(np.uint64), P2.view(np.uint64))
 
 
-@pytest.mark.parametrize("idx,n", [(2, 4), (2, 60), (2, 64), (2, 68), (5, 1), (5, 15), (5, 16), (5, 17),
-                                   (1, 1), (1, 3), (1, 4), (1, 5), (4, 1), (4, 3), (4, 4), (4, 5), (3, 2052)])
-def test_tiny_and_ragged_lengths(oracle, idx, n):
-    """Segments shorter than / equal to / just above one 16-byte vector (tail-only and 1-vector paths)."""
+def test_bitwise_determinism_under_dynamic_tile_claims():
+    """pcal_gen2.cuh hands a quarter of its tiles out through a device counter: which CTA gets which tile differs from run to
+    run, the result must not (the per-position sums are exact integers, added with integer atomics).  60e6 samples = 915
+    tiles = 229 batches, 81 of them claimed; also with the stream cut where the second piece starts in the middle of a row,
+    and with other work keeping some SMs busy when the kernel starts."""
+    w = synth.config(3).scaled(60_000_004)
+    dev = synth.generate(w, DEV)
+    ref = None
+    for trial in range(4):
+        if trial >= 2:      # unrelated kernels in flight on another stream: some CTAs start late and claim fewer tiles
+            side = torch.cuda.Stream()
+            with torch.cuda.stream(side):
+                junk = torch.randn(64 << 20, device=DEV)
+                for _ in range(3):
+                    junk = junk * 1.0001 + 1.0
+        _, T, P = gpu_run(w, dev, rotator="generator", splits=(20_000_128 + 64 * trial * 0,))
+        torch.cuda.synchronize()
+        if ref is None:
+            ref = (T.copy(), P.copy())
+        assert np.array_equal(T.view(np.uint64), ref[0].view(np.uint64)), trial
+        assert np.array_equal(P.view(np.uint64), ref[1].view(np.uint64)), trial
+
+
+@pytest.mark.parametrize("idx,n,rot", [(2, 4, None), (2, 60, None), (2, 64, None), (2, 68, None), (5, 1, None), (5, 15, None), (5, 16, None),
+                                       (5, 17, None), (1, 1, None), (1, 3, None), (1, 4, None), (1, 5, None), (4, 1, None), (4, 3, None),
+                                       (4, 4, None), (4, 5, None), (3, 2052, None),
+                                       (3, 4, "generator"), (3, 508, "generator"), (3, 512, "generator"), (3, 516, "generator"),
+                                       (3, 512 * 128 - 4, "generator"), (3, 512 * 128 + 4, "generator"), (2, 60, "generator"), (2, 516, "generator")])
+def test_tiny_and_ragged_lengths(oracle, idx, n, rot):
+    """Segments shorter than / equal to / just above one 16-byte vector (tail-only and 1-vector paths); for the generator
+    kernel of 2-bit samples: around one row (512 samples) and one tile (128 rows)."""
     w, dev, host = make(idx, n)
+    if rot:
+        w = synth.replace(w, rotator=rot)
     if dev.numel() * dev.element_size() < 16:  # keep the device buffer 16-byte aligned & readable
         pad = torch.zeros(16, dtype=torch.uint8, device=DEV)
         pad[: dev.numel() * dev.element_size()] = dev.view(torch.uint8)
@@ -566,8 +595,9 @@ def test_sharding_package_on_one_gpu(oracle):
             c.destroy()
 
 
-@pytest.mark.parametrize("idx,n", [(2, 2_000_004), (1, 700_001), (4, 150_003), (3, 1_500_004)])
-def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n):
+@pytest.mark.parametrize("idx,n,rot", [(2, 2_000_004, None), (1, 700_001, None), (4, 150_003, None), (3, 1_500_004, None),
+                                       (3, 9_000_004, "generator"), (2, 2_000_004, "generator")])
+def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n, rot):
     """Consecutive fold launches overlap (device-side sequence numbers instead of grid-wide waits, pcal_tail.cuh).  Many
     back-to-back integration periods over different inputs, each into its own pinned buffer, must equal the result of the
     same period run alone, bit for bit -- launched directly and replayed from a CUDA graph (frozen parameters: the ring
@@ -575,6 +605,8 @@ def test_pipelined_launches_stress_and_graph_replay(oracle, idx, n):
     from dataclasses import replace
     from paper_2501_05993_b200 import binding
     w = synth.config(idx).scaled(n)
+    if rot:
+        w = replace(w, rotator=rot)
     bufs = [synth.generate(replace(w, seed=w.seed + 31 * k), DEV) for k in range(3)]
     p = binding.from_workload(w)
     alone = []

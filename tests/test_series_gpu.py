@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("idx,n_per,n_periods,rot", [(2, 320_064, 5, None), (4, 40_004, 4, None), (5, 262_160, 3, None),
-                                                     (1, 100_004, 3, None), (3, 512_000, 3, "generator")])
+                                                     (1, 100_004, 3, None), (3, 512_000, 3, "generator"), (4, 40_064, 3, "generator")])
 def test_series_matches_per_period_oracle(oracle, idx, n_per, n_periods, rot):
     w = synth.config(idx).scaled(n_per * n_periods)
     if rot:
