@@ -404,7 +404,14 @@ static int prepare(pcal_ctx* c) {
         else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
         if (occ < 1) return PCAL_ERR_DEVICE;
         c->gen_grid = (uint32_t)(c->sm_count * occ);
-        CU(cudaMalloc(&c->d_gen_partial, (size_t)c->gen_grid * c->n_bins * sizeof(double2)));
+        // The fused tail pays while the partial bins of a launch are few (its finishing CTAs hold the slots of CTAs of the next
+        // launch, whose tile assignment is static); config 5 (296 CTAs x 1024 bins) keeps the separate post and DFT kernels.
+        c->gen_fused = !c->gen_mma && (uint64_t)c->gen_grid * c->n_bins <= (1u << 16);       // (FFMA2 kernel only)
+        CU(cudaMalloc(&c->d_gen_partial, (size_t)(c->gen_fused ? kTailSlots : 1) * c->gen_grid * c->n_bins * sizeof(double2)));
+        CU(cudaMalloc(&c->d_g2_ctr, kTailSlots * 2 * sizeof(uint32_t)));     // arrival counters of the generator tail
+        CU(cudaMalloc(&c->d_tail_state, sizeof(TailState)));
+        CU(cudaMemsetAsync(c->d_g2_ctr, 0, kTailSlots * 2 * sizeof(uint32_t), c->stream));
+        CU(cudaMemsetAsync(c->d_tail_state, 0, sizeof(TailState), c->stream));
     }
     c->prepared = true;
     return PCAL_OK;
@@ -564,8 +571,9 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
     uint64_t n_loads = n_bytes / load_bytes;
     if (c->gen_mma) n_loads -= n_loads % (kMmaSpan / spt);        // whole 2048-sample rows; the rest goes to the post kernel
     const uint64_t Fs = c->Fs, Fo = c->Feff[0];
-    if (n_loads) {
+    if (n_loads || c->gen_fused) {   // (fused tail: also for a piece without a complete load -- the kernel's last CTA adds the ragged tail)
         GenParams gp;
+        memset(&gp, 0, sizeof(gp));
         gp.data = data; gp.n_loads = n_loads;
         // FFMA2 kernel: a CTA iteration covers gen_span samples (a multiple of N_bins), a tile 2^16 / (kThreads * spt) iterations
         const uint64_t span = c->gen_mma ? (uint64_t)kThreads * spt : c->gen_span;
@@ -579,9 +587,18 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         gp.rho = phasor_neg_host(mulmod_host(span, Fo, Fs), Fs);
         gp.rho2 = phasor_neg_host(mulmod_host(2 * span, Fo, Fs), Fs);
         for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
-        gp.partial = c->d_gen_partial; gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
+        gp.n_bins = c->n_bins; gp.sign_mag = c->sign_mag;
         gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
         gp.input_ready = c->input_ready ? 1 : 0;
+        GenTailParams& tp = gp.tail;
+        tp.st = c->gen_fused ? c->d_tail_state : nullptr; tp.cnt = c->d_g2_ctr; tp.partial = c->d_gen_partial; tp.P = c->d_P;
+        tp.tail = data + n_loads * load_bytes;
+        tp.n0 = c->n_processed; tp.n_body = n_loads * spt; tp.n_total = n; tp.Fs = Fs; tp.Foff = Fo;
+        tp.n_bins = c->n_bins; tp.kind = c->kind; tp.sign_mag = c->sign_mag; tp.overwrite = c->zero_pending ? 1 : 0;
+        if (c->fuse_req) {
+            tp.fuse_dft = 1; tp.dft_n1 = dft_n1_of(c->n_bins); tp.k_shift = (uint32_t)c->k_shift; tp.W = c->d_W;
+            tp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; tp.T_host = c->fuse_out; tp.P_copy = c->fuse_P_copy;
+        }
         const size_t smem = c->gen_smem;
         prof_mark(c, st);
         if (c->gen_mma) launch_chain(gen_mma_kernel<KIND_I8, false>, c->gen_grid, kThreads, smem, st, gp);
@@ -591,14 +608,16 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         prof_mark(c, st);
         c->launches += 1;
     }
-    GenPostParams gr;
-    gr.partial = c->d_gen_partial; gr.P = c->d_P; gr.tail = data + n_loads * load_bytes;
-    gr.n0 = c->n_processed; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
-    gr.grid = n_loads ? c->gen_grid : 0; gr.n_bins = c->n_bins; gr.kind = c->kind; gr.sign_mag = c->sign_mag;
-    gr.overwrite = c->zero_pending ? 1 : 0;
-    launch_chain(post_gen_kernel, (c->n_bins + 31) / 32, kPostThreads, 0, st, gr);
+    if (!c->gen_fused) {
+        GenPostParams gr;
+        gr.partial = c->d_gen_partial; gr.P = c->d_P; gr.tail = data + n_loads * load_bytes;
+        gr.n0 = c->n_processed; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
+        gr.grid = n_loads ? c->gen_grid : 0; gr.n_bins = c->n_bins; gr.kind = c->kind; gr.sign_mag = c->sign_mag;
+        gr.overwrite = c->zero_pending ? 1 : 0;
+        launch_chain(post_gen_kernel, (c->n_bins + 31) / 32, kPostThreads, 0, st, gr);
+        c->launches += 1;
+    }
     c->zero_pending = false;
-    c->launches += 1;
     CU(cudaGetLastError());
     return PCAL_OK;
 }
@@ -736,6 +755,13 @@ static bool can_fuse_dft(const pcal_ctx* c) {
         return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) &&
                2 * (size_t)c->n_bins * c->C * sizeof(double2) + 2 * kG2Fields * sizeof(long long) <= ring;
     }
+    if (c->prepared && c->rot_eff == PCAL_ROT_GENERATOR) {
+        if (!c->gen_fused) return false;
+        // int8 / float32 generator kernels: the CTA that finishes last (pcal_gen_tail.cuh); bins, DFT scratch and the slice sums
+        // of the reduction in the kernel's dynamic shared memory
+        const uint32_t n1 = dft_n1_of(c->n_bins);
+        return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) && (2 * (size_t)c->n_bins + 512) * sizeof(double2) <= c->gen_smem;
+    }
     if (!(c->prepared && c->rot_eff == PCAL_ROT_LUT && c->fused)) return false;
     // the last finishing CTA of the fold kernel: two-stage DFT cheap enough for a serial stage, and 2 * C * N_bins complex
     // values (P and as much scratch) fit in the kernel's shared scratch (4096 / 2048 / 1024 doubles)
@@ -751,7 +777,7 @@ static int enqueue_dft(pcal_ctx* c, double2* second_dst) {
     const uint32_t opw = dft_opw(c), per_cta = kDftThreads / 32 * opw;
     launch_chain(dft_kernel, dim3((c->n_bins + per_cta - 1) / per_cta, c->C), kDftThreads, smem, c->stream,
                  (const double2*)c->d_P, (const double2*)c->d_W, c->d_T, second_dst, c->n_bins, (uint32_t)c->k_shift, opw,
-                 (c->rot_eff == PCAL_ROT_LUT && c->fused) || (c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) ? c->d_tail_state : (TailState*)nullptr,
+                 (c->rot_eff == PCAL_ROT_LUT && c->fused) || (c->rot_eff == PCAL_ROT_GENERATOR && (c->gen2 || c->gen_fused)) ? c->d_tail_state : (TailState*)nullptr,
                  can_fuse_dft(c) ? 1 : 0);
     c->launches += 1;
     CU(cudaGetLastError());

@@ -26,6 +26,7 @@ struct pcal_ctx {
     // generator-mode geometry
     uint32_t gen_grid, gen_spt, gen_span;   // (gen_span: samples per CTA iteration of the FFMA2 kernel, a multiple of N_bins)
     bool gen_mma;                   // int8 samples, N_bins | 2048: tensor-core generator kernel (pcal_gen_mma.cuh)
+    bool gen_fused;                 // int8 / float32 generator kernels: reduction, tail and DFT by their last CTAs (pcal_gen_tail.cuh)
     bool gen2;                      // 2-bit samples: warp-specialised tensor-core generator kernel (pcal_gen2.cuh)
     uint32_t g2_span_t, g2_chunks;  // ... its row: time samples, 16-byte chunks
     uint32_t g2_cpw, g2_rt;         // ... chunks per consumer warp (1, 2, 4), rows per tile (128, 64, 32)

@@ -25,6 +25,7 @@
 #pragma once
 #include <type_traits>
 #include "pcal_common.cuh"
+#include "pcal_gen_tail.cuh"
 
 namespace pcal {
 
@@ -40,7 +41,7 @@ struct GenParams {
     double2 rho;             // exp(-j w * kThreads*SPT): oscillator step per CTA iteration
     double2 rho2;            // rho^2 (from the exactly reduced phase of two steps)
     double2 tw[16];          // exp(-j w k), k = 0..15: post-twiddle within a load
-    double2* partial;        // [device] [cta][n_bins]
+    GenTailParams tail;      // reduction, ragged tail, accumulation (and DFT) by the CTA that finishes last (pcal_gen_tail.cuh)
     uint32_t n_bins;
     int sign_mag;
     int input_ready;              // caller promised the input is complete: stream it before pdl_wait()
@@ -151,9 +152,9 @@ constexpr size_t gen_smem_bytes() {
 }
 
 template <int KIND>
-__global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
-    pdl_release();
+__global__ void __launch_bounds__(kThreads, 2) gen_kernel(const __grid_constant__ GenParams P) {
     if (!P.input_ready) pdl_wait();
+    __shared__ uint32_t s_gen[4];
     constexpr int SPT = GenTraits<KIND>::SPT;
     constexpr int LB = GenCfg<KIND>::LB, LPT = GenCfg<KIND>::LPT, RUN = GenCfg<KIND>::RUN, DEPTH = GenCfg<KIND>::DEPTH;
     constexpr uint32_t SPAN = kThreads * SPT;                // samples per CTA iteration at most (a tile: LPT iterations, <= 2^16 samples)
@@ -171,19 +172,6 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
 
     // this CTA's tiles: T_i = blockIdx.x + i * gridDim.x, i < nt
     const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
-    // ---- resync table: the exactly reduced INTEGER phase of every tile start -> fp64 phasor ----
-    {
-        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
-        if (k_cta >= P.Fs) k_cta -= P.Fs;
-        for (uint32_t i = tid; i < nt; i += kThreads) {
-            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
-            if (k >= P.Fs) k -= P.Fs;
-            base[i] = phasor_neg(k, P.Fs);
-        }
-    }
-    const double2 theta = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * SPT, P.Fs), P.Fs);   // exp(-j w tid SPT)
-    __syncthreads();
-
     const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
     unsigned char* my_ring = ring + (size_t)tid * LB;
     constexpr size_t RING_STRIDE = (size_t)kThreads * LB;                // bytes between a thread's ring slots
@@ -205,6 +193,22 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
             cp_async_own<LB>(my_ring + (size_t)j * RING_STRIDE, gdata + off + j * LOAD_STRIDE);
         if (j & 1) cp_async_commit();                        // one commit group per pair of loads
     }
+    // (the first loads are in flight: now the ticket and the tables)
+    if (tid == kThreads - 1) { if (P.tail.st) gen_take_ticket(P.tail, s_gen); }      // (published by the barrier below)
+    // ---- resync table: the exactly reduced INTEGER phase of every tile start -> fp64 phasor ----
+    {
+        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
+        if (k_cta >= P.Fs) k_cta -= P.Fs;
+        for (uint32_t i = tid; i < nt; i += kThreads) {
+            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
+            if (k >= P.Fs) k -= P.Fs;
+            base[i] = phasor_neg(k, P.Fs);
+        }
+    }
+    const double2 theta = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * SPT, P.Fs), P.Fs);   // exp(-j w tid SPT)
+    __syncthreads();
+    pdl_release();            // the ticket is taken: the next launch may become resident
+
     const float rho_c = (float)P.rho.x, rho_s = (float)P.rho.y;
 
     // one tile; CHECK = false when this tile and the next one are complete (no per-load tests).
@@ -293,12 +297,16 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(GenParams P) {
 #pragma unroll
     for (int k = 0; k < SPT; ++k) { pos_re[tid * SPT + k] = zr[k]; pos_im[tid * SPT + k] = zi[k]; }
     __syncthreads();
-    pdl_wait();   // the partial bins of the previous launch may still be read by its post kernel
+    // fused tail (small grid x N_bins): ring slot of this launch; else slot 0, read by post_gen_kernel, whose previous
+    // reader must have finished
+    if (!P.tail.st) pdl_wait();
+    double2* partial = P.tail.st ? gen_partial_of(P.tail, s_gen) : P.tail.partial + (size_t)blockIdx.x * P.n_bins;
     for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
         double re = 0.0, im = 0.0;
         for (uint32_t pos = sb; pos < P.span; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
-        P.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
+        partial[sb] = make_double2(re, im);
     }
+    if (P.tail.st) gen_tail(P.tail, s_gen, reinterpret_cast<double2*>(gen_smem));
 }
 
 }  // namespace pcal

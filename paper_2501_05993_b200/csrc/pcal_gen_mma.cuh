@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_mma_kernel(const __grid_const
     for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
         double re = 0.0, im = 0.0;
         for (uint32_t pos = sb; pos < kMmaSpan; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
-        P.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
+        P.tail.partial[(size_t)blockIdx.x * P.n_bins + sb] = make_double2(re, im);
     }
 }
 

@@ -3,7 +3,7 @@
 //                       (the "binary tree stepping" the paper leaves to the host)
 //   rotate_fold_kernel  A[r] * exp(-j w_off r) folded to N_bins (eq. 2.3 + 2.2 after the reordering
 //                       of PAPER.md:200), ragged tail (< 1 vector), accumulate into the context
-//   post_gen_kernel     per-CTA generator partials -> bins, ragged tail, accumulate
+//   post_gen_kernel     per-CTA generator partials -> bins, ragged tail, accumulate (large N_bins; else pcal_gen_tail.cuh)
 //   dft_kernel          T[i] = sum_b P[b] exp(-j 2 pi i b / N_bins)
 // All sums run in a fixed order (no floating-point atomics): two runs give bit-identical results.
 #pragma once
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(kPostThreads) rotate_fold_kernel(RotateParams 
     if (P.integer_exact) P.Pint[pp] = ai;
 }
 
-// ---- generator path: per-CTA partial bins -> context bins ------------------------------------
+// ---- generator path, un-fused (large grid x N_bins: pcal_gen_tail.cuh explains): per-CTA partial bins -> context bins ------------------------------------
 struct GenPostParams {
     const double2* partial;  // [device] [grid][n_bins], bin index relative to the piece start
     double2* P;              // [device] [n_bins] accumulated into (or overwritten)
