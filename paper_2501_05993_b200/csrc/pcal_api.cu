@@ -285,7 +285,11 @@ static int prepare(pcal_ctx* c) {
                 // the shortest row with at least 8 chunks (one per consumer warp): few positions, few accumulators.  A row of
                 // more than 32 chunks (2048 fields) is served in column blocks of 32 chunks, one launch each.
                 const uint32_t lam_chunks = (uint32_t)(lam * (uint64_t)c->C / 64u);
-                const uint32_t m = lam_chunks >= 8u ? 1u : (8u + lam_chunks - 1u) / lam_chunks;
+                // Several channels: as many rows of <= 16 chunks as fit (the generator warp's work per tile is per channel and row).
+                const char* mc = getenv("PCAL_G2_CHUNKS");       // (tests: other row lengths)
+                uint32_t m = lam_chunks >= 8u ? 1u : (8u + lam_chunks - 1u) / lam_chunks;
+                if (c->C > 1 && 16u / lam_chunks > m) m = 16u / lam_chunks;
+                if (mc && (uint32_t)atoi(mc) / lam_chunks >= 1u) m = (uint32_t)atoi(mc) / lam_chunks;
                 c->gen2 = true;
                 c->g2_span_t = (uint32_t)lam * m;
                 c->g2_chunks = lam_chunks * m;
@@ -749,9 +753,9 @@ static bool can_fuse_dft(const pcal_ctx* c) {
     if (c->prepared && c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) {
         if (c->C > 4 || c->g2_blocks > 1) return false;   // several launches per piece
         // two-stage DFT in the last CTA: cheap enough to sit in the serial final stage, and P and the scratch fit behind the
-        // position sums in the tile ring
+        // position sums in the kernel's rings (everything before its barriers and bookkeeping words)
         const uint32_t n1 = dft_n1_of(c->n_bins);
-        const size_t ring = (c->C == 4 ? 4u : 5u) * (size_t)kG2StageBytes;
+        const size_t ring = c->gen_smem - 1024;
         return (uint64_t)c->n_bins * (n1 + c->n_bins / n1) <= (1u << 17) &&
                2 * (size_t)c->n_bins * c->C * sizeof(double2) + 2 * kG2Fields * sizeof(long long) <= ring;
     }

@@ -62,8 +62,20 @@ constexpr uint32_t kG2Invalid = 0xFFFFFFFFu;
 constexpr uint32_t kG2TabRows = 512, kG2TabLo = 256, kG2TabHi = 128;      // generator tables per channel: rows of a batch, lo, hi
 constexpr uint32_t kG2TabStride = kG2TabRows + kG2TabLo + kG2TabHi;
 
-// ring depths: sample tiles / digit matrices (the generator runs that far ahead of the consumers)
-template <int C> struct G2Depth { static constexpr int TILES = C == 4 ? 4 : 5, DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4); };
+// Shared memory of a CTA (two CTAs share an SM): ring of sample tiles | ring of digit matrices (the generator runs that far
+// ahead of the consumers) | the generator's row table of one batch (4 tiles; when it fits) | barriers and bookkeeping
+constexpr size_t kG2SmemBudget = 115712 - 256;                // (228 KB - 2 x 1 KB reserved) / 2, less the kernel's static variables
+template <int C, int CPW> struct G2Cfg {
+    static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
+    static constexpr int DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4);
+    static constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;             // digit matrices of a tile: [C][KG][8 columns][32 rows]
+    static constexpr uint32_t TAB_BYTES = (uint32_t)C * 4 * RT * 16;          // exp(-j w_c span_t r), r < rows of a batch
+    static constexpr size_t FIXED = (size_t)DIGITS * DIG_BYTES + 1024;
+    static constexpr bool FIT5 = 5 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
+    static constexpr bool TAB_SMEM = FIT5 || 4 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
+    static constexpr int TILES = FIT5 ? 5 : 4;
+    static constexpr size_t BYTES = (size_t)TILES * kG2StageBytes + FIXED + (TAB_SMEM ? TAB_BYTES : 0u);
+};
 
 struct Gen2Params {
     const unsigned char* data;     // [device] packed samples of this piece, 16-byte aligned
@@ -105,7 +117,7 @@ struct Gen2Params {
 
 template <int C, int CPW>
 constexpr size_t gen2_smem_bytes() {
-    return (size_t)G2Depth<C>::TILES * kG2StageBytes + (size_t)G2Depth<C>::DIGITS * C * (4 / CPW) * 256 + 1024;
+    return G2Cfg<C, CPW>::BYTES;
 }
 
 // ---- mbarrier / cp.async / ldmatrix helpers -----------------------------------------------------------------
@@ -176,13 +188,15 @@ template <int C, bool SIGN_MAG, int CPW>
 __global__ void __launch_bounds__(kG2Threads + 64, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
 const __grid_constant__ Gen2Params P) {
     if (!P.input_ready) pdl_wait();
-    constexpr int KG = 4 / CPW, RT = 32 * KG;                                 // row groups (K = 32 rows each) and rows per tile
-    constexpr int DEPTH = G2Depth<C>::TILES, DIGD = G2Depth<C>::DIGITS;
-    constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;                    // digit matrices of a tile: [C][KG][8 columns][32 rows]
+    using Cfg = G2Cfg<C, CPW>;
+    constexpr int KG = Cfg::KG, RT = Cfg::RT;
+    constexpr int DEPTH = Cfg::TILES, DIGD = Cfg::DIGITS;
+    constexpr uint32_t DIG_BYTES = Cfg::DIG_BYTES;
     extern __shared__ __align__(128) unsigned char g2_smem[];
     unsigned char* ring = g2_smem;                                            // [DEPTH] padded sample tiles
     unsigned char* dig = ring + (size_t)DEPTH * kG2StageBytes;                // [DIGD][C][KG][8][32]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(dig + (size_t)DIGD * DIG_BYTES);   // full, empty [DEPTH]; digfull, digempty [DIGD]; ticket
+    double2* tab_s = reinterpret_cast<double2*>(dig + (size_t)DIGD * DIG_BYTES);    // [C][4 tiles][4][RT / 4] row phasors of a batch (TAB_SMEM)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(dig + (size_t)DIGD * DIG_BYTES + (Cfg::TAB_SMEM ? Cfg::TAB_BYTES : 0u));   // full, empty [DEPTH]; digfull, digempty [DIGD]; ticket
     uint32_t* dig_tile = reinterpret_cast<uint32_t*>(bars + 2 * DEPTH + 2 * DIGD + 1);   // [DIGD] tile of a digit entry
     uint32_t* s_gen = dig_tile + DIGD;                                         // [0] sequence number, [1] dft_started seen, [3] arrival, [4], [5] first claims
     __shared__ long long s_rsum[kG2MaxCh][2];                                  // sum of the quantised phasors of this CTA's valid rows
@@ -213,18 +227,30 @@ const __grid_constant__ Gen2Params P) {
         // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
         // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
         // batch number past the end.
-        // Lane l builds rows 4l .. 4l+3 of a tile (row group l / 8, K slots 4 (l % 8) ..): the four digit bytes of a column
-        // are one 32-bit word of the B fragment.  Digit bytes of v: the low bytes of v, v1 = (v + 128) >> 8, v2 = (v1 + 128) >> 8,
-        // v3 = (v2 + 128) >> 8 (signed base-256 digits; columns 0..3 = Re, 4..7 = Im).
-        long long rs_re[C], rs_im[C];
+        // The four digit bytes of a column for rows 4q .. 4q+3 are one 32-bit word of the B fragment (row group q / 8, K slots
+        // 4 (q % 8) ..; columns 0..3 = Re digits, 4..7 = Im digits).
+        // Work items: (channel, four consecutive rows).  A tile has Q = RT / 4 row quads; lane l serves quad l % Q of channel
+        // k * (32 / Q) + l / Q, k = 0 .. KI-1 -- with rows of 8 C chunks (RT = 128 / C) that is one item per lane and tile
+        // whatever C is.  Digits: round(rho 2^30) = v in [-2^30, 2^30]; the bytes of (v + 0x80808080) ^ 0x80808080 ARE the four
+        // signed base-256 digits of v (adding 128 to every digit makes them unsigned bytes without carries; ^ 0x80 takes the
+        // 128 off again in two's complement), and a 4 x 4 byte transpose (8 PRMT) puts digit d of the four rows into the
+        // word of column d.  Rounding by the 1.5 * 2^52 addend (round to nearest even, as cvt.rni).
+        constexpr int Q = RT / 4, CHP = 32 / Q, KI = (C + CHP - 1) / CHP;
+        const int g_ch0 = lane / Q, g_quad = lane % Q;
+        // the row phasors of a batch, from shared memory (an L2 round trip per tile is what this warp cannot afford): row
+        // r = RT j + 4 q + i of channel c at [c][j][i][q], so that the lanes of a load are neighbours
+        if (Cfg::TAB_SMEM) {
+            for (int x = lane; x < C * 4 * RT; x += 32) {
+                const int c = x / (4 * RT), r = x % (4 * RT);
+                tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
+            }
+            __syncwarp();
+        }
+        long long rs_re[KI], rs_im[KI];
 #pragma unroll
-        for (int c = 0; c < C; ++c) { rs_re[c] = 0; rs_im[c] = 0; }
+        for (int k = 0; k < KI; ++k) { rs_re[k] = 0; rs_im[k] = 0; }
         auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
-        auto pack4 = [](int v0, int v1, int v2, int v3) {      // low bytes of four values, v0 in byte 0
-            return __byte_perm(__byte_perm((uint32_t)v0, (uint32_t)v1, 0x0040), __byte_perm((uint32_t)v2, (uint32_t)v3, 0x0040), 0x5410);
-        };
-        const bool g_active = 4 * lane < RT;                   // (KG < 4: the upper lanes have no rows)
-        const uint32_t g_word = (uint32_t)(lane >> 3) * 64u + (uint32_t)(lane & 7);       // word of (row group, column 0, K slots) in a channel's digits
+        const uint32_t g_word = (uint32_t)(g_quad >> 3) * 64u + (uint32_t)(g_quad & 7);   // word of (row group, column 0, K slots) in a channel's digits
         // The CTA's batch sequence: positions 0 .. n_static-1 are its own (index + position * grid: most of the launch,
         // no round trips), the rest are claims from the launch's counter.  Claims are two positions ahead -- the first two
         // were made by the ticket thread -- so a claim has two batches' time to come back.
@@ -234,24 +260,26 @@ const __grid_constant__ Gen2Params P) {
         bool have_seq = false;
         uint32_t* ctr = nullptr;
         const uint32_t dyn0 = P.n_static * gridDim.x;          // first claimed batch number
-        auto load_tabs = [&](uint32_t b, double2 (&thi)[C], double2 (&tlo)[C]) {
+        auto load_tabs = [&](uint32_t b, double2 (&thi)[KI], double2 (&tlo)[KI]) {
 #pragma unroll
-            for (int c = 0; c < C; ++c) {
-                const double2* tab = P.gtab + (size_t)c * kG2TabStride;
-                thi[c] = __ldg(tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
-                tlo[c] = __ldg(tab + kG2TabRows + (b & 255u));
+            for (int k = 0; k < KI; ++k) {
+                const int ch = k * CHP + g_ch0;
+                const double2* tab = P.gtab + (size_t)(ch < C ? ch : 0) * kG2TabStride;
+                thi[k] = __ldg(tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
+                tlo[k] = __ldg(tab + kG2TabRows + (b & 255u));
             }
         };
-        double2 thi[C], tlo[C];
+        double2 thi[KI], tlo[KI];
         load_tabs(batch, thi, tlo);
         while (batch < P.n_batches) {
             const uint32_t tile0 = batch * kG2Batch;
             const uint32_t nt = P.n_tiles - tile0 < kG2Batch ? P.n_tiles - tile0 : kG2Batch;
-            double2 base[C];                                    // batch phasor, scaled by 2^30
+            double2 base[KI];                                   // batch phasor of this lane's channels, scaled by 2^30
 #pragma unroll
-            for (int c = 0; c < C; ++c) {
-                base[c] = cmul(cmul(P.base0[c], thi[c]), tlo[c]);
-                base[c].x *= 1073741824.0; base[c].y *= 1073741824.0;
+            for (int k = 0; k < KI; ++k) {
+                const int ch = k * CHP + g_ch0;
+                base[k] = cmul(cmul(P.base0[ch < C ? ch : 0], thi[k]), tlo[k]);
+                base[k].x *= 1073741824.0; base[k].y *= 1073741824.0;
             }
             // the next batch of the sequence, and its table entries on their way while this batch is built
             uint32_t nbatch;
@@ -272,35 +300,39 @@ const __grid_constant__ Gen2Params P) {
             }
             load_tabs(nbatch, thi, tlo);
             // UJ tiles at a time: their (independent) phasor chains overlap
-            constexpr uint32_t UJ = C == 1 ? 4u : (C == 2 ? 2u : 1u);
+            constexpr uint32_t UJ = KI == 1 ? 4u : (KI == 2 ? 2u : 1u);
 #pragma unroll 1
             for (uint32_t j0 = 0; j0 < nt; j0 += UJ) {
-                uint32_t w[UJ][C][8];
-                if (g_active) {
+                uint32_t w[UJ][KI][8];
 #pragma unroll
-                    for (uint32_t ju = 0; ju < UJ; ++ju) {
-                        const uint32_t rb = (j0 + ju) * RT + 4u * (uint32_t)lane;             // first of this lane's rows in the batch
-                        const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
-                        const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
+                for (uint32_t ju = 0; ju < UJ; ++ju) {
+                    const uint32_t rb = (j0 + ju) * RT + 4u * (uint32_t)g_quad;           // first of this lane's rows in the batch
+                    const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
+                    const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
 #pragma unroll
-                        for (int c = 0; c < C; ++c) {
-                            int vr[4], vi[4];
+                    for (int k = 0; k < KI; ++k) {
+                        const int ch = k * CHP + g_ch0;
+                        const int chc = ch < C ? ch : 0;
+                        uint32_t vr[4], vi[4];
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const double2 rho = cmul(base[c], __ldg(P.gtab + (size_t)c * kG2TabStride + (rb + i) % kG2TabRows));
-                                vr[i] = (uint32_t)i < nv ? __double2int_rn(rho.x) : 0;
-                                vi[i] = (uint32_t)i < nv ? __double2int_rn(rho.y) : 0;
-                            }
-                            rs_re[c] += ((long long)vr[0] + vr[1]) + ((long long)vr[2] + vr[3]);
-                            rs_im[c] += ((long long)vi[0] + vi[1]) + ((long long)vi[2] + vi[3]);
-#pragma unroll
-                            for (int d = 0; d < 4; ++d) {
-                                w[ju][c][d] = pack4(vr[0], vr[1], vr[2], vr[3]);
-                                w[ju][c][4 + d] = pack4(vi[0], vi[1], vi[2], vi[3]);
-#pragma unroll
-                                for (int i = 0; i < 4; ++i) { vr[i] = (vr[i] + 128) >> 8; vi[i] = (vi[i] + 128) >> 8; }
-                            }
+                        for (int i = 0; i < 4; ++i) {
+                            const double2 row = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + ((j0 + ju) * 4 + i) * Q + g_quad]
+                                                              : __ldg(P.gtab + (size_t)chc * kG2TabStride + (rb + i) % kG2TabRows);
+                            const double2 rho = cmul(base[k], row);
+                            const int xr = __double2loint(rho.x + 6755399441055744.0), xi = __double2loint(rho.y + 6755399441055744.0);
+                            const bool ok = (uint32_t)i < nv;
+                            rs_re[k] += ok ? xr : 0; rs_im[k] += ok ? xi : 0;
+                            vr[i] = ok ? ((uint32_t)xr + 0x80808080u) ^ 0x80808080u : 0u;
+                            vi[i] = ok ? ((uint32_t)xi + 0x80808080u) ^ 0x80808080u : 0u;
                         }
+                        const uint32_t r01l = __byte_perm(vr[0], vr[1], 0x5140), r23l = __byte_perm(vr[2], vr[3], 0x5140);
+                        const uint32_t r01h = __byte_perm(vr[0], vr[1], 0x7362), r23h = __byte_perm(vr[2], vr[3], 0x7362);
+                        const uint32_t i01l = __byte_perm(vi[0], vi[1], 0x5140), i23l = __byte_perm(vi[2], vi[3], 0x5140);
+                        const uint32_t i01h = __byte_perm(vi[0], vi[1], 0x7362), i23h = __byte_perm(vi[2], vi[3], 0x7362);
+                        w[ju][k][0] = __byte_perm(r01l, r23l, 0x5410); w[ju][k][1] = __byte_perm(r01l, r23l, 0x7632);
+                        w[ju][k][2] = __byte_perm(r01h, r23h, 0x5410); w[ju][k][3] = __byte_perm(r01h, r23h, 0x7632);
+                        w[ju][k][4] = __byte_perm(i01l, i23l, 0x5410); w[ju][k][5] = __byte_perm(i01l, i23l, 0x7632);
+                        w[ju][k][6] = __byte_perm(i01h, i23h, 0x5410); w[ju][k][7] = __byte_perm(i01h, i23h, 0x7632);
                     }
                 }
 #pragma unroll
@@ -309,12 +341,14 @@ const __grid_constant__ Gen2Params P) {
                     if (j < nt) {
                         const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
                         mbar_wait(dempty0 + 8 * e, ph ^ 1u);          // the consumers are done with the entry's previous tile
-                        if (g_active) {
-                            uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES) + g_word;
+                        uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES) + g_word;
 #pragma unroll
-                            for (int c = 0; c < C; ++c)
+                        for (int k = 0; k < KI; ++k) {
+                            const int ch = k * CHP + g_ch0;
+                            if (ch < C) {
 #pragma unroll
-                                for (int col = 0; col < 8; ++col) dg[c * KG * 64 + col * 8] = w[ju][c][col];
+                                for (int col = 0; col < 8; ++col) dg[ch * KG * 64 + col * 8] = w[ju][k][col];
+                            }
                         }
                         if (lane == 0) dig_tile[e] = tile0 + j;
                         __syncwarp();
@@ -331,13 +365,14 @@ const __grid_constant__ Gen2Params P) {
             if (lane == 0) { dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
         }
 #pragma unroll
-        for (int c = 0; c < C; ++c) {
+        for (int k = 0; k < KI; ++k) {
 #pragma unroll
-            for (int sh = 16; sh > 0; sh >>= 1) {
-                rs_re[c] += __shfl_xor_sync(0xFFFFFFFFu, rs_re[c], sh);
-                rs_im[c] += __shfl_xor_sync(0xFFFFFFFFu, rs_im[c], sh);
+            for (int sh = Q / 2; sh > 0; sh >>= 1) {           // the lanes of a channel: Q consecutive ones
+                rs_re[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_re[k], sh);
+                rs_im[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_im[k], sh);
             }
-            if (lane == 0) { s_rsum[c][0] = rs_re[c]; s_rsum[c][1] = rs_im[c]; }
+            const int ch = k * CHP + g_ch0;
+            if (g_quad == 0 && ch < C) { s_rsum[ch][0] = rs_re[k]; s_rsum[ch][1] = rs_im[k]; }
         }
     } else if (warp == 0) {
         // ---------------- loader: copy each tile as it lies, 512 contiguous bytes per instruction ----------------
@@ -422,14 +457,13 @@ const __grid_constant__ Gen2Params P) {
             mbar_wait(full0 + 8 * s, ph);
             const uint32_t tile = dig_tile[e];
             const uint32_t* dg32 = reinterpret_cast<const uint32_t*>(dig + (size_t)e * DIG_BYTES);
-            uint32_t bf[KG][C][2];
-#pragma unroll
-            for (int kg = 0; kg < KG; ++kg)
+            auto load_bf = [&](int kg, uint32_t (&bf)[C][2]) {
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
-                    bf[kg][c][0] = dg32[(c * KG + kg) * 64 + g * 8 + t];
-                    bf[kg][c][1] = dg32[(c * KG + kg) * 64 + g * 8 + 4 + t];
+                    bf[c][0] = dg32[(c * KG + kg) * 64 + g * 8 + t];
+                    bf[c][1] = dg32[(c * KG + kg) * 64 + g * 8 + 4 + t];
                 }
+            };
             const uint32_t base = my + s * kG2StageBytes;
             if (nch == (uint32_t)CPW) {
                 // complete rows (the usual case): every operand load of the tile is issued before the first MMA
@@ -440,21 +474,27 @@ const __grid_constant__ Gen2Params P) {
                     for (int c = 0; c < CPW; ++c) ldsm_t8_x2(base + kg * kg_step + 16u * c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3]);
                 if (tile == kG2Invalid) break;
 #pragma unroll
-                for (int kg = 0; kg < KG; ++kg)
+                for (int kg = 0; kg < KG; ++kg) {
+                    uint32_t bf[C][2];
+                    load_bf(kg, bf);
 #pragma unroll
-                    for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf[kg]);
+                    for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf);
+                }
             } else {
                 if (tile == kG2Invalid) break;
 #pragma unroll
-                for (int kg = 0; kg < KG; ++kg)
+                for (int kg = 0; kg < KG; ++kg) {
+                    uint32_t bf[C][2];
+                    load_bf(kg, bf);
 #pragma unroll
                     for (int c = 0; c < CPW; ++c) {
                         if ((uint32_t)c < nch) {
                             uint32_t a0, a1, a2, a3;
                             ldsm_t8_x2(base + kg * kg_step + 16u * c, a0, a1, a2, a3);
-                            chunk_mma(c, a0, a1, a2, a3, bf[kg]);
+                            chunk_mma(c, a0, a1, a2, a3, bf);
                         }
                     }
+                }
             }
             __syncwarp();
             if (lane == 0) { mbar_arrive(empty0 + 8 * s); mbar_arrive(dempty0 + 8 * e); }
