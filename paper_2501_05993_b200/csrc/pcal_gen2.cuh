@@ -52,7 +52,7 @@
 namespace pcal {
 
 constexpr int kG2Consumers = 8;                               // consumer warps
-constexpr int kG2Threads = (kG2Consumers + 2) * 32;           // + loader + generator
+constexpr int kG2Threads = (kG2Consumers + 2) * 32;           // + loader + generator (a second generator warp: G2Cfg::THREADS)
 constexpr uint32_t kG2StageBytes = 18432;                     // a padded tile: 128 rows x 144 B (8 chunks) ... 32 rows x 528 B (32 chunks)
 constexpr uint32_t kG2Fields = 2048;                          // fields (positions) per row at most
 constexpr uint32_t kG2Batch = 4;                              // tiles per claim
@@ -69,6 +69,8 @@ template <int C, int CPW> struct G2Cfg {
     static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
     static constexpr int DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4);
     static constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;             // digit matrices of a tile: [C][KG][8 columns][32 rows]
+    // generator work items per tile and lane: (channel, row quad) pairs / 32; two generator warps when that is two or more
+    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = KI >= 2 ? 2 : 1, THREADS = (kG2Consumers + 1 + NG) * 32;
     static constexpr uint32_t TAB_BYTES = (uint32_t)C * 4 * RT * 16;          // exp(-j w_c span_t r), r < rows of a batch
     static constexpr size_t FIXED = (size_t)DIGITS * DIG_BYTES + 1024;
     static constexpr bool FIT5 = 5 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
@@ -191,6 +193,7 @@ const __grid_constant__ Gen2Params P) {
     using Cfg = G2Cfg<C, CPW>;
     constexpr int KG = Cfg::KG, RT = Cfg::RT;
     constexpr int DEPTH = Cfg::TILES, DIGD = Cfg::DIGITS;
+    constexpr int NG = Cfg::NG, NT = Cfg::THREADS;                            // generator warps, threads of the CTA
     constexpr uint32_t DIG_BYTES = Cfg::DIG_BYTES;
     extern __shared__ __align__(128) unsigned char g2_smem[];
     unsigned char* ring = g2_smem;                                            // [DEPTH] padded sample tiles
@@ -198,7 +201,7 @@ const __grid_constant__ Gen2Params P) {
     double2* tab_s = reinterpret_cast<double2*>(dig + (size_t)DIGD * DIG_BYTES);    // [C][4 tiles][4][RT / 4] row phasors of a batch (TAB_SMEM)
     uint64_t* bars = reinterpret_cast<uint64_t*>(dig + (size_t)DIGD * DIG_BYTES + (Cfg::TAB_SMEM ? Cfg::TAB_BYTES : 0u));   // full, empty [DEPTH]; digfull, digempty [DIGD]; ticket
     uint32_t* dig_tile = reinterpret_cast<uint32_t*>(bars + 2 * DEPTH + 2 * DIGD + 1);   // [DIGD] tile of a digit entry
-    uint32_t* s_gen = dig_tile + DIGD;                                         // [0] sequence number, [1] dft_started seen, [3] arrival, [4], [5] first claims
+    uint32_t* s_gen = dig_tile + DIGD;                                         // [0] sequence number, [1] dft_started seen, [3] arrival, [4], [5] first claims, [6], [7] next batch (second generator warp)
     __shared__ long long s_rsum[kG2MaxCh][2];                                  // sum of the quantised phasors of this CTA's valid rows
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t full0 = smem_u32(bars), empty0 = full0 + 8 * DEPTH, dfull0 = empty0 + 8 * DEPTH,
@@ -209,7 +212,7 @@ const __grid_constant__ Gen2Params P) {
             mbar_init(full0 + 8 * s, 33);                 // 32 cp.async arrivals of the loader + 1 plain arrival (it has seen the digits)
             mbar_init(empty0 + 8 * s, kG2Consumers);
         }
-        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, 1); mbar_init(dempty0 + 8 * e, kG2Consumers); }
+        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, NG); mbar_init(dempty0 + 8 * e, kG2Consumers); }
         mbar_init(seqbar, 1);
     }
     __syncthreads();
@@ -222,7 +225,8 @@ const __grid_constant__ Gen2Params P) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) acc[c][u][k] = 0;
 
-    if (warp == 1) {
+    if (warp >= 1 && warp <= NG) {
+        const int gw = warp - 1;                                  // generator warp gw serves items k = gw, gw + NG, ...
         // ---------------- generator: owns the CTA's tile sequence; digit matrices of a batch of tiles, lane = row ----------------
         // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
         // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
@@ -235,14 +239,16 @@ const __grid_constant__ Gen2Params P) {
         // signed base-256 digits of v (adding 128 to every digit makes them unsigned bytes without carries; ^ 0x80 takes the
         // 128 off again in two's complement), and a 4 x 4 byte transpose (8 PRMT) puts digit d of the four rows into the
         // word of column d.  Rounding by the 1.5 * 2^52 addend (round to nearest even, as cvt.rni).
-        constexpr int Q = RT / 4, CHP = 32 / Q, KI = (C + CHP - 1) / CHP;
-        const int g_ch0 = lane / Q, g_quad = lane % Q;
+        constexpr int Q = RT / 4, CHP = 32 / Q, KI = Cfg::KI / NG;            // (items of this warp)
+        const int g_ch0 = gw * CHP + lane / Q, g_quad = lane % Q;
+        constexpr int KS = NG * CHP;                                            // channel step from item to item
         // the row phasors of a batch, from shared memory (an L2 round trip per tile is what this warp cannot afford): row
         // r = RT j + 4 q + i of channel c at [c][j][i][q], so that the lanes of a load are neighbours
         if (Cfg::TAB_SMEM) {
-            for (int x = lane; x < C * 4 * RT; x += 32) {
-                const int c = x / (4 * RT), r = x % (4 * RT);
-                tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
+            for (int x = lane; x < KI * CHP * 4 * RT; x += 32) {
+                const int cl = x / (4 * RT), r = x % (4 * RT);
+                const int c = (cl / CHP) * KS + gw * CHP + cl % CHP;            // this warp's channels
+                if (c < C) tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
             }
             __syncwarp();
         }
@@ -263,7 +269,7 @@ const __grid_constant__ Gen2Params P) {
         auto load_tabs = [&](uint32_t b, double2 (&thi)[KI], double2 (&tlo)[KI]) {
 #pragma unroll
             for (int k = 0; k < KI; ++k) {
-                const int ch = k * CHP + g_ch0;
+                const int ch = k * KS + g_ch0;
                 const double2* tab = P.gtab + (size_t)(ch < C ? ch : 0) * kG2TabStride;
                 thi[k] = __ldg(tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
                 tlo[k] = __ldg(tab + kG2TabRows + (b & 255u));
@@ -277,7 +283,7 @@ const __grid_constant__ Gen2Params P) {
             double2 base[KI];                                   // batch phasor of this lane's channels, scaled by 2^30
 #pragma unroll
             for (int k = 0; k < KI; ++k) {
-                const int ch = k * CHP + g_ch0;
+                const int ch = k * KS + g_ch0;
                 base[k] = cmul(cmul(P.base0[ch < C ? ch : 0], thi[k]), tlo[k]);
                 base[k].x *= 1073741824.0; base[k].y *= 1073741824.0;
             }
@@ -285,6 +291,8 @@ const __grid_constant__ Gen2Params P) {
             uint32_t nbatch;
             if (pos + 1 < P.n_static) {
                 nbatch = blockIdx.x + (pos + 1) * gridDim.x;
+            } else if (gw != 0) {
+                nbatch = 0;           // (from warp 1, below)
             } else {
                 if (!have_seq) {      // (the ticket and its two claims have long arrived by now)
                     mbar_wait(seqbar, 0u);
@@ -297,6 +305,11 @@ const __grid_constant__ Gen2Params P) {
                 // a claimed batch is always processed: claiming stops with the first batch number past the end
                 pend[0] = pend[1]; pend[1] = kG2Invalid;
                 if (lane == 0 && nbatch < P.n_batches && pos + 3 - P.n_static < kG2CapBatches) pend[1] = dyn0 + atomicAdd(ctr, 1u);
+            }
+            if (NG > 1 && pos + 1 >= P.n_static) {      // the claimed part of the sequence is warp 1's: one named barrier per batch
+                if (gw == 0 && lane == 0) s_gen[6 + (pos & 1u)] = nbatch;
+                asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
+                nbatch = s_gen[6 + (pos & 1u)];
             }
             load_tabs(nbatch, thi, tlo);
             // UJ tiles at a time: their (independent) phasor chains overlap
@@ -311,7 +324,7 @@ const __grid_constant__ Gen2Params P) {
                     const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
 #pragma unroll
                     for (int k = 0; k < KI; ++k) {
-                        const int ch = k * CHP + g_ch0;
+                        const int ch = k * KS + g_ch0;
                         const int chc = ch < C ? ch : 0;
                         uint32_t vr[4], vi[4];
 #pragma unroll
@@ -344,13 +357,13 @@ const __grid_constant__ Gen2Params P) {
                         uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES) + g_word;
 #pragma unroll
                         for (int k = 0; k < KI; ++k) {
-                            const int ch = k * CHP + g_ch0;
+                            const int ch = k * KS + g_ch0;
                             if (ch < C) {
 #pragma unroll
                                 for (int col = 0; col < 8; ++col) dg[ch * KG * 64 + col * 8] = w[ju][k][col];
                             }
                         }
-                        if (lane == 0) dig_tile[e] = tile0 + j;
+                        if (gw == 0 && lane == 0) dig_tile[e] = tile0 + j;
                         __syncwarp();
                         if (lane == 0) mbar_arrive(dfull0 + 8 * e);
                     }
@@ -362,7 +375,7 @@ const __grid_constant__ Gen2Params P) {
         {   // terminator: the entry after the last tile carries "no tile"
             const uint32_t e = it % DIGD, ph = (it / DIGD) & 1u;
             mbar_wait(dempty0 + 8 * e, ph ^ 1u);
-            if (lane == 0) { dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
+            if (lane == 0) { if (gw == 0) dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
         }
 #pragma unroll
         for (int k = 0; k < KI; ++k) {
@@ -371,7 +384,7 @@ const __grid_constant__ Gen2Params P) {
                 rs_re[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_re[k], sh);
                 rs_im[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_im[k], sh);
             }
-            const int ch = k * CHP + g_ch0;
+            const int ch = k * KS + g_ch0;
             if (g_quad == 0 && ch < C) { s_rsum[ch][0] = rs_re[k]; s_rsum[ch][1] = rs_im[k]; }
         }
     } else if (warp == 0) {
@@ -415,8 +428,8 @@ const __grid_constant__ Gen2Params P) {
         }
     } else {
         // ---------------- consumers: warp cw owns chunks CPW cw .. CPW cw + CPW - 1 of every row ----------------
-        const int cw = warp - 2, g = lane >> 2, t = lane & 3;
-        if (warp == 2 && lane == 0) {
+        const int cw = warp - 1 - NG, g = lane >> 2, t = lane & 3;
+        if (cw == 0 && lane == 0) {
             // ticket: sequence number of this launch, derived on the device (pcal_tail.cuh, "Pipelining"); taken before the
             // loader lets the dependent grid start.  The slot's previous user (launch seq - kTailSlots) must have finished
             // before the slot's counters are touched.
@@ -506,8 +519,8 @@ const __grid_constant__ Gen2Params P) {
 
     // ---- epilogue: digit sums -> exact per-position int64 (re, im) * 2^30 -> red.add into the launch's accumulators ----
     long long* pos_s = reinterpret_cast<long long*>(ring);                  // [kG2Fields][2]
-    if (warp >= 2) {
-        const int cw = warp - 2, g = lane >> 2, t = lane & 3;
+    if (warp >= 1 + NG) {
+        const int cw = warp - 1 - NG, g = lane >> 2, t = lane & 3;
 #pragma unroll
         for (int c = 0; c < CPW; ++c) {
             // field sums from the combination sums (exact: every U is a sum of non-negative multiples of the S)
@@ -547,7 +560,7 @@ const __grid_constant__ Gen2Params P) {
     const uint32_t nval = 2u * 64u * P.chunks;                              // values of the positions that exist
     {
         long long* dst = P.posacc + (size_t)slot * 2 * kG2Fields;
-        for (uint32_t i = tid; i < nval; i += kG2Threads) { const long long v = pos_s[i]; if (v) red_add_s64(dst + i, v); }
+        for (uint32_t i = tid; i < nval; i += NT) { const long long v = pos_s[i]; if (v) red_add_s64(dst + i, v); }
     }
     __syncthreads();                  // every thread's reds happen before thread 0's release below
     if (tid == 0) s_gen[3] = arrive_acq_rel(ctr + 1);
@@ -559,7 +572,7 @@ const __grid_constant__ Gen2Params P) {
     uint32_t seen_done = 0, seen_dft = 0;
     if (tid == 0) { seen_done = ld_acquire_u32(&P.st->n_done); seen_dft = ld_acquire_u32(&P.st->dft_finished); }
     long long* gacc = P.posacc + (size_t)slot * 2 * kG2Fields;
-    for (uint32_t i = tid; i < nval; i += kG2Threads) { pos_s[i] = __ldcg(gacc + i); gacc[i] = 0; }     // and ready for the slot's next launch
+    for (uint32_t i = tid; i < nval; i += NT) { pos_s[i] = __ldcg(gacc + i); gacc[i] = 0; }     // and ready for the slot's next launch
     const uint32_t pairs = (uint32_t)C * P.n_bins, n_tail = (uint32_t)(P.n_total - P.n_body);
     double2* sP = reinterpret_cast<double2*>(ring + 2 * kG2Fields * sizeof(long long));               // [pairs] (fused DFT)
     const uint32_t dft_x = s_gen[1];
@@ -575,7 +588,7 @@ const __grid_constant__ Gen2Params P) {
         }
         __syncthreads();
     };
-    for (uint32_t pp0 = 0; pp0 < pairs; pp0 += kG2Threads) {          // uniform trip count
+    for (uint32_t pp0 = 0; pp0 < pairs; pp0 += NT) {          // uniform trip count
         const uint32_t pp = pp0 + tid;
         const bool mine = pp < pairs;
         const uint32_t c = mine ? pp / P.n_bins : 0u, b = mine ? pp % P.n_bins : 0u;
@@ -611,7 +624,7 @@ const __grid_constant__ Gen2Params P) {
     if (P.fuse_dft) {   // T[c] = DFT(P[c]), channel by channel, from shared memory
         __syncthreads();
         double2* sY = sP + pairs;
-        dft_in_cta(sP, sY, P.W, (uint32_t)C, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev, P.T_host, kG2Threads);
+        dft_in_cta(sP, sY, P.W, (uint32_t)C, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev, P.T_host, NT);
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
     __syncthreads();
