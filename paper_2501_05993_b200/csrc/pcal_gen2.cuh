@@ -185,6 +185,33 @@ template <int C> __device__ __forceinline__ constexpr uint32_t g2_mask(int u) {
 }
 template <int C> __device__ __forceinline__ constexpr int g2_chan(int u) { return C == 1 ? 0 : (C == 2 ? (u & 1) : u); }
 
+// Digit words of four consecutive rows of one channel: rho = base * row[i] (base carries the 2^30), v = round(rho) in
+// [-2^30, 2^30].  The addend 1.5 * 2^52 + 0x80808080 rounds to nearest even (as cvt.rni would) and leaves v + 0x80808080 in
+// the low word; its bytes ^ 0x80 ARE the four signed base-256 digits of v (adding 128 to every digit makes them unsigned
+// bytes without carries between them; ^ 0x80 takes the 128 off again in two's complement).  A 4 x 4 byte transpose (8 PRMT)
+// then puts digit d of the four rows into the word of column d (0..3 Re, 4..7 Im).  FULL: all four rows exist; else rows
+// i >= nv get zero digits.
+template <bool FULL>
+__device__ __forceinline__ void g2_item_digits(const double2 base, const double2 (&row)[4], uint32_t nv, uint32_t (&w)[8]) {
+    constexpr double kRound = 6755399441055744.0 + 2155905152.0;
+    uint32_t vr[4], vi[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double re = base.x * row[i].x - base.y * row[i].y, im = base.x * row[i].y + base.y * row[i].x;
+        vr[i] = (uint32_t)__double2loint(re + kRound) ^ 0x80808080u;
+        vi[i] = (uint32_t)__double2loint(im + kRound) ^ 0x80808080u;
+        if (!FULL && (uint32_t)i >= nv) { vr[i] = 0u; vi[i] = 0u; }
+    }
+    const uint32_t r01l = __byte_perm(vr[0], vr[1], 0x5140), r23l = __byte_perm(vr[2], vr[3], 0x5140);
+    const uint32_t r01h = __byte_perm(vr[0], vr[1], 0x7362), r23h = __byte_perm(vr[2], vr[3], 0x7362);
+    const uint32_t i01l = __byte_perm(vi[0], vi[1], 0x5140), i23l = __byte_perm(vi[2], vi[3], 0x5140);
+    const uint32_t i01h = __byte_perm(vi[0], vi[1], 0x7362), i23h = __byte_perm(vi[2], vi[3], 0x7362);
+    w[0] = __byte_perm(r01l, r23l, 0x5410); w[1] = __byte_perm(r01l, r23l, 0x7632);
+    w[2] = __byte_perm(r01h, r23h, 0x5410); w[3] = __byte_perm(r01h, r23h, 0x7632);
+    w[4] = __byte_perm(i01l, i23l, 0x5410); w[5] = __byte_perm(i01l, i23l, 0x7632);
+    w[6] = __byte_perm(i01h, i23h, 0x5410); w[7] = __byte_perm(i01h, i23h, 0x7632);
+}
+
 // CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
 template <int C, bool SIGN_MAG, int CPW>
 __global__ void __launch_bounds__(kG2Threads + 64, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
@@ -233,12 +260,8 @@ const __grid_constant__ Gen2Params P) {
         // batch number past the end.
         // The four digit bytes of a column for rows 4q .. 4q+3 are one 32-bit word of the B fragment (row group q / 8, K slots
         // 4 (q % 8) ..; columns 0..3 = Re digits, 4..7 = Im digits).
-        // Work items: (channel, four consecutive rows).  A tile has Q = RT / 4 row quads; lane l serves quad l % Q of channel
-        // k * (32 / Q) + l / Q, k = 0 .. KI-1 -- with rows of 8 C chunks (RT = 128 / C) that is one item per lane and tile
-        // whatever C is.  Digits: round(rho 2^30) = v in [-2^30, 2^30]; the bytes of (v + 0x80808080) ^ 0x80808080 ARE the four
-        // signed base-256 digits of v (adding 128 to every digit makes them unsigned bytes without carries; ^ 0x80 takes the
-        // 128 off again in two's complement), and a 4 x 4 byte transpose (8 PRMT) puts digit d of the four rows into the
-        // word of column d.  Rounding by the 1.5 * 2^52 addend (round to nearest even, as cvt.rni).
+        // Work items: (channel, four consecutive rows), g2_item_digits.  A tile has Q = RT / 4 row quads; lane l of generator
+        // warp gw serves quad l % Q of channels gw (32 / Q) + l / Q + k NG (32 / Q), k = 0 .. KI-1.
         constexpr int Q = RT / 4, CHP = 32 / Q, KI = Cfg::KI / NG;            // (items of this warp)
         const int g_ch0 = gw * CHP + lane / Q, g_quad = lane % Q;
         constexpr int KS = NG * CHP;                                            // channel step from item to item
@@ -252,10 +275,14 @@ const __grid_constant__ Gen2Params P) {
             }
             __syncwarp();
         }
-        long long rs_re[KI], rs_im[KI];
-#pragma unroll
-        for (int k = 0; k < KI; ++k) { rs_re[k] = 0; rs_im[k] = 0; }
         auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
+        // column sums of the digit matrices of this lane's items: the sum of the quantised phasors over the CTA's rows, which
+        // the level offset -3 of every sample needs (rows that do not exist have zero digits; four digits of at most 128 per tile and lane: no overflow)
+        int dsum[KI][8];
+#pragma unroll
+        for (int k = 0; k < KI; ++k)
+#pragma unroll
+            for (int d = 0; d < 8; ++d) dsum[k][d] = 0;
         const uint32_t g_word = (uint32_t)(g_quad >> 3) * 64u + (uint32_t)(g_quad & 7);   // word of (row group, column 0, K slots) in a channel's digits
         // The CTA's batch sequence: positions 0 .. n_static-1 are its own (index + position * grid: most of the launch,
         // no round trips), the rest are claims from the launch's counter.  Claims are two positions ahead -- the first two
@@ -280,6 +307,7 @@ const __grid_constant__ Gen2Params P) {
         while (batch < P.n_batches) {
             const uint32_t tile0 = batch * kG2Batch;
             const uint32_t nt = P.n_tiles - tile0 < kG2Batch ? P.n_tiles - tile0 : kG2Batch;
+            const bool all_rows = (uint64_t)(tile0 + kG2Batch) * RT <= P.n_rows;      // (all but the last batch of a piece)
             double2 base[KI];                                   // batch phasor of this lane's channels, scaled by 2^30
 #pragma unroll
             for (int k = 0; k < KI; ++k) {
@@ -320,32 +348,22 @@ const __grid_constant__ Gen2Params P) {
 #pragma unroll
                 for (uint32_t ju = 0; ju < UJ; ++ju) {
                     const uint32_t rb = (j0 + ju) * RT + 4u * (uint32_t)g_quad;           // first of this lane's rows in the batch
-                    const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
-                    const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
 #pragma unroll
                     for (int k = 0; k < KI; ++k) {
                         const int ch = k * KS + g_ch0;
                         const int chc = ch < C ? ch : 0;
-                        uint32_t vr[4], vi[4];
+                        double2 row[4];
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const double2 row = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + ((j0 + ju) * 4 + i) * Q + g_quad]
-                                                              : __ldg(P.gtab + (size_t)chc * kG2TabStride + (rb + i) % kG2TabRows);
-                            const double2 rho = cmul(base[k], row);
-                            const int xr = __double2loint(rho.x + 6755399441055744.0), xi = __double2loint(rho.y + 6755399441055744.0);
-                            const bool ok = (uint32_t)i < nv;
-                            rs_re[k] += ok ? xr : 0; rs_im[k] += ok ? xi : 0;
-                            vr[i] = ok ? ((uint32_t)xr + 0x80808080u) ^ 0x80808080u : 0u;
-                            vi[i] = ok ? ((uint32_t)xi + 0x80808080u) ^ 0x80808080u : 0u;
+                        for (int i = 0; i < 4; ++i)
+                            row[i] = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + ((j0 + ju) * 4 + i) * Q + g_quad]
+                                                   : __ldg(P.gtab + (size_t)chc * kG2TabStride + (rb + i) % kG2TabRows);
+                        if (all_rows) {
+                            g2_item_digits<true>(base[k], row, 4u, w[ju][k]);
+                        } else {
+                            const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
+                            const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
+                            g2_item_digits<false>(base[k], row, nv, w[ju][k]);
                         }
-                        const uint32_t r01l = __byte_perm(vr[0], vr[1], 0x5140), r23l = __byte_perm(vr[2], vr[3], 0x5140);
-                        const uint32_t r01h = __byte_perm(vr[0], vr[1], 0x7362), r23h = __byte_perm(vr[2], vr[3], 0x7362);
-                        const uint32_t i01l = __byte_perm(vi[0], vi[1], 0x5140), i23l = __byte_perm(vi[2], vi[3], 0x5140);
-                        const uint32_t i01h = __byte_perm(vi[0], vi[1], 0x7362), i23h = __byte_perm(vi[2], vi[3], 0x7362);
-                        w[ju][k][0] = __byte_perm(r01l, r23l, 0x5410); w[ju][k][1] = __byte_perm(r01l, r23l, 0x7632);
-                        w[ju][k][2] = __byte_perm(r01h, r23h, 0x5410); w[ju][k][3] = __byte_perm(r01h, r23h, 0x7632);
-                        w[ju][k][4] = __byte_perm(i01l, i23l, 0x5410); w[ju][k][5] = __byte_perm(i01l, i23l, 0x7632);
-                        w[ju][k][6] = __byte_perm(i01h, i23h, 0x5410); w[ju][k][7] = __byte_perm(i01h, i23h, 0x7632);
                     }
                 }
 #pragma unroll
@@ -360,7 +378,10 @@ const __grid_constant__ Gen2Params P) {
                             const int ch = k * KS + g_ch0;
                             if (ch < C) {
 #pragma unroll
-                                for (int col = 0; col < 8; ++col) dg[ch * KG * 64 + col * 8] = w[ju][k][col];
+                                for (int col = 0; col < 8; ++col) {
+                                    dg[ch * KG * 64 + col * 8] = w[ju][k][col];
+                                    dsum[k][col] = __dp4a((int)w[ju][k][col], 0x01010101, dsum[k][col]);
+                                }
                             }
                         }
                         if (gw == 0 && lane == 0) dig_tile[e] = tile0 + j;
@@ -379,13 +400,15 @@ const __grid_constant__ Gen2Params P) {
         }
 #pragma unroll
         for (int k = 0; k < KI; ++k) {
+            long long re = (long long)dsum[k][0] + ((long long)dsum[k][1] << 8) + ((long long)dsum[k][2] << 16) + ((long long)dsum[k][3] << 24);
+            long long im = (long long)dsum[k][4] + ((long long)dsum[k][5] << 8) + ((long long)dsum[k][6] << 16) + ((long long)dsum[k][7] << 24);
 #pragma unroll
             for (int sh = Q / 2; sh > 0; sh >>= 1) {           // the lanes of a channel: Q consecutive ones
-                rs_re[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_re[k], sh);
-                rs_im[k] += __shfl_xor_sync(0xFFFFFFFFu, rs_im[k], sh);
+                re += __shfl_xor_sync(0xFFFFFFFFu, re, sh);
+                im += __shfl_xor_sync(0xFFFFFFFFu, im, sh);
             }
             const int ch = k * KS + g_ch0;
-            if (g_quad == 0 && ch < C) { s_rsum[ch][0] = rs_re[k]; s_rsum[ch][1] = rs_im[k]; }
+            if (g_quad == 0 && ch < C) { s_rsum[ch][0] = re; s_rsum[ch][1] = im; }
         }
     } else if (warp == 0) {
         // ---------------- loader: copy each tile as it lies, 512 contiguous bytes per instruction ----------------
