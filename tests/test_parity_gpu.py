@@ -435,6 +435,35 @@ def test_every_power_of_two_channel_count(oracle, C, enc, rot):
     p.destroy()
 
 
+@pytest.mark.parametrize("chunks", [8, 16, 32])
+@pytest.mark.parametrize("C,enc", [(1, 0), (2, 1), (4, 0), (16, 1)])
+def test_generator_row_lengths(oracle, monkeypatch, C, enc, chunks):
+    """The 2-bit generator kernel with rows of 8, 16 and 32 sixteen-byte chunks (PCAL_G2_CHUNKS, read when the context is set
+    up): every combination of chunks per consumer warp, generator warps and items per generator lane, with the row table in
+    shared memory and without.  A length with a ragged last tile and a ragged tail; tones through the fused DFT."""
+    from paper_2501_05993_b200 import binding
+    monkeypatch.setenv("PCAL_G2_CHUNKS", str(chunks))
+    n = 1_300_004
+    rs = np.random.RandomState(4300 + 10 * C + chunks)
+    packed = rs.randint(0, 256, size=n * 2 * C // 8).astype(np.uint8)
+    offs = [1234.567 + 100321.0123 * c for c in range(C)]
+    p = binding.Pcal(64e6, 1e6, 0.0, 2, enc, C)
+    p.set_channel_offsets(offs)
+    p.set_rotator(binding.ROT_GENERATOR)
+    dev = torch.from_numpy(packed).cuda()
+    out = torch.empty((C, 64), dtype=torch.complex128).pin_memory()
+    p.integrate(dev.data_ptr(), n, out.data_ptr())
+    torch.cuda.synchronize()
+    assert p.info().rotator_in_effect == binding.ROT_GENERATOR
+    P = p.get_folded()
+    fmt = oracle.TWO_BIT_SIGN_MAG if enc else oracle.TWO_BIT_OFFSET_BINARY
+    for c in range(C):
+        pr, pi = oracle.fold_ld(packed, fmt, C, c, 0, 1, n, 0, 64e6, 1e6, offs[c], tabulated=False)
+        assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"C={C} chunks={chunks} ch{c} folded")
+        assert_close(out[c].numpy(), oracle.dft(pr, pi), f"C={C} chunks={chunks} ch{c} tones")
+    p.destroy()
+
+
 def test_exchange_step_in_one_launch(oracle):
     """What bench.py does per step with N ranks, emulated on one GPU: every "rank" folds its time shard at
     its absolute start index, the bins are gathered into one buffer (stand-in for the NCCL all-gather) and
