@@ -183,7 +183,19 @@ def roofline_of(key, w, step_s, isolated_us, floor_us, launches_per_step, pipe_p
     pipe = row.get("pipe") or "lop3"
     pipe_peak = (pipe_peaks or {}).get(pipe)
     alu_s = samples * ips / pipe_peak if (ips and pipe_peak) else None
+    # legacy tensor path of the generator kernels: warp-level IMMA per sample (from the kernels' tiling: gen2_kernel 4 x m16n8k32
+    # per 16 bytes x 32 rows = 2048 samples, times the passes over 8 / 16-channel words; gen_mma_kernel one m16n8k16 per 256)
+    kname = row.get("kernel") or ""
+    mma = None
+    if kname.startswith("gen2_kernel"):
+        mma = ("imma_k32", (1.0 / 512.0) * max(1, w.n_channels // 4))
+    elif kname.startswith("gen_mma_kernel"):
+        mma = ("imma_k16", 1.0 / 256.0)
+    mma_peak = (pipe_peaks or {}).get(mma[0]) if mma else None
+    mma_s = samples * mma[1] / mma_peak if mma_peak else None
     bound = "alu" if (alu_s is not None and alu_s > hbm_s) else "hbm"
+    if mma_s is not None and mma_s > max(hbm_s, alu_s or 0.0):
+        bound = "tensor"
     achieved_gbs = w.n_bytes / step_s / 1e9
     r = {"bound": bound, "kernel": row.get("kernel") or ("generator kernel" if rotator == "generator" else "fold kernel incl. fused tail"),
          "algorithmic_bytes_per_launch": w.n_bytes, "avg_launch_us": step_s * 1e6, "launches_per_step": launches_per_step,
@@ -191,6 +203,9 @@ def roofline_of(key, w, step_s, isolated_us, floor_us, launches_per_step, pipe_p
          "alu": None if alu_s is None else {
              "thread_instr_per_sample": ips, "pipe": pipe, "pipe_peak_thread_instr_per_s": pipe_peak, "bound_us": alu_s * 1e6,
              "frac": alu_s / step_s, "source": f"{KERNEL_TABLE} (ncu smsp__inst_executed.sum x 32 / samples) and pcal_pipe_probe"},
+         "tensor": None if mma_s is None else {
+             "warp_mma_per_sample": mma[1], "pipe": mma[0], "pipe_peak_warp_mma_per_s": mma_peak, "bound_us": mma_s * 1e6,
+             "frac": mma_s / step_s, "source": "MMA count from the kernel's tiling (DESIGN.md 5.2) and pcal_pipe_probe"},
          "traffic": int(row["dram_bytes_per_launch"]) if row.get("dram_bytes_per_launch") else None,
          "traffic_source": f"{KERNEL_TABLE}: dram__bytes_read.sum + dram__bytes_write.sum of one launch, committed ncu --set full capture "
                            "(profiles/r2_kernels.md), not measured in this run" if row.get("dram_bytes_per_launch") else None,
@@ -201,6 +216,8 @@ def roofline_of(key, w, step_s, isolated_us, floor_us, launches_per_step, pipe_p
                 "the same kernel bracketed by events launch by launch (serialised: the latency of one integration on its own)"}
     if bound == "hbm":
         r.update({"achieved": achieved_gbs, "peak": peak, "unit": "GB/s", "frac": achieved_gbs / peak})
+    elif bound == "tensor":
+        r.update({"achieved": samples * mma[1] / step_s, "peak": mma_peak, "unit": "warp-MMA/s", "frac": mma_s / step_s})
     else:
         r.update({"achieved": samples * ips / step_s, "peak": pipe_peak, "unit": "thread-instr/s", "frac": alu_s / step_s})
     if floor_us:
@@ -499,7 +516,7 @@ def main():
     # measured issue-rate ceilings of this GPU: the ALU side of every roofline object
     pipe_peaks = None
     if not args.quick:
-        pipe_peaks = {"ffma": _b.pipe_probe(0), "lop3": _b.pipe_probe(1), "imma_k16": _b.pipe_probe(2)}
+        pipe_peaks = {"ffma": _b.pipe_probe(0), "lop3": _b.pipe_probe(1), "imma_k16": _b.pipe_probe(2), "imma_k32": _b.pipe_probe(3)}
     res, w = measure(args.config, args.steps, args.warmup, rank, world, device, n_override=args.samples or None,
                      rotator=args.rotator, no_graph=args.no_graph, exchange=args.force_exchange, do_e2e=not args.quick,
                      min_warm_s=0.0 if args.quick else 0.5, pipe_peaks=pipe_peaks, ktab=ktab, regions=0 if args.quick else 5)
@@ -518,7 +535,7 @@ def main():
             "launches_per_step": res["launches_per_step"], "finalize_alone_us": res["finalize_alone_us"],
             "roofline": res["roofline"], "hot_kernel_us": res["hot_kernel_us"]}
     if world == 1 and rank == 0 and not args.quick:
-        line["pipe_peaks"] = dict(pipe_peaks, unit="thread-instr/s (ffma, lop3), warp-instr/s (imma_k16)",
+        line["pipe_peaks"] = dict(pipe_peaks, unit="thread-instr/s (ffma, lop3), warp-instr/s (imma_k16: m16n8k16 s8, imma_k32: m16n8k32 u8 x s8)",
                                   how="pcal_pipe_probe: 8 independent chains per thread, 8 CTAs x 256 threads per SM, best of 3")
         line["parity"] = parity_sample(w, device, min(w.n_samples, 1 << 24))
         # the oracle as it stands on this box's host cores: ~20 core-seconds on a bounded sample

@@ -27,8 +27,9 @@ int pcal_get_profile(pcal_ctx *ctx, double *hot_kernel_ms, uint64_t *hot_kernel_
 int pcal_read_probe(pcal_ctx *ctx, const void *dev, uint64_t n_bytes, void *cuda_stream);
 
 /* Calibration: the measured issue rate of one pipe of the current device.  kind 0 = FFMA (fp32 FMA pipe), 1 = LOP3
- * (integer/logic pipe), 2 = IMMA m16n8k16 s8 (the legacy tensor path of the generator kernels).  out_per_s [host]:
- * thread-instructions per second (kind 0, 1) or warp-level MMA instructions per second (kind 2) with every SM busy.
+ * (integer/logic pipe), 2 = IMMA m16n8k16 s8, 3 = IMMA m16n8k32 u8 x s8 (the legacy tensor path of the generator kernels: int8 / 2-bit).
+ * out_per_s [host]: thread-instructions per second (kind 0, 1) or warp-level MMA instructions per second (kind 2, 3) with
+ * every SM busy.
  * Synchronous, default stream, no context needed. */
 int pcal_pipe_probe(int kind, double *out_per_s);
 

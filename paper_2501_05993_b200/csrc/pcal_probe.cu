@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(kThreads, 3) read_probe_kernel(const uint4* __
 
 // ---- calibration: issue-rate ceilings of the pipes the kernels lean on ----------------
 // kind 0: FFMA (fp32 FMA pipe), 1: LOP3 (integer/logic pipe), 2: IMMA m16n8k16 s8 (legacy tensor path used by
-// gen_mma_kernel).  Eight independent dependency chains per thread, `iters` trips; the result is written so that
+// gen_mma_kernel), 3: IMMA m16n8k32 u8 x s8 (gen2_kernel).  Eight independent dependency chains per thread, `iters` trips; the result is written so that
 // nothing is optimised away.  The host times the launch and reports instructions per second.
 template <int KIND_P>
 __global__ void __launch_bounds__(kThreads) pipe_probe_kernel(uint32_t iters, uint32_t* out) {
@@ -49,8 +49,10 @@ __global__ void __launch_bounds__(kThreads) pipe_probe_kernel(uint32_t iters, ui
         for (int j = 0; j < 8; ++j) {
             if (KIND_P == 0) f[j] = __fmaf_rn(f[j], m, q);
             else if (KIND_P == 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[j]) : "r"(x), "r"(y));
-            else asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
+            else if (KIND_P == 2) asm volatile("mma.sync.aligned.m16n8k16.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
                               : "+r"(d[j][0]), "+r"(d[j][1]), "+r"(d[j][2]), "+r"(d[j][3]) : "r"(x), "r"(y), "r"(a[j]));
+            else asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                              : "+r"(d[j][0]), "+r"(d[j][1]), "+r"(d[j][2]), "+r"(d[j][3]) : "r"(x), "r"(y), "r"(x ^ y), "r"(y + 1u), "r"(a[j]), "r"(a[j] ^ x));
         }
     }
     uint32_t s = 0;
@@ -83,7 +85,7 @@ extern "C" int pcal_read_probe(pcal_ctx* c, const void* dev, uint64_t n_bytes, v
 }
 
 extern "C" int pcal_pipe_probe(int kind, double* out_per_s) {
-    if (!out_per_s || kind < 0 || kind > 2) return PCAL_ERR_INVALID;
+    if (!out_per_s || kind < 0 || kind > 3) return PCAL_ERR_INVALID;
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -97,7 +99,8 @@ extern "C" int pcal_pipe_probe(int kind, double* out_per_s) {
         cudaEventRecord(e0);
         if (kind == 0) pipe_probe_kernel<0><<<grid, kThreads>>>(iters, d_out);
         else if (kind == 1) pipe_probe_kernel<1><<<grid, kThreads>>>(iters, d_out);
-        else pipe_probe_kernel<2><<<grid, kThreads>>>(iters, d_out);
+        else if (kind == 2) pipe_probe_kernel<2><<<grid, kThreads>>>(iters, d_out);
+        else pipe_probe_kernel<3><<<grid, kThreads>>>(iters, d_out);
         cudaEventRecord(e1);
         if (cudaEventSynchronize(e1) != cudaSuccess) break;
         float ms = 0.f;
@@ -107,7 +110,7 @@ extern "C" int pcal_pipe_probe(int kind, double* out_per_s) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
     if (cudaGetLastError() != cudaSuccess || !(best < 1e29f)) return PCAL_ERR_DEVICE;
     const double per_thread = (double)iters * 8.0, threads = (double)grid * kThreads;
-    *out_per_s = (kind == 2 ? per_thread * threads / 32.0 : per_thread * threads) / (best * 1e-3);
+    *out_per_s = (kind >= 2 ? per_thread * threads / 32.0 : per_thread * threads) / (best * 1e-3);
     return PCAL_OK;
 }
 
