@@ -413,6 +413,10 @@ static int prepare(pcal_ctx* c) {
         else { c->gen_smem = gen_smem_bytes<KIND_F32>(); CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->gen_smem)); occ = occupancy_of(gen_kernel<KIND_F32>, c->gen_smem); }
         if (occ < 1) return PCAL_ERR_DEVICE;
         c->gen_grid = (uint32_t)(c->sm_count * occ);
+        // float32: one CTA per SM and launch (64 KB of loads in flight each): the CTAs of consecutive launches share the SMs, so the
+        // prologue and the tail of one launch hide under the streaming of the next (64 MB per step: 17 -> 12 us; 1 GB: 154 -> 150 us)
+        if (!c->gen_mma && c->kind == KIND_F32) c->gen_grid = (uint32_t)c->sm_count;
+        if (const char* gg = getenv("PCAL_GEN_GRID")) { if (!c->gen_mma && atoi(gg) > 0) c->gen_grid = (uint32_t)atoi(gg); }   // tuning runs only
         // The fused tail pays while the partial bins of a launch are few (its finishing CTAs hold the slots of CTAs of the next
         // launch, whose tile assignment is static); config 5 (296 CTAs x 1024 bins) keeps the separate post and DFT kernels.
         c->gen_fused = !c->gen_mma && (uint64_t)c->gen_grid * c->n_bins <= (1u << 16);       // (FFMA2 kernel only)
@@ -589,6 +593,7 @@ static int extract_piece_gen(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaS
         const uint64_t tile = c->gen_mma ? kTileSamples : gen_tile_samples(c);
         gp.span = (uint32_t)span;
         gp.n_tiles = (n_loads * spt + tile - 1) / tile;
+        gp.n_iters = (n_loads * spt + span - 1) / span;
         gp.Fs = Fs; gp.Foff = Fo;
         gp.k0 = mulmod_host(c->n_processed % Fs, Fo, Fs);
         gp.E = mulmod_host(tile, Fo, Fs);

@@ -16,9 +16,11 @@
 // the start of every 2^16-sample tile it is re-derived from the exactly reduced INTEGER phase
 // (n * F_off) mod F_s -- BASELINE.json config 5's "fp64 phase resync every 2^16 samples".
 //
-// Mapping: a CTA iteration covers kThreads*SPT consecutive samples (thread t owns samples
-// t*SPT .. t*SPT+SPT-1 of it); 65536/(kThreads*SPT) iterations form a tile; tiles are dealt
-// round-robin to CTAs.  N_bins must divide kThreads*SPT so every thread keeps fixed bins.
+// Mapping: a CTA iteration covers `span` consecutive samples (thread t owns samples
+// t*SPT .. t*SPT+SPT-1 of it; span = a multiple of lcm(N_bins, SPT), so every thread keeps fixed
+// bins).  gen_kernel: the piece's iterations are split into gridDim.x equal contiguous ranges (a
+// short piece still loads every SM alike), a range is walked in tiles of 65536/(kThreads*SPT)
+// iterations, the last one partial.  gen_mma_kernel: whole tiles dealt round-robin to CTAs.
 // Per-sample work: decode (2 integer ops) + one packed FFMA2 issue (re and im of two samples).
 // fp32 partial sums live for one tile (<= 64 additions), then are added to fp64 accumulators in
 // shared memory.
@@ -34,7 +36,8 @@ constexpr uint32_t kTileSamples = 1u << 16;
 struct GenParams {
     const void* data;        // [device] packed samples
     uint64_t n_loads;        // complete per-thread loads available (vectors of SPT samples)
-    uint64_t n_tiles;
+    uint64_t n_tiles;        // gen_mma_kernel: tiles in the piece
+    uint64_t n_iters;        // gen_kernel: CTA iterations in the piece (the last one may be partial)
     uint32_t span;           // samples per CTA iteration: the largest multiple of lcm(N_bins, SPT) <= kThreads*SPT (threads past it idle)
     uint64_t Fs, k0, E, D;   // micro-hertz sample rate; (n0*Foff)%Fs; (tile*Foff)%Fs; (grid*E)%Fs
     uint64_t Foff;
@@ -170,17 +173,18 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(const __grid_constant_
 #pragma unroll
     for (int k = 0; k < SPT; ++k) acc[k * kThreads + tid] = make_double2(0.0, 0.0);
 
-    // this CTA's tiles: T_i = blockIdx.x + i * gridDim.x, i < nt
-    const uint32_t nt = blockIdx.x < P.n_tiles ? (uint32_t)((P.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    // this CTA's iterations: an equal share [it_lo, it_hi) of the piece, walked in tiles of LPT iterations
+    const uint64_t it_lo = P.n_iters * blockIdx.x / gridDim.x, it_hi = P.n_iters * (blockIdx.x + 1ull) / gridDim.x;
+    const uint32_t nt = (uint32_t)((it_hi - it_lo + LPT - 1) / LPT);
     const unsigned char* gdata = reinterpret_cast<const unsigned char*>(P.data);
     unsigned char* my_ring = ring + (size_t)tid * LB;
     constexpr size_t RING_STRIDE = (size_t)kThreads * LB;                // bytes between a thread's ring slots
     static_assert(LPT % DEPTH == 0, "ring slot of load j is j % DEPTH, a compile-time constant");
     const uint64_t LOAD_STRIDE = (uint64_t)(P.span / SPT) * LB;          // bytes between a thread's loads
     const uint64_t TILE_BYTES = (uint64_t)LPT * LOAD_STRIDE;
-    const uint64_t end_off = P.n_loads * LB;                              // first byte past the last complete load
-    const uint64_t tile_stride = (uint64_t)gridDim.x * TILE_BYTES;
-    uint64_t off = (uint64_t)blockIdx.x * TILE_BYTES + (uint64_t)tid * LB;   // this thread's load 0 of tile i
+    const uint64_t end_off = it_hi * LOAD_STRIDE < P.n_loads * LB ? it_hi * LOAD_STRIDE : P.n_loads * LB;   // first byte past this CTA's last load
+    const uint64_t tile_stride = TILE_BYTES;
+    uint64_t off = it_lo * LOAD_STRIDE + (uint64_t)tid * LB;              // this thread's load 0 of tile i
 
     float2 ar[SPT / 2], ai[SPT / 2];
 #pragma unroll
@@ -196,14 +200,10 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(const __grid_constant_
     // (the first loads are in flight: now the ticket and the tables)
     if (tid == kThreads - 1) { if (P.tail.st) gen_take_ticket(P.tail, s_gen); }      // (published by the barrier below)
     // ---- resync table: the exactly reduced INTEGER phase of every tile start -> fp64 phasor ----
-    {
-        uint64_t k_cta = P.k0 + mulmod_u64(P.E, blockIdx.x, P.Fs);
-        if (k_cta >= P.Fs) k_cta -= P.Fs;
-        for (uint32_t i = tid; i < nt; i += kThreads) {
-            uint64_t k = k_cta + mulmod_u64(P.D, i, P.Fs);
-            if (k >= P.Fs) k -= P.Fs;
-            base[i] = phasor_neg(k, P.Fs);
-        }
+    for (uint32_t i = tid; i < nt; i += kThreads) {       // (k0 = phase of the piece's first sample)
+        uint64_t k = P.k0 + mulmod_u64(P.Foff, (it_lo + (uint64_t)i * LPT) * P.span % P.Fs, P.Fs);
+        if (k >= P.Fs) k -= P.Fs;
+        base[i] = phasor_neg(k, P.Fs);
     }
     const double2 theta = phasor_neg(mulmod_u64(P.Foff, (uint64_t)tid * SPT, P.Fs), P.Fs);   // exp(-j w tid SPT)
     __syncthreads();
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(const __grid_constant_
         const double2 ph0 = make_double2(b.x * theta.x - b.y * theta.y, b.x * theta.y + b.y * theta.x);
         const uint64_t tile0 = off - (uint64_t)tid * LB;     // first byte of tile i
         const bool next_exists = i + 1 < nt;
-        const bool fast = next_exists && tile0 + tile_stride + TILE_BYTES <= end_off;   // tiles i and i+1 complete
+        const bool fast = tile0 + TILE_BYTES + (uint64_t)DEPTH * LOAD_STRIDE <= end_off;   // tile i and the first DEPTH iterations of tile i+1 complete
         if (fast) tile_body(std::false_type{}, ph0, true);
         else tile_body(std::true_type{}, ph0, next_exists);
         if ((i + 1) % RUN == 0 || i + 1 == nt) {
