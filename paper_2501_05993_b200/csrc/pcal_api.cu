@@ -245,11 +245,8 @@ static size_t gen2_smem_c(uint32_t cpw) { return cpw == 1 ? gen2_smem_bytes<C, 1
 static size_t gen2_smem_of(const pcal_ctx* c) {
     return c->C == 1 ? gen2_smem_c<1>(c->g2_cpw) : (c->C == 2 ? gen2_smem_c<2>(c->g2_cpw) : gen2_smem_c<4>(c->g2_cpw));
 }
-// threads of a gen2 CTA: loader + generator warp(s) + consumers (G2Cfg::THREADS)
-static uint32_t gen2_threads_of(const pcal_ctx* c) {
-    const uint32_t ck = (uint32_t)gen2_ck(c), items = (ck + c->g2_cpw - 1u) / c->g2_cpw;
-    return (uint32_t)(kG2Consumers + 1 + (items >= 2u ? 2 : 1)) * 32u;
-}
+// threads of a gen2 CTA: loader + two generator warps + consumers (G2Cfg::THREADS)
+static uint32_t gen2_threads_of(const pcal_ctx*) { return (uint32_t)(kG2Consumers + 3) * 32u; }
 static const void* gen2_fn(const pcal_ctx* c) { return reinterpret_cast<const void*>(gen2_kernel_of(c)); }
 
 static int prepare(pcal_ctx* c) {

@@ -69,8 +69,10 @@ template <int C, int CPW> struct G2Cfg {
     static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
     static constexpr int DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4);
     static constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;             // digit matrices of a tile: [C][KG][8 columns][32 rows]
-    // generator work items per tile and lane: (channel, row quad) pairs / 32; two generator warps when that is two or more
-    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = KI >= 2 ? 2 : 1, THREADS = (kG2Consumers + 1 + NG) * 32;
+    // generator work items per tile and lane: (channel, row quad) pairs / 32.  Two generator warps: with two or more items each
+    // takes half of the channels of every tile, with one they take the tiles of a batch in turn (TS)
+    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = 2, THREADS = (kG2Consumers + 1 + NG) * 32;
+    static constexpr bool TS = KI == 1;
     static constexpr uint32_t TAB_BYTES = (uint32_t)C * 4 * RT * 16;          // exp(-j w_c span_t r), r < rows of a batch
     static constexpr size_t FIXED = (size_t)DIGITS * DIG_BYTES + 1024;
     static constexpr bool FIT5 = 5 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
@@ -239,8 +241,10 @@ const __grid_constant__ Gen2Params P) {
             mbar_init(full0 + 8 * s, 33);                 // 32 cp.async arrivals of the loader + 1 plain arrival (it has seen the digits)
             mbar_init(empty0 + 8 * s, kG2Consumers);
         }
-        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, NG); mbar_init(dempty0 + 8 * e, kG2Consumers); }
+        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, Cfg::TS ? 1 : NG); mbar_init(dempty0 + 8 * e, kG2Consumers); }
         mbar_init(seqbar, 1);
+#pragma unroll
+        for (int c = 0; c < (int)kG2MaxCh; ++c) { s_rsum[c][0] = 0; s_rsum[c][1] = 0; }
     }
     __syncthreads();
 
@@ -253,7 +257,8 @@ const __grid_constant__ Gen2Params P) {
             for (int k = 0; k < 4; ++k) acc[c][u][k] = 0;
 
     if (warp >= 1 && warp <= NG) {
-        const int gw = warp - 1;                                  // generator warp gw serves items k = gw, gw + NG, ...
+        const int gw = warp - 1;                                  // generator warp gw: channels gw, gw + NG, ... of a tile, or (TS) tiles gw, gw + NG of a batch
+        constexpr bool TS = Cfg::TS;
         // ---------------- generator: owns the CTA's tile sequence; digit matrices of a batch of tiles, lane = row ----------------
         // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
         // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
@@ -261,19 +266,20 @@ const __grid_constant__ Gen2Params P) {
         // The four digit bytes of a column for rows 4q .. 4q+3 are one 32-bit word of the B fragment (row group q / 8, K slots
         // 4 (q % 8) ..; columns 0..3 = Re digits, 4..7 = Im digits).
         // Work items: (channel, four consecutive rows), g2_item_digits.  A tile has Q = RT / 4 row quads; lane l of generator
-        // warp gw serves quad l % Q of channels gw (32 / Q) + l / Q + k NG (32 / Q), k = 0 .. KI-1.
-        constexpr int Q = RT / 4, CHP = 32 / Q, KI = Cfg::KI / NG;            // (items of this warp)
-        const int g_ch0 = gw * CHP + lane / Q, g_quad = lane % Q;
+        // warp gw serves quad l % Q of channels gw (32 / Q) + l / Q + k NG (32 / Q), k = 0 .. KI-1 (TS: of channel l / Q).
+        constexpr int Q = RT / 4, CHP = 32 / Q, KI = TS ? 1 : Cfg::KI / NG;   // (items of this warp per tile)
+        const int g_ch0 = (TS ? 0 : gw * CHP) + lane / Q, g_quad = lane % Q;
         constexpr int KS = NG * CHP;                                            // channel step from item to item
         // the row phasors of a batch, from shared memory (an L2 round trip per tile is what this warp cannot afford): row
         // r = RT j + 4 q + i of channel c at [c][j][i][q], so that the lanes of a load are neighbours
         if (Cfg::TAB_SMEM) {
-            for (int x = lane; x < KI * CHP * 4 * RT; x += 32) {
+            for (int x = TS ? lane + 32 * gw : lane; x < KI * CHP * 4 * RT; x += TS ? 64 : 32) {
                 const int cl = x / (4 * RT), r = x % (4 * RT);
-                const int c = (cl / CHP) * KS + gw * CHP + cl % CHP;            // this warp's channels
+                const int c = TS ? cl : (cl / CHP) * KS + gw * CHP + cl % CHP;  // this warp's channels (TS: half of the entries of all)
                 if (c < C) tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
             }
-            __syncwarp();
+            if (TS) asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
+            else __syncwarp();
         }
         auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
         // column sums of the digit matrices of this lane's items: the sum of the quantised phasors over the CTA's rows, which
@@ -334,20 +340,23 @@ const __grid_constant__ Gen2Params P) {
                 pend[0] = pend[1]; pend[1] = kG2Invalid;
                 if (lane == 0 && nbatch < P.n_batches && pos + 3 - P.n_static < kG2CapBatches) pend[1] = dyn0 + atomicAdd(ctr, 1u);
             }
-            if (NG > 1 && pos + 1 >= P.n_static) {      // the claimed part of the sequence is warp 1's: one named barrier per batch
+            if (pos + 1 >= P.n_static) {      // the claimed part of the sequence is warp 1's: one named barrier per batch
                 if (gw == 0 && lane == 0) s_gen[6 + (pos & 1u)] = nbatch;
                 asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
                 nbatch = s_gen[6 + (pos & 1u)];
             }
             load_tabs(nbatch, thi, tlo);
             // UJ tiles at a time: their (independent) phasor chains overlap
-            constexpr uint32_t UJ = KI == 1 ? 4u : (KI == 2 ? 2u : 1u);
+            constexpr uint32_t UJ = TS ? 2u : (KI == 1 ? 4u : (KI == 2 ? 2u : 1u));
+            constexpr uint32_t JS = TS ? (uint32_t)NG : 1u;    // tile step of this warp inside a batch
+            const uint32_t jf = TS ? (uint32_t)gw : 0u;         // its first tile
 #pragma unroll 1
-            for (uint32_t j0 = 0; j0 < nt; j0 += UJ) {
+            for (uint32_t j0 = jf; j0 < nt; j0 += UJ * JS) {
                 uint32_t w[UJ][KI][8];
 #pragma unroll
                 for (uint32_t ju = 0; ju < UJ; ++ju) {
-                    const uint32_t rb = (j0 + ju) * RT + 4u * (uint32_t)g_quad;           // first of this lane's rows in the batch
+                    const uint32_t jt = j0 + ju * JS;                                       // tile of the batch
+                    const uint32_t rb = jt * RT + 4u * (uint32_t)g_quad;                    // first of this lane's rows in the batch
 #pragma unroll
                     for (int k = 0; k < KI; ++k) {
                         const int ch = k * KS + g_ch0;
@@ -355,7 +364,7 @@ const __grid_constant__ Gen2Params P) {
                         double2 row[4];
 #pragma unroll
                         for (int i = 0; i < 4; ++i)
-                            row[i] = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + ((j0 + ju) * 4 + i) * Q + g_quad]
+                            row[i] = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + (jt * 4 + i) * Q + g_quad]
                                                    : __ldg(P.gtab + (size_t)chc * kG2TabStride + (rb + i) % kG2TabRows);
                         if (all_rows) {
                             g2_item_digits<true>(base[k], row, 4u, w[ju][k]);
@@ -368,7 +377,7 @@ const __grid_constant__ Gen2Params P) {
                 }
 #pragma unroll
                 for (uint32_t ju = 0; ju < UJ; ++ju) {
-                    const uint32_t j = j0 + ju;
+                    const uint32_t j = j0 + ju * JS;
                     if (j < nt) {
                         const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
                         mbar_wait(dempty0 + 8 * e, ph ^ 1u);          // the consumers are done with the entry's previous tile
@@ -384,7 +393,7 @@ const __grid_constant__ Gen2Params P) {
                                 }
                             }
                         }
-                        if (gw == 0 && lane == 0) dig_tile[e] = tile0 + j;
+                        if ((TS || gw == 0) && lane == 0) dig_tile[e] = tile0 + j;
                         __syncwarp();
                         if (lane == 0) mbar_arrive(dfull0 + 8 * e);
                     }
@@ -396,7 +405,7 @@ const __grid_constant__ Gen2Params P) {
         {   // terminator: the entry after the last tile carries "no tile"
             const uint32_t e = it % DIGD, ph = (it / DIGD) & 1u;
             mbar_wait(dempty0 + 8 * e, ph ^ 1u);
-            if (lane == 0) { if (gw == 0) dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
+            if (lane == 0 && (gw == 0 || !TS)) { if (gw == 0) dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
         }
 #pragma unroll
         for (int k = 0; k < KI; ++k) {
@@ -408,7 +417,10 @@ const __grid_constant__ Gen2Params P) {
                 im += __shfl_xor_sync(0xFFFFFFFFu, im, sh);
             }
             const int ch = k * KS + g_ch0;
-            if (g_quad == 0 && ch < C) { s_rsum[ch][0] = re; s_rsum[ch][1] = im; }
+            if (g_quad == 0 && ch < C) {      // (TS: both warps hold a part)
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][0]), (unsigned long long)re);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][1]), (unsigned long long)im);
+            }
         }
     } else if (warp == 0) {
         // ---------------- loader: copy each tile as it lies, 512 contiguous bytes per instruction ----------------
