@@ -245,8 +245,6 @@ static size_t gen2_smem_c(uint32_t cpw) { return cpw == 1 ? gen2_smem_bytes<C, 1
 static size_t gen2_smem_of(const pcal_ctx* c) {
     return c->C == 1 ? gen2_smem_c<1>(c->g2_cpw) : (c->C == 2 ? gen2_smem_c<2>(c->g2_cpw) : gen2_smem_c<4>(c->g2_cpw));
 }
-// threads of a gen2 CTA: loader + two generator warps + consumers (G2Cfg::THREADS)
-static uint32_t gen2_threads_of(const pcal_ctx*) { return (uint32_t)(kG2Consumers + 3) * 32u; }
 static const void* gen2_fn(const pcal_ctx* c) { return reinterpret_cast<const void*>(gen2_kernel_of(c)); }
 
 static int prepare(pcal_ctx* c) {
@@ -561,7 +559,7 @@ static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cuda
             gp.T_dev = c->fuse_T_dev ? c->fuse_T_dev : c->d_T; gp.T_host = c->fuse_out; gp.P_copy = c->fuse_P_copy;
         }
         prof_mark(c, st);
-        launch_chain(gen2_kernel_of(c), c->gen_grid, gen2_threads_of(c), c->gen_smem, st, gp);
+        launch_chain(gen2_kernel_of(c), c->gen_grid, kG2Threads, c->gen_smem, st, gp);
         prof_mark(c, st);
         c->launches += 1;
     }

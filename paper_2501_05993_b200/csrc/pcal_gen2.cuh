@@ -21,12 +21,14 @@
 // row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-31 quantisation.
 //
 // Structure (profiles/r2_ncu_full.md has the before/after against the round-1 kernel):
-//   * warp roles, no CTA-wide barrier in the loop.  Warp 1 (generator) owns the CTA's tile sequence -- its own batches
-//     first, then batches claimed from a device counter, each claim issued two batches ahead -- and writes the digit
-//     matrices into a ring of entries.  Warp 0 (loader) follows the sequence and copies each tile as it lies in memory
-//     (one cp.async instruction per 512 contiguous bytes) into a ring of padded tiles; completion arrives on the
-//     stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 2..9 (consumers) wait for "full", read their operands
-//     and release stage and digit entry on "empty" barriers.  Nobody waits for anybody else's loads.
+//   * warp roles, no CTA-wide barrier in the loop.  Warps 1 and 2 (generators) write the digit matrices of the CTA's tile
+//     sequence -- its own batches first, then batches that warp 1 claims from a device counter, each claim issued two
+//     batches ahead -- into a ring of entries; they split the channels of a tile, or, with one work item per lane and tile,
+//     the tiles of a batch.  They are the critical resource of the kernel: row phasors of a batch in shared memory, digits
+//     by one fp64 add and one xor (g2_item_digits).  Warp 0 (loader) follows the sequence and copies each tile as it
+//     lies in memory (one cp.async instruction per 512 contiguous bytes) into a ring of padded tiles; completion arrives
+//     on the stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 3..10 (consumers) wait for "full", read their
+//     operands and release stage and digit entry on "empty" barriers.  Nobody waits for anybody else's loads.
 //   * the 4x4 byte transpose (four rows of one position into one register) is done by the load itself:
 //     ldmatrix.m16n16.trans.b8 (SASS LDSM.8.MT1616, new on sm_100) returns exactly the A fragment of m16n8k32, lane
 //     (g, t): byte column g / g + 8 of rows 4t..4t+3 (+16).  The row pitch is an odd number of 16-byte chunks, which keeps
@@ -35,7 +37,7 @@
 //     U3 = & 0xC0 (3 LOP3 instead of 4; single channel), the field sums S_f are differences of the U sums, exact.
 //     With C = 2 / 4 channels field f belongs to channel f mod C and is masked accordingly (digits per channel).
 //   * hybrid tile assignment: three quarters of the batches are a CTA's own (index + k * grid), the rest are claimed from a
-//     device counter -- a CTA that starts late simply takes fewer.  A CTA is half an SM (320 threads, 80 registers) and
+//     device counter -- a CTA that starts late simply takes fewer.  A CTA is half an SM (352 threads, 80 registers) and
 //     lets its dependent grid start as soon as its ticket is taken: consecutive launches share the SMs pairwise and HBM
 //     keeps streaming while one of them is in its epilogue.
 //   * the per-position sums of a CTA are exact int64 and are added to the launch's accumulators with integer
@@ -52,7 +54,7 @@
 namespace pcal {
 
 constexpr int kG2Consumers = 8;                               // consumer warps
-constexpr int kG2Threads = (kG2Consumers + 2) * 32;           // + loader + generator (a second generator warp: G2Cfg::THREADS)
+constexpr int kG2Threads = (kG2Consumers + 3) * 32;           // + loader + two generator warps
 constexpr uint32_t kG2StageBytes = 18432;                     // a padded tile: 128 rows x 144 B (8 chunks) ... 32 rows x 528 B (32 chunks)
 constexpr uint32_t kG2Fields = 2048;                          // fields (positions) per row at most
 constexpr uint32_t kG2Batch = 4;                              // tiles per claim
@@ -216,7 +218,7 @@ __device__ __forceinline__ void g2_item_digits(const double2 base, const double2
 
 // CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
 template <int C, bool SIGN_MAG, int CPW>
-__global__ void __launch_bounds__(kG2Threads + 64, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
+__global__ void __launch_bounds__(kG2Threads + 32, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
 const __grid_constant__ Gen2Params P) {
     if (!P.input_ready) pdl_wait();
     using Cfg = G2Cfg<C, CPW>;
