@@ -229,10 +229,15 @@ def test_bitwise_determinism_under_dynamic_tile_claims():
                                        (5, 17, None), (1, 1, None), (1, 3, None), (1, 4, None), (1, 5, None), (4, 1, None), (4, 3, None),
                                        (4, 4, None), (4, 5, None), (3, 2052, None),
                                        (3, 4, "generator"), (3, 508, "generator"), (3, 512, "generator"), (3, 516, "generator"),
-                                       (3, 512 * 128 - 4, "generator"), (3, 512 * 128 + 4, "generator"), (2, 60, "generator"), (2, 516, "generator")])
+                                       (3, 512 * 128 - 4, "generator"), (3, 512 * 128 + 4, "generator"), (2, 60, "generator"), (2, 516, "generator"),
+                                       (8, 1, "generator"), (8, 3, "generator"), (8, 1020, "generator"), (8, 1024, "generator"), (8, 1028, "generator"),
+                                       (8, 1024 * 147 + 8, "generator"), (8, 1024 * 148, "generator"), (8, 1024 * 149 - 4, "generator"),
+                                       (8, 1024 * 64 * 148 + 1024 * 3 + 4, "generator")])
 def test_tiny_and_ragged_lengths(oracle, idx, n, rot):
     """Segments shorter than / equal to / just above one 16-byte vector (tail-only and 1-vector paths); for the generator
-    kernel of 2-bit samples: around one row (512 samples) and one tile (128 rows)."""
+    kernel of 2-bit samples: around one row (512 samples) and one tile (128 rows); for the float32 generator kernel: around
+    one CTA iteration (1024 samples), one iteration per CTA (fewer iterations than CTAs, exactly as many, one more) and a
+    little more than one full tile per CTA."""
     w, dev, host = make(idx, n)
     if rot:
         w = synth.replace(w, rotator=rot)
@@ -249,8 +254,9 @@ def test_tiny_and_ragged_lengths(oracle, idx, n, rot):
         if (~empty).any():
             assert_close(P[c][~empty], want[~empty], f"cfg{idx} n={n} ch{c} folded")
         wt = oracle.dft(pr, pi)
-        assert np.abs(T[c] - wt).max() <= 1e-5 * np.abs(wt).max() * 1e-3 + 1e-300, (idx, n, c)     # every tone to 1e-8 of the largest ...
-        big = np.abs(wt) >= 1e-3 * np.abs(wt).max()
+        small = 1e-2 if w.bits == 32 else 1e-3               # reading R28: "small" tones, float32 input: 1e-2 of the largest
+        assert np.abs(T[c] - wt).max() <= 1e-5 * np.abs(wt).max() * small + 1e-300, (idx, n, c)    # every tone to 1e-8 (1e-7) of the largest ...
+        big = np.abs(wt) >= small * np.abs(wt).max()
         assert_close(T[c][big], wt[big], f"cfg{idx} n={n} ch{c} tones")                              # ... and per tone where it is not a cancellation
 
 
