@@ -79,6 +79,19 @@ __device__ __forceinline__ uint64_t mulmod_u64(uint64_t a, uint64_t b, uint64_t 
     return r;
 }
 
+// Exact division of small numbers by a run-time divisor without the ~150-cycle dependent sequence of a hardware-assisted
+// udiv -- the serial tails of the kernels (one CTA, two warps per scheduler) are chains of such latencies.
+// q = (x * ceil(2^40 / d)) >> 40 is exact for x * d < 2^40 (here: x < 2^24, d <= 2^12 .. 2^16).  The constant comes from ONE
+// fp64 division: 2^40 / d is an integer (d a power of two) or at least 2^-16 away from one, which fp64 resolves (53 bits).
+struct FastDiv {
+    uint64_t m;
+    uint32_t d;
+    __device__ __forceinline__ explicit FastDiv(uint32_t div) : m((uint64_t)ceil(1099511627776.0 / (double)div)), d(div) {}
+    __device__ __forceinline__ uint32_t div(uint32_t x) const { return (uint32_t)(((uint64_t)x * m) >> 40); }
+    __device__ __forceinline__ uint32_t mod(uint32_t x) const { return x - div(x) * d; }
+    __device__ __forceinline__ void divmod(uint32_t x, uint32_t& q, uint32_t& r) const { q = div(x); r = x - q * d; }
+};
+
 // exp(-j 2 pi k / m) in fp64 for an exactly reduced numerator 0 <= k < m.
 __device__ __forceinline__ double2 phasor_neg(uint64_t k, uint64_t m) {
     double s, c;

@@ -625,16 +625,20 @@ const __grid_constant__ Gen2Params P) {
         }
         __syncthreads();
     };
+    const FastDiv dBins(P.n_bins);                            // (dividends below 2^24: pcal_common.cuh)
+    const uint32_t tau_first = dBins.mod(2u * P.n_bins - P.n0_mod_bins - dBins.mod(P.tau0));      // time offset of bin 0 in this launch's columns
     for (uint32_t pp0 = 0; pp0 < pairs; pp0 += NT) {          // uniform trip count
         const uint32_t pp = pp0 + tid;
         const bool mine = pp < pairs;
-        const uint32_t c = mine ? pp / P.n_bins : 0u, b = mine ? pp % P.n_bins : 0u;
+        uint32_t c = 0u, b = 0u;
+        if (mine) dBins.divmod(pp, c, b);
         double re = 0.0, im = 0.0;
         if (mine) {
             const double2* tw = P.tw + (size_t)c * P.span_t + P.tau0;
             const uint32_t n_tau = 64u * P.chunks / ((uint32_t)C * P.cls_count);       // time offsets in this launch's columns
             // tau0 + tau = b - n0 (mod N_bins), in order
-            for (uint32_t tau = (b + 2u * P.n_bins - P.n0_mod_bins - P.tau0 % P.n_bins) % P.n_bins; tau < n_tau; tau += P.n_bins) {
+            uint32_t tau = b + tau_first; if (tau >= P.n_bins) tau -= P.n_bins;
+            for (; tau < n_tau; tau += P.n_bins) {
                 const uint32_t F = (tau * P.cls_count + P.cls) * C + c;
                 const double xr = (double)pos_s[2 * F] * (1.0 / 1073741824.0), xi = (double)pos_s[2 * F + 1] * (1.0 / 1073741824.0);
                 const double2 w = __ldg(tw + tau);

@@ -80,7 +80,7 @@ __device__ __forceinline__ void gen_tail(const GenTailParams& T, uint32_t* s_gen
     for (uint32_t b0 = bin_lo; b0 < bin_hi; b0 += 32u) {     // uniform trip count
         const uint32_t b = b0 + lane;
         const bool ok = b < bin_hi;
-        const uint32_t s = ok ? (b + T.n_bins - shift) % T.n_bins : 0u;
+        uint32_t s = ok ? b + T.n_bins - shift : 0u; if (s >= T.n_bins) s -= T.n_bins;
         double re = 0.0, im = 0.0;
         if (ok) {
             for (uint32_t c0 = sl; c0 < gridDim.x; c0 += 64u) {        // eight loads in flight, added in CTA order

@@ -337,37 +337,44 @@ __device__ __forceinline__ void dft_in_cta(const double2* sP, double2* sY, const
                                            uint32_t N1, uint32_t k_shift, double2* T_dev, double2* T_host, uint32_t nthreads,
                                            double2* sOut = nullptr) {
     const uint32_t N2 = N / N1, tid = threadIdx.x, total = n_ch * N;
-    for (uint32_t oo = tid; oo < total; oo += nthreads) {
-        const uint32_t c = oo / N, o = oo % N;
-        const uint32_t k1 = o / N2, b2 = o % N2;
-        const uint32_t step = (uint32_t)(((uint64_t)N2 * k1) % N);
-        const double2* p0 = sP + c * N + b2;
+    const FastDiv dN(N), dN1(N1), dN2(N2);                 // (indices below 2^24, divisors <= 4096)
+    // sum_{j < n} x[j * stride] * W[(j * step) mod N] in index order; eight loads of each operand in flight at a time
+    auto dot = [&](const double2* x, uint32_t stride, uint32_t n, uint32_t step, double& re, double& im) {
         uint32_t idx = 0;
-        double re = 0.0, im = 0.0;
-        for (uint32_t b1 = 0; b1 < N1; ++b1) {
-            const double2 p = p0[N2 * b1], w = __ldg(W + idx);
-            re += p.x * w.x - p.y * w.y;
-            im += p.x * w.y + p.y * w.x;
-            idx += step; if (idx >= N) idx -= N;
+        re = 0.0; im = 0.0;
+        for (uint32_t j0 = 0; j0 < n; j0 += 8u) {
+            double2 xv[8], wv[8];
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) {
+                const bool in = j0 + j < n;
+                xv[j] = in ? x[(j0 + j) * stride] : make_double2(0.0, 0.0);
+                wv[j] = in ? __ldg(W + idx) : make_double2(0.0, 0.0);
+                idx += step; if (idx >= N) idx -= N;
+            }
+#pragma unroll
+            for (uint32_t j = 0; j < 8u; ++j) {
+                re += xv[j].x * wv[j].x - xv[j].y * wv[j].y;
+                im += xv[j].x * wv[j].y + xv[j].y * wv[j].x;
+            }
         }
-        const double2 w = __ldg(W + (uint32_t)(((uint64_t)k1 * b2) % N));
+    };
+    for (uint32_t oo = tid; oo < total; oo += nthreads) {
+        uint32_t c, o, k1, b2;
+        dN.divmod(oo, c, o);
+        dN2.divmod(o, k1, b2);
+        double re, im;
+        dot(sP + c * N + b2, N2, N1, dN.mod(N2 * k1), re, im);
+        const double2 w = __ldg(W + dN.mod(k1 * b2));
         sY[c * N + b2 * N1 + k1] = make_double2(re * w.x - im * w.y, re * w.y + im * w.x);
     }
     __syncthreads();
     for (uint32_t oo = tid; oo < total; oo += nthreads) {
-        const uint32_t c = oo / N, o = oo % N;
-        const uint32_t k1 = o % N1, k2 = o / N1;
-        const uint32_t step = (uint32_t)(((uint64_t)N1 * k2) % N);
-        const double2* y0 = sY + c * N + k1;
-        uint32_t idx = 0;
-        double re = 0.0, im = 0.0;
-        for (uint32_t b2 = 0; b2 < N2; ++b2) {
-            const double2 y = y0[b2 * N1], w = __ldg(W + idx);
-            re += y.x * w.x - y.y * w.y;
-            im += y.x * w.y + y.y * w.x;
-            idx += step; if (idx >= N) idx -= N;
-        }
-        const uint32_t i = c * N + (o + k_shift) % N;
+        uint32_t c, o, k1, k2;
+        dN.divmod(oo, c, o);
+        dN1.divmod(o, k2, k1);
+        double re, im;
+        dot(sY + c * N + k1, N1, N2, dN.mod(N1 * k2), re, im);
+        const uint32_t i = c * N + dN.mod(o + k_shift);
         if (sOut) { sOut[i] = make_double2(re, im); continue; }
         T_dev[i] = make_double2(re, im);
         if (T_host) T_host[i] = make_double2(re, im);

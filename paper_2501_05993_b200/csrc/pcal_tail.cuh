@@ -178,8 +178,10 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     // B1: thread t multiplies the elements t, t+256, ... by their phasors -- all table loads of a thread
     //     in flight at once -- and leaves the products in shared memory (in place of the sums);
     // B2: tpp threads per (channel, bin) pair add the pair's products in a fixed order.
-    const uint32_t pairs = T.C * T.n_bins, W = 32u * T.spv, tpp = T.tpp;
-    const uint32_t base_b = (uint32_t)((T.n0_mod_bins + (uint64_t)p * W) % T.n_bins);
+    const uint32_t n_bins = T.n_bins;      // (the parameters sit behind a reference: every use is a load -- the loops keep copies)
+    const FastDiv dBins(n_bins), dC(T.C);  // (dividends below 2^24)
+    const uint32_t pairs = T.C * n_bins, W = 32u * T.spv, tpp = T.tpp;
+    const uint32_t base_b = dBins.mod(T.n0_mod_bins + p * W);
     {
         constexpr uint32_t EPT = (E + kThreads - 1) / kThreads;       // 8, 2, 1
         double v[EPT];
@@ -189,7 +191,9 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
             const uint32_t e = tid + j * kThreads;
             v[j] = 0.0; ph[j] = make_double2(1.0, 0.0);
             if (e < E) {
-                const uint32_t f = e >> 5, ln = e & 31u, t = f / T.C, c = f % T.C;
+                const uint32_t f = e >> 5, ln = e & 31u;
+                uint32_t t, c;
+                dC.divmod(f, t, c);
                 const uint32_t L = T.lut_len[c];
                 v[j] = scratch[e];
                 if (L > 1) ph[j] = __ldg(T.lut + T.lut_off[c] + (T.n0_mod_L[c] + p * W + ln * T.spv + t) % L);
@@ -206,26 +210,30 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
     }
     const double2* G = T.G + (size_t)slot * q * pairs;
     double2* Gp = T.G + ((size_t)slot * q + p) * pairs;
-    for (uint32_t s0 = 0; s0 < pairs * tpp; s0 += kThreads) {          // uniform trip count: shuffles below
-        const uint32_t slot = s0 + tid;
-        const bool active = slot < pairs * tpp;
-        const uint32_t pp = active ? slot / tpp : 0u, u = slot % tpp;
-        const uint32_t c = pp / T.n_bins, b = pp % T.n_bins;
-        double are = 0.0, aim = 0.0;
-        if (active) {
-            const double2* prod = reinterpret_cast<const double2*>(scratch);
-            const uint32_t d0 = (b + T.n_bins - base_b) % T.n_bins;
-            const uint32_t dstep = tpp * T.n_bins;
-            for (uint32_t d = d0 + u * T.n_bins; d < W; d += dstep) {
-                const double2 x = prod[(((d & (T.spv - 1u)) * T.C + c) << 5) + (d >> T.spv_log2)];
-                are += x.x; aim += x.y;
+    {
+        const uint32_t nC = T.C, spv_m1 = T.spv - 1u, spv_log2 = T.spv_log2, tpp_log2 = 31u - (uint32_t)__clz(tpp);   // tpp: a power of two
+        const double2* prod = reinterpret_cast<const double2*>(scratch);
+        const uint32_t dstep = tpp * n_bins, slots = pairs * tpp;
+        for (uint32_t s0 = 0; s0 < slots; s0 += kThreads) {               // uniform trip count: shuffles below
+            const uint32_t sl_ = s0 + tid;
+            const bool active = sl_ < slots;
+            const uint32_t pp = active ? sl_ >> tpp_log2 : 0u, u = sl_ & (tpp - 1u);
+            uint32_t c, b;
+            dBins.divmod(pp, c, b);
+            double are = 0.0, aim = 0.0;
+            if (active) {
+                uint32_t d0 = b + n_bins - base_b; if (d0 >= n_bins) d0 -= n_bins;
+                for (uint32_t d = d0 + u * n_bins; d < W; d += dstep) {
+                    const double2 x = prod[(((d & spv_m1) * nC + c) << 5) + (d >> spv_log2)];
+                    are += x.x; aim += x.y;
+                }
             }
+            for (uint32_t sh = tpp >> 1; sh > 0; sh >>= 1) {
+                are += __shfl_xor_sync(0xFFFFFFFFu, are, sh);
+                aim += __shfl_xor_sync(0xFFFFFFFFu, aim, sh);
+            }
+            if (active && u == 0) Gp[pp] = make_double2(are, aim);
         }
-        for (uint32_t sh = tpp >> 1; sh > 0; sh >>= 1) {
-            are += __shfl_xor_sync(0xFFFFFFFFu, are, sh);
-            aim += __shfl_xor_sync(0xFFFFFFFFu, aim, sh);
-        }
-        if (active && u == 0) Gp[pp] = make_double2(are, aim);
     }
 
     __syncthreads();
@@ -292,7 +300,8 @@ __device__ __noinline__ void fold_tail(const TailParams& T, const void* partial,
             if (sl == 0) for (uint32_t k = 0; k < ns; ++k) { are += s_re[k * ppc + e0]; aim += s_im[k * ppc + e0]; }
         }
         const bool mine = sl == 0 && pp < pair_hi;
-        const uint32_t c = mine ? pp / T.n_bins : 0u, b = mine ? pp % T.n_bins : 0u;
+        uint32_t c = 0u, b = 0u;
+        if (mine) dBins.divmod(pp, c, b);
         if (mine && n_tail) {   // samples NT .. n_total-1 (fewer than one vector)
             const uint32_t L = T.lut_len[c];
             const double2* lut = T.lut + T.lut_off[c];
