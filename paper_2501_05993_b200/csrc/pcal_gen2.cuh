@@ -21,14 +21,15 @@
 // row) -- so there is no drift to bound; the error of rho is ~4e-16 before the 2^-31 quantisation.
 //
 // Structure (profiles/r2_ncu_full.md has the before/after against the round-1 kernel):
-//   * warp roles, no CTA-wide barrier in the loop.  Warps 1 and 2 (generators) write the digit matrices of the CTA's tile
+//   * warp roles, no CTA-wide barrier in the loop.  Warps 1..3 (generators) write the digit matrices of the CTA's tile
 //     sequence -- its own batches first, then batches that warp 1 claims from a device counter, each claim issued two
-//     batches ahead -- into a ring of entries; they split the channels of a tile, or, with one work item per lane and tile,
-//     the tiles of a batch.  They are the critical resource of the kernel: row phasors of a batch in shared memory, digits
-//     by one fp64 add and one xor (g2_item_digits).  Warp 0 (loader) follows the sequence and copies each tile as it
-//     lies in memory (one cp.async instruction per 512 contiguous bytes) into a ring of padded tiles; completion arrives
-//     on the stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 3..10 (consumers) wait for "full", read their
-//     operands and release stage and digit entry on "empty" barriers.  Nobody waits for anybody else's loads.
+//     batches ahead -- into a ring of entries, taking the tiles of the sequence in turn.  Their latency per tile is the
+//     critical resource of the kernel (one warp: 0.86 of the copy peak on config 3, two: 0.92, three: 0.97): row phasors
+//     of a batch in shared memory, digits by one fp64 add and one xor (g2_item_digits).  Warp 0 (loader) follows the
+//     sequence and copies each tile as it lies in memory (one cp.async instruction per 512 contiguous bytes) into a ring
+//     of padded tiles; completion arrives on the stage's mbarrier (cp.async.mbarrier.arrive.noinc).  Warps 4..11
+//     (consumers) wait for "full", read their operands and release stage and digit entry on "empty" barriers.  Nobody
+//     waits for anybody else's loads.
 //   * the 4x4 byte transpose (four rows of one position into one register) is done by the load itself:
 //     ldmatrix.m16n16.trans.b8 (SASS LDSM.8.MT1616, new on sm_100) returns exactly the A fragment of m16n8k32, lane
 //     (g, t): byte column g / g + 8 of rows 4t..4t+3 (+16).  The row pitch is an odd number of 16-byte chunks, which keeps
@@ -37,7 +38,7 @@
 //     U3 = & 0xC0 (3 LOP3 instead of 4; single channel), the field sums S_f are differences of the U sums, exact.
 //     With C = 2 / 4 channels field f belongs to channel f mod C and is masked accordingly (digits per channel).
 //   * hybrid tile assignment: three quarters of the batches are a CTA's own (index + k * grid), the rest are claimed from a
-//     device counter -- a CTA that starts late simply takes fewer.  A CTA is half an SM (352 threads, 80 registers) and
+//     device counter -- a CTA that starts late simply takes fewer.  A CTA is half an SM (384 threads, 80 registers) and
 //     lets its dependent grid start as soon as its ticket is taken: consecutive launches share the SMs pairwise and HBM
 //     keeps streaming while one of them is in its epilogue.
 //   * the per-position sums of a CTA are exact int64 and are added to the launch's accumulators with integer
@@ -54,7 +55,7 @@
 namespace pcal {
 
 constexpr int kG2Consumers = 8;                               // consumer warps
-constexpr int kG2Threads = (kG2Consumers + 3) * 32;           // + loader + two generator warps
+constexpr int kG2Threads = (kG2Consumers + 4) * 32;           // + loader + at most three generator warps
 constexpr uint32_t kG2StageBytes = 18432;                     // a padded tile: 128 rows x 144 B (8 chunks) ... 32 rows x 528 B (32 chunks)
 constexpr uint32_t kG2Fields = 2048;                          // fields (positions) per row at most
 constexpr uint32_t kG2Batch = 4;                              // tiles per claim
@@ -71,10 +72,9 @@ template <int C, int CPW> struct G2Cfg {
     static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
     static constexpr int DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4);
     static constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;             // digit matrices of a tile: [C][KG][8 columns][32 rows]
-    // generator work items per tile and lane: (channel, row quad) pairs / 32.  Two generator warps: with two or more items each
-    // takes half of the channels of every tile, with one they take the tiles of a batch in turn (TS)
-    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = 2, THREADS = (kG2Consumers + 1 + NG) * 32;
-    static constexpr bool TS = KI == 1;
+    // generator work items per tile and lane: (channel, row quad) pairs / 32.  Three generator warps take the tiles of the
+    // CTA's sequence in turn.
+    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = 3, THREADS = (kG2Consumers + 1 + NG) * 32;
     static constexpr uint32_t TAB_BYTES = (uint32_t)C * 4 * RT * 16;          // exp(-j w_c span_t r), r < rows of a batch
     static constexpr size_t FIXED = (size_t)DIGITS * DIG_BYTES + 1024;
     static constexpr bool FIT5 = 5 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
@@ -218,7 +218,7 @@ __device__ __forceinline__ void g2_item_digits(const double2 base, const double2
 
 // CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
 template <int C, bool SIGN_MAG, int CPW>
-__global__ void __launch_bounds__(kG2Threads + 32, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
+__global__ void __launch_bounds__(kG2Threads, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
 const __grid_constant__ Gen2Params P) {
     if (!P.input_ready) pdl_wait();
     using Cfg = G2Cfg<C, CPW>;
@@ -243,7 +243,7 @@ const __grid_constant__ Gen2Params P) {
             mbar_init(full0 + 8 * s, 33);                 // 32 cp.async arrivals of the loader + 1 plain arrival (it has seen the digits)
             mbar_init(empty0 + 8 * s, kG2Consumers);
         }
-        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, Cfg::TS ? 1 : NG); mbar_init(dempty0 + 8 * e, kG2Consumers); }
+        for (int e = 0; e < DIGD; ++e) { mbar_init(dfull0 + 8 * e, 1); mbar_init(dempty0 + 8 * e, kG2Consumers); }
         mbar_init(seqbar, 1);
 #pragma unroll
         for (int c = 0; c < (int)kG2MaxCh; ++c) { s_rsum[c][0] = 0; s_rsum[c][1] = 0; }
@@ -259,8 +259,7 @@ const __grid_constant__ Gen2Params P) {
             for (int k = 0; k < 4; ++k) acc[c][u][k] = 0;
 
     if (warp >= 1 && warp <= NG) {
-        const int gw = warp - 1;                                  // generator warp gw: channels gw, gw + NG, ... of a tile, or (TS) tiles gw, gw + NG of a batch
-        constexpr bool TS = Cfg::TS;
+        const int gw = warp - 1;                                  // generator warp gw: tiles gw, gw + NG, ... of the CTA's sequence
         // ---------------- generator: owns the CTA's tile sequence; digit matrices of a batch of tiles, lane = row ----------------
         // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
         // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
@@ -268,20 +267,19 @@ const __grid_constant__ Gen2Params P) {
         // The four digit bytes of a column for rows 4q .. 4q+3 are one 32-bit word of the B fragment (row group q / 8, K slots
         // 4 (q % 8) ..; columns 0..3 = Re digits, 4..7 = Im digits).
         // Work items: (channel, four consecutive rows), g2_item_digits.  A tile has Q = RT / 4 row quads; lane l of generator
-        // warp gw serves quad l % Q of channels gw (32 / Q) + l / Q + k NG (32 / Q), k = 0 .. KI-1 (TS: of channel l / Q).
-        constexpr int Q = RT / 4, CHP = 32 / Q, KI = TS ? 1 : Cfg::KI / NG;   // (items of this warp per tile)
-        const int g_ch0 = (TS ? 0 : gw * CHP) + lane / Q, g_quad = lane % Q;
-        constexpr int KS = NG * CHP;                                            // channel step from item to item
+        // a generator warp serves quad l % Q of channels l / Q + k (32 / Q), k = 0 .. KI-1.
+        constexpr int Q = RT / 4, CHP = 32 / Q, KI = Cfg::KI;
+        const int g_ch0 = lane / Q, g_quad = lane % Q;
+        constexpr int KS = CHP;                                                 // channel step from item to item
         // the row phasors of a batch, from shared memory (an L2 round trip per tile is what this warp cannot afford): row
         // r = RT j + 4 q + i of channel c at [c][j][i][q], so that the lanes of a load are neighbours
         if (Cfg::TAB_SMEM) {
-            for (int x = TS ? lane + 32 * gw : lane; x < KI * CHP * 4 * RT; x += TS ? 64 : 32) {
+            for (int x = lane + 32 * gw; x < KI * CHP * 4 * RT; x += 32 * NG) {                 // (each warp a third of the entries)
                 const int cl = x / (4 * RT), r = x % (4 * RT);
-                const int c = TS ? cl : (cl / CHP) * KS + gw * CHP + cl % CHP;  // this warp's channels (TS: half of the entries of all)
+                const int c = cl;
                 if (c < C) tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
             }
-            if (TS) asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
-            else __syncwarp();
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
         }
         auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
         // column sums of the digit matrices of this lane's items: the sum of the quantised phasors over the CTA's rows, which
@@ -349,15 +347,15 @@ const __grid_constant__ Gen2Params P) {
             }
             load_tabs(nbatch, thi, tlo);
             // UJ tiles at a time: their (independent) phasor chains overlap
-            constexpr uint32_t UJ = TS ? 2u : (KI == 1 ? 4u : (KI == 2 ? 2u : 1u));
-            constexpr uint32_t JS = TS ? (uint32_t)NG : 1u;    // tile step of this warp inside a batch
-            const uint32_t jf = TS ? (uint32_t)gw : 0u;         // its first tile
+            constexpr uint32_t UJ = KI == 1 ? 2u : 1u;
+            constexpr uint32_t JS = (uint32_t)NG;               // tile step of this warp inside a batch
+            const uint32_t jf = ((uint32_t)gw + NG - it % NG) % NG;               // its first tile: tiles of the CTA's sequence in turn
 #pragma unroll 1
             for (uint32_t j0 = jf; j0 < nt; j0 += UJ * JS) {
                 uint32_t w[UJ][KI][8];
 #pragma unroll
                 for (uint32_t ju = 0; ju < UJ; ++ju) {
-                    const uint32_t jt = j0 + ju * JS;                                       // tile of the batch
+                    const uint32_t jt = j0 + ju * JS < kG2Batch ? j0 + ju * JS : kG2Batch - 1u;   // tile of the batch (past the batch: computed, not stored)
                     const uint32_t rb = jt * RT + 4u * (uint32_t)g_quad;                    // first of this lane's rows in the batch
 #pragma unroll
                     for (int k = 0; k < KI; ++k) {
@@ -395,7 +393,7 @@ const __grid_constant__ Gen2Params P) {
                                 }
                             }
                         }
-                        if ((TS || gw == 0) && lane == 0) dig_tile[e] = tile0 + j;
+                        if (lane == 0) dig_tile[e] = tile0 + j;
                         __syncwarp();
                         if (lane == 0) mbar_arrive(dfull0 + 8 * e);
                     }
@@ -407,7 +405,7 @@ const __grid_constant__ Gen2Params P) {
         {   // terminator: the entry after the last tile carries "no tile"
             const uint32_t e = it % DIGD, ph = (it / DIGD) & 1u;
             mbar_wait(dempty0 + 8 * e, ph ^ 1u);
-            if (lane == 0 && (gw == 0 || !TS)) { if (gw == 0) dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
+            if (lane == 0 && gw == 0) { dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
         }
 #pragma unroll
         for (int k = 0; k < KI; ++k) {
@@ -419,7 +417,7 @@ const __grid_constant__ Gen2Params P) {
                 im += __shfl_xor_sync(0xFFFFFFFFu, im, sh);
             }
             const int ch = k * KS + g_ch0;
-            if (g_quad == 0 && ch < C) {      // (TS: both warps hold a part)
+            if (g_quad == 0 && ch < C) {      // (every generator warp holds a part)
                 atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][0]), (unsigned long long)re);
                 atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][1]), (unsigned long long)im);
             }
