@@ -41,7 +41,8 @@ enum {
     PCAL_ERR_STATE = -3,       /* call not legal in the current state */
     PCAL_ERR_UNSUPPORTED = -4, /* valid request this build cannot serve (e.g. LUT of impractical length) */
     PCAL_ERR_DEVICE = -5,      /* CUDA error / no device */
-    PCAL_ERR_NOMEM = -6
+    PCAL_ERR_NOMEM = -6,
+    PCAL_ERR_LIMIT = -7        /* size beyond the fixed scratch of the no-allocation entry point (pcal_noalloc.h) */
 };
 
 /* Sample encodings (PAPER.md:31 says only "2-bit or higher"; tables defined here, R15).

@@ -99,6 +99,7 @@ def lib():
             "pcal_set_profiling": (i32, [vp, i32]),
             "pcal_get_profile": (i32, [vp, ctypes.POINTER(dbl), ctypes.POINTER(u64)]),
             "pcal_pipe_probe": (i32, [i32, ctypes.POINTER(dbl)]),
+            "pcal_fold_noalloc": (i32, [vp, u64, u64, dbl, dbl, dbl, i32, i32, i32, vp, vp]),
             "pcal_reset": (i32, [vp]),
             "pcal_destroy": (None, [vp]),
             "pcal_info": (i32, [vp, ctypes.POINTER(InfoT)]),
@@ -320,6 +321,17 @@ def pipe_probe(kind: int) -> float:
     v = ctypes.c_double()
     _check(lib().pcal_pipe_probe(kind, ctypes.byref(v)), "pcal_pipe_probe")
     return v.value
+
+
+def fold_noalloc(dev_samples, n_samples: int, start_index: int, f_s_hz: float, f_comb_hz: float, f_offset_hz: float,
+                 bits: int, encoding: int, accumulate: bool, dev_out_bins, stream=None):
+    """pcal_fold_noalloc (include/pcal_noalloc.h): rotate + fold one single-channel segment into the caller's device bins
+    without any allocation in the library (N_bins <= 1024; every call on a device shares one scratch array).
+    Tensors or raw addresses; asynchronous.  Marshalling only."""
+    src = dev_samples.data_ptr() if hasattr(dev_samples, "data_ptr") else int(dev_samples)
+    dst = dev_out_bins.data_ptr() if hasattr(dev_out_bins, "data_ptr") else int(dev_out_bins)
+    _check(lib().pcal_fold_noalloc(src, n_samples, start_index, f_s_hz, f_comb_hz, f_offset_hz, bits, encoding,
+                                   1 if accumulate else 0, dst, _stream_handle(stream)), "pcal_fold_noalloc")
 
 
 def from_workload(w) -> "Pcal":

@@ -8,9 +8,11 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
+#include "../../include/pcal_noalloc.h"
 #include "pcal_ctx.h"
 #include "pcal_fold.cuh"
 #include "pcal_gen.cuh"
@@ -71,6 +73,7 @@ extern "C" const char* pcal_strerror(int code) {
         case PCAL_ERR_UNSUPPORTED: return "unsupported configuration";
         case PCAL_ERR_DEVICE: return "CUDA device error";
         case PCAL_ERR_NOMEM: return "out of memory";
+        case PCAL_ERR_LIMIT: return "size exceeds the fixed scratch of the no-allocation entry point (N_bins <= 1024, one channel)";
         default: return "unknown error";
     }
 }
@@ -1073,4 +1076,120 @@ extern "C" int pcal_generator_study(const pcal_gen_case_t* cases, uint32_t n_cas
     }
     cudaFree(d_cases); cudaFree(d_err); cudaGetLastError();
     return rc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// pcal_fold_noalloc (include/pcal_noalloc.h): rotate + fold one segment without allocating anything.
+// gen_kernel and post_gen_kernel as they are; their scratch -- the per-CTA partial bins -- is this file-scope array
+// instead of cudaMalloc'd memory.  Every device that loads the library holds its 2.5 MiB until the process exits.
+// In HOST code the name of a __device__ array is a host-side stand-in, not a device address: the kernels get the
+// address that cudaGetSymbolAddress returns for the current device (looked up once per device, below).
+// Shared by every call on the device, never cleared: gen_kernel writes all n_bins partial bins of each of its CTAs
+// before post_gen_kernel reads exactly those; calls that overlap on the GPU race on it (pcal_noalloc.h).
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[PCAL_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+struct NoAllocDevice {
+    bool ready;
+    double2* scratch;      // device address of g_noalloc_scratch on this device
+    int sm_count;
+};
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;
+
+// once per device, with that device current: address of the scratch array, SM count, shared-memory attribute of the kernels
+int noalloc_setup(int dev, NoAllocDevice** out) {
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return PCAL_ERR_DEVICE;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoAllocDevice& d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        void* ptr = nullptr;
+        CU(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+        if (!ptr || ((uintptr_t)ptr & 255u)) return PCAL_ERR_DEVICE;
+        CU(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaFuncSetAttribute(gen_kernel<KIND_2BIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes<KIND_2BIT>()));
+        CU(cudaFuncSetAttribute(gen_kernel<KIND_I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes<KIND_I8>()));
+        CU(cudaFuncSetAttribute(gen_kernel<KIND_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes<KIND_F32>()));
+        d.scratch = reinterpret_cast<double2*>(ptr);
+        d.ready = true;
+    }
+    *out = &d;
+    return PCAL_OK;
+}
+}  // namespace
+
+extern "C" int pcal_fold_noalloc(const void* dev_samples, uint64_t n_samples, uint64_t start_index, double f_s_hz, double f_comb_hz,
+                                 double f_offset_hz, int bits, int encoding, int accumulate, double* dev_out_bins, void* cuda_stream) {
+    if (!dev_out_bins || (!dev_samples && n_samples)) return PCAL_ERR_INVALID;
+    if (!(f_s_hz > 0) || !(f_comb_hz > 0) || !(f_offset_hz >= 0) || !(f_offset_hz < f_s_hz)) return PCAL_ERR_INVALID;
+    const uint64_t Fs = to_uhz(f_s_hz), Fc = to_uhz(f_comb_hz), Fo = to_uhz(f_offset_hz);
+    if (Fs == 0 || Fc == 0 || Fs % Fc != 0 || Fs / Fc < 2 || Fs >= (1ull << 62)) return PCAL_ERR_INVALID;
+    int kind;
+    if (bits == 2 && (encoding == PCAL_ENC_OFFSET_BINARY || encoding == PCAL_ENC_SIGN_MAG)) kind = KIND_2BIT;
+    else if (bits == 8 && encoding == PCAL_ENC_TWOS_COMPLEMENT) kind = KIND_I8;
+    else if (bits == 32 && encoding == PCAL_ENC_IEEE_FLOAT) kind = KIND_F32;
+    else return PCAL_ERR_INVALID;
+    if (Fs / Fc > PCAL_NOALLOC_MAX_BINS) return PCAL_ERR_LIMIT;          // the scratch array holds 160 x 1024 bins
+    const uint32_t n_bins = (uint32_t)(Fs / Fc);
+    if (((uintptr_t)dev_samples & 15u) || ((uintptr_t)dev_out_bins & 15u) || (n_samples * (uint64_t)bits) % 8u) return PCAL_ERR_ALIGNMENT;
+    // a CTA iteration of gen_kernel: the largest multiple of lcm(N_bins, samples per load) that 256 loads hold
+    const uint32_t spt = kind == KIND_F32 ? 4u : 16u;
+    const uint64_t unit = lcm_sat(n_bins, spt, 1u << 20), cap = (uint64_t)kThreads * spt;
+    if (unit > cap) return PCAL_ERR_UNSUPPORTED;
+    const uint32_t span = (uint32_t)(unit * (cap / unit));
+
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    NoAllocDevice* nd = nullptr;
+    const int rc = noalloc_setup(dev, &nd);
+    if (rc != PCAL_OK) return rc;
+    const uint32_t grid = (uint32_t)nd->sm_count < PCAL_NOALLOC_MAX_CTAS ? (uint32_t)nd->sm_count : PCAL_NOALLOC_MAX_CTAS;
+    if ((size_t)grid * n_bins * sizeof(double2) > PCAL_NOALLOC_SCRATCH_BYTES) return PCAL_ERR_LIMIT;     // (cannot happen: both capped above)
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint8_t* data = reinterpret_cast<const uint8_t*>(dev_samples);
+    const uint64_t load_bytes = kind == KIND_2BIT ? 4 : 16;
+    const uint64_t tile = (uint64_t)(kTileSamples / (kThreads * spt)) * span;          // samples per tile of a CTA
+    const uint64_t piece = (uint64_t)(small_pieces() ? 2 : kGenMaxTiles) * grid * tile;   // the resync table of a CTA holds 256 tiles (PCAL_SMALL_PIECES: tests)
+    uint64_t done = 0;
+    bool first = true;
+    do {
+        const uint64_t n = n_samples - done < piece ? n_samples - done : piece;
+        const uint8_t* base = data + done * (uint64_t)bits / 8;
+        const uint64_t n0 = start_index + done;
+        const uint64_t n_loads = n * (uint64_t)bits / 8 / load_bytes;
+        if (n_loads) {
+            GenParams gp;
+            memset(&gp, 0, sizeof(gp));
+            gp.data = base; gp.n_loads = n_loads; gp.span = span;
+            gp.n_tiles = (n_loads * spt + tile - 1) / tile;
+            gp.n_iters = (n_loads * spt + span - 1) / span;
+            gp.Fs = Fs; gp.Foff = Fo;
+            gp.k0 = mulmod_host(n0 % Fs, Fo, Fs);
+            gp.rho = phasor_neg_host(mulmod_host(span, Fo, Fs), Fs);
+            gp.rho2 = phasor_neg_host(mulmod_host(2ull * span, Fo, Fs), Fs);
+            for (uint32_t k = 0; k < 16; ++k) gp.tw[k] = phasor_neg_host(mulmod_host(k, Fo, Fs), Fs);
+            gp.n_bins = n_bins; gp.sign_mag = encoding == PCAL_ENC_SIGN_MAG;
+            gp.dec_mask = 0x00600000u; gp.dec_one = 0x3F800000u;
+            gp.input_ready = 0;                       // the samples may come from earlier work on the stream
+            gp.tail.st = nullptr;                     // no fused tail: partial bins of CTA i at scratch + i * n_bins
+            gp.tail.partial = nd->scratch;
+            if (kind == KIND_2BIT) launch_chain(gen_kernel<KIND_2BIT>, grid, kThreads, gen_smem_bytes<KIND_2BIT>(), st, gp);
+            else if (kind == KIND_I8) launch_chain(gen_kernel<KIND_I8>, grid, kThreads, gen_smem_bytes<KIND_I8>(), st, gp);
+            else launch_chain(gen_kernel<KIND_F32>, grid, kThreads, gen_smem_bytes<KIND_F32>(), st, gp);
+        }
+        GenPostParams gr;
+        memset(&gr, 0, sizeof(gr));
+        gr.partial = nd->scratch; gr.P = reinterpret_cast<double2*>(dev_out_bins);
+        gr.tail = base + n_loads * load_bytes;
+        gr.n0 = n0; gr.n_done = n_loads * spt; gr.n_total = n; gr.Fs = Fs; gr.Foff = Fo;
+        gr.grid = n_loads ? grid : 0; gr.n_bins = n_bins; gr.kind = kind; gr.sign_mag = encoding == PCAL_ENC_SIGN_MAG;
+        gr.overwrite = (first && !accumulate) ? 1 : 0;
+        if (n || gr.overwrite) launch_chain(post_gen_kernel, (n_bins + 31) / 32, kPostThreads, 0, st, gr);
+        first = false;
+        done += n;
+    } while (done < n_samples);
+    CU(cudaGetLastError());
+    return PCAL_OK;
 }
