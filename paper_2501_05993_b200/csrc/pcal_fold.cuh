@@ -230,8 +230,11 @@ __global__ void __launch_bounds__(kThreads, 3) fold_i8_kernel(const __grid_const
 }
 
 // ---------------------------------------------------------------------------------------------
-// float32 samples: 4 fields per vector.  fp32 runs of 16 additions, flushed into fp64
-// (runs <= 64 keep every bin within 1.3e-6 relative).
+// float32 samples: 4 fields per vector.  Every sample is converted (exactly) and added in fp64: the folded bins of unrotated
+// float32 input are REAL sums in which signal and noise cancel to a few per cent of a typical bin about once in a hundred
+// bins, and fp32 runs of 16 additions (the first version: 1.7e-7 of a typical bin) put such bins outside 1e-5 relative.
+// The price is two fp64-pipe instructions per sample (62 per clock and SM on B200): 0.4 us on a 16 MiB step
+// (DESIGN.md "Accumulation precision").
 // Output: double partial[cta][4][32].
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_constant__ FoldParams P) {
@@ -243,27 +246,21 @@ __global__ void __launch_bounds__(kThreads, 3) fold_f32_kernel(const __grid_cons
     const uint64_t stride = (uint64_t)P.R * kWarps * P.q * 32u;
     fold_ticket_and_release(P.tail, s_gen);
     double tot[4] = {0.0, 0.0, 0.0, 0.0};
-    for (uint32_t i = 0; i < P.n_iter; i += 2 * kUnroll) {
-        float run[4] = {0.f, 0.f, 0.f, 0.f};
+    for (uint32_t i = 0; i < P.n_iter; i += kUnroll) {
+        uint4 v[kUnroll];
 #pragma unroll
-        for (int half = 0; half < 2; ++half) {
-            uint4 v[kUnroll];
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u) {
-                const uint64_t a = idx + (uint64_t)u * stride;
-                v[u] = (a < P.n_vec) ? ldg_stream(P.data + a) : make_uint4(0, 0, 0, 0);
-            }
-            idx += (uint64_t)kUnroll * stride;
-#pragma unroll
-            for (int u = 0; u < kUnroll; ++u) {
-                run[0] += __uint_as_float(v[u].x);
-                run[1] += __uint_as_float(v[u].y);
-                run[2] += __uint_as_float(v[u].z);
-                run[3] += __uint_as_float(v[u].w);
-            }
+        for (int u = 0; u < kUnroll; ++u) {
+            const uint64_t a = idx + (uint64_t)u * stride;
+            v[u] = (a < P.n_vec) ? ldg_stream(P.data + a) : make_uint4(0, 0, 0, 0);
         }
+        idx += (uint64_t)kUnroll * stride;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) tot[k] += (double)run[k];
+        for (int u = 0; u < kUnroll; ++u) {
+            tot[0] += (double)__uint_as_float(v[u].x);
+            tot[1] += (double)__uint_as_float(v[u].y);
+            tot[2] += (double)__uint_as_float(v[u].z);
+            tot[3] += (double)__uint_as_float(v[u].w);
+        }
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) sh[w][k][lane] = tot[k];

@@ -508,9 +508,9 @@ def test_float32_odd_slot_group_counts(oracle, n_bins, unfused, monkeypatch):
     host = dev.cpu().numpy()
     p, T, P = gpu_run(w, dev)
     pr, pi = oracle_folded(oracle, w, host, 0)
-    # (reading R28: without rotation the bins are REAL sums of ~4000 float32 samples each -- a Gaussian variable lies within
-    #  1 % of its median magnitude of zero with probability ~0.5 %, so a few of the N_bins bins are that small)
-    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"N_bins={n_bins} folded", max_small=n_bins // 64, small_bin=1e-2)
+    # (without rotation the bins are REAL sums of ~4000 float32 samples each, of which a few per cent cancel to ~1 % of a typical
+    #  bin: the fold kernel adds float32 samples in fp64 for that reason, and no bin needs the rule of reading R28)
+    assert_close(P[0], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"N_bins={n_bins} folded")
     assert_close(T[0][1:n_bins // 2], oracle.dft(pr, pi)[1:n_bins // 2], f"N_bins={n_bins} in-band tones")
     p.destroy()
 
