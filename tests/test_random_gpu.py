@@ -3,6 +3,8 @@ of two and not), per-channel offsets (zero, rational, non-rational), rotator req
 are all drawn from the seed.  Every folded bin and every tone of the checked channels is held to north_star's bar
 (pcal_testlib.assert_close).  The point is the combinations the hand-written cases do not list.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -52,7 +54,7 @@ def draw(seed):
                 start=start, data=data, rs=rs)
 
 
-@pytest.mark.parametrize("seed", range(28))
+@pytest.mark.parametrize("seed", range(int(os.environ.get("PCAL_RANDOM_CASES", "28"))))     # (more seeds: a longer search)
 def test_random_configuration(oracle, seed):
     from paper_2501_05993_b200 import binding
     d = draw(seed)
