@@ -76,14 +76,24 @@ def test_random_configuration(oracle, seed):
             p.extract(flat[lo:hi], b - a)
         T, P = p.finalize(), p.get_folded()
         in_effect = p.info().rotator_in_effect
+        # the same data as ONE integration period through pcal_integrate, twice back to back (launches overlap; where the
+        # geometry allows, reduction and DFT run inside the hot kernel): tones delivered to pinned host memory
+        Ti = None
+        if not d["start"]:
+            outs = [torch.empty((C, d["n_bins"]), dtype=torch.complex128).pin_memory() for _ in range(2)]
+            for o in outs:
+                p.integrate(flat, n, o)
+            torch.cuda.synchronize()
+            assert torch.equal(outs[0].view(torch.float64), outs[1].view(torch.float64)), what
+            Ti = outs[1].numpy()
         p.destroy()
-        return T, P, in_effect
+        return T, P, in_effect, Ti
 
     try:
-        T, P, in_effect = run(d["rot"])
+        T, P, in_effect, Ti = run(d["rot"])
     except binding.PcalError as e:             # a generator request the kernels' geometry cannot serve: documented, then AUTO must work
         assert e.code == -4 and d["rot"] == "generator", what
-        T, P, in_effect = run("auto")
+        T, P, in_effect, Ti = run("auto")
     fmt = {"f32": oracle.F32, "i8": oracle.I8}.get(d["kind"], oracle.TWO_BIT_SIGN_MAG if d["enc"] else oracle.TWO_BIT_OFFSET_BINARY)
     chans = list(range(C)) if C <= 4 else sorted(set(int(x) for x in d["rs"].randint(0, C, size=4)))
     # reading R28: a few outputs of a noise-only integration may cancel below 1e-3 of the median (1e-2 where float32
@@ -99,6 +109,8 @@ def test_random_configuration(oracle, seed):
             assert_close(P[c][~empty], want[~empty], what + f" ch{c} folded", **small)
         wt = oracle.dft(pr, pi)
         assert_close(T[c], wt, what + f" ch{c} tones", **small)
+        if Ti is not None:
+            assert_close(Ti[c], wt, what + f" ch{c} tones (pcal_integrate)", **small)
         if d["offs"][c] == 0.0 and d["kind"] != "f32" and in_effect == binding.ROT_LUT:      # (unrotated integer sums: bit-exact)
             wi = oracle.fold_i64(d["data"], fmt, C, c, 0, 1, n, d["start"], d["n_bins"])
             assert np.array_equal(P[c].real, wi.astype(np.float64)) and not P[c].imag.any(), what + f" ch{c} exact integers"
