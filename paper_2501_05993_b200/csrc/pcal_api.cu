@@ -227,25 +227,30 @@ static uint32_t dft_n1_of(uint32_t n) {
     return best;
 }
 
-// the gen2_kernel instantiation of a context: <channels, SIGN_MAG, chunks per consumer warp>
+// the gen2_kernel instantiation of a context: <channels per byte, SIGN_MAG, chunks per consumer warp, byte classes per launch>
 typedef void (*gen2_kfn)(const Gen2Params);
-template <int C, int CPW>
-static gen2_kfn gen2_pick_sm(bool sm) { return sm ? gen2_kernel<C, true, CPW> : gen2_kernel<C, false, CPW>; }
+template <int C, int CPW, int NCLS>
+static gen2_kfn gen2_pick_sm(bool sm) { return sm ? gen2_kernel<C, true, CPW, NCLS> : gen2_kernel<C, false, CPW, NCLS>; }
 template <int C>
 static gen2_kfn gen2_pick_cpw(uint32_t cpw, bool sm) {
-    return cpw == 1 ? gen2_pick_sm<C, 1>(sm) : (cpw == 2 ? gen2_pick_sm<C, 2>(sm) : gen2_pick_sm<C, 4>(sm));
+    return cpw == 1 ? gen2_pick_sm<C, 1, 1>(sm) : (cpw == 2 ? gen2_pick_sm<C, 2, 1>(sm) : gen2_pick_sm<C, 4, 1>(sm));
 }
-// (words of 8 / 16 channels are served four channels -- one byte of the time sample -- per launch)
-static int gen2_ck(const pcal_ctx* c) { return c->C < 4 ? c->C : 4; }
+// words of 8 / 16 channels: a time sample is 2 / 4 bytes ("classes" of four channels).  A launch serves g2_ncls classes: all of
+// them where the accumulators fit (rows of <= 16 chunks), else one class per launch and as many passes over the data.
+static int gen2_ck(const pcal_ctx* c) { return c->C < 4 ? c->C : 4 * (int)c->g2_ncls; }       // channels per launch
 static gen2_kfn gen2_kernel_of(const pcal_ctx* c) {
     const bool sm = c->sign_mag != 0;
     if (c->C == 1) return gen2_pick_cpw<1>(c->g2_cpw, sm);
     if (c->C == 2) return gen2_pick_cpw<2>(c->g2_cpw, sm);
+    if (c->g2_ncls == 2) return c->g2_cpw == 1 ? gen2_pick_sm<4, 1, 2>(sm) : gen2_pick_sm<4, 2, 2>(sm);
+    if (c->g2_ncls == 4) return c->g2_cpw == 1 ? gen2_pick_sm<4, 1, 4>(sm) : gen2_pick_sm<4, 2, 4>(sm);
     return gen2_pick_cpw<4>(c->g2_cpw, sm);
 }
 template <int C>
-static size_t gen2_smem_c(uint32_t cpw) { return cpw == 1 ? gen2_smem_bytes<C, 1>() : (cpw == 2 ? gen2_smem_bytes<C, 2>() : gen2_smem_bytes<C, 4>()); }
+static size_t gen2_smem_c(uint32_t cpw) { return cpw == 1 ? gen2_smem_bytes<C, 1, 1>() : (cpw == 2 ? gen2_smem_bytes<C, 2, 1>() : gen2_smem_bytes<C, 4, 1>()); }
 static size_t gen2_smem_of(const pcal_ctx* c) {
+    if (c->g2_ncls == 2) return c->g2_cpw == 1 ? gen2_smem_bytes<4, 1, 2>() : gen2_smem_bytes<4, 2, 2>();
+    if (c->g2_ncls == 4) return c->g2_cpw == 1 ? gen2_smem_bytes<4, 1, 4>() : gen2_smem_bytes<4, 2, 4>();
     return c->C == 1 ? gen2_smem_c<1>(c->g2_cpw) : (c->C == 2 ? gen2_smem_c<2>(c->g2_cpw) : gen2_smem_c<4>(c->g2_cpw));
 }
 static const void* gen2_fn(const pcal_ctx* c) { return reinterpret_cast<const void*>(gen2_kernel_of(c)); }
@@ -299,6 +304,10 @@ static int prepare(pcal_ctx* c) {
                 c->g2_blocks = (c->g2_chunks + 31u) / 32u;
                 c->g2_cpw = c->g2_chunks <= 8u ? 1u : (c->g2_chunks <= 16u ? 2u : 4u);
                 c->g2_rt = 32u * (4u / c->g2_cpw);
+                // byte classes per launch (8 / 16 channels): all of them when a thread's accumulators fit (PCAL_G2_NCLS: A/B runs, tests)
+                c->g2_ncls = 1;
+                if (c->C > 4 && c->g2_cpw <= 2u && c->g2_blocks == 1u) c->g2_ncls = (uint32_t)c->C / 4u;
+                if (const char* nc = getenv("PCAL_G2_NCLS")) { const uint32_t v = (uint32_t)atoi(nc); if (c->g2_ncls > 1 && (v == 1 || v == 2) && v <= c->g2_ncls) c->g2_ncls = v; }
             }
         }
     }
@@ -525,11 +534,12 @@ static bool can_fuse_dft(const pcal_ctx* c);
 // pcal_gen2.cuh over n time samples starting at data: rows, tail and accumulation in ONE kernel (one launch per group of
 // four channels for words of 8 / 16 channels)
 static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cudaStream_t st) {
-    const int ck = gen2_ck(c);
-    const uint32_t n_cls = (uint32_t)c->C / (uint32_t)ck;
+    const int ck = gen2_ck(c);                                     // channels per launch
+    const uint32_t n_cls = c->C > 4 ? (uint32_t)c->C / 4u : 1u;    // byte classes of a time sample
+    const uint32_t cls_step = c->g2_ncls;                          // classes per launch
     const bool was_pending = c->zero_pending;
     for (uint32_t blk = 0; blk < c->g2_blocks; ++blk)
-    for (uint32_t cls = 0; cls < n_cls; ++cls) {
+    for (uint32_t cls = 0; cls < n_cls; cls += cls_step) {
         Gen2Params gp;
         memset(&gp, 0, sizeof(gp));
         const uint64_t n_bytes = n * 2ull * c->C / 8;
@@ -539,7 +549,7 @@ static int extract_piece_gen2(pcal_ctx* c, const uint8_t* data, uint64_t n, cuda
         gp.row_stride = (uint64_t)c->g2_chunks * 16u; gp.col_off = 512ull * blk;
         gp.tau0 = 2048u * blk / (uint32_t)c->C; gp.do_tail = blk == 0 ? 1 : 0;
         gp.pitch = gp.row_bytes + ((gp.chunks & 1u) ? 0u : 16u);      // an odd number of 16-byte chunks
-        gp.cls_count = n_cls; gp.cls = cls; gp.c_real = (uint32_t)c->C; gp.c_base = cls * (uint32_t)ck;
+        gp.cls_count = n_cls; gp.cls = cls; gp.c_real = (uint32_t)c->C; gp.c_base = c->C > 4 ? cls * 4u : 0u;
         gp.n_rows = n_bytes / gp.row_stride;
         gp.n_tiles = (uint32_t)((gp.n_rows + c->g2_rt - 1) / c->g2_rt);
         gp.n_batches = (gp.n_tiles + kG2Batch - 1) / kG2Batch;
@@ -759,7 +769,7 @@ static uint32_t dft_ctas(const pcal_ctx* c) {
 // stage C of the fold kernel can take the DFT itself: small N_bins, and C*N_bins complex values fit in its scratch
 static bool can_fuse_dft(const pcal_ctx* c) {
     if (c->prepared && c->rot_eff == PCAL_ROT_GENERATOR && c->gen2) {
-        if (c->C > 4 || c->g2_blocks > 1) return false;   // several launches per piece
+        if ((c->C > 4 && 4u * c->g2_ncls != (uint32_t)c->C) || c->g2_blocks > 1) return false;   // several launches per piece
         // two-stage DFT in the last CTA: cheap enough to sit in the serial final stage, and P and the scratch fit behind the
         // position sums in the kernel's rings (everything before its barriers and bookkeeping words)
         const uint32_t n1 = dft_n1_of(c->n_bins);

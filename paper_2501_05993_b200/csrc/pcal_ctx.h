@@ -31,6 +31,7 @@ struct pcal_ctx {
     uint32_t g2_span_t, g2_chunks;  // ... its row: time samples, 16-byte chunks
     uint32_t g2_cpw, g2_rt;         // ... chunks per consumer warp (1, 2, 4), rows per tile (128, 64, 32)
     uint32_t g2_blocks;             // ... column blocks of a row (rows longer than 32 chunks are served 32 chunks per launch)
+    uint32_t g2_ncls;               // ... byte classes (four channels each) of 8 / 16-channel words served by one launch (1, 2, 4)
     double2 *d_g2_rtab, *d_g2_tw;   // ... stride phasors [C][32], position factors [C][span_t]
     uint32_t* d_g2_ctr;             // ... [slot][2] batch and arrival counters
     long long* d_g2_posacc;         // ... [slot][2*2048] exact per-position sums

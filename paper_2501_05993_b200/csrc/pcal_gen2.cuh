@@ -46,8 +46,11 @@
 //     arrives last converts to fp64, applies the position factor, folds positions to bins in a fixed order, adds the
 //     ragged tail and accumulates into the context (same TailState protocol as pcal_tail.cuh) and, for pcal_integrate /
 //     pcal_extract_series, takes the DFT in two stages (dft_in_cta).
-//   * words of 8 / 16 channels: four channels (one byte of the time sample) per launch; rows longer than 2048 fields: column
-//     blocks of 32 chunks, one launch each.
+//   * words of 8 / 16 channels: a time sample is 2 / 4 bytes ("classes" of four channels).  An MMA's 16 byte columns hold every
+//     class while its digit matrix belongs to one channel: the masked operand meets the digits of channel u of every class in turn
+//     (NCLS MMAs), each lane keeps the sums of its own class.  All classes in one launch when the accumulators fit (rows of <= 16
+//     chunks: NCLS = 2 or 4, one CTA per SM), else one class per launch.  Rows longer than 2048 fields: column blocks of 32
+//     chunks, one launch each.
 #pragma once
 #include "pcal_gen.cuh"
 #include "pcal_tail.cuh"
@@ -60,26 +63,37 @@ constexpr uint32_t kG2StageBytes = 18432;                     // a padded tile: 
 constexpr uint32_t kG2Fields = 2048;                          // fields (positions) per row at most
 constexpr uint32_t kG2Batch = 4;                              // tiles per claim
 constexpr uint32_t kG2CapBatches = 256;                       // claims per CTA per launch: <= 1032 tiles keep the int32 digit sums exact
-constexpr uint32_t kG2MaxCh = 4;
+constexpr uint32_t kG2MaxCh = 16;                             // channels per launch at most (four per byte class, four classes)
 constexpr uint32_t kG2Invalid = 0xFFFFFFFFu;
+constexpr uint32_t kG2DigRG = 72;                             // words of a digit matrix (one channel, one group of 32 rows): 64 + 8 of padding
 constexpr uint32_t kG2TabRows = 512, kG2TabLo = 256, kG2TabHi = 128;      // generator tables per channel: rows of a batch, lo, hi
 constexpr uint32_t kG2TabStride = kG2TabRows + kG2TabLo + kG2TabHi;
 
 // Shared memory of a CTA (two CTAs share an SM): ring of sample tiles | ring of digit matrices (the generator runs that far
 // ahead of the consumers) | the generator's row table of one batch (4 tiles; when it fits) | barriers and bookkeeping
 constexpr size_t kG2SmemBudget = 115712 - 256;                // (228 KB - 2 x 1 KB reserved) / 2, less the kernel's static variables
-template <int C, int CPW> struct G2Cfg {
+constexpr size_t kG2SmemBudgetAlone = 232448 - 1024;          // one CTA per SM (several byte classes per launch: the accumulators need the registers)
+// C = channels per byte (1, 2, 4); NCLS = byte classes served by one launch (words of 8 / 16 channels: a time sample is 2 / 4 bytes,
+// "classes"; else 1); CPW = chunks per consumer warp
+template <int C, int CPW, int NCLS> struct G2Cfg {
+    static constexpr int CT = C * NCLS;                                        // channels of a launch
     static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
     static constexpr int DIGITS = C == 1 ? 8 : (C == 2 ? 6 : 4);
-    static constexpr uint32_t DIG_BYTES = (uint32_t)C * KG * 256;             // digit matrices of a tile: [C][KG][8 columns][32 rows]
     // generator work items per tile and lane: (channel, row quad) pairs / 32.  Three generator warps take the tiles of the
-    // CTA's sequence in turn.
-    static constexpr int KI = (C * RT / 4 + 31) / 32, NG = 3, THREADS = (kG2Consumers + 1 + NG) * 32;
-    static constexpr uint32_t TAB_BYTES = (uint32_t)C * 4 * RT * 16;          // exp(-j w_c span_t r), r < rows of a batch
+    // CTA's sequence in turn.  With more than 32 items LC = 32 / CT lanes share a channel; the per-channel strides of the
+    // digit matrices and of the row table are padded by LC words / entries, which spreads the lanes of a warp over the banks.
+    static constexpr int KI = (CT * RT / 4 + 31) / 32, NG = 3, THREADS = (kG2Consumers + 1 + NG) * 32;
+    static constexpr int LC = CT * RT / 4 <= 32 ? RT / 4 : 32 / CT;                                // lanes per channel
+    static constexpr int DIG_CH = KG * (int)kG2DigRG + (KI > 1 ? LC : 0);     // words of a channel's digit matrices [KG][8 columns][8 quads] (+ pad)
+    static constexpr uint32_t DIG_BYTES = (uint32_t)CT * DIG_CH * 4;          // digit matrices of a tile
+    static constexpr int TAB_CH = 4 * RT + (KI > 1 && LC < 8 ? LC : 0);       // entries of a channel's row table (+ pad)
+    static constexpr uint32_t TAB_BYTES = (uint32_t)CT * TAB_CH * 16;         // exp(-j w_c span_t r), r < rows of a batch
     static constexpr size_t FIXED = (size_t)DIGITS * DIG_BYTES + 1024;
-    static constexpr bool FIT5 = 5 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
-    static constexpr bool TAB_SMEM = FIT5 || 4 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= kG2SmemBudget;
-    static constexpr int TILES = FIT5 ? 5 : 4;
+    static constexpr size_t BUDGET = NCLS == 1 ? kG2SmemBudget : kG2SmemBudgetAlone;
+    static constexpr int MAXT = NCLS == 1 ? 5 : 8;                            // (alone on the SM: a deeper ring keeps as many bytes in flight as two CTAs would)
+    static constexpr bool TAB_SMEM = 4 * (size_t)kG2StageBytes + FIXED + TAB_BYTES <= BUDGET;
+    static constexpr size_t ROOM = BUDGET - FIXED - (TAB_SMEM ? TAB_BYTES : 0u);
+    static constexpr int TILES = ROOM / kG2StageBytes >= (size_t)MAXT ? MAXT : (int)(ROOM / kG2StageBytes);
     static constexpr size_t BYTES = (size_t)TILES * kG2StageBytes + FIXED + (TAB_SMEM ? TAB_BYTES : 0u);
 };
 
@@ -95,8 +109,8 @@ struct Gen2Params {
     int do_tail;                   // this launch also adds the ragged tail of the piece
     uint32_t pitch;                // row pitch in shared memory: row_bytes (+16 if chunks is even)
     uint32_t span_t;               // time samples per row (multiple of N_bins)
-    uint32_t cls_count, cls;       // words of 8 / 16 channels: a time sample is cls_count bytes, this launch serves byte `cls` of each
-                                   // (channels 4 cls .. 4 cls + 3; the other bytes' sums are not used); else 1, 0
+    uint32_t cls_count, cls;       // words of 8 / 16 channels: a time sample is cls_count bytes ("classes"), this launch serves bytes
+                                   // cls .. cls + NCLS - 1 of each (channels 4 cls ..; the other bytes' sums are not used); else 1, 0
     uint32_t c_real, c_base;       // channels in the stream; first channel of this launch
     uint64_t Fs;
     uint64_t Foff[kG2MaxCh];       // rotator frequency per channel (micro-hertz, k-shift included): ragged tail
@@ -121,9 +135,9 @@ struct Gen2Params {
     double2 *T_dev, *T_host, *P_copy;
 };
 
-template <int C, int CPW>
+template <int C, int CPW, int NCLS>
 constexpr size_t gen2_smem_bytes() {
-    return G2Cfg<C, CPW>::BYTES;
+    return G2Cfg<C, CPW, NCLS>::BYTES;
 }
 
 // ---- mbarrier / cp.async / ldmatrix helpers -----------------------------------------------------------------
@@ -217,18 +231,19 @@ __device__ __forceinline__ void g2_item_digits(const double2 base, const double2
 }
 
 // CPW = chunks per consumer warp (1, 2 or 4: rows of <= 8, 16, 32 chunks); a tile has KG = 4 / CPW groups of 32 rows
-template <int C, bool SIGN_MAG, int CPW>
-__global__ void __launch_bounds__(kG2Threads, 2) gen2_kernel(     // (bound for 384 threads: <= 80 registers, so that two CTAs leave room for a DFT CTA)
+template <int C, bool SIGN_MAG, int CPW, int NCLS>
+__global__ void __launch_bounds__(kG2Threads, NCLS == 1 ? 2 : 1) gen2_kernel(     // (two CTAs per SM: <= 80 registers; several classes: one CTA, <= 168)
 const __grid_constant__ Gen2Params P) {
+    static_assert(NCLS == 1 || C == 4, "several byte classes per launch: words of 8 / 16 channels");
     if (!P.input_ready) pdl_wait();
-    using Cfg = G2Cfg<C, CPW>;
-    constexpr int KG = Cfg::KG, RT = Cfg::RT;
+    using Cfg = G2Cfg<C, CPW, NCLS>;
+    constexpr int KG = Cfg::KG, RT = Cfg::RT, CT = Cfg::CT;
     constexpr int DEPTH = Cfg::TILES, DIGD = Cfg::DIGITS;
     constexpr int NG = Cfg::NG, NT = Cfg::THREADS;                            // generator warps, threads of the CTA
     constexpr uint32_t DIG_BYTES = Cfg::DIG_BYTES;
     extern __shared__ __align__(128) unsigned char g2_smem[];
     unsigned char* ring = g2_smem;                                            // [DEPTH] padded sample tiles
-    unsigned char* dig = ring + (size_t)DEPTH * kG2StageBytes;                // [DIGD][C][KG][8][32]
+    unsigned char* dig = ring + (size_t)DEPTH * kG2StageBytes;                // [DIGD][CT] digit matrices (Cfg::DIG_CH words each)
     double2* tab_s = reinterpret_cast<double2*>(dig + (size_t)DIGD * DIG_BYTES);    // [C][4 tiles][4][RT / 4] row phasors of a batch (TAB_SMEM)
     uint64_t* bars = reinterpret_cast<uint64_t*>(dig + (size_t)DIGD * DIG_BYTES + (Cfg::TAB_SMEM ? Cfg::TAB_BYTES : 0u));   // full, empty [DEPTH]; digfull, digempty [DIGD]; ticket
     uint32_t* dig_tile = reinterpret_cast<uint32_t*>(bars + 2 * DEPTH + 2 * DIGD + 1);   // [DIGD] tile of a digit entry
@@ -250,46 +265,47 @@ const __grid_constant__ Gen2Params P) {
     }
     __syncthreads();
 
-    int acc[CPW][4][4];               // [chunk of this warp][combination u][C fragment]
+    int acc[NCLS][CPW][4][4];         // [byte class][chunk of this warp][combination u][C fragment]
 #pragma unroll
-    for (int c = 0; c < CPW; ++c)
+    for (int q = 0; q < NCLS; ++q)
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int c = 0; c < CPW; ++c)
 #pragma unroll
-            for (int k = 0; k < 4; ++k) acc[c][u][k] = 0;
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc[q][c][u][k] = 0;
 
     if (warp >= 1 && warp <= NG) {
         const int gw = warp - 1;                                  // generator warp gw: tiles gw, gw + NG, ... of the CTA's sequence
-        // ---------------- generator: owns the CTA's tile sequence; digit matrices of a batch of tiles, lane = row ----------------
+        // ---------------- generators: own the CTA's tile sequence; digit matrices of a batch of tiles ----------------
         // Batches: the CTA's own index and index + grid first (no round trip before the first tiles), then claims from the
-        // launch's counter, each issued one batch ahead.  A claimed batch is always processed: claiming stops with the first
+        // launch's counter, each issued two batches ahead.  A claimed batch is always processed: claiming stops with the first
         // batch number past the end.
         // The four digit bytes of a column for rows 4q .. 4q+3 are one 32-bit word of the B fragment (row group q / 8, K slots
         // 4 (q % 8) ..; columns 0..3 = Re digits, 4..7 = Im digits).
-        // Work items: (channel, four consecutive rows), g2_item_digits.  A tile has Q = RT / 4 row quads; lane l of generator
-        // a generator warp serves quad l % Q of channels l / Q + k (32 / Q), k = 0 .. KI-1.
-        constexpr int Q = RT / 4, CHP = 32 / Q, KI = Cfg::KI;
-        const int g_ch0 = lane / Q, g_quad = lane % Q;
-        constexpr int KS = CHP;                                                 // channel step from item to item
-        // the row phasors of a batch, from shared memory (an L2 round trip per tile is what this warp cannot afford): row
+        // Work items: (channel, four consecutive rows), g2_item_digits.  A tile has Q = RT / 4 row quads per channel.  A lane
+        // serves ONE channel (one batch phasor, one set of digit sums): with CT Q <= 32 items lane l takes quad l % Q of
+        // channel l / Q; else 32 / CT lanes share a channel and take its quads in turn (KI items per lane and tile).
+        constexpr int Q = RT / 4, KI = Cfg::KI;
+        constexpr int LC = Cfg::LC, DIG_CH = Cfg::DIG_CH, TAB_CH = Cfg::TAB_CH;   // lanes per channel; padded per-channel strides
+        const int g_ch = lane / LC, g_sub = lane % LC;                          // channel, first quad (quads g_sub + k LC)
+        const bool g_on = g_ch < CT;
+        const int g_chc = g_on ? g_ch : 0;
+        // the row phasors of a batch, from shared memory (an L2 round trip per tile is what these warps cannot afford): row
         // r = RT j + 4 q + i of channel c at [c][j][i][q], so that the lanes of a load are neighbours
         if (Cfg::TAB_SMEM) {
-            for (int x = lane + 32 * gw; x < KI * CHP * 4 * RT; x += 32 * NG) {                 // (each warp a third of the entries)
-                const int cl = x / (4 * RT), r = x % (4 * RT);
-                const int c = cl;
-                if (c < C) tab_s[c * 4 * RT + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
+            for (int x = lane + 32 * gw; x < CT * 4 * RT; x += 32 * NG) {                       // (each warp a third of the entries)
+                const int c = x / (4 * RT), r = x % (4 * RT);
+                tab_s[c * TAB_CH + ((r / RT) * 4 + (r & 3)) * Q + (r % RT) / 4] = __ldg(P.gtab + (size_t)c * kG2TabStride + r);
             }
             asm volatile("bar.sync 1, %0;" ::"n"(32 * NG) : "memory");
         }
         auto cmul = [](const double2 a, const double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); };
         // column sums of the digit matrices of this lane's items: the sum of the quantised phasors over the CTA's rows, which
-        // the level offset -3 of every sample needs (rows that do not exist have zero digits; four digits of at most 128 per tile and lane: no overflow)
-        int dsum[KI][8];
+        // the level offset -3 of every sample needs (rows that do not exist have zero digits; four digits of at most 128 per item: no overflow)
+        int dsum[8];
 #pragma unroll
-        for (int k = 0; k < KI; ++k)
-#pragma unroll
-            for (int d = 0; d < 8; ++d) dsum[k][d] = 0;
-        const uint32_t g_word = (uint32_t)(g_quad >> 3) * 64u + (uint32_t)(g_quad & 7);   // word of (row group, column 0, K slots) in a channel's digits
+        for (int d = 0; d < 8; ++d) dsum[d] = 0;
         // The CTA's batch sequence: positions 0 .. n_static-1 are its own (index + position * grid: most of the launch,
         // no round trips), the rest are claims from the launch's counter.  Claims are two positions ahead -- the first two
         // were made by the ticket thread -- so a claim has two batches' time to come back.
@@ -299,28 +315,19 @@ const __grid_constant__ Gen2Params P) {
         bool have_seq = false;
         uint32_t* ctr = nullptr;
         const uint32_t dyn0 = P.n_static * gridDim.x;          // first claimed batch number
-        auto load_tabs = [&](uint32_t b, double2 (&thi)[KI], double2 (&tlo)[KI]) {
-#pragma unroll
-            for (int k = 0; k < KI; ++k) {
-                const int ch = k * KS + g_ch0;
-                const double2* tab = P.gtab + (size_t)(ch < C ? ch : 0) * kG2TabStride;
-                thi[k] = __ldg(tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
-                tlo[k] = __ldg(tab + kG2TabRows + (b & 255u));
-            }
+        const double2* g_tab = P.gtab + (size_t)g_chc * kG2TabStride;
+        auto load_tabs = [&](uint32_t b, double2& thi, double2& tlo) {
+            thi = __ldg(g_tab + kG2TabRows + kG2TabLo + ((b >> 8) & (kG2TabHi - 1u)));
+            tlo = __ldg(g_tab + kG2TabRows + (b & 255u));
         };
-        double2 thi[KI], tlo[KI];
+        double2 thi, tlo;
         load_tabs(batch, thi, tlo);
         while (batch < P.n_batches) {
             const uint32_t tile0 = batch * kG2Batch;
             const uint32_t nt = P.n_tiles - tile0 < kG2Batch ? P.n_tiles - tile0 : kG2Batch;
             const bool all_rows = (uint64_t)(tile0 + kG2Batch) * RT <= P.n_rows;      // (all but the last batch of a piece)
-            double2 base[KI];                                   // batch phasor of this lane's channels, scaled by 2^30
-#pragma unroll
-            for (int k = 0; k < KI; ++k) {
-                const int ch = k * KS + g_ch0;
-                base[k] = cmul(cmul(P.base0[ch < C ? ch : 0], thi[k]), tlo[k]);
-                base[k].x *= 1073741824.0; base[k].y *= 1073741824.0;
-            }
+            double2 base = cmul(cmul(P.base0[g_chc], thi), tlo);                      // batch phasor of this lane's channel, scaled by 2^30
+            base.x *= 1073741824.0; base.y *= 1073741824.0;
             // the next batch of the sequence, and its table entries on their way while this batch is built
             uint32_t nbatch;
             if (pos + 1 < P.n_static) {
@@ -346,57 +353,75 @@ const __grid_constant__ Gen2Params P) {
                 nbatch = s_gen[6 + (pos & 1u)];
             }
             load_tabs(nbatch, thi, tlo);
-            // UJ tiles at a time: their (independent) phasor chains overlap
-            constexpr uint32_t UJ = KI == 1 ? 2u : 1u;
+            // digit words of item k of tile jt of the batch
+            auto item = [&](uint32_t jt, int k, uint32_t (&w)[8]) {
+                const uint32_t quad = (uint32_t)(g_sub + k * LC);
+                const uint32_t rb = jt * RT + 4u * quad;                                // first of the item's rows in the batch
+                double2 row[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    row[i] = Cfg::TAB_SMEM ? tab_s[g_chc * TAB_CH + (jt * 4 + i) * Q + quad]
+                                           : __ldg(g_tab + (rb + i) % kG2TabRows);
+                if (all_rows) {
+                    g2_item_digits<true>(base, row, 4u, w);
+                } else {
+                    const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
+                    const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
+                    g2_item_digits<false>(base, row, nv, w);
+                }
+            };
+            auto store = [&](uint32_t* dg, int k, const uint32_t (&w)[8]) {
+                const uint32_t quad = (uint32_t)(g_sub + k * LC);
+                // word of (channel, row group, column, K slots 4 q7 ..), q7 = quad % 8: at column * 8 + 2 (q7 % 4) + q7 / 4, so that the
+                // two B-fragment registers of consumer lane (g = column, t = q7 % 4) are ONE 64-bit load at word 2 * lane; row groups
+                // are kG2DigRG = 72 words apart, which spreads the 32 quads of a single-channel tile over all banks
+                uint32_t* d = dg + g_ch * DIG_CH + (quad >> 3) * kG2DigRG + 2u * (quad & 3u) + ((quad >> 2) & 1u);
+#pragma unroll
+                for (int col = 0; col < 8; ++col) {
+                    d[col * 8] = w[col];
+                    dsum[col] = __dp4a((int)w[col], 0x01010101, dsum[col]);
+                }
+            };
             constexpr uint32_t JS = (uint32_t)NG;               // tile step of this warp inside a batch
             const uint32_t jf = ((uint32_t)gw + NG - it % NG) % NG;               // its first tile: tiles of the CTA's sequence in turn
+            if constexpr (KI == 1) {
+                // two tiles at a time: their (independent) phasor chains overlap; computed before the entry is waited for
 #pragma unroll 1
-            for (uint32_t j0 = jf; j0 < nt; j0 += UJ * JS) {
-                uint32_t w[UJ][KI][8];
+                for (uint32_t j0 = jf; j0 < nt; j0 += 2 * JS) {
+                    uint32_t w[2][8];
 #pragma unroll
-                for (uint32_t ju = 0; ju < UJ; ++ju) {
-                    const uint32_t jt = j0 + ju * JS < kG2Batch ? j0 + ju * JS : kG2Batch - 1u;   // tile of the batch (past the batch: computed, not stored)
-                    const uint32_t rb = jt * RT + 4u * (uint32_t)g_quad;                    // first of this lane's rows in the batch
+                    for (uint32_t ju = 0; ju < 2; ++ju)
+                        item(j0 + ju * JS < kG2Batch ? j0 + ju * JS : kG2Batch - 1u, 0, w[ju]);      // (past the batch: computed, not stored)
 #pragma unroll
-                    for (int k = 0; k < KI; ++k) {
-                        const int ch = k * KS + g_ch0;
-                        const int chc = ch < C ? ch : 0;
-                        double2 row[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            row[i] = Cfg::TAB_SMEM ? tab_s[chc * 4 * RT + (jt * 4 + i) * Q + g_quad]
-                                                   : __ldg(P.gtab + (size_t)chc * kG2TabStride + (rb + i) % kG2TabRows);
-                        if (all_rows) {
-                            g2_item_digits<true>(base[k], row, 4u, w[ju][k]);
-                        } else {
-                            const uint64_t r_abs = (uint64_t)tile0 * RT + rb;
-                            const uint32_t nv = r_abs < P.n_rows ? (P.n_rows - r_abs < 4u ? (uint32_t)(P.n_rows - r_abs) : 4u) : 0u;   // valid rows from there on
-                            g2_item_digits<false>(base[k], row, nv, w[ju][k]);
+                    for (uint32_t ju = 0; ju < 2; ++ju) {
+                        const uint32_t j = j0 + ju * JS;
+                        if (j < nt) {
+                            const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
+                            mbar_wait(dempty0 + 8 * e, ph ^ 1u);          // the consumers are done with the entry's previous tile
+                            if (g_on) store(reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES), 0, w[ju]);
+                            if (lane == 0) dig_tile[e] = tile0 + j;
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(dfull0 + 8 * e);
                         }
                     }
                 }
-#pragma unroll
-                for (uint32_t ju = 0; ju < UJ; ++ju) {
-                    const uint32_t j = j0 + ju * JS;
-                    if (j < nt) {
-                        const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
-                        mbar_wait(dempty0 + 8 * e, ph ^ 1u);          // the consumers are done with the entry's previous tile
-                        uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES) + g_word;
-#pragma unroll
-                        for (int k = 0; k < KI; ++k) {
-                            const int ch = k * KS + g_ch0;
-                            if (ch < C) {
-#pragma unroll
-                                for (int col = 0; col < 8; ++col) {
-                                    dg[ch * KG * 64 + col * 8] = w[ju][k][col];
-                                    dsum[k][col] = __dp4a((int)w[ju][k][col], 0x01010101, dsum[k][col]);
-                                }
-                            }
-                        }
-                        if (lane == 0) dig_tile[e] = tile0 + j;
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(dfull0 + 8 * e);
+            } else {
+                // several items per lane and tile: item by item into the entry (two in flight)
+#pragma unroll 1
+                for (uint32_t j = jf; j < nt; j += JS) {
+                    const uint32_t e = (it + j) % DIGD, ph = ((it + j) / DIGD) & 1u;
+                    mbar_wait(dempty0 + 8 * e, ph ^ 1u);
+                    uint32_t* dg = reinterpret_cast<uint32_t*>(dig + (size_t)e * DIG_BYTES);
+#pragma unroll 1
+                    for (int k = 0; k < KI; k += 2) {
+                        uint32_t w[2][8];
+                        item(j, k, w[0]);
+                        item(j, k + 1, w[1]);
+                        if (g_on) { store(dg, k, w[0]); store(dg, k + 1, w[1]); }
                     }
+                    if (lane == 0) dig_tile[e] = tile0 + j;
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(dfull0 + 8 * e);
                 }
             }
             it += nt;
@@ -407,19 +432,17 @@ const __grid_constant__ Gen2Params P) {
             mbar_wait(dempty0 + 8 * e, ph ^ 1u);
             if (lane == 0 && gw == 0) { dig_tile[e] = kG2Invalid; mbar_arrive(dfull0 + 8 * e); }
         }
+        {
+            long long re = (long long)dsum[0] + ((long long)dsum[1] << 8) + ((long long)dsum[2] << 16) + ((long long)dsum[3] << 24);
+            long long im = (long long)dsum[4] + ((long long)dsum[5] << 8) + ((long long)dsum[6] << 16) + ((long long)dsum[7] << 24);
 #pragma unroll
-        for (int k = 0; k < KI; ++k) {
-            long long re = (long long)dsum[k][0] + ((long long)dsum[k][1] << 8) + ((long long)dsum[k][2] << 16) + ((long long)dsum[k][3] << 24);
-            long long im = (long long)dsum[k][4] + ((long long)dsum[k][5] << 8) + ((long long)dsum[k][6] << 16) + ((long long)dsum[k][7] << 24);
-#pragma unroll
-            for (int sh = Q / 2; sh > 0; sh >>= 1) {           // the lanes of a channel: Q consecutive ones
+            for (int sh = LC / 2; sh > 0; sh >>= 1) {          // the lanes of a channel: LC consecutive ones
                 re += __shfl_xor_sync(0xFFFFFFFFu, re, sh);
                 im += __shfl_xor_sync(0xFFFFFFFFu, im, sh);
             }
-            const int ch = k * KS + g_ch0;
-            if (g_quad == 0 && ch < C) {      // (every generator warp holds a part)
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][0]), (unsigned long long)re);
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[ch][1]), (unsigned long long)im);
+            if (g_sub == 0 && g_on) {         // (every generator warp holds a part)
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[g_ch][0]), (unsigned long long)re);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_rsum[g_ch][1]), (unsigned long long)im);
             }
         }
     } else if (warp == 0) {
@@ -463,7 +486,7 @@ const __grid_constant__ Gen2Params P) {
         }
     } else {
         // ---------------- consumers: warp cw owns chunks CPW cw .. CPW cw + CPW - 1 of every row ----------------
-        const int cw = warp - 1 - NG, g = lane >> 2, t = lane & 3;
+        const int cw = warp - 1 - NG;
         if (cw == 0 && lane == 0) {
             // ticket: sequence number of this launch, derived on the device (pcal_tail.cuh, "Pipelining"); taken before the
             // loader lets the dependent grid start.  The slot's previous user (launch seq - kTailSlots) must have finished
@@ -486,7 +509,9 @@ const __grid_constant__ Gen2Params P) {
         const uint32_t nch = P.chunks > first ? (P.chunks - first < (uint32_t)CPW ? P.chunks - first : (uint32_t)CPW) : 0u;   // this warp's chunks
         const uint32_t kg_step = 32u * P.pitch;
         // one chunk of one row group: byte column -> four masked operands -> four MMAs
-        auto chunk_mma = [&](int c, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, const uint32_t (&bf)[C][2]) {
+        // (several classes: the masked operand meets the digits of channel u of EVERY class -- an MMA's 16 byte columns hold all
+        //  classes, each lane keeps the sums of its own; the B fragments come straight from the digit entry, `dgk` = row group kg)
+        auto chunk_mma = [&](int c, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, const uint32_t (&bf)[C][2], const uint32_t* dgk) {
             if (SIGN_MAG) {
                 a0 = signmag_to_offset_binary(a0); a1 = signmag_to_offset_binary(a1);
                 a2 = signmag_to_offset_binary(a2); a3 = signmag_to_offset_binary(a3);
@@ -495,8 +520,17 @@ const __grid_constant__ Gen2Params P) {
             for (int u = 0; u < 4; ++u) {
                 const uint32_t m = g2_mask<C>(u);
                 const int ch = g2_chan<C>(u);
-                if (m == 0xFFFFFFFFu) mma_u8s8_k32(acc[c][u], a0, a1, a2, a3, bf[ch][0], bf[ch][1]);
-                else mma_u8s8_k32(acc[c][u], a0 & m, a1 & m, a2 & m, a3 & m, bf[ch][0], bf[ch][1]);
+                if constexpr (NCLS == 1) {
+                    if (m == 0xFFFFFFFFu) mma_u8s8_k32(acc[0][c][u], a0, a1, a2, a3, bf[ch][0], bf[ch][1]);
+                    else mma_u8s8_k32(acc[0][c][u], a0 & m, a1 & m, a2 & m, a3 & m, bf[ch][0], bf[ch][1]);
+                } else {
+                    const uint32_t x0 = a0 & m, x1 = a1 & m, x2 = a2 & m, x3 = a3 & m;
+#pragma unroll
+                    for (int q = 0; q < NCLS; ++q) {
+                        const uint2 b = *reinterpret_cast<const uint2*>(dgk + (q * C + ch) * Cfg::DIG_CH + 2 * lane);
+                        mma_u8s8_k32(acc[q][c][u], x0, x1, x2, x3, b.x, b.y);
+                    }
+                }
             }
         };
         for (uint32_t it = 0;; ++it) {
@@ -506,10 +540,12 @@ const __grid_constant__ Gen2Params P) {
             const uint32_t tile = dig_tile[e];
             const uint32_t* dg32 = reinterpret_cast<const uint32_t*>(dig + (size_t)e * DIG_BYTES);
             auto load_bf = [&](int kg, uint32_t (&bf)[C][2]) {
+                if constexpr (NCLS == 1) {
 #pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    bf[c][0] = dg32[(c * KG + kg) * 64 + g * 8 + t];
-                    bf[c][1] = dg32[(c * KG + kg) * 64 + g * 8 + 4 + t];
+                    for (int c = 0; c < C; ++c) {
+                        const uint2 b = *reinterpret_cast<const uint2*>(dg32 + c * Cfg::DIG_CH + kg * kG2DigRG + 2 * lane);
+                        bf[c][0] = b.x; bf[c][1] = b.y;
+                    }
                 }
             };
             const uint32_t base = my + s * kG2StageBytes;
@@ -521,12 +557,42 @@ const __grid_constant__ Gen2Params P) {
 #pragma unroll
                     for (int c = 0; c < CPW; ++c) ldsm_t8_x2(base + kg * kg_step + 16u * c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3]);
                 if (tile == kG2Invalid) break;
+                if constexpr (NCLS == 1) {
 #pragma unroll
-                for (int kg = 0; kg < KG; ++kg) {
-                    uint32_t bf[C][2];
-                    load_bf(kg, bf);
+                    for (int kg = 0; kg < KG; ++kg) {
+                        uint32_t bf[C][2];
+                        load_bf(kg, bf);
 #pragma unroll
-                    for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf);
+                        for (int c = 0; c < CPW; ++c) chunk_mma(c, a[kg][c][0], a[kg][c][1], a[kg][c][2], a[kg][c][3], bf, dg32 + kg * kG2DigRG);
+                    }
+                } else {
+                    // several classes: per row group and combination u the B fragments of channel u of every class are loaded
+                    // once (2 NCLS registers) and meet the masked operands of all of this warp's chunks
+#pragma unroll
+                    for (int kg = 0; kg < KG; ++kg) {
+                        if (SIGN_MAG) {
+#pragma unroll
+                            for (int c = 0; c < CPW; ++c)
+#pragma unroll
+                                for (int r = 0; r < 4; ++r) a[kg][c][r] = signmag_to_offset_binary(a[kg][c][r]);
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            uint32_t bq[NCLS][2];
+#pragma unroll
+                            for (int q = 0; q < NCLS; ++q) {
+                                const uint2 b = *reinterpret_cast<const uint2*>(dg32 + kg * kG2DigRG + (q * C + g2_chan<C>(u)) * Cfg::DIG_CH + 2 * lane);
+                                bq[q][0] = b.x; bq[q][1] = b.y;
+                            }
+                            const uint32_t m = g2_mask<C>(u);
+#pragma unroll
+                            for (int c = 0; c < CPW; ++c) {
+                                const uint32_t x0 = a[kg][c][0] & m, x1 = a[kg][c][1] & m, x2 = a[kg][c][2] & m, x3 = a[kg][c][3] & m;
+#pragma unroll
+                                for (int q = 0; q < NCLS; ++q) mma_u8s8_k32(acc[q][c][u], x0, x1, x2, x3, bq[q][0], bq[q][1]);
+                            }
+                        }
+                    }
                 }
             } else {
                 if (tile == kG2Invalid) break;
@@ -539,7 +605,7 @@ const __grid_constant__ Gen2Params P) {
                         if ((uint32_t)c < nch) {
                             uint32_t a0, a1, a2, a3;
                             ldsm_t8_x2(base + kg * kg_step + 16u * c, a0, a1, a2, a3);
-                            chunk_mma(c, a0, a1, a2, a3, bf);
+                            chunk_mma(c, a0, a1, a2, a3, bf, dg32 + kg * kG2DigRG);
                         }
                     }
                 }
@@ -558,18 +624,30 @@ const __grid_constant__ Gen2Params P) {
         const int cw = warp - 1 - NG, g = lane >> 2, t = lane & 3;
 #pragma unroll
         for (int c = 0; c < CPW; ++c) {
+            // this lane's byte columns (g, g + 8 of every chunk) belong to one byte class: the sums of that class
+            const uint32_t kcls = (uint32_t)g % P.cls_count - P.cls;          // class index inside the launch (wraps when below it)
+            const bool mine = kcls < (uint32_t)NCLS;                           // (8 / 16 channels: the bytes of this launch's channels)
+            int A[4][4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    A[u][k] = acc[0][c][u][k];
+#pragma unroll
+                    for (int q = 1; q < NCLS; ++q) if (kcls == (uint32_t)q) A[u][k] = acc[q][c][u][k];
+                }
             // field sums from the combination sums (exact: every U is a sum of non-negative multiples of the S)
             int S[4][4];              // [field f][C fragment], field f scaled by 4^f
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 if (C == 1) {
-                    S[0][k] = acc[c][0][k] - acc[c][1][k]; S[1][k] = acc[c][1][k] - acc[c][2][k];
-                    S[2][k] = acc[c][2][k] - acc[c][3][k]; S[3][k] = acc[c][3][k];
+                    S[0][k] = A[0][k] - A[1][k]; S[1][k] = A[1][k] - A[2][k];
+                    S[2][k] = A[2][k] - A[3][k]; S[3][k] = A[3][k];
                 } else if (C == 2) {
-                    S[0][k] = acc[c][0][k] - acc[c][2][k]; S[1][k] = acc[c][1][k] - acc[c][3][k];
-                    S[2][k] = acc[c][2][k]; S[3][k] = acc[c][3][k];
+                    S[0][k] = A[0][k] - A[2][k]; S[1][k] = A[1][k] - A[3][k];
+                    S[2][k] = A[2][k]; S[3][k] = A[3][k];
                 } else {
-                    S[0][k] = acc[c][0][k]; S[1][k] = acc[c][1][k]; S[2][k] = acc[c][2][k]; S[3][k] = acc[c][3][k];
+                    S[0][k] = A[0][k]; S[1][k] = A[1][k]; S[2][k] = A[2][k]; S[3][k] = A[3][k];
                 }
             }
 #pragma unroll
@@ -585,8 +663,7 @@ const __grid_constant__ Gen2Params P) {
                     if (!(t & 1)) {
                         const uint32_t bytecol = (uint32_t)(cw * CPW + c) * 16u + (uint32_t)g + 8u * hi;
                         const uint32_t F = 4u * bytecol + (uint32_t)f;
-                        const bool mine = bytecol % P.cls_count == P.cls;       // (8 / 16 channels: the bytes of this launch's channels)
-                        pos_s[2 * F + ri] = mine ? 2 * v - 3 * s_rsum[f % C][ri] : 0;    // codes 0..3 -> levels 2 code - 3
+                        pos_s[2 * F + ri] = mine ? 2 * v - 3 * s_rsum[kcls * C + f % C][ri] : 0;    // codes 0..3 -> levels 2 code - 3
                     }
                 }
         }
@@ -608,7 +685,7 @@ const __grid_constant__ Gen2Params P) {
     if (tid == 0) { seen_done = ld_acquire_u32(&P.st->n_done); seen_dft = ld_acquire_u32(&P.st->dft_finished); }
     long long* gacc = P.posacc + (size_t)slot * 2 * kG2Fields;
     for (uint32_t i = tid; i < nval; i += NT) { pos_s[i] = __ldcg(gacc + i); gacc[i] = 0; }     // and ready for the slot's next launch
-    const uint32_t pairs = (uint32_t)C * P.n_bins, n_tail = (uint32_t)(P.n_total - P.n_body);
+    const uint32_t pairs = (uint32_t)CT * P.n_bins, n_tail = (uint32_t)(P.n_total - P.n_body);
     double2* sP = reinterpret_cast<double2*>(ring + 2 * kG2Fields * sizeof(long long));               // [pairs] (fused DFT)
     const uint32_t dft_x = s_gen[1];
     __syncthreads();
@@ -637,7 +714,7 @@ const __grid_constant__ Gen2Params P) {
             // tau0 + tau = b - n0 (mod N_bins), in order
             uint32_t tau = b + tau_first; if (tau >= P.n_bins) tau -= P.n_bins;
             for (; tau < n_tau; tau += P.n_bins) {
-                const uint32_t F = (tau * P.cls_count + P.cls) * C + c;
+                const uint32_t F = (tau * P.cls_count + P.cls + c / C) * C + c % C;       // (class of channel c: c / C)
                 const double xr = (double)pos_s[2 * F] * (1.0 / 1073741824.0), xi = (double)pos_s[2 * F + 1] * (1.0 / 1073741824.0);
                 const double2 w = __ldg(tw + tau);
                 re += xr * w.x - xi * w.y;
@@ -663,7 +740,7 @@ const __grid_constant__ Gen2Params P) {
     if (P.fuse_dft) {   // T[c] = DFT(P[c]), channel by channel, from shared memory
         __syncthreads();
         double2* sY = sP + pairs;
-        dft_in_cta(sP, sY, P.W, (uint32_t)C, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev, P.T_host, NT);
+        dft_in_cta(sP, sY, P.W, (uint32_t)CT, P.n_bins, P.dft_n1, P.k_shift % P.n_bins, P.T_dev, P.T_host, NT);
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
     __syncthreads();
