@@ -470,6 +470,31 @@ def test_generator_row_lengths(oracle, monkeypatch, C, enc, chunks):
     p.destroy()
 
 
+@pytest.mark.parametrize("C,ncls", [(8, "1"), (16, "1"), (16, "2")])
+def test_generator_byte_classes_per_launch(oracle, monkeypatch, C, ncls):
+    """Words of 8 / 16 channels through the 2-bit generator kernel with fewer byte classes per launch than the default (all of
+    them in one launch): PCAL_G2_NCLS = 1 (one launch per four channels) and 2 (16 channels in two launches)."""
+    from paper_2501_05993_b200 import binding
+    monkeypatch.setenv("PCAL_G2_NCLS", ncls)
+    n = 700_004
+    rs = np.random.RandomState(4400 + C + int(ncls))
+    packed = rs.randint(0, 256, size=n * 2 * C // 8).astype(np.uint8)
+    offs = [1234.567 + 100321.0123 * c for c in range(C)]
+    p = binding.Pcal(64e6, 1e6, 0.0, 2, 1, C)
+    p.set_channel_offsets(offs)
+    p.set_rotator(binding.ROT_GENERATOR)
+    dev = torch.from_numpy(packed).cuda()
+    launches0 = p.info().kernel_launches
+    p.extract(dev, n)
+    assert p.info().kernel_launches - launches0 == C // 4 // int(ncls)
+    T, P = p.finalize(), p.get_folded()
+    for c in sorted(set(int(x) for x in rs.randint(0, C, size=5))):
+        pr, pi = oracle.fold_ld(packed, oracle.TWO_BIT_SIGN_MAG, C, c, 0, 1, n, 0, 64e6, 1e6, offs[c], tabulated=False, threads=8)
+        assert_close(P[c], pr.astype(np.float64) + 1j * pi.astype(np.float64), f"C={C} ncls={ncls} ch{c} folded")
+        assert_close(T[c], oracle.dft(pr, pi), f"C={C} ncls={ncls} ch{c} tones")
+    p.destroy()
+
+
 def test_exchange_step_in_one_launch(oracle):
     """What bench.py does per step with N ranks, emulated on one GPU: every "rank" folds its time shard at
     its absolute start index, the bins are gathered into one buffer (stand-in for the NCCL all-gather) and
