@@ -78,7 +78,7 @@ constexpr size_t kG2SmemBudgetAlone = 232448 - 1024;          // one CTA per SM 
 template <int C, int CPW, int NCLS> struct G2Cfg {
     static constexpr int CT = C * NCLS;                                        // channels of a launch
     static constexpr int KG = 4 / CPW, RT = 32 * KG;                          // row groups (K = 32 rows each) and rows per tile
-    static constexpr int DIGITS = NCLS == 1 ? (C == 1 ? 8 : (C == 2 ? 6 : 4)) : (NCLS == 2 ? 8 : 8);   // digit entries: how far the generators run ahead
+    static constexpr int DIGITS = 8;   // digit entries: how far the generators run ahead
     // generator work items per tile and lane: (channel, row quad) pairs / 32.  Three generator warps take the tiles of the
     // CTA's sequence in turn.  With more than 32 items LC = 32 / CT lanes share a channel; the per-channel strides of the
     // digit matrices and of the row table are padded by LC words / entries, which spreads the lanes of a warp over the banks.
