@@ -301,10 +301,22 @@ __global__ void __launch_bounds__(kThreads, 2) gen_kernel(const __grid_constant_
     // reader must have finished
     if (!P.tail.st) pdl_wait();
     double2* partial = P.tail.st ? gen_partial_of(P.tail, s_gen) : P.tail.partial + (size_t)blockIdx.x * P.n_bins;
-    for (uint32_t sb = tid; sb < P.n_bins; sb += kThreads) {
+    // positions -> bins: tpb threads per bin (a power of two, consecutive lanes; with few bins a single thread per bin would add
+    // span / N_bins values one after the other -- 1 us for 16 bins), each adds every tpb-th position of its bin, then a shuffle tree:
+    // a fixed order
+    uint32_t tpb = 1;
+    while (tpb < 32u && 2u * tpb * P.n_bins <= (uint32_t)kThreads) tpb *= 2u;
+    const uint32_t bins_per_pass = (uint32_t)kThreads / tpb;
+    for (uint32_t sb0 = 0; sb0 < P.n_bins; sb0 += bins_per_pass) {          // uniform trip count (shuffles below)
+        const uint32_t sb = sb0 + (uint32_t)tid / tpb, j = (uint32_t)tid % tpb;
         double re = 0.0, im = 0.0;
-        for (uint32_t pos = sb; pos < P.span; pos += P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
-        partial[sb] = make_double2(re, im);
+        if (sb < P.n_bins)
+            for (uint32_t pos = sb + j * P.n_bins; pos < P.span; pos += tpb * P.n_bins) { re += pos_re[pos]; im += pos_im[pos]; }
+        for (uint32_t sh = tpb >> 1; sh > 0; sh >>= 1) {
+            re += __shfl_xor_sync(0xFFFFFFFFu, re, sh);
+            im += __shfl_xor_sync(0xFFFFFFFFu, im, sh);
+        }
+        if (sb < P.n_bins && j == 0) partial[sb] = make_double2(re, im);
     }
     if (P.tail.st) gen_tail(P.tail, s_gen, reinterpret_cast<double2*>(gen_smem));
 }
