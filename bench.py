@@ -432,7 +432,7 @@ def measure(idx: int, steps: int, warmup: int, rank: int, world: int, device, do
     return res, w
 
 
-ROWS = [(1, None), (2, None), (3, "lut"), (3, "generator"), (4, None), (5, None), (8, "lut"), (8, "generator")]   # 8 = the paper's own benchmark shape
+ROWS = [(1, None), (2, None), (3, "lut"), (3, "generator"), (4, None), (4, "generator"), (5, None), (8, "lut"), (8, "generator")]   # 8 = the paper's own benchmark shape
 
 
 def reference_line(args):
