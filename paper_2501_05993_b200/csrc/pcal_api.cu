@@ -351,6 +351,13 @@ static int prepare(pcal_ctx* c) {
             // and for the CTAs of a DFT kernel: the next launch must become resident in one wave
             const uint32_t reserve = 2 * (q + 1) + dft_ctas(c) + 8;
             if (slots > reserve + q) c->R = (slots - reserve) / q;
+            // Half of that when it still gives every SM a CTA: the CTAs of TWO consecutive launches then fit on the machine, so a
+            // launch streams while its predecessor is in its prologue or tail instead of waiting for the predecessor's slots
+            // (measured, steps back to back: config 1 4.5 (or 6.0: two regimes) -> 3.6 us, config 2 11.3 -> 10.0 us, config 3
+            // 19.5 -> 18.4 us, config 4 40.4 -> 36.0 us; a launch on its own is 5-20 % slower).  PCAL_FOLD_FULL_GRID=1: the full grid.
+            const char* fg = getenv("PCAL_FOLD_FULL_GRID");
+            if (!(fg && fg[0] == '1') && slots > reserve + 2 * q && (slots - reserve) / (2 * q) * q >= (uint32_t)c->sm_count)
+                c->R = (slots - reserve) / (2 * q);
             const uint32_t W = 32u * c->spv, per = W / c->n_bins ? W / c->n_bins : 1u;
             uint32_t tpp = 1; while (tpp * 2 <= per && tpp < 32) tpp *= 2;
             c->tail_tpp = tpp;
