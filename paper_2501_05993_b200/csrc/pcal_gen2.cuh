@@ -491,9 +491,10 @@ const __grid_constant__ Gen2Params P) {
             // ticket: sequence number of this launch, derived on the device (pcal_tail.cuh, "Pipelining"); taken before the
             // loader lets the dependent grid start.  The slot's previous user (launch seq - kTailSlots) must have finished
             // before the slot's counters are touched.
+            const unsigned long long tk = atomicAdd(&P.st->tick, 1ull);   // (ticket and acquire load in flight together: pcal_tail.cuh)
             uint32_t done, x;
             ld_acquire_done_started(P.st, done, x);
-            const uint32_t sq = (uint32_t)(atomicAdd(&P.st->tick, 1ull) / gridDim.x);
+            const uint32_t sq = (uint32_t)(tk / gridDim.x);
             s_gen[0] = sq; s_gen[1] = x;
             if ((int32_t)(done - (sq - kTailSlots + 1u)) < 0)
                 while ((int32_t)(ld_acquire_u32(&P.st->n_done) - (sq - kTailSlots + 1u)) < 0) __nanosleep(64);

@@ -30,9 +30,10 @@ struct GenTailParams {
 // returns once the slot's previous user (launch seq - kTailSlots) has finished.  The caller's next barrier publishes s_gen;
 // only after it may the CTA release its dependent grid.
 __device__ __forceinline__ void gen_take_ticket(const GenTailParams& T, uint32_t* s_gen) {
+    const unsigned long long tk = atomicAdd(&T.st->tick, 1ull);       // (ticket and acquire load in flight together: pcal_tail.cuh)
     uint32_t done, x;
     ld_acquire_done_started(T.st, done, x);
-    const uint32_t seq = (uint32_t)(atomicAdd(&T.st->tick, 1ull) / gridDim.x);
+    const uint32_t seq = (uint32_t)(tk / gridDim.x);
     s_gen[0] = seq; s_gen[1] = x;
     if ((int32_t)(done - (seq - kTailSlots + 1u)) < 0)
         while ((int32_t)(ld_acquire_u32(&T.st->n_done) - (seq - kTailSlots + 1u)) < 0) __nanosleep(64);

@@ -103,9 +103,12 @@ __device__ __forceinline__ uint32_t arrive_acq_rel(uint32_t* p) {
 __device__ __forceinline__ void fold_ticket_and_release(const TailParams& T, uint32_t* s_gen) {
     if (T.enabled) {
         if (threadIdx.x == 0) {
+            // (the ticket first, the acquire load behind it: both are in flight together -- one round trip, not two; X only has to
+            //  be read before this CTA releases its dependents, see above)
+            const unsigned long long tk = atomicAdd(&T.st->tick, 1ull);
             uint32_t done, x;
             ld_acquire_done_started(T.st, done, x);
-            const uint32_t seq = (uint32_t)(atomicAdd(&T.st->tick, 1ull) / gridDim.x);
+            const uint32_t seq = (uint32_t)(tk / gridDim.x);
             s_gen[0] = seq; s_gen[1] = x;
             s_gen[2] = ((int32_t)(done - (seq - kTailSlots + 1u)) >= 0) ? 1u : 0u;
         }
