@@ -430,6 +430,12 @@ static int prepare(pcal_ctx* c) {
         // float32: one CTA per SM and launch (64 KB of loads in flight each): the CTAs of consecutive launches share the SMs, so the
         // prologue and the tail of one launch hide under the streaming of the next (64 MB per step: 17 -> 12 us; 1 GB: 154 -> 150 us)
         if (!c->gen_mma && c->kind == KIND_F32) c->gen_grid = (uint32_t)c->sm_count;
+        // ... and one CTA per TWO SMs when the first segment (or period) the context sees is short (< 128 MB, ~20 us of streaming):
+        // the fixed cost of a CTA (ticket, tables, epilogue: ~4 us) is then spread over twice the data, and four launches are
+        // resident together instead of two (the paper's shape, 64 MB per step: 11.3 -> 9.7 us; on its own 27 -> 31 us).  The grid
+        // stays as chosen for the life of the geometry: the launch sequence numbers are tickets / grid (pcal_tail.cuh).
+        if (!c->gen_mma && c->kind == KIND_F32 && c->first_bytes && c->first_bytes < (128ull << 20) && c->sm_count >= 2)
+            c->gen_grid = (uint32_t)c->sm_count / 2u;
         if (const char* gg = getenv("PCAL_GEN_GRID")) { if (!c->gen_mma && atoi(gg) > 0) c->gen_grid = (uint32_t)atoi(gg); }   // tuning runs only
         // The fused tail pays while the partial bins of a launch are few (its finishing CTAs hold the slots of CTAs of the next
         // launch, whose tile assignment is static); config 5 (296 CTAs x 1024 bins) keeps the separate post and DFT kernels.
@@ -688,6 +694,7 @@ extern "C" int pcal_extract(pcal_ctx* c, const void* dev_samples, uint64_t n_sam
     if ((uintptr_t)dev_samples & 15u) return PCAL_ERR_ALIGNMENT;
     if ((n_samples * (uint64_t)c->bits * c->C) % 8) return PCAL_ERR_ALIGNMENT;
     c->stream = (cudaStream_t)cuda_stream;       // prepare() issues its set-up copies on the caller's stream
+    if (!c->prepared) c->first_bytes = n_samples * (uint64_t)c->bits * c->C / 8;
     const int rc = prepare(c);
     if (rc != PCAL_OK) return rc;
     c->started = true;
@@ -706,6 +713,7 @@ extern "C" int pcal_extract_series(pcal_ctx* c, const void* dev_samples, uint64_
     if (((uintptr_t)dev_samples & 15u) || bits_per_period % 128) return PCAL_ERR_ALIGNMENT;   // every period 16-byte aligned
     if (dev_out_folded && c->k_shift) return PCAL_ERR_STATE;
     c->stream = (cudaStream_t)cuda_stream;
+    if (!c->prepared) c->first_bytes = bits_per_period / 8;
     const int rc = prepare(c);
     if (rc != PCAL_OK) return rc;
     c->started = true;
@@ -841,6 +849,7 @@ extern "C" int pcal_integrate(pcal_ctx* c, const void* dev_samples, uint64_t n_s
     int r = pcal_reset(c);
     if (r != PCAL_OK) return r;
     c->stream = (cudaStream_t)cuda_stream;
+    if (!c->prepared) c->first_bytes = n_samples * (uint64_t)c->bits * c->C / 8;
     r = prepare(c);
     if (r != PCAL_OK) return r;
     // One launch for the whole period when the fold kernel can deliver T itself: a small DFT, the period is one

@@ -51,6 +51,7 @@ struct pcal_ctx {
     size_t partial_slot_bytes;
     uint32_t tail_tpp;              // threads per (channel, bin) pair in stage B of the fused tail
     uint32_t rot_tpp;               // threads per (channel, bin) pair in rotate_fold_kernel
+    uint64_t first_bytes;           // bytes of the first segment / period seen before the geometry was fixed (prepare): a size hint
     bool input_ready;               // pcal_set_input_ready: sample buffers are complete when extract is called
     bool zero_pending;              // reset happened, accumulators not yet overwritten or zeroed
     double* h_pinned;
